@@ -1,0 +1,149 @@
+/*
+ * radiusfps.h -- C-ABI of the B200-native RadiusFPS hot path.
+ *
+ * Exact farthest point sampling accelerated by spherical-voxel pruning
+ * (arxiv/paper_2606_06255; PAPER.md = the paper's text).  The library computes, for every
+ * cloud of a batch, the sequence defined by Eq. 3
+ *
+ *     s_j = argmax_{p in P}  min_{s in S_{j-1}}  d2(p, s),      j = 1 .. M-1,   s_0 = P[start_idx]
+ *
+ * under the exactness contract of PAPER.md:179 (same seed, same floating-point precision, argmax
+ * ties -> smallest original input index), with
+ *
+ *     d2(p, s) = ((dx*dx + dy*dy) + dz*dz),  dx = p.x - s.x, ...   fp32, round-to-nearest-even,
+ *                                                                   no FMA contraction
+ *
+ * (BASELINE.json north_star; the paper itself writes the Euclidean norm, Eq. 1/29).  The result
+ * is bit-identical to classical FPS (Alg. 1); the voxel index only removes work
+ * that cannot change it (Eq. 20-30).
+ *
+ * Conventions
+ *   - Every pointer named "DEVICE" is a CUDA device pointer on the current device; every other
+ *     pointer is a host pointer.  No torch types appear anywhere in this interface.
+ *   - The caller owns points, out_idx and out_mindist.  The library owns everything inside a
+ *     handle and frees it in fps_index_destroy.
+ *   - Functions returning int return FPS_OK (0) or a negative fps_status.  fps_last_error()
+ *     returns a thread-local, NUL-terminated description of the last failure on this thread.
+ *   - A handle holds mutable sampling state (Dist_p, Dist_v): calls on ONE handle must not
+ *     overlap; different handles are independent.
+ */
+#ifndef RADIUSFPS_H
+#define RADIUSFPS_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct fps_index fps_index_t;   /* opaque */
+
+typedef enum {
+    FPS_OK            =  0,
+    FPS_ERR_INVALID   = -1,  /* bad argument: N<1, B<1, M<1, M>N, start_idx outside [0,N), NULL pointer,
+                                unsupported option value                                              */
+    FPS_ERR_CUDA      = -2,  /* a CUDA runtime call or kernel launch failed                           */
+    FPS_ERR_NONFINITE = -3,  /* a coordinate is NaN or +-inf (the method has no defined answer)       */
+    FPS_ERR_NOMEM     = -4   /* device or host allocation failed                                      */
+} fps_status;
+
+/* Build options.  NOTHING here may change the sampled indices or min-distances: the options only
+ * move work around (the voxel resolution n_vox is a free parameter of the method, PAPER.md:192,
+ * :695; results are identical for every value).  Zero-initialise, then set what you need.       */
+typedef struct {
+    int32_t n_vox;         /* voxel bins per axis (Eq. 7); 0 = choose from N; 1..1024   */
+    int32_t tile_points;   /* split voxels holding more points than this into tiles with their own
+                              bounding sphere; 0 = default, -1 = never split (the paper's layout)      */
+    int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1,2,4,8,16            */
+    int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
+    int32_t flags;         /* FPS_FLAG_* below                                                          */
+    void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
+} fps_build_opts;
+
+enum {
+    FPS_FLAG_NO_PRUNE = 1,  /* ablation: visit every voxel (Eq. 25 never taken)                         */
+    FPS_FLAG_NO_SKIP  = 2,  /* ablation: no coordinate-wise point skip (Eq. 28 never taken)             */
+    FPS_FLAG_STATS    = 4   /* count voxel tests / visited voxels / visited points / effective updates  */
+};
+
+/* Counters and layout facts, summed over the B clouds (fps_get_stats).                             */
+typedef struct {
+    int32_t B, N;
+    int32_t n_vox;            /* resolution actually used                                             */
+    int32_t cluster_size, block_threads, voxels_per_thread;
+    int64_t K_total;          /* active (tiled) voxels over all clouds                                */
+    int32_t K_max;            /* largest per-cloud K                                                  */
+    int32_t max_voxel_points; /* largest segment                                                      */
+    int64_t device_bytes;     /* memory owned by the handle                                           */
+    /* the following are filled only when FPS_FLAG_STATS was set, for the LAST fps_sample call:      */
+    int64_t iterations;       /* sum over clouds of (M-1)                                             */
+    int64_t voxel_tests;      /* Eq. 25 evaluations                                                   */
+    int64_t voxels_visited;   /* voxels that survived the prune                                       */
+    int64_t points_visited;   /* points in visited voxels                                             */
+    int64_t points_computed;  /* points that passed the skip test                                     */
+    int64_t effective;        /* strict decreases of Dist_p (Eq. 2)                     */
+} fps_stats;
+
+/*
+ * fps_index_build -- steps a1-a6 of the hot path: on-device spherical-voxel index
+ * (Alg. 2 Phases 1-3; Eq. 6-10).
+ *
+ *   points  DEVICE, fp32, contiguous [B][N][3] (array of structures, row-major).  Read during the
+ *           call only; not referenced afterwards.
+ *   N       points per cloud, >= 1.     B  clouds, >= 1.  Every cloud gets its own bounding box,
+ *           grid, active-voxel list and sorted structure-of-arrays copy.
+ *
+ * Work is issued on the legacy default stream (fps_index_build) or on opts->stream (_ex); the
+ * call returns when the index is complete (it synchronises that stream).  Returns NULL on
+ * failure; fps_last_error() says why (FPS_ERR_NONFINITE if a coordinate is not finite).
+ */
+fps_index_t *fps_index_build(const float *points, int32_t N, int32_t B);
+fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const fps_build_opts *opts);
+
+/*
+ * fps_sample -- steps a7-a13: M-1 fused iterations of {select, radius prune (Eq. 25), point skip
+ * (Eq. 28), fp32 min-distance update (Eq. 29), per-voxel max (Eq. 30), global argmax (Eq. 15-18)}
+ * in ONE persistent kernel launch, for all B clouds at once.
+ *
+ *   M            samples per cloud, 1 <= M <= N.       start_idx  first sample of every cloud.
+ *   out_idx      DEVICE int32 [B][M]: ORIGINAL input indices in selection order; out_idx[b][0] ==
+ *                start_idx.
+ *   out_mindist  DEVICE fp32 [B][M]: squared fp32 distance of sample j to the nearest earlier
+ *                sample at the moment it was chosen (= max_i Dist_p[i]); out_mindist[b][0] = +inf.
+ *   stream       cudaStream_t (as void*) the launch is enqueued on; the call does not synchronise.
+ *
+ * May be called any number of times on one handle (any M, any start_idx); every call restarts
+ * from Dist_p = +inf.  On a negative return nothing has been enqueued.
+ */
+int fps_sample(fps_index_t *h, int32_t M, int32_t start_idx,
+               int32_t *out_idx, float *out_mindist, void *stream);
+
+/* Frees the handle and all device memory it owns.  NULL is allowed. */
+void fps_index_destroy(fps_index_t *h);
+
+/* Layout facts and (with FPS_FLAG_STATS) the counters of the last fps_sample; synchronises the
+ * stream of that call.  out: host pointer. */
+int fps_get_stats(fps_index_t *h, fps_stats *out);
+
+/*
+ * fps_sample_host -- the same path for callers whose data lives in HOST memory: copies
+ * points [B][N][3] to the device, builds the index, samples, copies out_idx / out_mindist
+ * (HOST, [B][M]) back and destroys the index.  Synchronous.  opts may be NULL.
+ */
+int fps_sample_host(const float *points_host, int32_t N, int32_t B, int32_t M, int32_t start_idx,
+                    int32_t *out_idx_host, float *out_mindist_host, const fps_build_opts *opts);
+
+/* Thread-local description of the last error on the calling thread ("" if none). */
+const char *fps_last_error(void);
+
+/* fps_status of the last fps_index_build / fps_index_build_ex on the calling thread (those return
+ * a pointer, so NULL alone cannot say why): FPS_OK after a success. */
+int fps_last_status(void);
+
+/* Library version string, e.g. "radiusfps-b200 0.1 (sm_100a)". */
+const char *fps_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RADIUSFPS_H */

@@ -28,8 +28,10 @@
  *   A9  Eq. 25 is proved over the reals; here it is applied with fp32 safety margins:
  *         build:  r_k = sqrtf(max_p d2(p,c_k)) * (1+2^-20)
  *         test:   dc = sqrtf(d2(s,c_k)) * (1-2^-20);  t = (dc - r_k) * (1-2^-20)
- *                 prune iff t > 0 and (t*t)*(1-2^-20) >= Dist_v[k] and Dist_v[k] >= 1e-30f
- *       (the last clause keeps the relative-error argument clear of underflow).
+ *                 prune iff Dist_v[k] == 0, or
+ *                           t > 0 and (t*t)*(1-2^-20) >= Dist_v[k] and Dist_v[k] >= 1e-30f
+ *       (Dist_v[k] == 0: no squared distance is < 0, so the strict-< update of Eq. 2 cannot fire;
+ *       the 1e-30f clause keeps the relative-error argument clear of underflow).
  *   A10 c_k = midpoint of the axis-aligned bounding box of the voxel's own points, r_k tight
  *       (any enclosing sphere is valid; Eq. 10's sqrt(3)/2 L is one).
  *   A11 Dist_v starts at +inf instead of 0, so iteration 1 prunes nothing and the "initial
@@ -180,7 +182,8 @@ int pruned_fps_cpu(const float *P, int32_t N, int32_t M, int32_t start, int32_t 
                 } else {
                     const float dc = sqrtf(d2c) * DN;
                     const float t = (dc - vr[k]) * DN;
-                    prune = (t > 0.0f) && ((t * t) * DN >= Dv[k]) && (Dv[k] >= 1e-30f);
+                    prune = (Dv[k] == 0.0f) ||
+                            ((t > 0.0f) && ((t * t) * DN >= Dv[k]) && (Dv[k] >= 1e-30f));
                 }
             }
             if (!prune) {

@@ -1,0 +1,201 @@
+"""Thin ctypes binding of the C-ABI in include/radiusfps.h -- argument marshalling only.
+
+Same names as the C entry points.  PyTorch is used for device memory and streams, nothing else:
+every step of the path runs in the CUDA kernels of ``csrc/``.  There is no CPU fallback: if
+``libradiusfps.so`` is missing this module raises at first use.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
+
+FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
+FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS = 1, 2, 4
+
+EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_sample", "fps_index_destroy", "fps_get_stats",
+           "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
+
+
+class fps_build_opts(ctypes.Structure):
+    _fields_ = [("n_vox", ctypes.c_int32), ("tile_points", ctypes.c_int32), ("cluster_size", ctypes.c_int32),
+                ("block_threads", ctypes.c_int32), ("flags", ctypes.c_int32), ("stream", ctypes.c_void_p)]
+
+
+class fps_stats(ctypes.Structure):
+    _fields_ = [("B", ctypes.c_int32), ("N", ctypes.c_int32), ("n_vox", ctypes.c_int32),
+                ("cluster_size", ctypes.c_int32), ("block_threads", ctypes.c_int32),
+                ("voxels_per_thread", ctypes.c_int32),
+                ("K_total", ctypes.c_int64), ("K_max", ctypes.c_int32), ("max_voxel_points", ctypes.c_int32),
+                ("device_bytes", ctypes.c_int64), ("iterations", ctypes.c_int64), ("voxel_tests", ctypes.c_int64),
+                ("voxels_visited", ctypes.c_int64), ("points_visited", ctypes.c_int64),
+                ("points_computed", ctypes.c_int64), ("effective", ctypes.c_int64)]
+
+    def as_dict(self) -> dict:
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class FpsError(RuntimeError):
+    def __init__(self, status: int, message: str):
+        super().__init__(f"radiusfps status {status}: {message}")
+        self.status = status
+
+
+_lib = None
+
+
+def load() -> ctypes.CDLL:
+    """dlopen the in-tree library; raises (no fallback) when it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise FileNotFoundError(
+            f"{LIB_PATH} is missing: build it with `python -m paper_2606_06255_b200.build` "
+            "(or __graft_entry__.build()); there is no CPU fallback")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, i32 = ctypes.c_void_p, ctypes.c_int32
+    lib.fps_index_build.restype = vp
+    lib.fps_index_build.argtypes = [vp, i32, i32]
+    lib.fps_index_build_ex.restype = vp
+    lib.fps_index_build_ex.argtypes = [vp, i32, i32, ctypes.POINTER(fps_build_opts)]
+    lib.fps_sample.restype = ctypes.c_int
+    lib.fps_sample.argtypes = [vp, i32, i32, vp, vp, vp]
+    lib.fps_index_destroy.restype = None
+    lib.fps_index_destroy.argtypes = [vp]
+    lib.fps_get_stats.restype = ctypes.c_int
+    lib.fps_get_stats.argtypes = [vp, ctypes.POINTER(fps_stats)]
+    lib.fps_sample_host.restype = ctypes.c_int
+    lib.fps_sample_host.argtypes = [vp, i32, i32, i32, i32, vp, vp, ctypes.POINTER(fps_build_opts)]
+    lib.fps_last_error.restype = ctypes.c_char_p
+    lib.fps_last_error.argtypes = []
+    lib.fps_version.restype = ctypes.c_char_p
+    lib.fps_version.argtypes = []
+    lib.fps_last_status.restype = ctypes.c_int
+    lib.fps_last_status.argtypes = []
+    _lib = lib
+    return lib
+
+
+def fps_last_error() -> str:
+    return load().fps_last_error().decode()
+
+
+def fps_version() -> str:
+    return load().fps_version().decode()
+
+
+def _check_points(points: torch.Tensor) -> tuple[int, int]:
+    if points.dtype != torch.float32 or not points.is_contiguous():
+        raise ValueError("points must be a contiguous float32 tensor")
+    if points.dim() == 2 and points.shape[1] == 3:
+        return 1, points.shape[0]
+    if points.dim() == 3 and points.shape[2] == 3:
+        return points.shape[0], points.shape[1]
+    raise ValueError("points must be [N,3] or [B,N,3]")
+
+
+def _opts(n_vox=0, tile_points=0, cluster_size=0, block_threads=0, flags=0, stream=None) -> fps_build_opts:
+    return fps_build_opts(n_vox, tile_points, cluster_size, block_threads, flags, stream or 0)
+
+
+class Index:
+    """Owner of one ``fps_index_t*``.  ``points``: CUDA float32 [B,N,3] (or [N,3])."""
+
+    def __init__(self, handle: int, B: int, N: int, device: torch.device):
+        self.handle, self.B, self.N, self.device = handle, B, N, device
+
+    def sample(self, M: int, start_idx: int = 0, out_idx: torch.Tensor | None = None,
+               out_mindist: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
+        return fps_sample(self, M, start_idx, out_idx, out_mindist, stream)
+
+    def stats(self) -> dict:
+        return fps_get_stats(self)
+
+    def destroy(self) -> None:
+        fps_index_destroy(self)
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def fps_index_build(points: torch.Tensor, *, n_vox: int = 0, tile_points: int = 0, cluster_size: int = 0,
+                    block_threads: int = 0, flags: int = 0, stream: torch.cuda.Stream | None = None) -> Index:
+    """fps_index_build / fps_index_build_ex.  The build is issued on ``stream`` (default: torch's
+    current stream) and is complete when this returns."""
+    lib = load()
+    if not points.is_cuda:
+        raise ValueError("points must live on a CUDA device (use fps_sample_host for host arrays)")
+    B, N = _check_points(points)
+    with torch.cuda.device(points.device):
+        s = stream if stream is not None else torch.cuda.current_stream()
+        o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, s.cuda_stream)
+        h = lib.fps_index_build_ex(points.data_ptr(), N, B, ctypes.byref(o))
+    if not h:
+        raise FpsError(lib.fps_last_status(), fps_last_error())
+    return Index(h, B, N, points.device)
+
+
+def fps_sample(index: Index, M: int, start_idx: int = 0, out_idx: torch.Tensor | None = None,
+               out_mindist: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
+    """fps_sample: enqueue on ``stream`` (default: torch's current stream); returns
+    (out_idx int32 [B,M], out_mindist float32 [B,M]) without synchronising."""
+    lib = load()
+    if index.handle is None:
+        raise ValueError("index was destroyed")
+    M = int(M)
+    with torch.cuda.device(index.device):
+        if out_idx is None:
+            out_idx = torch.empty((index.B, max(M, 0)), dtype=torch.int32, device=index.device)
+        if out_mindist is None:
+            out_mindist = torch.empty((index.B, max(M, 0)), dtype=torch.float32, device=index.device)
+        if out_idx.dtype != torch.int32 or out_mindist.dtype != torch.float32 or not out_idx.is_contiguous() \
+                or not out_mindist.is_contiguous() or out_idx.numel() < index.B * M or out_mindist.numel() < index.B * M:
+            raise ValueError("out_idx must be contiguous int32 [B,M] and out_mindist contiguous float32 [B,M]")
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.fps_sample(index.handle, M, int(start_idx), out_idx.data_ptr(), out_mindist.data_ptr(), s.cuda_stream)
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return out_idx, out_mindist
+
+
+def fps_index_destroy(index: Index) -> None:
+    if index.handle is not None:
+        load().fps_index_destroy(index.handle)
+        index.handle = None
+
+
+def fps_get_stats(index: Index) -> dict:
+    st = fps_stats()
+    rc = load().fps_get_stats(index.handle, ctypes.byref(st))
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return st.as_dict()
+
+
+def fps_sample_host(points_host: torch.Tensor, M: int, start_idx: int = 0, *, n_vox: int = 0, tile_points: int = 0,
+                    cluster_size: int = 0, block_threads: int = 0, flags: int = 0,
+                    out_idx: torch.Tensor | None = None, out_mindist: torch.Tensor | None = None):
+    """fps_sample_host: HOST float32 [B,N,3] in, HOST int32/float32 [B,M] out; copies, index build and
+    sampling all happen inside the C call (synchronous)."""
+    lib = load()
+    if points_host.is_cuda:
+        raise ValueError("fps_sample_host takes host tensors")
+    B, N = _check_points(points_host)
+    if out_idx is None:
+        out_idx = torch.empty((B, M), dtype=torch.int32, pin_memory=torch.cuda.is_available())
+    if out_mindist is None:
+        out_mindist = torch.empty((B, M), dtype=torch.float32, pin_memory=torch.cuda.is_available())
+    o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, None)
+    rc = lib.fps_sample_host(points_host.data_ptr(), N, B, int(M), int(start_idx), out_idx.data_ptr(),
+                             out_mindist.data_ptr(), ctypes.byref(o))
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return out_idx, out_mindist

@@ -1,0 +1,577 @@
+// index_build.cu -- steps a1-a6 of the hot path: the on-device spherical-voxel index.
+//
+// Follows Alg. 2 Phases 1-3 of the paper and Eq. 6-10:
+//   a1 bounding box           Eq. 6-7   (k_bbox)
+//   a2 voxel id per point     Eq. 8, 31 (k_keys)
+//   a3 radix sort by voxel id Alg. 2 l.11 (radix_sort_pairs: hand-written stable LSD radix sort)
+//   a4 gather AoS -> SoA      Alg. 2 Phase 2 (k_gather)
+//   a5 active-voxel segments  Alg. 2 Phase 3 (k_heads + scan + k_voxel_segments)
+//   a6 per-voxel sphere       Eq. 10 / north_star "per-voxel center, radius" (k_sphere)
+// What differs from the paper:
+//   * the sort key carries a few Morton bits of the position INSIDE the voxel below V_id, so that
+//     a voxel holding more than `tile_points` points can be cut into spatially compact tiles;
+//     every tile is a "spherical voxel" of its own (own centre, own tight radius).  Any
+//     partition with conservative spheres leaves the result unchanged (Eq. 20-26).
+//   * c_k is the midpoint of the tile's own bounding box and r_k its tight radius rounded up,
+//     instead of the cell centre and sqrt(3)/2 L (reading A10).
+#include <cfloat>
+#include <cmath>
+#include <cstdlib>
+#include <cstring>
+#include <vector>
+
+#include "internal.h"
+
+namespace rfps {
+
+// ---------------------------------------------------------------------------------------------
+// small helpers
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned f2ord(float f)
+{   // monotone map float -> uint (for atomicMin/Max on floats of either sign)
+    unsigned u = __float_as_uint(f);
+    return (u & 0x80000000u) ? ~u : (u | 0x80000000u);
+}
+__device__ __forceinline__ float ord2f(unsigned u)
+{
+    return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
+}
+
+struct DevBuf {   // RAII for build-time scratch
+    void *p = nullptr;
+    ~DevBuf() { if (p) cudaFree(p); }
+    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 4); }
+    template <class T> T *as() { return reinterpret_cast<T *>(p); }
+};
+
+// ---------------------------------------------------------------------------------------------
+// a1: bounding box (Eq. 6) + non-finite detection.  bbox[b] = {minx,miny,minz,maxx,maxy,maxz} as
+// order-preserving uints; bbox[b][6] = non-finite flag.
+// ---------------------------------------------------------------------------------------------
+constexpr int BBOX_STRIDE = 8;
+
+__global__ void k_bbox_init(unsigned *bbox, int B)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < B * BBOX_STRIDE) {
+        int c = i % BBOX_STRIDE;
+        bbox[i] = c < 3 ? 0xFFFFFFFFu : 0u;
+    }
+}
+
+__global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, int N, unsigned *bbox)
+{
+    const int b = blockIdx.y;
+    const float *P = pts + (size_t)b * N * 3;
+    float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+    bool bad = false;
+    for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            float v = P[3 * (size_t)i + a];
+            bad |= !(fabsf(v) <= FLT_MAX);   // NaN or inf
+            mn[a] = fminf(mn[a], v);
+            mx[a] = fmaxf(mx[a], v);
+        }
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        for (int o = 16; o > 0; o >>= 1) {
+            mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+            mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+        }
+    bad = __any_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0) {
+        unsigned *bb = bbox + b * BBOX_STRIDE;
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            if (mn[a] <= mx[a]) {
+                atomicMin(bb + a, f2ord(mn[a]));
+                atomicMax(bb + 3 + a, f2ord(mx[a]));
+            }
+        }
+        if (bad) atomicOr(bb + 6, 1u);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a2: sort key per point.  key = V_id << (3*sb) | morton(sub-cell), V_id per Eq. 31; val = i.
+// Voxel coordinates per Eq. 8 (floor, then clamp; reading A14); L per Eq. 7 with alpha = 1 + 1e-3.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned spread3(unsigned v)
+{   // 0b abcd -> 0b a00b00c00d (up to 10 bits)
+    v &= 0x3ffu;
+    v = (v | (v << 16)) & 0x030000ffu;
+    v = (v | (v << 8)) & 0x0300f00fu;
+    v = (v | (v << 4)) & 0x030c30c3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int N, const unsigned *__restrict__ bbox,
+                                               int n_vox, int sb, unsigned *__restrict__ keys, int *__restrict__ vals)
+{
+    const int b = blockIdx.y;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const unsigned *bb = bbox + b * BBOX_STRIDE;
+    const float lo[3] = {ord2f(bb[0]), ord2f(bb[1]), ord2f(bb[2])};
+    const float hi[3] = {ord2f(bb[3]), ord2f(bb[4]), ord2f(bb[5])};
+    float E = fmaxf(fmaxf(hi[0] - lo[0], hi[1] - lo[1]), hi[2] - lo[2]);
+    float L = (1.0f + 1e-3f) * E / (float)n_vox;
+    if (!(L > 0.0f)) L = 1.0f;
+    const float invsub = (float)(1 << sb);
+    unsigned v[3], s[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        float t = (pts[((size_t)b * N + i) * 3 + a] - lo[a]) / L;
+        float f = floorf(t);
+        int c = (int)f;
+        c = max(0, min(n_vox - 1, c));
+        int sc = (int)floorf((t - (float)c) * invsub);
+        sc = max(0, min((1 << sb) - 1, sc));
+        v[a] = (unsigned)c;
+        s[a] = (unsigned)sc;
+    }
+    unsigned vid = (v[2] * (unsigned)n_vox + v[1]) * (unsigned)n_vox + v[0];
+    unsigned sub = sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
+    keys[(size_t)b * N + i] = (vid << (3 * sb)) | sub;
+    vals[(size_t)b * N + i] = i;
+}
+
+// ---------------------------------------------------------------------------------------------
+// batched exclusive scan of int32: three kernels (block sums, scan of block sums, apply)
+// ---------------------------------------------------------------------------------------------
+constexpr int SCAN_T = 256, SCAN_ITEMS = 8, SCAN_TILE = SCAN_T * SCAN_ITEMS;
+
+__device__ __forceinline__ int block_excl_scan(int v, int *total, int *sm /*[33]*/)
+{   // exclusive scan of one int per thread across a 256-thread block
+    const int lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    int inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+    }
+    if (lane == 31) sm[w] = inc;
+    __syncthreads();
+    if (w == 0) {
+        int s = lane < (SCAN_T / 32) ? sm[lane] : 0;
+        int si = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int t = __shfl_up_sync(0xffffffffu, si, o);
+            if (lane >= o) si += t;
+        }
+        if (lane < (SCAN_T / 32)) sm[lane] = si - s;
+        if (lane == 31) sm[32] = si;
+    }
+    __syncthreads();
+    int r = inc - v + sm[w];
+    *total = sm[32];
+    __syncthreads();
+    return r;
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_blocksum(const int *__restrict__ in, int n, int stride, int nblk,
+                                                           int *__restrict__ bsum)
+{
+    __shared__ int sm[33];
+    const int b = blockIdx.y;
+    const int *src = in + (size_t)b * stride;
+    int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i)
+        if (base + i < n) s += src[base + i];
+    int tot;
+    block_excl_scan(s, &tot, sm);
+    if (threadIdx.x == 0) bsum[(size_t)b * nblk + blockIdx.x] = tot;
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_bsums(int *bsum, int nblk, int *totals)
+{
+    __shared__ int sm[33];
+    const int b = blockIdx.x;
+    int *s = bsum + (size_t)b * nblk;
+    int carry = 0;
+    for (int base = 0; base < nblk; base += SCAN_T) {
+        int i = base + threadIdx.x;
+        int v = i < nblk ? s[i] : 0;
+        int tot;
+        int e = block_excl_scan(v, &tot, sm);
+        if (i < nblk) s[i] = e + carry;
+        carry += tot;
+    }
+    if (threadIdx.x == 0 && totals) totals[b] = carry;
+}
+
+__global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ in, int *__restrict__ out, int n, int stride,
+                                                        int nblk, const int *__restrict__ bsum)
+{
+    __shared__ int sm[33];
+    const int b = blockIdx.y;
+    const int *src = in + (size_t)b * stride;
+    int *dst = out + (size_t)b * stride;
+    int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
+    int v[SCAN_ITEMS], s = 0;
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        v[i] = base + i < n ? src[base + i] : 0;
+        s += v[i];
+    }
+    int tot;
+    int e = block_excl_scan(s, &tot, sm) + bsum[(size_t)b * nblk + blockIdx.x];
+#pragma unroll
+    for (int i = 0; i < SCAN_ITEMS; ++i) {
+        if (base + i < n) dst[base + i] = e;
+        e += v[i];
+    }
+}
+
+// exclusive scan of B arrays of n ints (per-array stride `stride`); totals[b] (device, may be null)
+static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
+                          cudaStream_t st)
+{
+    const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
+    k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp);
+    k_scan_bsums<<<B, SCAN_T, 0, st>>>(bsum_tmp, nblk, totals);
+    k_scan_apply<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, out, n, stride, nblk, bsum_tmp);
+    RFPS_CUDA(cudaGetLastError());
+    return FPS_OK;
+}
+static inline int scan_tmp_ints(int n, int B) { return ((n + SCAN_TILE - 1) / SCAN_TILE) * B + 1; }
+
+// ---------------------------------------------------------------------------------------------
+// a3: stable LSD radix sort of (key, val) pairs, 8 bits per pass, batched over clouds.
+// One warp owns a chunk of RS_CHUNK consecutive keys; its 256 digit counters live in shared
+// memory.  The counter table is digit-major ([digit][chunk]) so that one exclusive scan gives
+// every (digit, chunk) its global output offset.  Stability: chunks are ordered by the table
+// layout, rounds inside a chunk run in order, lanes inside a round are ranked by lane id
+// (__match_any_sync + popc of lower lanes).
+// ---------------------------------------------------------------------------------------------
+constexpr int RS_CHUNK = 2048, RS_WARPS = 4;
+
+__global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, int N, int nchunk, int shift,
+                                                               int *__restrict__ table)
+{
+    __shared__ int h[RS_WARPS][256];
+    const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c = blockIdx.x * RS_WARPS + w;
+    for (int d = lane; d < 256; d += 32) h[w][d] = 0;
+    __syncwarp();
+    if (c < nchunk) {
+        const unsigned *k = keys + (size_t)b * N;
+        const int end = min(N, (c + 1) * RS_CHUNK);
+        for (int p = c * RS_CHUNK + lane; p < end; p += 32) atomicAdd(&h[w][(k[p] >> shift) & 255u], 1);
+        __syncwarp();
+        int *t = table + (size_t)b * 256 * nchunk;
+        for (int d = lane; d < 256; d += 32) t[(size_t)d * nchunk + c] = h[w][d];
+    }
+}
+
+__global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned *__restrict__ keys, const int *__restrict__ vals,
+                                                                  int N, int nchunk, int shift, const int *__restrict__ table,
+                                                                  unsigned *__restrict__ okeys, int *__restrict__ ovals)
+{
+    __shared__ int base[RS_WARPS][256];
+    const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const int c = blockIdx.x * RS_WARPS + w;
+    if (c >= nchunk) return;
+    const int *t = table + (size_t)b * 256 * nchunk;
+    for (int d = lane; d < 256; d += 32) base[w][d] = t[(size_t)d * nchunk + c];
+    __syncwarp();
+    const unsigned *k = keys + (size_t)b * N;
+    const int *v = vals + (size_t)b * N;
+    unsigned *ok = okeys + (size_t)b * N;
+    int *ov = ovals + (size_t)b * N;
+    const int end = min(N, (c + 1) * RS_CHUNK);
+    const unsigned lt = (1u << lane) - 1u;
+    for (int p0 = c * RS_CHUNK; p0 < end; p0 += 32) {
+        const int p = p0 + lane;
+        const bool valid = p < end;
+        unsigned key = valid ? k[p] : 0u;
+        int val = valid ? v[p] : 0;
+        unsigned d = valid ? ((key >> shift) & 255u) : 256u;
+        unsigned peers = __match_any_sync(0xffffffffu, d);
+        int rank = __popc(peers & lt);
+        int dst = 0;
+        if (valid) dst = base[w][d] + rank;
+        __syncwarp();
+        if (valid && rank == 0) base[w][d] += __popc(peers);
+        __syncwarp();
+        if (valid) { ok[dst] = key; ov[dst] = val; }
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a5: active voxels.  heads[p] = 1 where the grid-voxel id changes; scan -> voxel rank.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_heads(const unsigned *__restrict__ keys, int N, int subbits, int *__restrict__ heads)
+{
+    const int b = blockIdx.y;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const unsigned *k = keys + (size_t)b * N;
+    heads[(size_t)b * N + p] = (p == 0 || (k[p] >> subbits) != (k[p - 1] >> subbits)) ? 1 : 0;
+}
+
+// voff[b][rank] = p for every head position p
+__global__ void __launch_bounds__(256) k_voxel_offsets(const int *__restrict__ heads, const int *__restrict__ rank, int N,
+                                                        int *__restrict__ voff)
+{
+    const int b = blockIdx.y;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    if (heads[(size_t)b * N + p]) voff[(size_t)b * N + rank[(size_t)b * N + p]] = p;
+}
+
+// number of tiles of each grid voxel: ceil(cnt / tile_points) (1 if tiling is off)
+__global__ void __launch_bounds__(256) k_ntiles(const int *__restrict__ voff, const int *__restrict__ Kv, int N, int tile_points,
+                                                 int *__restrict__ ntiles)
+{
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= N) return;
+    const int kv = Kv[b];
+    int nt = 0;
+    if (k < kv) {
+        const int off = voff[(size_t)b * N + k];
+        const int cnt = (k + 1 < kv ? voff[(size_t)b * N + k + 1] : N) - off;
+        nt = tile_points > 0 ? (cnt + tile_points - 1) / tile_points : 1;
+    }
+    ntiles[(size_t)b * N + k] = nt;
+}
+
+// vseg[b][tbase[k] + t] = {off + t*chunk, len}: equal-size tiles of the (Morton-ordered) voxel run
+__global__ void __launch_bounds__(256) k_tiles(const int *__restrict__ voff, const int *__restrict__ Kv, const int *__restrict__ ntiles,
+                                                const int *__restrict__ tbase, int N, int K_cap, int2 *__restrict__ vseg)
+{
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    const int kv = Kv[b];
+    if (k >= kv) return;
+    const int off = voff[(size_t)b * N + k];
+    const int cnt = (k + 1 < kv ? voff[(size_t)b * N + k + 1] : N) - off;
+    const int nt = ntiles[(size_t)b * N + k];
+    const int chunk = (cnt + nt - 1) / nt;
+    int2 *dst = vseg + (size_t)b * K_cap + tbase[(size_t)b * N + k];
+    for (int t = 0; t < nt; ++t) {
+        const int s = t * chunk;
+        dst[t] = make_int2(off + s, min(chunk, cnt - s));
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// a4: gather AoS -> sorted SoA (+ permutation and its inverse)
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pts, const int *__restrict__ order, int N,
+                                                 float *__restrict__ px, float *__restrict__ py, float *__restrict__ pz,
+                                                 int *__restrict__ porig, int *__restrict__ pinv)
+{
+    const int b = blockIdx.y;
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= N) return;
+    const size_t o = (size_t)b * N;
+    const int i = order[o + p];
+    const float *s = pts + (o + i) * 3;
+    px[o + p] = s[0];
+    py[o + p] = s[1];
+    pz[o + p] = s[2];
+    porig[o + p] = i;
+    pinv[o + i] = p;
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6: per-voxel bounding sphere, one warp per voxel.
+//   c_k = midpoint of the axis-aligned bounding box of the voxel's points (reading A10)
+//   R_k = sqrt_rn(max_p d2(p, c_k)) * (1 + 2^-20)      (reading A9: rounded UP past every fp32
+//         error of d2 and sqrt, so that ||p - c_k|| <= R_k holds over the reals)
+// d2 is the library's one distance expression, ((dx*dx + dy*dy) + dz*dz) without FMA.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ float d2_rn(float x, float y, float z, float sx, float sy, float sz)
+{
+    const float dx = __fsub_rn(x, sx), dy = __fsub_rn(y, sy), dz = __fsub_rn(z, sz);
+    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
+}
+
+__global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, const float *__restrict__ py,
+                                                 const float *__restrict__ pz, const int2 *__restrict__ vseg,
+                                                 const int *__restrict__ K, int N, int K_cap, float4 *__restrict__ vgeom,
+                                                 int *__restrict__ maxcnt)
+{
+    const int b = blockIdx.y;
+    const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (k >= K[b]) return;
+    const int2 sg = vseg[(size_t)b * K_cap + k];
+    const float *x = px + (size_t)b * N, *y = py + (size_t)b * N, *z = pz + (size_t)b * N;
+    float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+    for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) {
+        mn[0] = fminf(mn[0], x[p]); mx[0] = fmaxf(mx[0], x[p]);
+        mn[1] = fminf(mn[1], y[p]); mx[1] = fmaxf(mx[1], y[p]);
+        mn[2] = fminf(mn[2], z[p]); mx[2] = fmaxf(mx[2], z[p]);
+    }
+#pragma unroll
+    for (int a = 0; a < 3; ++a)
+        for (int o = 16; o > 0; o >>= 1) {
+            mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+            mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+        }
+    const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+    const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+    const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+    float r2 = 0.0f;
+    for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) r2 = fmaxf(r2, d2_rn(x[p], y[p], z[p], cx, cy, cz));
+    for (int o = 16; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+    if (lane == 0) {
+        const float R = __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f);
+        vgeom[(size_t)b * K_cap + k] = make_float4(cx, cy, cz, R);
+        atomicMax(maxcnt, sg.y);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// host orchestration
+// ---------------------------------------------------------------------------------------------
+static int ilog2_ceil(unsigned long long v)
+{
+    int b = 0;
+    while ((1ull << b) < v) ++b;
+    return b;
+}
+
+static int auto_n_vox(int N)
+{   // nearest power of two to N^(1/3): a few points per active voxel on surface-like clouds.
+    // A free parameter of the method; results do not depend on it.
+    double c = std::cbrt((double)N);
+    int n = 1;
+    while (n * 2 <= 1024 && std::fabs(std::log2((double)n * 2) - std::log2(c)) <= std::fabs(std::log2((double)n) - std::log2(c))) n *= 2;
+    return n < 2 ? 2 : n;
+}
+
+template <class T>
+static int dev_alloc(T *&p, size_t count, int64_t &total)
+{
+    void *q = nullptr;
+    size_t bytes = (count ? count : 1) * sizeof(T);
+    cudaError_t e = cudaMalloc(&q, bytes);
+    if (e != cudaSuccess) {
+        set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
+        return FPS_ERR_NOMEM;
+    }
+    p = reinterpret_cast<T *>(q);
+    total += (int64_t)bytes;
+    return FPS_OK;
+}
+
+void free_index(DeviceIndex &ix)
+{
+    cudaFree(ix.px); cudaFree(ix.py); cudaFree(ix.pz);
+    cudaFree(ix.porig); cudaFree(ix.pinv); cudaFree(ix.Dp);
+    cudaFree(ix.vgeom); cudaFree(ix.vseg); cudaFree(ix.vstate);
+    cudaFree(ix.K_dev); cudaFree(ix.counters);
+    free(ix.K_host);
+    ix = DeviceIndex();
+}
+
+int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
+{
+    const int B = ix.B, N = ix.N;
+    cudaStream_t st = (cudaStream_t)o.stream;
+    int n_vox = o.n_vox > 0 ? o.n_vox : auto_n_vox(N);
+    if (n_vox > 1024) { set_error("n_vox=%d out of range [1,1024]", n_vox); return FPS_ERR_INVALID; }
+    int tile_points = o.tile_points == 0 ? 64 : (o.tile_points < 0 ? 0 : o.tile_points);
+    const int vbits = ilog2_ceil((unsigned long long)n_vox * n_vox * n_vox);
+    int sb = tile_points > 0 ? (32 - vbits) / 3 : 0;
+    if (sb > 4) sb = 4;
+    const int keybits = vbits + 3 * sb;
+    ix.n_vox = n_vox;
+    ix.tile_points = tile_points;
+    ix.flags = o.flags;
+
+    const size_t BN = (size_t)B * N;
+    const int nchunk = (N + RS_CHUNK - 1) / RS_CHUNK;
+    const size_t table_n = (size_t)256 * nchunk;       // per cloud
+    DevBuf bbox, kA, kB, vA, vB, table, bsum, heads, rank, voff, ntl, tbase, Kv;
+    if (bbox.alloc(sizeof(unsigned) * B * BBOX_STRIDE) || kA.alloc(4 * BN) || kB.alloc(4 * BN) || vA.alloc(4 * BN) ||
+        vB.alloc(4 * BN) || table.alloc(4 * table_n * B) ||
+        bsum.alloc(4 * (size_t)(scan_tmp_ints((int)std::max((size_t)N, table_n), B))) || heads.alloc(4 * BN) ||
+        rank.alloc(4 * BN) || voff.alloc(4 * BN) || ntl.alloc(4 * BN) || tbase.alloc(4 * BN) || Kv.alloc(4 * B)) {
+        set_error("cudaMalloc of build scratch failed (B=%d, N=%d)", B, N);
+        return FPS_ERR_NOMEM;
+    }
+    int rc;
+    if ((rc = dev_alloc(ix.K_dev, B, ix.device_bytes)) != FPS_OK) return rc;
+
+    const dim3 gN((N + 255) / 256, B);
+    k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(bbox.as<unsigned>(), B);
+    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, bbox.as<unsigned>());
+    k_keys<<<gN, 256, 0, st>>>(points, N, bbox.as<unsigned>(), n_vox, sb, kA.as<unsigned>(), vA.as<int>());
+    RFPS_CUDA(cudaGetLastError());
+
+    // a3: LSD radix sort, 8 bits per pass
+    unsigned *kin = kA.as<unsigned>(), *kout = kB.as<unsigned>();
+    int *vin = vA.as<int>(), *vout = vB.as<int>();
+    const dim3 gR((nchunk + RS_WARPS - 1) / RS_WARPS, B);
+    for (int shift = 0; shift < keybits; shift += 8) {
+        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, N, nchunk, shift, table.as<int>());
+        if ((rc = scan_exclusive(table.as<int>(), table.as<int>(), (int)table_n, (int)table_n, B, nullptr, bsum.as<int>(), st)))
+            return rc;
+        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, N, nchunk, shift, table.as<int>(), kout, vout);
+        std::swap(kin, kout);
+        std::swap(vin, vout);
+    }
+    RFPS_CUDA(cudaGetLastError());
+
+    // a5: grid voxels -> (tiled) segments
+    k_heads<<<gN, 256, 0, st>>>(kin, N, 3 * sb, heads.as<int>());
+    if ((rc = scan_exclusive(heads.as<int>(), rank.as<int>(), N, N, B, Kv.as<int>(), bsum.as<int>(), st))) return rc;
+    k_voxel_offsets<<<gN, 256, 0, st>>>(heads.as<int>(), rank.as<int>(), N, voff.as<int>());
+    k_ntiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), N, tile_points, ntl.as<int>());
+    if ((rc = scan_exclusive(ntl.as<int>(), tbase.as<int>(), N, N, B, ix.K_dev, bsum.as<int>(), st))) return rc;
+    RFPS_CUDA(cudaGetLastError());
+
+    // the one host round-trip of the build: K per cloud + the non-finite flags
+    ix.K_host = (int32_t *)malloc(sizeof(int32_t) * B);
+    std::vector<unsigned> hb((size_t)B * BBOX_STRIDE);
+    if (!ix.K_host) { set_error("host malloc failed"); return FPS_ERR_NOMEM; }
+    RFPS_CUDA(cudaMemcpyAsync(ix.K_host, ix.K_dev, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, st));
+    RFPS_CUDA(cudaMemcpyAsync(hb.data(), bbox.p, sizeof(unsigned) * B * BBOX_STRIDE, cudaMemcpyDeviceToHost, st));
+    RFPS_CUDA(cudaStreamSynchronize(st));
+    for (int b = 0; b < B; ++b)
+        if (hb[(size_t)b * BBOX_STRIDE + 6]) {
+            set_error("cloud %d holds a NaN or infinite coordinate", b);
+            return FPS_ERR_NONFINITE;
+        }
+    ix.K_max = 0;
+    ix.K_total = 0;
+    for (int b = 0; b < B; ++b) {
+        ix.K_max = std::max(ix.K_max, ix.K_host[b]);
+        ix.K_total += ix.K_host[b];
+    }
+    ix.K_cap = ix.K_max;
+
+    if ((rc = dev_alloc(ix.px, BN, ix.device_bytes)) || (rc = dev_alloc(ix.py, BN, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.pz, BN, ix.device_bytes)) || (rc = dev_alloc(ix.porig, BN, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.pinv, BN, ix.device_bytes)) || (rc = dev_alloc(ix.Dp, BN, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.vgeom, (size_t)B * ix.K_cap, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.vseg, (size_t)B * ix.K_cap, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.vstate, (size_t)B * ix.K_cap, ix.device_bytes)) ||
+        (rc = dev_alloc(ix.counters, 8, ix.device_bytes)))
+        return rc;
+
+    int *maxcnt = reinterpret_cast<int *>(ix.counters);   // borrowed as scratch during the build
+    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    k_tiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), ntl.as<int>(), tbase.as<int>(), N, ix.K_cap, ix.vseg);
+    k_gather<<<gN, 256, 0, st>>>(points, vin, N, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
+    k_sphere<<<dim3((ix.K_cap + 7) / 8, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, N, ix.K_cap, ix.vgeom,
+                                                          maxcnt);
+    RFPS_CUDA(cudaGetLastError());
+    RFPS_CUDA(cudaMemcpyAsync(&ix.max_voxel_points, maxcnt, sizeof(int), cudaMemcpyDeviceToHost, st));
+    RFPS_CUDA(cudaStreamSynchronize(st));
+    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    return choose_launch_shape(ix, o);
+}
+
+}  // namespace rfps

@@ -1,0 +1,78 @@
+// internal.h -- shared declarations of the radiusfps CUDA library (not installed; the public
+// interface is include/radiusfps.h).  Nothing here is used by, or taken from, oracle/.
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <cstdarg>
+#include <cstdio>
+
+#include "radiusfps.h"
+
+namespace rfps {
+
+// ---------------------------------------------------------------------------------------------
+// error plumbing: thread-local message + status
+// ---------------------------------------------------------------------------------------------
+void set_error(const char *fmt, ...);
+
+#define RFPS_CUDA(call)                                                                          \
+    do {                                                                                         \
+        cudaError_t e__ = (call);                                                                \
+        if (e__ != cudaSuccess) {                                                                \
+            ::rfps::set_error("%s:%d: %s failed: %s", __FILE__, __LINE__, #call,                 \
+                              cudaGetErrorString(e__));                                          \
+            return FPS_ERR_CUDA;                                                                 \
+        }                                                                                        \
+    } while (0)
+
+// ---------------------------------------------------------------------------------------------
+// per-voxel records (one "voxel" = one segment of the sorted SoA arrays with its own bounding
+// sphere; with tiling a grid voxel of Eq. 8 may be split into several of them)
+// ---------------------------------------------------------------------------------------------
+// VoxelGeom  (constant after build)   {cx, cy, cz, R}   R >= max_p ||p - c||  (rounded up, A9)
+// VoxelSeg   (constant after build)   {off, cnt}        segment [off, off+cnt) of the cloud's arrays
+// VoxelState (rewritten on every visit) {dv_bits, ~orig, pos, thr_bits}:
+//     dv_bits  fp32 bits of Dist_v[k] = max Dist_p in the voxel            (Eq. 30)
+//     ~orig    0xFFFFFFFF - (lowest original index attaining it)           (tie-break)
+//     pos      sorted position of that point
+//     thr_bits fp32 bits of the prune threshold: the voxel is pruned iff d2(s_j, c_k) >= thr
+//              (sqrt-free squared-domain form of Eq. 25 with fp32 safety margins)
+
+struct DeviceIndex {
+    int32_t B = 0, N = 0;
+    int32_t n_vox = 0, tile_points = 0;
+    int32_t K_max = 0, K_cap = 0;       // largest per-cloud K; per-cloud stride of the voxel arrays
+    int64_t K_total = 0;
+    int32_t max_voxel_points = 0;
+    int32_t cluster_size = 0, block_threads = 0, vpt = 0;   // sampling-kernel launch shape
+    int32_t flags = 0;
+    // point arrays, [B][N], sorted by voxel
+    float *px = nullptr, *py = nullptr, *pz = nullptr;
+    int32_t *porig = nullptr;           // sorted position -> original index
+    int32_t *pinv = nullptr;            // original index  -> sorted position
+    float *Dp = nullptr;                // Dist_p
+    // voxel arrays, [B][K_cap]
+    float4 *vgeom = nullptr;
+    int2 *vseg = nullptr;
+    uint4 *vstate = nullptr;
+    int32_t *K_dev = nullptr;           // [B]
+    int32_t *K_host = nullptr;          // [B] (malloc)
+    unsigned long long *counters = nullptr;   // [8] device, FPS_FLAG_STATS
+    int64_t device_bytes = 0;
+    int64_t last_iterations = 0;
+    cudaStream_t last_stream = nullptr;
+};
+
+int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o);
+void free_index(DeviceIndex &ix);
+int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
+                  cudaStream_t stream);
+int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o);
+
+}  // namespace rfps
+
+struct fps_index {
+    rfps::DeviceIndex ix;
+};
