@@ -75,6 +75,8 @@ typedef struct {
     int32_t K_max;            /* largest per-cloud K                                                  */
     int32_t max_voxel_points; /* largest segment                                                      */
     int64_t device_bytes;     /* memory owned by the handle                                           */
+    int32_t build_launches;   /* kernels fps_index_build launched (a1-a6); fps_sample launches ONE    */
+    int32_t reserved;
     /* the following are filled only when FPS_FLAG_STATS was set, for the LAST fps_sample call:      */
     int64_t iterations;       /* sum over clouds of (M-1)                                             */
     int64_t voxel_tests;      /* Eq. 25 evaluations                                                   */

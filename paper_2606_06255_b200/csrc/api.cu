@@ -97,6 +97,7 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
     out->cluster_size = ix.cluster_size; out->block_threads = ix.block_threads; out->voxels_per_thread = ix.vpt;
     out->K_total = ix.K_total; out->K_max = ix.K_max; out->max_voxel_points = ix.max_voxel_points;
     out->device_bytes = ix.device_bytes;
+    out->build_launches = ix.build_launches;
     if (ix.flags & FPS_FLAG_STATS) {
         unsigned long long c[8];
         RFPS_CUDA(cudaStreamSynchronize(ix.last_stream));

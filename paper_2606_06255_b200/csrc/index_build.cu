@@ -230,9 +230,12 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ i
 }
 
 // exclusive scan of B arrays of n ints (per-array stride `stride`); totals[b] (device, may be null)
+static int g_launches = 0;   // kernels launched by the build in progress (host-side bookkeeping only)
+
 static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
                           cudaStream_t st)
 {
+    g_launches += 3;
     const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
     k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp);
     k_scan_bsums<<<B, SCAN_T, 0, st>>>(bsum_tmp, nblk, totals);
@@ -504,11 +507,13 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     int rc;
     if ((rc = dev_alloc(ix.K_dev, B, ix.device_bytes)) != FPS_OK) return rc;
 
+    g_launches = 0;
     const dim3 gN((N + 255) / 256, B);
     k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(bbox.as<unsigned>(), B);
     k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, bbox.as<unsigned>());
     k_keys<<<gN, 256, 0, st>>>(points, N, bbox.as<unsigned>(), n_vox, sb, kA.as<unsigned>(), vA.as<int>());
     RFPS_CUDA(cudaGetLastError());
+    g_launches += 3;
 
     // a3: LSD radix sort, 8 bits per pass
     unsigned *kin = kA.as<unsigned>(), *kout = kB.as<unsigned>();
@@ -521,6 +526,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, N, nchunk, shift, table.as<int>(), kout, vout);
         std::swap(kin, kout);
         std::swap(vin, vout);
+        g_launches += 2;
     }
     RFPS_CUDA(cudaGetLastError());
 
@@ -531,6 +537,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     k_ntiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), N, tile_points, ntl.as<int>());
     if ((rc = scan_exclusive(ntl.as<int>(), tbase.as<int>(), N, N, B, ix.K_dev, bsum.as<int>(), st))) return rc;
     RFPS_CUDA(cudaGetLastError());
+    g_launches += 3 + 3;   // heads, voxel_offsets, ntiles + tiles, gather, sphere below
 
     // the one host round-trip of the build: K per cloud + the non-finite flags
     ix.K_host = (int32_t *)malloc(sizeof(int32_t) * B);
@@ -571,6 +578,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     RFPS_CUDA(cudaMemcpyAsync(&ix.max_voxel_points, maxcnt, sizeof(int), cudaMemcpyDeviceToHost, st));
     RFPS_CUDA(cudaStreamSynchronize(st));
     RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    ix.build_launches = g_launches;
     return choose_launch_shape(ix, o);
 }
 

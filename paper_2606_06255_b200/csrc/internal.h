@@ -48,6 +48,7 @@ struct DeviceIndex {
     int32_t max_voxel_points = 0;
     int32_t cluster_size = 0, block_threads = 0, vpt = 0;   // sampling-kernel launch shape
     int32_t flags = 0;
+    int32_t build_launches = 0;         // kernels launched by fps_index_build (a1-a6)
     // point arrays, [B][N], sorted by voxel
     float *px = nullptr, *py = nullptr, *pz = nullptr;
     int32_t *porig = nullptr;           // sorted position -> original index

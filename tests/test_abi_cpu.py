@@ -1,0 +1,86 @@
+"""CPU-only checks of the boundary: the C-ABI library builds for sm_100a, loads, and exports every
+symbol include/radiusfps.h declares; the Python binding marshals and validates without a GPU."""
+import ctypes
+import os
+import re
+
+import pytest
+import torch
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    from paper_2606_06255_b200 import build
+    return ctypes.CDLL(build.build())
+
+
+def declared_functions():
+    text = open(os.path.join(ROOT, "include", "radiusfps.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(fps_[a-z_]+)\s*\(", text)))
+
+
+def test_header_declares_the_north_star_calls():
+    names = declared_functions()
+    for must in ("fps_index_build", "fps_sample", "fps_index_destroy", "fps_last_error"):
+        assert must in names
+
+
+def test_library_exports_every_declared_symbol(lib):
+    for name in declared_functions():
+        assert hasattr(lib, name), name
+
+
+def test_binding_lists_every_declared_symbol():
+    from paper_2606_06255_b200 import binding
+    assert sorted(binding.EXPORTS) == declared_functions()
+
+
+def test_struct_sizes_match_header(lib):
+    # fps_build_opts: 5 x int32 + pointer (8-aligned) = 32 bytes; fps_stats: see header
+    from paper_2606_06255_b200 import binding
+    assert ctypes.sizeof(binding.fps_build_opts) == 32
+    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8
+
+
+def test_version_and_error_strings(lib):
+    lib.fps_version.restype = ctypes.c_char_p
+    lib.fps_last_error.restype = ctypes.c_char_p
+    assert b"sm_100a" in lib.fps_version()
+    assert lib.fps_last_error() == b""
+
+
+def test_null_and_bad_arguments_fail_without_a_gpu(lib):
+    lib.fps_index_build.restype = ctypes.c_void_p
+    lib.fps_last_error.restype = ctypes.c_char_p
+    assert lib.fps_index_build(None, 10, 1) is None
+    assert b"NULL" in lib.fps_last_error()
+    assert lib.fps_last_status() == -1
+    buf = (ctypes.c_float * 3)()
+    assert lib.fps_index_build(buf, 0, 1) is None
+    assert lib.fps_sample(None, 1, 0, None, None, None) == -1
+    assert lib.fps_sample_host(buf, 1, 1, 2, 0, buf, buf, None) == -1      # M > N
+    lib.fps_index_destroy(None)                                             # allowed
+
+
+def test_binding_rejects_host_tensor_and_wrong_dtype():
+    from paper_2606_06255_b200 import binding
+    with pytest.raises(ValueError):
+        binding.fps_index_build(torch.zeros(8, 3))                 # not on a CUDA device
+    with pytest.raises(ValueError):
+        binding._check_points(torch.zeros(8, 3, dtype=torch.float64))
+    with pytest.raises(ValueError):
+        binding._check_points(torch.zeros(8, 4))
+    assert binding._check_points(torch.zeros(2, 8, 3)) == (2, 8)
+
+
+def test_product_path_does_not_import_oracle():
+    pkg = os.path.join(ROOT, "paper_2606_06255_b200")
+    for dirpath, _, files in os.walk(pkg):
+        for f in files:
+            if f.endswith((".py", ".cu", ".h")):
+                src = open(os.path.join(dirpath, f)).read()
+                assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
+                assert "oracle/" not in src or f == "inputs.py" or "Nothing here is used by" in src, f

@@ -1,0 +1,264 @@
+"""GPU parity: the CUDA path (through the C-ABI) against the CPU oracle, element by element.
+
+Bar (BASELINE.json north_star): indices with 0 mismatches, out_mindist with 0 ULP difference --
+both are compared as raw bits.  Small cases span several voxels/tiles, ragged tails and the
+degenerate inputs of the method; the five full-size configurations run in the launch configuration
+bench.py times (library defaults) and are compared with the live oracle (C1-C4) and with the
+stored oracle hashes of tests/golden/full_size.json (all five; written by
+tests/golden/make_golden.py from the oracle alone).
+"""
+import hashlib
+import json
+import os
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_2606_06255_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden", "full_size.json")
+
+
+@pytest.fixture(scope="module")
+def rf():
+    from paper_2606_06255_b200 import binding
+    binding.load()            # raises if the CUDA library is missing: no fallback
+    assert torch.cuda.is_available()
+    return binding
+
+
+def run_gpu(rf, P, M, start=0, **opts):
+    Pd = torch.from_numpy(np.ascontiguousarray(P)).cuda()
+    ix = rf.fps_index_build(Pd, **opts)
+    try:
+        idx, mind = rf.fps_sample(ix, M, start)
+        torch.cuda.synchronize()
+        st = rf.fps_get_stats(ix)
+    finally:
+        rf.fps_index_destroy(ix)
+    return idx.cpu().numpy(), mind.cpu().numpy(), st
+
+
+def assert_same(got_idx, got_mind, ref_idx, ref_mind):
+    got_idx = got_idx.reshape(ref_idx.shape)
+    got_mind = got_mind.reshape(ref_mind.shape)
+    bad = np.nonzero((got_idx != ref_idx).reshape(-1))[0]
+    assert bad.size == 0, f"{bad.size} index mismatches, first at flat position {bad[0]}"
+    badm = np.nonzero((got_mind.view(np.uint32) != ref_mind.view(np.uint32)).reshape(-1))[0]
+    assert badm.size == 0, f"{badm.size} min-distance bit mismatches, first at {badm[0]}"
+
+
+SMALL = {
+    "uniform4096": lambda: (inputs.uniform_cube(4096, 1234), 1024),
+    "room": lambda: (inputs.room(6000, 11), 1500),
+    "room_dense": lambda: (inputs.room(5000, 12, size=(20.0, 15.0, 3.0), n_boxes=60, dense_half=True), 1250),
+    "lidar": lambda: (inputs.lidar(6000, 13, n_azimuth=94), 1500),
+    "clustered": lambda: (inputs.clustered(5000, 14), 1250),
+    "lattice": lambda: (inputs.shuffled_lattice(16, 15), 1024),
+    "dups": lambda: (inputs.with_duplicates(3000, 16, 700), 1000),
+    "line": lambda: (inputs.integer_line(513), 513),
+    "ragged_tail": lambda: (inputs.uniform_cube(4099, 5), 1031),
+}
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_small_clouds_default_config(rf, name):
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, _ = run_gpu(rf, P, M)
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("cluster", [1, 2, 4, 8, 16])
+@pytest.mark.parametrize("name", ["room", "lattice", "lidar"])
+def test_every_cluster_size(rf, name, cluster):
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, cluster_size=cluster)
+    assert st["cluster_size"] == cluster
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("n_vox", [1, 2, 7, 16, 24, 64, 128])
+@pytest.mark.parametrize("name", ["room", "lattice", "clustered"])
+def test_result_independent_of_n_vox(rf, name, n_vox):
+    # PAPER.md:695 "largely insensitive" is about speed; the RESULT must be identical for every n_vox
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, n_vox=n_vox)
+    assert st["n_vox"] == n_vox
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("tile", [-1, 8, 32, 200])
+@pytest.mark.parametrize("name", ["lidar", "clustered", "dups"])
+def test_result_independent_of_tiling(rf, name, tile):
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, tile_points=tile, n_vox=8)
+    if tile > 0:
+        assert st["max_voxel_points"] <= tile
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("threads", [64, 128, 256, 1024])
+def test_block_sizes(rf, threads):
+    P, M = SMALL["room"]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, block_threads=threads, cluster_size=2)
+    assert st["block_threads"] == threads
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("flags", [1, 2, 3, 4, 7])
+def test_ablations_and_stats_are_bit_identical(rf, flags):
+    # Table 4 structure: prune off / skip off / both off must not change a bit
+    P, M = SMALL["room"]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, flags=flags)
+    assert_same(gi, gm, *ref)
+    if flags & rf.FPS_FLAG_STATS:
+        assert st["iterations"] == M - 1
+        assert st["voxel_tests"] == st["K_total"] * (M - 1)
+        if flags & rf.FPS_FLAG_NO_PRUNE:
+            assert st["voxels_visited"] == st["K_total"] * (M - 1)
+            assert st["points_visited"] == P.shape[0] * (M - 1)
+        if flags & rf.FPS_FLAG_NO_SKIP:
+            assert st["points_computed"] == st["points_visited"]
+
+
+def test_stats_match_cpu_pruned_variant_effective_updates(rf):
+    # the number of EFFECTIVE updates (Eq. 2) is a property of the data, not of the index
+    P, M = SMALL["room"]()
+    _, _, cpu = oracle.pruned_fps(P, M, 0, n_vox=16)
+    _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS)
+    assert st["effective"] == cpu["effective"]
+    assert st["points_visited"] < 0.2 * P.shape[0] * (M - 1)
+
+
+@pytest.mark.parametrize("N,M,start", [(1, 1, 0), (2, 2, 1), (3, 1, 2), (33, 33, 32), (64, 64, 7), (1000, 1000, 999)])
+def test_degenerate_sizes_and_starts(rf, N, M, start):
+    P = inputs.uniform_cube(N, 3)
+    ref = oracle.fps(P, M, start)
+    gi, gm, _ = run_gpu(rf, P, M, start)
+    assert_same(gi, gm, *ref)
+
+
+def test_identical_points(rf):
+    P = np.full((100, 3), 0.25, dtype=np.float32)
+    ref = oracle.fps(P, 10, 3)
+    gi, gm, _ = run_gpu(rf, P, 10, 3)
+    assert_same(gi, gm, *ref)
+    assert gi.reshape(-1).tolist() == [3] + [0] * 9
+
+
+def test_closed_form_line_and_corners(rf):
+    gi, gm, _ = run_gpu(rf, inputs.integer_line(9), 9)
+    assert gi.reshape(-1).tolist() == [0, 8, 4, 2, 6, 1, 3, 5, 7]
+    assert gm.reshape(-1).tolist() == [np.inf, 64, 16, 4, 4, 1, 1, 1, 1]
+    gi, gm, _ = run_gpu(rf, inputs.cube_corners(), 8)
+    assert gi.reshape(-1).tolist() == [0, 7, 1, 2, 3, 4, 5, 6]
+
+
+def test_large_coordinates_and_tiny_extent(rf):
+    base = inputs.uniform_cube(3000, 8)
+    for P in ((base * np.float32(1e6)).astype(np.float32), (base * np.float32(1e-6)).astype(np.float32),
+              (base + np.float32(1000.0)).astype(np.float32)):
+        ref = oracle.fps(P, 600, 0)
+        gi, gm, _ = run_gpu(rf, P, 600)
+        assert_same(gi, gm, *ref)
+
+
+def test_batch_of_clouds_and_repeat_calls(rf):
+    w = inputs.scaled("C2", 3000, 700, B=5)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    Pd = torch.from_numpy(P).cuda()
+    ix = rf.fps_index_build(Pd)
+    try:
+        for _ in range(2):                                   # a handle is reusable: state resets per call
+            idx, mind = rf.fps_sample(ix, w.M, 0)
+            torch.cuda.synchronize()
+            assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+        idx, mind = rf.fps_sample(ix, 100, 17)               # other M / start on the same handle
+        torch.cuda.synchronize()
+        assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *oracle.fps(P, 100, 17))
+    finally:
+        rf.fps_index_destroy(ix)
+
+
+def test_host_entry_point(rf):
+    w = inputs.scaled("C4", 4000, 900, B=2)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    idx, mind = rf.fps_sample_host(torch.from_numpy(P), w.M, 0)
+    assert_same(idx.numpy(), mind.numpy(), *ref)
+
+
+def test_errors(rf):
+    P = torch.from_numpy(inputs.uniform_cube(100, 1)).cuda()
+    ix = rf.fps_index_build(P)
+    for M, start in [(0, 0), (101, 0), (10, -1), (10, 100)]:
+        with pytest.raises(rf.FpsError) as e:
+            rf.fps_sample(ix, M, start)
+        assert e.value.status == rf.FPS_ERR_INVALID
+    rf.fps_index_destroy(ix)
+    bad = P.clone()
+    bad[5, 1] = float("nan")
+    with pytest.raises(rf.FpsError) as e:
+        rf.fps_index_build(bad)
+    assert e.value.status == rf.FPS_ERR_NONFINITE
+    with pytest.raises(rf.FpsError):
+        rf.fps_index_build(P, cluster_size=3)
+
+
+# ---------------------------------------------------------------------------------------------
+# full-size configurations, library-default launch configuration (= what bench.py times)
+# ---------------------------------------------------------------------------------------------
+def sha(a):
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
+def test_full_size_against_live_oracle(rf, name):
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, w.start_idx)
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx)
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
+def test_full_size_against_stored_oracle_hashes(rf, name):
+    gold = json.load(open(GOLDEN))[name]
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    assert sha(P) == gold["input_sha256"], "input generator drifted from the one the golden was made with"
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx)
+    assert gi.reshape(w.B, w.M)[0, :8].tolist() == gold["idx_head"]
+    assert sha(gi.astype(np.int32)) == gold["idx_sha256"]
+    assert sha(gm.astype(np.float32)) == gold["mindist_sha256"]
+
+
+def test_C5_properties_and_sampled_recomputation(rf):
+    """N = 10^6: properties that hold at any size + min-distances recomputed for sampled outputs."""
+    w = inputs.WORKLOADS["C5"]
+    P = inputs.make_batch(w)
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx)
+    gi, gm, P = gi.reshape(-1), gm.reshape(-1), P[0]
+    assert gi[0] == w.start_idx and np.isinf(gm[0])
+    assert np.all(gm[1:] <= gm[:-1])
+    assert np.unique(gi).size == w.M
+    S = P[gi]
+    rng = np.random.default_rng(0)
+    for j in [1, 2, 3, w.M - 1] + rng.integers(4, w.M, size=60).tolist():
+        d = (S[:j] - S[j]).astype(np.float32)
+        d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
+        assert d2.min().view(np.uint32) == gm[j].view(np.uint32), j
+    # the second pick is one library argmax over all 10^6 points
+    d = (P - P[w.start_idx]).astype(np.float32)
+    d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
+    assert gi[1] == int(np.argmax(d2)) and gm[1].view(np.uint32) == d2.max().view(np.uint32)
