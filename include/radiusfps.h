@@ -58,15 +58,22 @@ typedef struct {
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
+    int32_t local_warps;   /* batched kernel: warps running the candidate-set FPS: 0 = choose; 1,2,4,8   */
+    int32_t cand_per_thread; /* batched kernel: candidates per thread (registers): 0 = choose; 4,8,16;
+                              candidate capacity = 32 * local_warps * cand_per_thread                   */
 } fps_build_opts;
 
 enum {
     FPS_FLAG_NO_PRUNE = 1,  /* ablation: visit every voxel (Eq. 25 never taken)                         */
     FPS_FLAG_NO_SKIP  = 2,  /* ablation: no coordinate-wise point skip (Eq. 28 never taken)             */
-    FPS_FLAG_STATS    = 4   /* count voxel tests / visited voxels / visited points / effective updates  */
+    FPS_FLAG_STATS    = 4,  /* count voxel tests / visited voxels / visited points / effective updates  */
+    FPS_FLAG_NO_BATCH = 8,  /* ablation: every batch of the batched kernel is the single global argmax  */
+    FPS_FLAG_PER_PICK = 16  /* run the per-pick persistent kernel (one cluster-wide exchange per sample,
+                               the paper's iteration structure) instead of exact batched picking        */
 };
 
-/* Counters and layout facts, summed over the B clouds (fps_get_stats).                             */
+/* Counters and layout facts, summed over the B clouds (fps_get_stats).  With the batched kernel
+ * voxel_tests / points_visited / points_computed count (voxel, pick) and (point, pick) pairs.      */
 typedef struct {
     int32_t B, N;
     int32_t n_vox;            /* resolution actually used                                             */
@@ -84,6 +91,14 @@ typedef struct {
     int64_t points_visited;   /* points in visited voxels                                             */
     int64_t points_computed;  /* points that passed the skip test                                     */
     int64_t effective;        /* strict decreases of Dist_p (Eq. 2)                     */
+    /* batched kernel only (zero for FPS_FLAG_PER_PICK):                                              */
+    int64_t rounds;           /* global rounds (apply + extract + local phase)                        */
+    int64_t extract_retries;  /* candidate extractions repeated because the buffer overflowed         */
+    int64_t single_picks;     /* rounds that fell back to the single global argmax                    */
+    int64_t candidates;       /* candidates handed to the local phase, summed over rounds             */
+    int64_t extract_voxels;   /* voxels scanned by the extraction                                     */
+    int64_t extract_points;   /* points scanned by the extraction                                     */
+    int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
 } fps_stats;
 
 /*

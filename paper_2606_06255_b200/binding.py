@@ -15,7 +15,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
 
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
-FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS = 1, 2, 4
+FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
 
 EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_sample", "fps_index_destroy", "fps_get_stats",
            "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
@@ -23,7 +23,8 @@ EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_sample", "fps_index_des
 
 class fps_build_opts(ctypes.Structure):
     _fields_ = [("n_vox", ctypes.c_int32), ("tile_points", ctypes.c_int32), ("cluster_size", ctypes.c_int32),
-                ("block_threads", ctypes.c_int32), ("flags", ctypes.c_int32), ("stream", ctypes.c_void_p)]
+                ("block_threads", ctypes.c_int32), ("flags", ctypes.c_int32), ("stream", ctypes.c_void_p),
+                ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
 
 
 class fps_stats(ctypes.Structure):
@@ -34,7 +35,10 @@ class fps_stats(ctypes.Structure):
                 ("device_bytes", ctypes.c_int64), ("build_launches", ctypes.c_int32), ("reserved", ctypes.c_int32),
                 ("iterations", ctypes.c_int64), ("voxel_tests", ctypes.c_int64),
                 ("voxels_visited", ctypes.c_int64), ("points_visited", ctypes.c_int64),
-                ("points_computed", ctypes.c_int64), ("effective", ctypes.c_int64)]
+                ("points_computed", ctypes.c_int64), ("effective", ctypes.c_int64),
+                ("rounds", ctypes.c_int64), ("extract_retries", ctypes.c_int64), ("single_picks", ctypes.c_int64),
+                ("candidates", ctypes.c_int64), ("extract_voxels", ctypes.c_int64), ("extract_points", ctypes.c_int64),
+                ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -100,8 +104,10 @@ def _check_points(points: torch.Tensor) -> tuple[int, int]:
     raise ValueError("points must be [N,3] or [B,N,3]")
 
 
-def _opts(n_vox=0, tile_points=0, cluster_size=0, block_threads=0, flags=0, stream=None) -> fps_build_opts:
-    return fps_build_opts(n_vox, tile_points, cluster_size, block_threads, flags, stream or 0)
+def _opts(n_vox=0, tile_points=0, cluster_size=0, block_threads=0, flags=0, stream=None, local_warps=0,
+          cand_per_thread=0) -> fps_build_opts:
+    return fps_build_opts(n_vox, tile_points, cluster_size, block_threads, flags, stream or 0, local_warps,
+                          cand_per_thread)
 
 
 class Index:
@@ -128,7 +134,8 @@ class Index:
 
 
 def fps_index_build(points: torch.Tensor, *, n_vox: int = 0, tile_points: int = 0, cluster_size: int = 0,
-                    block_threads: int = 0, flags: int = 0, stream: torch.cuda.Stream | None = None) -> Index:
+                    block_threads: int = 0, flags: int = 0, stream: torch.cuda.Stream | None = None,
+                    local_warps: int = 0, cand_per_thread: int = 0) -> Index:
     """fps_index_build / fps_index_build_ex.  The build is issued on ``stream`` (default: torch's
     current stream) and is complete when this returns."""
     lib = load()
@@ -137,7 +144,7 @@ def fps_index_build(points: torch.Tensor, *, n_vox: int = 0, tile_points: int = 
     B, N = _check_points(points)
     with torch.cuda.device(points.device):
         s = stream if stream is not None else torch.cuda.current_stream()
-        o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, s.cuda_stream)
+        o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, s.cuda_stream, local_warps, cand_per_thread)
         h = lib.fps_index_build_ex(points.data_ptr(), N, B, ctypes.byref(o))
     if not h:
         raise FpsError(lib.fps_last_status(), fps_last_error())
@@ -182,7 +189,8 @@ def fps_get_stats(index: Index) -> dict:
 
 
 def fps_sample_host(points_host: torch.Tensor, M: int, start_idx: int = 0, *, n_vox: int = 0, tile_points: int = 0,
-                    cluster_size: int = 0, block_threads: int = 0, flags: int = 0,
+                    cluster_size: int = 0, block_threads: int = 0, flags: int = 0, local_warps: int = 0,
+                    cand_per_thread: int = 0,
                     out_idx: torch.Tensor | None = None, out_mindist: torch.Tensor | None = None):
     """fps_sample_host: HOST float32 [B,N,3] in, HOST int32/float32 [B,M] out; copies, index build and
     sampling all happen inside the C call (synchronous)."""
@@ -194,7 +202,7 @@ def fps_sample_host(points_host: torch.Tensor, M: int, start_idx: int = 0, *, n_
         out_idx = torch.empty((B, M), dtype=torch.int32, pin_memory=torch.cuda.is_available())
     if out_mindist is None:
         out_mindist = torch.empty((B, M), dtype=torch.float32, pin_memory=torch.cuda.is_available())
-    o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, None)
+    o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, None, local_warps, cand_per_thread)
     rc = lib.fps_sample_host(points_host.data_ptr(), N, B, int(M), int(start_idx), out_idx.data_ptr(),
                              out_mindist.data_ptr(), ctypes.byref(o))
     if rc != FPS_OK:

@@ -14,7 +14,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libradiusfps.so")
-SOURCES = ["api.cu", "index_build.cu", "sample_kernel.cu"]
+SOURCES = ["api.cu", "index_build.cu", "sample_kernel.cu", "sample_batched.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",

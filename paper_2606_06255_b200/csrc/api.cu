@@ -77,7 +77,9 @@ int fps_sample(fps_index_t *h, int32_t M, int32_t start_idx, int32_t *out_idx, f
         set_error("start_idx=%d must be in [0, N=%d)", start_idx, h->ix.N);
         return FPS_ERR_INVALID;
     }
-    return rfps::launch_sample(h->ix, M, start_idx, out_idx, out_mindist, (cudaStream_t)stream);
+    if (h->ix.flags & FPS_FLAG_PER_PICK)
+        return rfps::launch_sample(h->ix, M, start_idx, out_idx, out_mindist, (cudaStream_t)stream);
+    return rfps::launch_sample_batched(h->ix, M, start_idx, out_idx, out_mindist, (cudaStream_t)stream);
 }
 
 void fps_index_destroy(fps_index_t *h)
@@ -98,8 +100,9 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
     out->K_total = ix.K_total; out->K_max = ix.K_max; out->max_voxel_points = ix.max_voxel_points;
     out->device_bytes = ix.device_bytes;
     out->build_launches = ix.build_launches;
+    out->local_warps = ix.local_warps; out->cand_per_thread = ix.cand_per_thread;
     if (ix.flags & FPS_FLAG_STATS) {
-        unsigned long long c[8];
+        unsigned long long c[rfps::NUM_COUNTERS];
         RFPS_CUDA(cudaStreamSynchronize(ix.last_stream));
         RFPS_CUDA(cudaMemcpy(c, ix.counters, sizeof c, cudaMemcpyDeviceToHost));
         out->iterations = ix.last_iterations;
@@ -108,6 +111,10 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
         out->points_visited = (int64_t)c[2];
         out->points_computed = (int64_t)c[3];
         out->effective = (int64_t)c[4];
+        if (!(ix.flags & FPS_FLAG_PER_PICK)) {
+            out->rounds = (int64_t)c[5]; out->extract_retries = (int64_t)c[6]; out->single_picks = (int64_t)c[7];
+            out->candidates = (int64_t)c[8]; out->extract_voxels = (int64_t)c[9]; out->extract_points = (int64_t)c[10];
+        }
     }
     return FPS_OK;
 }

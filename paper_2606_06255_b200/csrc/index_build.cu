@@ -565,11 +565,11 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         (rc = dev_alloc(ix.vgeom, (size_t)B * ix.K_cap, ix.device_bytes)) ||
         (rc = dev_alloc(ix.vseg, (size_t)B * ix.K_cap, ix.device_bytes)) ||
         (rc = dev_alloc(ix.vstate, (size_t)B * ix.K_cap, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.counters, 8, ix.device_bytes)))
+        (rc = dev_alloc(ix.counters, NUM_COUNTERS, ix.device_bytes)))
         return rc;
 
     int *maxcnt = reinterpret_cast<int *>(ix.counters);   // borrowed as scratch during the build
-    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
     k_tiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), ntl.as<int>(), tbase.as<int>(), N, ix.K_cap, ix.vseg);
     k_gather<<<gN, 256, 0, st>>>(points, vin, N, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
     k_sphere<<<dim3((ix.K_cap + 7) / 8, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, N, ix.K_cap, ix.vgeom,
@@ -577,9 +577,9 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     RFPS_CUDA(cudaGetLastError());
     RFPS_CUDA(cudaMemcpyAsync(&ix.max_voxel_points, maxcnt, sizeof(int), cudaMemcpyDeviceToHost, st));
     RFPS_CUDA(cudaStreamSynchronize(st));
-    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
     ix.build_launches = g_launches;
-    return choose_launch_shape(ix, o);
+    return (o.flags & FPS_FLAG_PER_PICK) ? choose_launch_shape(ix, o) : choose_batched_shape(ix, o);
 }
 
 }  // namespace rfps

@@ -40,6 +40,8 @@ void set_error(const char *fmt, ...);
 //     thr_bits fp32 bits of the prune threshold: the voxel is pruned iff d2(s_j, c_k) >= thr
 //              (sqrt-free squared-domain form of Eq. 25 with fp32 safety margins)
 
+constexpr int NUM_COUNTERS = 16;
+
 struct DeviceIndex {
     int32_t B = 0, N = 0;
     int32_t n_vox = 0, tile_points = 0;
@@ -47,6 +49,7 @@ struct DeviceIndex {
     int64_t K_total = 0;
     int32_t max_voxel_points = 0;
     int32_t cluster_size = 0, block_threads = 0, vpt = 0;   // sampling-kernel launch shape
+    int32_t local_warps = 0, cand_per_thread = 0, Kc_cap = 0;   // batched kernel: local-phase shape, voxels per CTA
     int32_t flags = 0;
     int32_t build_launches = 0;         // kernels launched by fps_index_build (a1-a6)
     // point arrays, [B][N], sorted by voxel
@@ -60,7 +63,7 @@ struct DeviceIndex {
     uint4 *vstate = nullptr;
     int32_t *K_dev = nullptr;           // [B]
     int32_t *K_host = nullptr;          // [B] (malloc)
-    unsigned long long *counters = nullptr;   // [8] device, FPS_FLAG_STATS
+    unsigned long long *counters = nullptr;   // [NUM_COUNTERS] device, FPS_FLAG_STATS
     int64_t device_bytes = 0;
     int64_t last_iterations = 0;
     cudaStream_t last_stream = nullptr;
@@ -71,6 +74,10 @@ void free_index(DeviceIndex &ix);
 int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
                   cudaStream_t stream);
 int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o);
+// exact batched picking (sample_batched.cu)
+int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
+                          cudaStream_t stream);
+int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o);
 
 }  // namespace rfps
 

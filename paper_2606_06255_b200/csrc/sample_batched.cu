@@ -1,0 +1,578 @@
+// sample_batched.cu -- steps a7-a13 with EXACT BATCHED PICKING: the same rules as the paper's
+// iteration (radius prune Eq. 25, point skip Eq. 28, fp32 min-distance update Eq. 29, per-voxel max
+// Eq. 30, lowest-index argmax Eq. 15-18), rescheduled so that the M-1
+// sequentially dependent picks no longer pay one cluster-wide exchange each.
+//
+// Why it is exact.  Let Dist_p be exact with respect to all picks so far and
+// tau < max Dist_p.  Put C = {p : Dist_p[p] > tau}.  Dist_p never increases, so every point outside
+// C stays <= tau for ever; hence, while the maximum over C is > tau, the argmax over C (same key:
+// distance, then lowest original index) IS the global argmax of Eq. 3 -- ties included, because all
+// points tied at the maximum are in C.  Plain FPS restricted to C therefore emits exactly the
+// oracle's picks until its maximum drops to <= tau.  The picks of such a batch are then applied to
+// the whole cloud at once: min is order-independent, so Dist_p ends bit-identical to applying them
+// one by one, and a voxel may be tested against a pick with a stale (larger) Dist_v because that
+// only makes the prune test of Eq. 25 more conservative.
+//
+// One round, one thread-block cluster per cloud (all CTAs unless noted):
+//   APPLY    the nb picks of the previous batch, 32 at a time: every thread tests the voxels it
+//            owns against the 32 picks (a9, squared-domain Eq. 25 with fp32 margins) and pushes
+//            (voxel, survivor mask) to a queue; warps walk the queued voxels' points (a10 skip,
+//            a11 update) and refresh the voxel key and threshold (a12).
+//   MAX      CTA argmax of the voxel keys, then cluster argmax over DSMEM (a8).
+//   EXTRACT  tau = Dmax * (1 - g): points with Dist_p > tau are appended to the candidate buffer in
+//            CTA 0's shared memory over DSMEM (atom.shared::cluster + st.shared::cluster).  If more
+//            than TC candidates turn up, tau is raised and the step repeated; if that fails the
+//            batch is the single global argmax (the paper's own per-pick iteration).
+//   LOCAL    (CTA 0, LW warps) register-resident FPS over the <= TC candidates: one named barrier
+//            per pick, no global memory in the loop; stops when the maximum is <= tau, after PB
+//            picks, or at M.  Picks go to out_idx / out_mindist and to the next round's batch.
+//
+// Arithmetic: d2 only via __fsub_rn/__fmul_rn/__fadd_rn (never FMA); the local phase uses
+// fminf(D, d2), which is value-identical to the strict '<' update for non-NaN operands.
+#include <cfloat>
+#include <cstring>
+
+#include "device_utils.cuh"
+#include "internal.h"
+
+namespace rfps {
+
+constexpr int BT = 512;        // threads per CTA
+constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
+constexpr int MAX_ATTEMPTS = 4;
+
+struct BatchParams {
+    const float *px, *py, *pz;
+    const int *porig, *pinv;
+    float *Dp;
+    const float4 *vgeom;
+    const int2 *vseg;
+    const int *K;
+    int N, K_cap, Kc_cap, M, start_idx;
+    int *out_idx;
+    float *out_mind;
+    unsigned long long *counters;
+};
+
+struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is the cluster's
+    unsigned ccount[MAX_ATTEMPTS];  // candidates found by extraction attempt a (may exceed TC)
+    unsigned best_hi, best_lo, best_pos, pad0;   // this CTA's best voxel key
+    int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
+};
+
+struct __align__(16) LSlot { unsigned hi, lo; float x, y, z; unsigned p0, p1, p2; };   // 32 B
+
+enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
+       CNT_XVOX, CNT_XPTS, CNT_N };
+
+// shared-memory carve-up (host and device must agree)
+struct SmemLayout {
+    size_t geom, vst, queue, bpick, cand, ctl, wbest, lslot, qn, total;
+};
+__host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
+{
+    SmemLayout L;
+    size_t o = 0;
+    L.geom = o;  o += sizeof(float4) * (size_t)Kc_cap;
+    L.vst = o;   o += sizeof(uint4) * (size_t)Kc_cap;
+    L.bpick = o; o += sizeof(float4) * PB;
+    L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
+    L.ctl = o;   o += sizeof(Ctl);
+    L.wbest = o; o += sizeof(uint4) * 32;
+    L.lslot = o; o += sizeof(LSlot) * 2 * 32;
+    L.queue = o; o += sizeof(int2) * (size_t)Kc_cap;
+    L.qn = o;    o += sizeof(int) * 4;
+    L.total = o;
+    return L;
+}
+
+// ---------------------------------------------------------------------------------------------
+// LOCAL: register-resident FPS over the candidate set (CTA 0, warps 0..LW-1).  Every thread keeps
+// CPT candidates {x, y, z, D, ~orig} in registers.  One pick = CPT d2 evaluations per thread, two
+// redux.sync per warp, one 32-byte slot per warp, one named barrier.  Slots are double-buffered by
+// pick parity, so a single barrier per pick is enough.
+// ---------------------------------------------------------------------------------------------
+template <int CPT, int LW>
+__device__ __forceinline__ void local_fps(const float *cX, const float *cY, const float *cZ, const float *cD,
+                                          const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
+                                          const int M, LSlot *lslot, float4 *bpick, int *out_idx, float *out_mind,
+                                          const int ltid)
+{
+    const int lane = ltid & 31, w = ltid >> 5;
+    float X[CPT], Y[CPT], Z[CPT], D[CPT];
+    unsigned O[CPT];
+#pragma unroll
+    for (int c = 0; c < CPT; ++c) {
+        const int i = c * (LW * 32) + ltid;
+        const bool ok = i < cnt;
+        X[c] = ok ? cX[i] : 0.0f;
+        Y[c] = ok ? cY[i] : 0.0f;
+        Z[c] = ok ? cZ[i] : 0.0f;
+        D[c] = ok ? cD[i] : 0.0f;      // padding: key (0, 0) is below every real key (real lo >= 2^31)
+        O[c] = ok ? cO[i] : 0u;
+    }
+    int par = 0;
+    nb = 0;
+    for (;;) {
+        float m = D[0];
+#pragma unroll
+        for (int c = 1; c < CPT; ++c) m = fmaxf(m, D[c]);
+        const unsigned hi = __float_as_uint(m);
+        const unsigned mhi = __reduce_max_sync(FULL, hi);
+        unsigned lo = 0u;
+        if (hi == mhi) {
+#pragma unroll
+            for (int c = 0; c < CPT; ++c)
+                if (D[c] == m) lo = max(lo, O[c]);
+        }
+        const unsigned mlo = __reduce_max_sync(FULL, lo);
+        if (hi == mhi && lo == mlo) {
+            float x = X[0], y = Y[0], z = Z[0];
+#pragma unroll
+            for (int c = 1; c < CPT; ++c)
+                if (D[c] == m && O[c] == lo) { x = X[c]; y = Y[c]; z = Z[c]; }
+            LSlot *s = &lslot[par * LW + w];
+            s->hi = mhi; s->lo = mlo; s->x = x; s->y = y; s->z = z;
+        }
+        if (LW > 1) named_bar_sync(1, LW * 32);
+        else __syncwarp();
+        unsigned shi = 0u, slo = 0u;
+        if (lane < LW) { shi = lslot[par * LW + lane].hi; slo = lslot[par * LW + lane].lo; }
+        unsigned ghi, glo;
+        const int win = warp_argmax_key(shi, slo, ghi, glo);
+        if (!(ghi > taubits)) break;        // restricted max <= tau: the candidate set no longer decides
+        const LSlot *ws = &lslot[par * LW + win];
+        const float sx = ws->x, sy = ws->y, sz = ws->z;
+        if (ltid == 0) {
+            out_idx[j] = (int)(~glo);
+            out_mind[j] = __uint_as_float(ghi);
+            bpick[nb] = make_float4(sx, sy, sz, 0.0f);
+        }
+        ++j;
+        ++nb;
+        if (j >= M || nb >= PB) break;
+#pragma unroll
+        for (int c = 0; c < CPT; ++c) D[c] = fminf(D[c], d2_rn(X[c], Y[c], Z[c], sx, sy, sz));
+        par ^= 1;
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// the kernel: one cluster per cloud; CTA `rank` owns the voxels k = rank + C*kl (round-robin, so
+// that dense regions of the cloud are spread over the CTAs)
+// ---------------------------------------------------------------------------------------------
+template <int CPT, int LW, bool STATS>
+__global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, const int flags)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    constexpr int TC = CPT * LW * 32;
+    constexpr int NW = BT / 32;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const unsigned lt = (1u << lane) - 1u;
+    const int C = (int)cluster_nctarank(), rank = (int)cluster_ctarank();
+    const int b = blockIdx.x / C;
+    const bool no_prune = flags & FPS_FLAG_NO_PRUNE, no_skip = flags & FPS_FLAG_NO_SKIP;
+    const bool no_batch = flags & FPS_FLAG_NO_BATCH;
+
+    const SmemLayout L = smem_layout(P.Kc_cap, TC, LW);
+    float4 *sgeom = reinterpret_cast<float4 *>(smem_raw + L.geom);    // [Kc] {cx, cy, cz, R}
+    uint4 *vst = reinterpret_cast<uint4 *>(smem_raw + L.vst);         // [Kc] {Dv bits, ~orig, pos, thr bits}
+    float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
+    float *cX = reinterpret_cast<float *>(smem_raw + L.cand), *cY = cX + TC, *cZ = cY + TC, *cD = cZ + TC;
+    unsigned *cO = reinterpret_cast<unsigned *>(cD + TC);
+    Ctl *ctl = reinterpret_cast<Ctl *>(smem_raw + L.ctl);
+    uint4 *wbest = reinterpret_cast<uint4 *>(smem_raw + L.wbest);
+    LSlot *lslot = reinterpret_cast<LSlot *>(smem_raw + L.lslot);
+    int2 *queue = reinterpret_cast<int2 *>(smem_raw + L.queue);
+    int *qn = reinterpret_cast<int *>(smem_raw + L.qn);
+
+    const size_t po = (size_t)b * P.N, vo = (size_t)b * P.K_cap;
+    const float *__restrict__ px = P.px + po;
+    const float *__restrict__ py = P.py + po;
+    const float *__restrict__ pz = P.pz + po;
+    const int *__restrict__ porig = P.porig + po;
+    float *Dp = P.Dp + po;
+    const float4 *__restrict__ vgeom = P.vgeom + vo;
+    const int2 *__restrict__ vseg = P.vseg + vo;
+    int *out_idx = P.out_idx + (size_t)b * P.M;
+    float *out_mind = P.out_mind + (size_t)b * P.M;
+    const int K = P.K[b];
+    const int Kc = K > rank ? (K - rank + C - 1) / C : 0;     // voxels owned by this CTA
+
+    // ---- a7: state reset.  Thresholds = NaN: nothing can be pruned by the first pick, which therefore
+    // performs the paper's "initial update" (Eq. 13-14).  Dist_p = +inf on this CTA's slice. ----
+    for (int kl = tid; kl < Kc; kl += BT) {
+        sgeom[kl] = vgeom[rank + C * kl];
+        vst[kl] = make_uint4(0u, 0u, 0u, F32_NAN_BITS);
+    }
+    {
+        const int chunk = (P.N + C - 1) / C;
+        const int p0 = min(P.N, rank * chunk), p1 = min(P.N, p0 + chunk);
+        const float inf = __uint_as_float(F32_INF_BITS);
+        for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
+    }
+    if (tid == 0) {
+        qn[0] = qn[1] = 0;
+#pragma unroll
+        for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
+        ctl->best_hi = ctl->best_lo = ctl->best_pos = 0u;
+        ctl->nb = 1;
+        ctl->j = 1;
+        const int p = P.pinv[po + P.start_idx];
+        bpick[0] = make_float4(px[p], py[p], pz[p], 0.0f);     // s_0 = the caller's start point
+        if (rank == 0) {
+            out_idx[0] = P.start_idx;
+            out_mind[0] = __uint_as_float(F32_INF_BITS);
+        }
+    }
+    int nb = 1, j = 1;
+    unsigned qpar = 0u;
+    float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
+    unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
+                       c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0;
+    cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
+
+    while (j < P.M) {
+        if (STATS && tid == 0 && rank == 0) c_rounds++;
+        // =====================================================================================
+        // APPLY: the nb picks in bpick[], 32 at a time
+        // =====================================================================================
+        for (int sub = 0; sub < nb; sub += 32) {
+            const int nsub = min(32, nb - sub);
+            // ---- a9: radius prune (Eq. 25) of the voxels this thread owns against the 32 picks ----
+            for (int base = 0; base < Kc; base += BT) {
+                const int kl = base + tid;
+                unsigned mask = 0u;
+                if (kl < Kc) {
+                    if (no_prune) mask = nsub == 32 ? FULL : ((1u << nsub) - 1u);
+                    else {
+                        const float4 gm = sgeom[kl];
+                        const float thr = __uint_as_float(vst[kl].w);
+                        for (int i = 0; i < nsub; ++i) {
+                            const float4 s = bpick[sub + i];
+                            const float d2c = d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z);
+                            if (!(d2c >= thr)) mask |= 1u << i;
+                        }
+                    }
+                    if (STATS) c_vtest += nsub;
+                }
+                const unsigned bal = __ballot_sync(FULL, mask != 0u);
+                if (bal) {
+                    int qb = 0;
+                    if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
+                    qb = __shfl_sync(FULL, qb, 0);
+                    if (mask) queue[qb + __popc(bal & lt)] = make_int2(kl, (int)mask);
+                }
+            }
+            __syncthreads();
+            const int nq = qn[qpar];
+            if (tid == 0) qn[qpar ^ 1u] = 0;
+            // ---- a10-a12: one warp per surviving voxel: point skip, update, voxel key + threshold ----
+            for (int qi = warp; qi < nq; qi += NW) {
+                const int2 e = queue[qi];
+                const int kl = e.x;
+                const unsigned mask = (unsigned)e.y;
+                const int2 sg = vseg[rank + C * kl];
+                const float R = sgeom[kl].w;
+                float bestD = -1.0f;
+                unsigned bestO = 0u;
+                int bestP = 0;
+                for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) {
+                    const float x = px[p], y = py[p], z = pz[p];
+                    const unsigned o = ~(unsigned)porig[p];
+                    const float D0 = Dp[p];
+                    float D = D0;
+                    unsigned m = mask;
+                    while (m) {
+                        const int i = __ffs(m) - 1;
+                        m &= m - 1u;
+                        const float4 s = bpick[sub + i];
+                        const float dx = __fsub_rn(x, s.x), dy = __fsub_rn(y, s.y), dz = __fsub_rn(z, s.z);
+                        const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                        if (no_skip || !(dx2 >= D || dy2 >= D || dz2 >= D)) {     // Eq. 28, squared domain
+                            const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                            if (STATS) c_pcomp++;
+                            if (d < D) {                                          // Eq. 29 / Eq. 2 (strict)
+                                D = d;
+                                if (STATS) c_eff++;
+                            }
+                        }
+                    }
+                    if (D < D0) Dp[p] = D;
+                    if (STATS) c_pvisit += __popc(mask);
+                    if (D > bestD || (D == bestD && o > bestO)) { bestD = D; bestO = o; bestP = p; }
+                }
+                const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
+                unsigned mhi, mlo;
+                const int win = warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
+                const int wpos = __shfl_sync(FULL, bestP, win);
+                if (lane == 0) {
+                    vst[kl] = make_uint4(mhi, mlo, (unsigned)wpos, __float_as_uint(prune_threshold(mhi, R)));
+                    if (STATS) c_vvisit++;
+                }
+            }
+            __syncthreads();
+            qpar ^= 1u;
+        }
+
+        // =====================================================================================
+        // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
+        // =====================================================================================
+        {
+            unsigned bhi = 0u, blo = 0u, bpos = 0u;
+            for (int kl = tid; kl < Kc; kl += BT) {
+                const uint4 s = vst[kl];
+                if (s.x > bhi || (s.x == bhi && s.y > blo)) { bhi = s.x; blo = s.y; bpos = s.z; }
+            }
+            unsigned mhi, mlo;
+            const int win = warp_argmax_key(bhi, blo, mhi, mlo);
+            const unsigned wpos = __shfl_sync(FULL, bpos, win);
+            if (lane == 0) wbest[warp] = make_uint4(mhi, mlo, wpos, 0u);
+        }
+        __syncthreads();
+        if (warp == 0) {
+            const uint4 wb = lane < NW ? wbest[lane] : make_uint4(0u, 0u, 0u, 0u);
+            unsigned chi, clo;
+            const int win = warp_argmax_key(wb.x, wb.y, chi, clo);
+            const unsigned cpos = __shfl_sync(FULL, wb.z, win);
+            if (lane == 0) {
+                ctl->best_hi = chi; ctl->best_lo = clo; ctl->best_pos = cpos;
+                if (rank == 0) {
+#pragma unroll
+                    for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
+                }
+            }
+        }
+        cluster_sync_all();
+        unsigned ghi, glo, gpos;
+        {
+            uint4 rb = make_uint4(0u, 0u, 0u, 0u);
+            if (lane < C) rb = ld_dsmem_v4(mapa(smem_u32(&ctl->best_hi), (unsigned)lane));
+            const int win = warp_argmax_key(rb.x, rb.y, ghi, glo);
+            gpos = __shfl_sync(FULL, rb.z, win);
+        }
+
+        // =====================================================================================
+        // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
+        // =====================================================================================
+        int cnt = 0;
+        unsigned taubits = ghi;
+        if (!no_batch && ghi > 0u && ghi < F32_INF_BITS) {
+            const float Dmax = __uint_as_float(ghi);
+            const unsigned cX0 = mapa(smem_u32(cX), 0u), cY0 = mapa(smem_u32(cY), 0u), cZ0 = mapa(smem_u32(cZ), 0u),
+                           cD0 = mapa(smem_u32(cD), 0u), cO0 = mapa(smem_u32(cO), 0u);
+            for (int a = 0; a < MAX_ATTEMPTS; ++a) {
+                const unsigned tb = __float_as_uint(__fmul_rn(Dmax, __fsub_rn(1.0f, g)));
+                if (!(tb < ghi)) break;                      // g too small to separate tau from Dmax
+                const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[a]), 0u);
+                for (int base = 0; base < Kc; base += BT) {
+                    const int kl = base + tid;
+                    const bool hit = kl < Kc && vst[kl].x > tb;
+                    const unsigned bal = __ballot_sync(FULL, hit);
+                    if (bal) {
+                        int qb = 0;
+                        if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
+                        qb = __shfl_sync(FULL, qb, 0);
+                        if (hit) queue[qb + __popc(bal & lt)] = make_int2(kl, 0);
+                    }
+                }
+                __syncthreads();
+                const int nq = qn[qpar];
+                if (tid == 0) qn[qpar ^ 1u] = 0;
+                for (int qi = warp; qi < nq; qi += NW) {
+                    const int2 sg = vseg[rank + C * queue[qi].x];
+                    if (STATS && lane == 0) c_xvox++;
+                    for (int p0 = sg.x; p0 < sg.x + sg.y; p0 += 32) {
+                        const int p = p0 + lane;
+                        const bool in = p < sg.x + sg.y;
+                        const unsigned db = in ? __float_as_uint(Dp[p]) : 0u;
+                        const bool is = db > tb;
+                        const unsigned bal = __ballot_sync(FULL, is);
+                        if (STATS && in) c_xpts++;
+                        if (bal) {
+                            unsigned cb = 0u;
+                            if (lane == 0) cb = atom_add_dsmem_u32(cnt_addr, (unsigned)__popc(bal));
+                            cb = __shfl_sync(FULL, cb, 0);
+                            const unsigned slot = cb + (unsigned)__popc(bal & lt);
+                            if (is && slot < (unsigned)TC) {
+                                st_dsmem_u32(cX0 + 4u * slot, __float_as_uint(px[p]));
+                                st_dsmem_u32(cY0 + 4u * slot, __float_as_uint(py[p]));
+                                st_dsmem_u32(cZ0 + 4u * slot, __float_as_uint(pz[p]));
+                                st_dsmem_u32(cD0 + 4u * slot, db);
+                                st_dsmem_u32(cO0 + 4u * slot, ~(unsigned)porig[p]);
+                            }
+                        }
+                    }
+                }
+                qpar ^= 1u;
+                cluster_sync_all();
+                const unsigned found = ld_dsmem_u32(cnt_addr);
+                if (found <= (unsigned)TC) {
+                    cnt = (int)found;
+                    taubits = tb;
+                    // aim the next round at ~5/8 of the buffer; move by at most 2x per round
+                    const float ratio = fminf(2.0f, fmaxf(0.5f, (0.625f * TC) / (float)max(found, 1u)));
+                    g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
+                    break;
+                }
+                if (STATS && tid == 0 && rank == 0) c_retries++;
+                g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
+            }
+        }
+
+        // =====================================================================================
+        // LOCAL (CTA 0): FPS restricted to the candidates; or the single global argmax
+        // =====================================================================================
+        if (rank == 0) {
+            if (cnt == 0) {
+                if (tid == 0) {
+                    out_idx[j] = (int)(~glo);
+                    out_mind[j] = __uint_as_float(ghi);
+                    bpick[0] = make_float4(px[gpos], py[gpos], pz[gpos], 0.0f);
+                    ctl->nb = 1;
+                    ctl->j = j + 1;
+                    if (STATS) c_singles++;
+                }
+            } else if (warp < LW) {
+                int lj = j, lnb = 0;
+                local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, lslot, bpick, out_idx, out_mind, tid);
+                if (tid == 0) {
+                    ctl->nb = lnb;
+                    ctl->j = lj;
+                    if (STATS) c_cands += (unsigned long long)cnt;
+                }
+            }
+        }
+        cluster_sync_all();
+        {
+            const uint4 r0 = ld_dsmem_v4(mapa(smem_u32(&ctl->nb), 0u));
+            nb = (int)r0.x;
+            j = (int)r0.y;
+        }
+        if (rank != 0 && j < P.M) {
+            const unsigned src = mapa(smem_u32(bpick), 0u);
+            for (int i = tid; i < nb; i += BT) {
+                const uint4 v = ld_dsmem_v4(src + 16u * (unsigned)i);
+                bpick[i] = make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), 0.0f);
+            }
+            __syncthreads();
+        }
+    }
+
+    if (STATS) {
+        atomicAdd(P.counters + CNT_VTEST, c_vtest);
+        atomicAdd(P.counters + CNT_VVISIT, c_vvisit);
+        atomicAdd(P.counters + CNT_PVISIT, c_pvisit);
+        atomicAdd(P.counters + CNT_PCOMP, c_pcomp);
+        atomicAdd(P.counters + CNT_EFF, c_eff);
+        atomicAdd(P.counters + CNT_XVOX, c_xvox);
+        atomicAdd(P.counters + CNT_XPTS, c_xpts);
+        if (tid == 0 && rank == 0) {
+            atomicAdd(P.counters + CNT_ROUNDS, c_rounds);
+            atomicAdd(P.counters + CNT_RETRIES, c_retries);
+            atomicAdd(P.counters + CNT_SINGLES, c_singles);
+            atomicAdd(P.counters + CNT_CANDS, c_cands);
+        }
+    }
+    cluster_sync_all();   // no CTA may exit while a peer can still read its shared memory
+}
+
+// ---------------------------------------------------------------------------------------------
+// host side: launch shape and launch
+// ---------------------------------------------------------------------------------------------
+static const int kMaxSmem = 227 * 1024;
+
+int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
+{
+    int LW = o.local_warps > 0 ? o.local_warps : 4;
+    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : 8;
+    if (!((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16))) {
+        set_error("local_warps=%d must be 1,2,4,8 and cand_per_thread=%d must be 4,8,16", LW, CPT);
+        return FPS_ERR_INVALID;
+    }
+    int C = o.cluster_size;
+    if (C != 0 && C != 1 && C != 2 && C != 4 && C != 8 && C != 16) { set_error("cluster_size=%d must be 0,1,2,4,8 or 16", C); return FPS_ERR_INVALID; }
+    if (o.block_threads != 0 && o.block_threads != BT) { set_error("block_threads=%d: the batched kernel runs %d threads per CTA", o.block_threads, BT); return FPS_ERR_INVALID; }
+    const int K = ix.K_max > 0 ? ix.K_max : 1;
+    const int TC = CPT * LW * 32;
+    auto fits = [&](int c) { return smem_layout((K + c - 1) / c, TC, LW).total <= (size_t)kMaxSmem; };
+    if (C == 0) {
+        C = 1;
+        while (C < 16 && (long long)C * 2 * ix.B <= 148 && (long long)ix.N > (long long)C * 2048) C *= 2;
+        while (C < 16 && !fits(C)) C *= 2;
+    }
+    if (!fits(C)) {
+        set_error("K_max=%d voxels do not fit the shared memory of %d CTAs; use a smaller n_vox or a larger tile_points", K, C);
+        return FPS_ERR_INVALID;
+    }
+    ix.cluster_size = C;
+    ix.block_threads = BT;
+    ix.vpt = 0;
+    ix.local_warps = LW;
+    ix.cand_per_thread = CPT;
+    ix.Kc_cap = (K + C - 1) / C;
+    return FPS_OK;
+}
+
+template <int CPT, int LW, bool STATS>
+static int launch_batched_one(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
+{
+    auto kern = k_fps_batched<CPT, LW, STATS>;
+    const size_t smem = smem_layout(ix.Kc_cap, CPT * LW * 32, LW).total;
+    RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    if (ix.cluster_size > 8) RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)(ix.B * ix.cluster_size));
+    cfg.blockDim = dim3(BT);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)ix.cluster_size;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    RFPS_CUDA(cudaLaunchKernelEx(&cfg, kern, bp, ix.flags));
+    return FPS_OK;
+}
+
+template <int CPT, int LW>
+static int launch_batched_s(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
+{
+    return (ix.flags & FPS_FLAG_STATS) ? launch_batched_one<CPT, LW, true>(bp, ix, st)
+                                       : launch_batched_one<CPT, LW, false>(bp, ix, st);
+}
+
+int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
+                          cudaStream_t st)
+{
+    BatchParams bp;
+    bp.px = ix.px; bp.py = ix.py; bp.pz = ix.pz;
+    bp.porig = ix.porig; bp.pinv = ix.pinv;
+    bp.Dp = ix.Dp;
+    bp.vgeom = ix.vgeom; bp.vseg = ix.vseg;
+    bp.K = ix.K_dev;
+    bp.N = ix.N; bp.K_cap = ix.K_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
+    bp.out_idx = out_idx; bp.out_mind = out_mindist;
+    bp.counters = ix.counters;
+    if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
+    ix.last_iterations = (int64_t)ix.B * (M - 1);
+    ix.last_stream = st;
+    const int key = ix.cand_per_thread * 100 + ix.local_warps;
+    switch (key) {
+        case 804: return launch_batched_s<8, 4>(bp, ix, st);
+        case 801: return launch_batched_s<8, 1>(bp, ix, st);
+        case 802: return launch_batched_s<8, 2>(bp, ix, st);
+        case 808: return launch_batched_s<8, 8>(bp, ix, st);
+        case 404: return launch_batched_s<4, 4>(bp, ix, st);
+        case 408: return launch_batched_s<4, 8>(bp, ix, st);
+        case 1604: return launch_batched_s<16, 4>(bp, ix, st);
+        case 1608: return launch_batched_s<16, 8>(bp, ix, st);
+    }
+    set_error("unsupported local shape cand_per_thread=%d local_warps=%d", ix.cand_per_thread, ix.local_warps);
+    return FPS_ERR_INVALID;
+}
+
+}  // namespace rfps

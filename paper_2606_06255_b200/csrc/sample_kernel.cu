@@ -36,12 +36,12 @@
 #include <cfloat>
 #include <cstring>
 
+#include "device_utils.cuh"
 #include "internal.h"
 
 namespace rfps {
 
 constexpr int MAX_CLUSTER = 16;
-constexpr unsigned FULL = 0xffffffffu;
 
 struct SampleParams {
     const float *px, *py, *pz;
@@ -62,77 +62,6 @@ struct __align__(16) XMsg {   // one candidate: 32 bytes = two st.async.v4.b32
     float x, y, z;             // coordinates of the candidate point
     unsigned pad0, pad1, pad2;
 };
-
-// --------------------------------------------------------------------------------------------
-// PTX wrappers (sm_90+ cluster / mbarrier / async-store instructions)
-// --------------------------------------------------------------------------------------------
-__device__ __forceinline__ unsigned smem_u32(const void *p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ unsigned cluster_ctarank()
-{
-    unsigned r;
-    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ unsigned cluster_nctarank()
-{
-    unsigned r;
-    asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
-    return r;
-}
-__device__ __forceinline__ void cluster_sync_all()
-{
-    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-__device__ __forceinline__ unsigned mapa(unsigned local_addr, unsigned rank)
-{
-    unsigned r;
-    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(local_addr), "r"(rank));
-    return r;
-}
-__device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity)
-{
-    asm volatile(
-        "{\n\t.reg .pred p;\n\t"
-        "WAIT_LOOP:\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
-        "@p bra WAIT_DONE;\n\t"
-        "bra WAIT_LOOP;\n\t"
-        "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
-}
-__device__ __forceinline__ void st_async_v4(unsigned remote_addr, unsigned a, unsigned b, unsigned c, unsigned d,
-                                            unsigned remote_bar)
-{
-    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];" ::"r"(
-                     remote_addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(remote_bar) : "memory");
-}
-
-// max of a (hi, lo) key over the warp; returns the winning lane (lowest lane on a full tie)
-__device__ __forceinline__ int warp_argmax_key(unsigned hi, unsigned lo, unsigned &mhi, unsigned &mlo)
-{
-    mhi = __reduce_max_sync(FULL, hi);
-    mlo = __reduce_max_sync(FULL, hi == mhi ? lo : 0u);
-    unsigned win = __ballot_sync(FULL, hi == mhi && lo == mlo);
-    return __ffs(win) - 1;
-}
-
-// prune threshold of a voxel from its Dist_v and radius: the voxel is pruned iff d2(s,c) >= thr.
-// thr >= (sqrt(Dv)*(1+3u) + R)^2 * (1+6u) over the reals (u = 2^-24), see DESIGN.md "Prune test".
-__device__ __forceinline__ float prune_threshold(unsigned dv_bits, float R)
-{
-    if (dv_bits == 0u) return 0.0f;   // Dist_v == +0: the strict '<' of Eq. 2 can never fire
-    const float q = __fadd_rn(__fmul_rn(__fsqrt_rn(__uint_as_float(dv_bits)), 1.0f + 0x1p-20f), 0x1p-40f);
-    const float a = __fadd_rn(q, R);
-    const float t = __fmul_rn(__fmul_rn(a, a), 1.0f + 0x1p-18f);
-    return (t < __uint_as_float(0x7f800000u)) ? t : __uint_as_float(0x7fc00000u);   // inf -> NaN: never prune
-}
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF };
 
@@ -444,7 +373,7 @@ int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_id
     sp.N = ix.N; sp.K_cap = ix.K_cap; sp.M = M; sp.start_idx = start_idx;
     sp.out_idx = out_idx; sp.out_mind = out_mindist;
     sp.counters = ix.counters;
-    if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, 8 * sizeof(unsigned long long), st));
+    if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
     ix.last_iterations = (int64_t)ix.B * (M - 1);
     ix.last_stream = st;
     const bool big = ix.block_threads > 512;
