@@ -98,6 +98,8 @@ typedef struct {
     int64_t candidates;       /* candidates handed to the local phase, summed over rounds             */
     int64_t extract_voxels;   /* voxels scanned by the extraction                                     */
     int64_t extract_points;   /* points scanned by the extraction                                     */
+    int64_t cycles_apply, cycles_max, cycles_extract, cycles_local;   /* SM cycles spent per phase, as seen
+                                 by thread 0 of each cloud's first CTA, summed over clouds             */
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
 } fps_stats;
 

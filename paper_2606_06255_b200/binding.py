@@ -38,6 +38,8 @@ class fps_stats(ctypes.Structure):
                 ("points_computed", ctypes.c_int64), ("effective", ctypes.c_int64),
                 ("rounds", ctypes.c_int64), ("extract_retries", ctypes.c_int64), ("single_picks", ctypes.c_int64),
                 ("candidates", ctypes.c_int64), ("extract_voxels", ctypes.c_int64), ("extract_points", ctypes.c_int64),
+                ("cycles_apply", ctypes.c_int64), ("cycles_max", ctypes.c_int64), ("cycles_extract", ctypes.c_int64),
+                ("cycles_local", ctypes.c_int64),
                 ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
 
     def as_dict(self) -> dict:

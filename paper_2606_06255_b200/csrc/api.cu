@@ -114,6 +114,8 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
         if (!(ix.flags & FPS_FLAG_PER_PICK)) {
             out->rounds = (int64_t)c[5]; out->extract_retries = (int64_t)c[6]; out->single_picks = (int64_t)c[7];
             out->candidates = (int64_t)c[8]; out->extract_voxels = (int64_t)c[9]; out->extract_points = (int64_t)c[10];
+            out->cycles_apply = (int64_t)c[11]; out->cycles_max = (int64_t)c[12];
+            out->cycles_extract = (int64_t)c[13]; out->cycles_local = (int64_t)c[14];
         }
     }
     return FPS_OK;

@@ -30,6 +30,7 @@
 // Arithmetic: d2 only via __fsub_rn/__fmul_rn/__fadd_rn (never FMA); the local phase uses
 // fminf(D, d2), which is value-identical to the strict '<' update for non-NaN operands.
 #include <cfloat>
+#include <algorithm>
 #include <cstring>
 
 #include "device_utils.cuh"
@@ -60,10 +61,9 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
     int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
 };
 
-struct __align__(16) LSlot { unsigned hi, lo; float x, y, z; unsigned p0, p1, p2; };   // 32 B
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_N };
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
@@ -79,7 +79,7 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
     L.ctl = o;   o += sizeof(Ctl);
     L.wbest = o; o += sizeof(uint4) * 32;
-    L.lslot = o; o += sizeof(LSlot) * 2 * 32;
+    L.lslot = o; o += sizeof(uint2) * 2 * 8;
     L.queue = o; o += sizeof(int2) * (size_t)Kc_cap;
     L.qn = o;    o += sizeof(int) * 4;
     L.total = o;
@@ -87,72 +87,139 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 }
 
 // ---------------------------------------------------------------------------------------------
-// LOCAL: register-resident FPS over the candidate set (CTA 0, warps 0..LW-1).  Every thread keeps
-// CPT candidates {x, y, z, D, ~orig} in registers.  One pick = CPT d2 evaluations per thread, two
-// redux.sync per warp, one 32-byte slot per warp, one named barrier.  Slots are double-buffered by
-// pick parity, so a single barrier per pick is enough.
+// packed fp32x2 arithmetic (sm_100: FADD2 / FMUL2).  Each half is an ordinary IEEE round-to-nearest
+// fp32 operation, so the results are bit-identical to the scalar __f*_rn intrinsics.
+// ---------------------------------------------------------------------------------------------
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float a, float b)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(a), "f"(b));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float &a, float &b) { asm("mov.b64 {%0, %1}, %2;" : "=f"(a), "=f"(b) : "l"(v)); }
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 r;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+// NOTE: there is deliberately no add2(): ptxas (12.9) contracts mul.rn.f32x2 + add.rn.f32x2 into FFMA2
+// even under --fmad=false, which changes the rounding.  The two additions of d2 are therefore done
+// with scalar __fadd_rn on the unpacked halves (scalar .rn adds are never contracted), and
+// tests/test_abi_cpu.py checks that the built library holds no FFMA2 at all.
+
+// ---------------------------------------------------------------------------------------------
+// LOCAL: register-resident FPS over the candidate set (CTA 0, warps 0..LW-1).  Thread t keeps the
+// candidates i = c*(LW*32) + t, c < CPT: coordinates (packed in pairs) and D in registers; the
+// original indices stay in shared memory and are only read to break exact ties and to emit.
+// One pick = CPT d2 evaluations per thread (FADD2/FMUL2 for the differences and squares), one redux + one vote per warp, one
+// 8-byte slot {D bits, candidate index} per warp, one named barrier.  Slots are double-buffered by
+// pick parity, so a single barrier per pick is enough.  Exact ties of the maximum (inside a lane,
+// between lanes, between warps) take a slow path that compares ~orig, i.e. lowest index wins.
 // ---------------------------------------------------------------------------------------------
 template <int CPT, int LW>
 __device__ __forceinline__ void local_fps(const float *cX, const float *cY, const float *cZ, const float *cD,
                                           const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
-                                          const int M, LSlot *lslot, float4 *bpick, int *out_idx, float *out_mind,
+                                          const int M, uint2 *lslot, float4 *bpick, int *out_idx, float *out_mind,
                                           const int ltid)
 {
+    static_assert(CPT % 2 == 0, "candidates are processed in pairs");
+    constexpr int H = CPT / 2, LT = LW * 32;
     const int lane = ltid & 31, w = ltid >> 5;
-    float X[CPT], Y[CPT], Z[CPT], D[CPT];
-    unsigned O[CPT];
+    f32x2 X[H], Y[H], Z[H];
+    float D[CPT];
 #pragma unroll
-    for (int c = 0; c < CPT; ++c) {
-        const int i = c * (LW * 32) + ltid;
-        const bool ok = i < cnt;
-        X[c] = ok ? cX[i] : 0.0f;
-        Y[c] = ok ? cY[i] : 0.0f;
-        Z[c] = ok ? cZ[i] : 0.0f;
-        D[c] = ok ? cD[i] : 0.0f;      // padding: key (0, 0) is below every real key (real lo >= 2^31)
-        O[c] = ok ? cO[i] : 0u;
+    for (int h = 0; h < H; ++h) {
+        const int i0 = (2 * h) * LT + ltid, i1 = (2 * h + 1) * LT + ltid;
+        const bool ok0 = i0 < cnt, ok1 = i1 < cnt;
+        X[h] = pack2(ok0 ? cX[i0] : 0.0f, ok1 ? cX[i1] : 0.0f);
+        Y[h] = pack2(ok0 ? cY[i0] : 0.0f, ok1 ? cY[i1] : 0.0f);
+        Z[h] = pack2(ok0 ? cZ[i0] : 0.0f, ok1 ? cZ[i1] : 0.0f);
+        D[2 * h] = ok0 ? cD[i0] : 0.0f;          // padding: D = 0 never exceeds tau
+        D[2 * h + 1] = ok1 ? cD[i1] : 0.0f;
     }
     int par = 0;
     nb = 0;
     for (;;) {
+        // ---- warp level: max D, its owner lane and candidate slot ----
         float m = D[0];
 #pragma unroll
         for (int c = 1; c < CPT; ++c) m = fmaxf(m, D[c]);
         const unsigned hi = __float_as_uint(m);
         const unsigned mhi = __reduce_max_sync(FULL, hi);
-        unsigned lo = 0u;
-        if (hi == mhi) {
+        const bool top = hi == mhi;
+        unsigned eq = 0u;                        // bit c set iff D[c] == m (only meaningful on top lanes)
 #pragma unroll
-            for (int c = 0; c < CPT; ++c)
-                if (D[c] == m) lo = max(lo, O[c]);
-        }
-        const unsigned mlo = __reduce_max_sync(FULL, lo);
-        if (hi == mhi && lo == mlo) {
-            float x = X[0], y = Y[0], z = Z[0];
+        for (int c = 0; c < CPT; ++c) eq |= (D[c] == m ? 1u : 0u) << c;
+        const unsigned tops = __ballot_sync(FULL, top);
+        const bool multi = __any_sync(FULL, top && (eq & (eq - 1u)));
+        int cstar = __ffs(eq) - 1;
+        int wlane = __ffs(tops) - 1;
+        if (multi || (tops & (tops - 1u))) {     // exact tie inside the warp: lowest original index wins
+            unsigned lo = 0u;
+            if (top) {
 #pragma unroll
-            for (int c = 1; c < CPT; ++c)
-                if (D[c] == m && O[c] == lo) { x = X[c]; y = Y[c]; z = Z[c]; }
-            LSlot *s = &lslot[par * LW + w];
-            s->hi = mhi; s->lo = mlo; s->x = x; s->y = y; s->z = z;
+                for (int c = 0; c < CPT; ++c)
+                    if (eq & (1u << c)) {
+                        const unsigned o = cO[c * LT + ltid];
+                        if (o >= lo) { lo = o; cstar = c; }
+                    }
+            }
+            const unsigned mlo = __reduce_max_sync(FULL, lo);
+            wlane = __ffs(__ballot_sync(FULL, top && lo == mlo)) - 1;
         }
-        if (LW > 1) named_bar_sync(1, LW * 32);
+        if (lane == wlane) lslot[par * LW + w] = make_uint2(mhi, (unsigned)(cstar * LT + ltid));
+        if (LW > 1) named_bar_sync(1, LT);
         else __syncwarp();
-        unsigned shi = 0u, slo = 0u;
-        if (lane < LW) { shi = lslot[par * LW + lane].hi; slo = lslot[par * LW + lane].lo; }
-        unsigned ghi, glo;
-        const int win = warp_argmax_key(shi, slo, ghi, glo);
-        if (!(ghi > taubits)) break;        // restricted max <= tau: the candidate set no longer decides
-        const LSlot *ws = &lslot[par * LW + win];
-        const float sx = ws->x, sy = ws->y, sz = ws->z;
+        // ---- CTA level: every thread reads the LW slots ----
+        unsigned ghi = 0u, gidx = 0u;
+        int nties = 0;
+#pragma unroll
+        for (int s = 0; s < LW; ++s) {
+            const uint2 v = lslot[par * LW + s];
+            if (v.x > ghi) { ghi = v.x; gidx = v.y; nties = 1; }
+            else if (v.x == ghi) ++nties;
+        }
+        if (!(ghi > taubits)) break;            // restricted max <= tau: the candidate set no longer decides
+        if (nties > 1) {                         // exact tie between warps: lowest original index wins
+            unsigned bo = 0u;
+#pragma unroll
+            for (int s = 0; s < LW; ++s) {
+                const uint2 v = lslot[par * LW + s];
+                if (v.x == ghi) {
+                    const unsigned o = cO[v.y];
+                    if (o >= bo) { bo = o; gidx = v.y; }
+                }
+            }
+        }
+        const float sx = cX[gidx], sy = cY[gidx], sz = cZ[gidx];
         if (ltid == 0) {
-            out_idx[j] = (int)(~glo);
+            out_idx[j] = (int)(~cO[gidx]);
             out_mind[j] = __uint_as_float(ghi);
             bpick[nb] = make_float4(sx, sy, sz, 0.0f);
         }
         ++j;
         ++nb;
         if (j >= M || nb >= PB) break;
+        // ---- update: D = min(D, d2(candidate, pick)), two candidates per instruction ----
+        const f32x2 SX = pack2(sx, sx), SY = pack2(sy, sy), SZ = pack2(sz, sz);
 #pragma unroll
-        for (int c = 0; c < CPT; ++c) D[c] = fminf(D[c], d2_rn(X[c], Y[c], Z[c], sx, sy, sz));
+        for (int h = 0; h < H; ++h) {
+            const f32x2 dx = sub2(X[h], SX), dy = sub2(Y[h], SY), dz = sub2(Z[h], SZ);
+            float x0, x1, y0, y1, z0, z1;
+            unpack2(mul2(dx, dx), x0, x1);
+            unpack2(mul2(dy, dy), y0, y1);
+            unpack2(mul2(dz, dz), z0, z1);
+            D[2 * h] = fminf(D[2 * h], __fadd_rn(__fadd_rn(x0, y0), z0));
+            D[2 * h + 1] = fminf(D[2 * h + 1], __fadd_rn(__fadd_rn(x1, y1), z1));
+        }
         par ^= 1;
     }
 }
@@ -182,7 +249,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned *cO = reinterpret_cast<unsigned *>(cD + TC);
     Ctl *ctl = reinterpret_cast<Ctl *>(smem_raw + L.ctl);
     uint4 *wbest = reinterpret_cast<uint4 *>(smem_raw + L.wbest);
-    LSlot *lslot = reinterpret_cast<LSlot *>(smem_raw + L.lslot);
+    uint2 *lslot = reinterpret_cast<uint2 *>(smem_raw + L.lslot);
     int2 *queue = reinterpret_cast<int2 *>(smem_raw + L.queue);
     int *qn = reinterpret_cast<int *>(smem_raw + L.qn);
 
@@ -230,10 +297,11 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
                        c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0;
+    long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
     cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
 
     while (j < P.M) {
-        if (STATS && tid == 0 && rank == 0) c_rounds++;
+        if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
         // =====================================================================================
         // APPLY: the nb picks in bpick[], 32 at a time
         // =====================================================================================
@@ -315,6 +383,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             qpar ^= 1u;
         }
 
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_apply += t1 - t0; t0 = t1; }
         // =====================================================================================
         // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
         // =====================================================================================
@@ -352,6 +421,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             gpos = __shfl_sync(FULL, rb.z, win);
         }
 
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
         // =====================================================================================
         // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
         // =====================================================================================
@@ -420,6 +490,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             }
         }
 
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
         // =====================================================================================
         // LOCAL (CTA 0): FPS restricted to the candidates; or the single global argmax
         // =====================================================================================
@@ -444,6 +515,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             }
         }
         cluster_sync_all();
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_local += t1 - t0; }
         {
             const uint4 r0 = ld_dsmem_v4(mapa(smem_u32(&ctl->nb), 0u));
             nb = (int)r0.x;
@@ -472,6 +544,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             atomicAdd(P.counters + CNT_RETRIES, c_retries);
             atomicAdd(P.counters + CNT_SINGLES, c_singles);
             atomicAdd(P.counters + CNT_CANDS, c_cands);
+            atomicAdd(P.counters + CNT_CYC_APPLY, (unsigned long long)t_apply);
+            atomicAdd(P.counters + CNT_CYC_MAX, (unsigned long long)t_max);
+            atomicAdd(P.counters + CNT_CYC_EXTRACT, (unsigned long long)t_extract);
+            atomicAdd(P.counters + CNT_CYC_LOCAL, (unsigned long long)t_local);
         }
     }
     cluster_sync_all();   // no CTA may exit while a peer can still read its shared memory
@@ -481,6 +557,32 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 // host side: launch shape and launch
 // ---------------------------------------------------------------------------------------------
 static const int kMaxSmem = 227 * 1024;
+
+template <int CPT, int LW, bool STATS>
+__global__ void k_fps_batched(const BatchParams P, const int flags);
+
+// how many clusters of `c` CTAs of the default kernel can be resident at once (0 on error)
+static int max_resident_clusters(int c, size_t smem)
+{
+    auto kern = k_fps_batched<8, 4, false>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)(c * 148));
+    cfg.blockDim = dim3(BT);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)c;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n;
+}
 
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
 {
@@ -500,6 +602,10 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         C = 1;
         while (C < 16 && (long long)C * 2 * ix.B <= 148 && (long long)ix.N > (long long)C * 2048) C *= 2;
         while (C < 16 && !fits(C)) C *= 2;
+        // all B clusters should be resident at once (a cluster lives inside one GPC, so fewer clusters
+        // fit than 148 / C suggests); otherwise the clouds run in waves
+        while (C > 1 && fits(C / 2) && max_resident_clusters(C, smem_layout((K + C - 1) / C, TC, LW).total) < std::min(ix.B, 148 / C))
+            C /= 2;
     }
     if (!fits(C)) {
         set_error("K_max=%d voxels do not fit the shared memory of %d CTAs; use a smaller n_vox or a larger tile_points", K, C);

@@ -39,10 +39,10 @@ def test_binding_lists_every_declared_symbol():
 
 
 def test_struct_sizes_match_header(lib):
-    # fps_build_opts: 5 x int32 + pointer (8-aligned) = 32 bytes; fps_stats: see header
+    # fps_build_opts: 5 x int32 + pointer (8-aligned) + 2 x int32 = 40 bytes; fps_stats: see header
     from paper_2606_06255_b200 import binding
-    assert ctypes.sizeof(binding.fps_build_opts) == 32
-    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8
+    assert ctypes.sizeof(binding.fps_build_opts) == 40
+    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8 + 10 * 8 + 2 * 4
 
 
 def test_version_and_error_strings(lib):
@@ -84,3 +84,33 @@ def test_product_path_does_not_import_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert not re.search(r"^\s*(import|from)\s+oracle\b", src, flags=re.M), f
                 assert "oracle/" not in src or f == "inputs.py" or "Nothing here is used by" in src, f
+
+
+def test_no_packed_fma_in_the_built_kernels():
+    """The one distance expression must never be contracted to FMA (BASELINE.json north_star).  The
+    scalar path uses __f*_rn intrinsics; the packed path (FADD2/FMUL2 in the candidate-set FPS) must
+    not contain FFMA2, which ptxas would produce from mul.f32x2 + add.f32x2 even under --fmad=false."""
+    import shutil
+    import subprocess
+    from paper_2606_06255_b200 import build
+    cuobjdump = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(cuobjdump):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([cuobjdump, "-sass", build.build()], capture_output=True, text=True, check=True).stdout
+    assert "FMUL2" in sass                      # the packed path is really there
+    assert "FFMA2" not in sass
+    # scalar FFMA may only come from the sqrt_rn / division sequences (MUFU + Newton steps), never from
+    # a distance: a few dozen at most per kernel, and always fewer than the FMUL of the distances
+    fn, counts = None, {}
+    for line in sass.splitlines():
+        m = re.search(r"Function : (\S+)", line)
+        if m:
+            fn = m.group(1)
+            counts[fn] = [0, 0]
+        elif fn and " FFMA" in line:
+            counts[fn][0] += 1
+        elif fn and (" FMUL " in line or " FMUL2 " in line):
+            counts[fn][1] += 1
+    for fn, (ffma, fmul) in counts.items():
+        if "k_fps_" in fn:
+            assert ffma <= 48 and fmul > ffma, (fn, ffma, fmul)

@@ -64,22 +64,54 @@ SMALL = {
 }
 
 
+# the two sampling kernels: exact batched picking (default) and the per-pick persistent kernel
+KERNELS = {"batched": 0, "per_pick": 16}
+
+
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("name", sorted(SMALL))
-def test_small_clouds_default_config(rf, name):
+def test_small_clouds_default_config(rf, name, kernel):
     P, M = SMALL[name]()
     ref = oracle.fps(P, M, 0)
-    gi, gm, _ = run_gpu(rf, P, M)
+    gi, gm, _ = run_gpu(rf, P, M, flags=KERNELS[kernel])
     assert_same(gi, gm, *ref)
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("cluster", [1, 2, 4, 8, 16])
 @pytest.mark.parametrize("name", ["room", "lattice", "lidar"])
-def test_every_cluster_size(rf, name, cluster):
+def test_every_cluster_size(rf, name, cluster, kernel):
     P, M = SMALL[name]()
     ref = oracle.fps(P, M, 0)
-    gi, gm, st = run_gpu(rf, P, M, cluster_size=cluster)
+    gi, gm, st = run_gpu(rf, P, M, cluster_size=cluster, flags=KERNELS[kernel])
     assert st["cluster_size"] == cluster
     assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("cpt", [4, 8, 16])
+@pytest.mark.parametrize("lw", [1, 2, 4, 8])
+@pytest.mark.parametrize("name", ["room", "lattice", "dups", "clustered"])
+def test_every_local_phase_shape(rf, name, lw, cpt):
+    # candidate capacity 32*lw*cpt from 128 to 4096: different thresholds, batches and tie paths
+    # (lattice: exact ties inside a lane, between lanes and between warps; dups: Dist reaches +0)
+    if (cpt, lw) not in {(8, 4), (8, 1), (8, 2), (8, 8), (4, 4), (4, 8), (16, 4), (16, 8)}:
+        pytest.skip("shape not instantiated")
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, local_warps=lw, cand_per_thread=cpt, flags=rf.FPS_FLAG_STATS)
+    assert (st["local_warps"], st["cand_per_thread"]) == (lw, cpt)
+    assert_same(gi, gm, *ref)
+    assert st["rounds"] >= 1 and st["rounds"] <= M
+    if name == "room":
+        assert st["rounds"] < M // 8            # batching really happens on ordinary data
+
+
+def test_batched_kernel_degenerates_to_per_pick_rounds_without_batching(rf):
+    P, M = SMALL["room"]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_NO_BATCH | rf.FPS_FLAG_STATS)
+    assert_same(gi, gm, *ref)
+    assert st["rounds"] == M - 1 and st["single_picks"] == M - 1 and st["candidates"] == 0
 
 
 @pytest.mark.parametrize("n_vox", [1, 2, 7, 16, 24, 64, 128])
@@ -108,24 +140,32 @@ def test_result_independent_of_tiling(rf, name, tile):
 def test_block_sizes(rf, threads):
     P, M = SMALL["room"]()
     ref = oracle.fps(P, M, 0)
-    gi, gm, st = run_gpu(rf, P, M, block_threads=threads, cluster_size=2)
+    gi, gm, st = run_gpu(rf, P, M, block_threads=threads, cluster_size=2, flags=rf.FPS_FLAG_PER_PICK)
     assert st["block_threads"] == threads
     assert_same(gi, gm, *ref)
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("flags", [1, 2, 3, 4, 7])
-def test_ablations_and_stats_are_bit_identical(rf, flags):
+def test_ablations_and_stats_are_bit_identical(rf, flags, kernel):
     # Table 4 structure: prune off / skip off / both off must not change a bit
     P, M = SMALL["room"]()
     ref = oracle.fps(P, M, 0)
-    gi, gm, st = run_gpu(rf, P, M, flags=flags)
+    gi, gm, st = run_gpu(rf, P, M, flags=flags | KERNELS[kernel])
     assert_same(gi, gm, *ref)
     if flags & rf.FPS_FLAG_STATS:
         assert st["iterations"] == M - 1
-        assert st["voxel_tests"] == st["K_total"] * (M - 1)
+        if kernel == "per_pick":
+            applied = M - 1                                      # every voxel is tested against every pick
+        else:
+            # ... except the picks of the last batch, which nothing needs to be updated for
+            applied = st["voxel_tests"] // st["K_total"]
+            assert st["voxel_tests"] == st["K_total"] * applied and M - 1 - 1024 <= applied <= M - 1
+        assert st["voxel_tests"] == st["K_total"] * applied
         if flags & rf.FPS_FLAG_NO_PRUNE:
-            assert st["voxels_visited"] == st["K_total"] * (M - 1)
-            assert st["points_visited"] == P.shape[0] * (M - 1)
+            if kernel == "per_pick":
+                assert st["voxels_visited"] == st["K_total"] * applied
+            assert st["points_visited"] == P.shape[0] * applied
         if flags & rf.FPS_FLAG_NO_SKIP:
             assert st["points_computed"] == st["points_visited"]
 
@@ -134,32 +174,39 @@ def test_stats_match_cpu_pruned_variant_effective_updates(rf):
     # the number of EFFECTIVE updates (Eq. 2) is a property of the data, not of the index
     P, M = SMALL["room"]()
     _, _, cpu = oracle.pruned_fps(P, M, 0, n_vox=16)
-    _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS)
-    assert st["effective"] == cpu["effective"]
-    assert st["points_visited"] < 0.2 * P.shape[0] * (M - 1)
+    for kernel, kflag in KERNELS.items():
+        _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS | kflag)
+        if kernel == "per_pick":
+            assert st["effective"] == cpu["effective"]
+        else:                       # the picks of the last batch are never applied (nothing needs them)
+            assert 0.8 * cpu["effective"] <= st["effective"] <= cpu["effective"]
+        assert st["points_visited"] < 0.2 * P.shape[0] * (M - 1)
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("N,M,start", [(1, 1, 0), (2, 2, 1), (3, 1, 2), (33, 33, 32), (64, 64, 7), (1000, 1000, 999)])
-def test_degenerate_sizes_and_starts(rf, N, M, start):
+def test_degenerate_sizes_and_starts(rf, N, M, start, kernel):
     P = inputs.uniform_cube(N, 3)
     ref = oracle.fps(P, M, start)
-    gi, gm, _ = run_gpu(rf, P, M, start)
+    gi, gm, _ = run_gpu(rf, P, M, start, flags=KERNELS[kernel])
     assert_same(gi, gm, *ref)
 
 
-def test_identical_points(rf):
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
+def test_identical_points(rf, kernel):
     P = np.full((100, 3), 0.25, dtype=np.float32)
     ref = oracle.fps(P, 10, 3)
-    gi, gm, _ = run_gpu(rf, P, 10, 3)
+    gi, gm, _ = run_gpu(rf, P, 10, 3, flags=KERNELS[kernel])
     assert_same(gi, gm, *ref)
     assert gi.reshape(-1).tolist() == [3] + [0] * 9
 
 
-def test_closed_form_line_and_corners(rf):
-    gi, gm, _ = run_gpu(rf, inputs.integer_line(9), 9)
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
+def test_closed_form_line_and_corners(rf, kernel):
+    gi, gm, _ = run_gpu(rf, inputs.integer_line(9), 9, flags=KERNELS[kernel])
     assert gi.reshape(-1).tolist() == [0, 8, 4, 2, 6, 1, 3, 5, 7]
     assert gm.reshape(-1).tolist() == [np.inf, 64, 16, 4, 4, 1, 1, 1, 1]
-    gi, gm, _ = run_gpu(rf, inputs.cube_corners(), 8)
+    gi, gm, _ = run_gpu(rf, inputs.cube_corners(), 8, flags=KERNELS[kernel])
     assert gi.reshape(-1).tolist() == [0, 7, 1, 2, 3, 4, 5, 6]
 
 
@@ -228,6 +275,8 @@ def test_full_size_against_live_oracle(rf, name):
     P = inputs.make_batch(w)
     ref = oracle.fps(P, w.M, w.start_idx)
     gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx)
+    assert_same(gi, gm, *ref)
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx, flags=rf.FPS_FLAG_PER_PICK)
     assert_same(gi, gm, *ref)
 
 
