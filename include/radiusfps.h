@@ -100,6 +100,8 @@ typedef struct {
     int64_t extract_points;   /* points scanned by the extraction                                     */
     int64_t cycles_apply, cycles_max, cycles_extract, cycles_local;   /* SM cycles spent per phase, as seen
                                  by thread 0 of each cloud's first CTA, summed over clouds             */
+    int64_t group_tests;      /* (group of 32 voxels, pick) prune tests; voxel_tests then counts only the
+                                 pairs whose group survived                                           */
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
 } fps_stats;
 

@@ -116,6 +116,7 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->candidates = (int64_t)c[8]; out->extract_voxels = (int64_t)c[9]; out->extract_points = (int64_t)c[10];
             out->cycles_apply = (int64_t)c[11]; out->cycles_max = (int64_t)c[12];
             out->cycles_extract = (int64_t)c[13]; out->cycles_local = (int64_t)c[14];
+            out->group_tests = (int64_t)c[15];
         }
     }
     return FPS_OK;
@@ -140,13 +141,13 @@ int fps_sample_host(const float *points_host, int32_t N, int32_t B, int32_t M, i
     int rc = FPS_OK;
     fps_index_t *h = nullptr;
     auto fail = [&](int code) {
-        cudaFree(d_pts); cudaFree(d_idx); cudaFree(d_mind);
+        rfps::dev_free_async(d_pts, st); rfps::dev_free_async(d_idx, st); rfps::dev_free_async(d_mind, st);
         if (h) fps_index_destroy(h);
         return code;
     };
-    if (cudaMalloc(&d_pts, pb) != cudaSuccess || cudaMalloc(&d_idx, ob) != cudaSuccess ||
-        cudaMalloc(&d_mind, ob) != cudaSuccess) {
-        set_error("cudaMalloc failed in fps_sample_host");
+    if (rfps::dev_alloc_async((void **)&d_pts, pb, st) != cudaSuccess || rfps::dev_alloc_async((void **)&d_idx, ob, st) != cudaSuccess ||
+        rfps::dev_alloc_async((void **)&d_mind, ob, st) != cudaSuccess) {
+        set_error("device allocation failed in fps_sample_host");
         cudaGetLastError();
         return fail(FPS_ERR_NOMEM);
     }

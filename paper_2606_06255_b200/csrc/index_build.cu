@@ -18,6 +18,7 @@
 #include <cmath>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <vector>
 
 #include "internal.h"
@@ -36,13 +37,6 @@ __device__ __forceinline__ float ord2f(unsigned u)
 {
     return __uint_as_float((u & 0x80000000u) ? (u & 0x7fffffffu) : ~u);
 }
-
-struct DevBuf {   // RAII for build-time scratch
-    void *p = nullptr;
-    ~DevBuf() { if (p) cudaFree(p); }
-    cudaError_t alloc(size_t bytes) { return cudaMalloc(&p, bytes ? bytes : 4); }
-    template <class T> T *as() { return reinterpret_cast<T *>(p); }
-};
 
 // ---------------------------------------------------------------------------------------------
 // a1: bounding box (Eq. 6) + non-finite detection.  bbox[b] = {minx,miny,minz,maxx,maxy,maxz} as
@@ -95,7 +89,7 @@ __global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, int
 }
 
 // ---------------------------------------------------------------------------------------------
-// a2: sort key per point.  key = V_id << (3*sb) | morton(sub-cell), V_id per Eq. 31; val = i.
+// a2: sort key per point.  key = V_id << (3*sb) | morton(sub-cell); val = i.
 // Voxel coordinates per Eq. 8 (floor, then clamp; reading A14); L per Eq. 7 with alpha = 1 + 1e-3.
 // ---------------------------------------------------------------------------------------------
 __device__ __forceinline__ unsigned spread3(unsigned v)
@@ -133,7 +127,10 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int
         v[a] = (unsigned)c;
         s[a] = (unsigned)sc;
     }
-    unsigned vid = (v[2] * (unsigned)n_vox + v[1]) * (unsigned)n_vox + v[0];
+    // voxel id: the Morton interleave of (v_x, v_y, v_z) instead of the row-major id of Eq. 31 -- any
+    // bijective id gives the same voxels; Morton order keeps consecutive active voxels spatially
+    // compact, which the sampling kernel's group-level prune relies on
+    unsigned vid = spread3(v[0]) | (spread3(v[1]) << 1) | (spread3(v[2]) << 2);
     unsigned sub = sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
     keys[(size_t)b * N + i] = (vid << (3 * sb)) | sub;
     vals[(size_t)b * N + i] = i;
@@ -404,11 +401,12 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
                                                  int *__restrict__ maxcnt)
 {
     const int b = blockIdx.y;
-    const int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
-    if (k >= K[b]) return;
-    const int2 sg = vseg[(size_t)b * K_cap + k];
     const float *x = px + (size_t)b * N, *y = py + (size_t)b * N, *z = pz + (size_t)b * N;
+    const int Kb = K[b];
+    int local_max = 0;
+    for (int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); k < Kb; k += gridDim.x * (blockDim.x >> 5)) {
+    const int2 sg = vseg[(size_t)b * K_cap + k];
     float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
     for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) {
         mn[0] = fminf(mn[0], x[p]); mx[0] = fmaxf(mx[0], x[p]);
@@ -430,7 +428,45 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
     if (lane == 0) {
         const float R = __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f);
         vgeom[(size_t)b * K_cap + k] = make_float4(cx, cy, cz, R);
-        atomicMax(maxcnt, sg.y);
+        local_max = max(local_max, sg.y);
+    }
+    }
+    if (lane == 0 && local_max > 0) atomicMax(maxcnt, local_max);
+}
+
+// ---------------------------------------------------------------------------------------------
+// a6': group spheres.  32 consecutive (Morton-ordered) voxels form a group; its sphere encloses the
+// member spheres:  c_g = midpoint of the box around the member spheres,
+//   R_g = max_l ( sqrt_rn(d2(c_l, c_g)) * (1 + 2^-20) + R_l ) * (1 + 2^-20)     (rounded up, as A9)
+// so every point p of a member voxel has ||p - c_g|| <= ||p - c_l|| + ||c_l - c_g|| <= R_g, and the
+// prune test of Eq. 25 can be applied to the whole group with Dist_v := max over its voxels.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_group_sphere(const float4 *__restrict__ vgeom, const int *__restrict__ K, int K_cap,
+                                                       int G_cap, float4 *__restrict__ ggeom)
+{
+    const int b = blockIdx.y;
+    const int lane = threadIdx.x & 31;
+    const int Kb = K[b];
+    const int G = (Kb + 31) / 32;
+    for (int g = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); g < G; g += gridDim.x * (blockDim.x >> 5)) {
+        const int k = g * 32 + lane;
+        const bool in = k < Kb;
+        const float4 v = in ? vgeom[(size_t)b * K_cap + k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float mn[3] = {in ? v.x - v.w : FLT_MAX, in ? v.y - v.w : FLT_MAX, in ? v.z - v.w : FLT_MAX};
+        float mx[3] = {in ? v.x + v.w : -FLT_MAX, in ? v.y + v.w : -FLT_MAX, in ? v.z + v.w : -FLT_MAX};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            for (int o = 16; o > 0; o >>= 1) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+            }
+        const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+        const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+        const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+        float r = 0.0f;
+        if (in) r = __fmul_rn(__fadd_rn(__fmul_rn(__fsqrt_rn(d2_rn(v.x, v.y, v.z, cx, cy, cz)), 1.0f + 0x1p-20f), v.w), 1.0f + 0x1p-20f);
+        for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
+        if (lane == 0) ggeom[(size_t)b * G_cap + g] = make_float4(cx, cy, cz, r);
     }
 }
 
@@ -453,39 +489,80 @@ static int auto_n_vox(int N)
     return n < 2 ? 2 : n;
 }
 
-template <class T>
-static int dev_alloc(T *&p, size_t count, int64_t &total)
+// Stream-ordered allocations from a private pool that keeps freed memory (release threshold = max),
+// so that a build + destroy cycle costs no cudaMalloc/cudaFree and no device synchronisation.
+static cudaMemPool_t build_pool()
 {
-    void *q = nullptr;
-    size_t bytes = (count ? count : 1) * sizeof(T);
-    cudaError_t e = cudaMalloc(&q, bytes);
-    if (e != cudaSuccess) {
-        set_error("cudaMalloc(%zu bytes) failed: %s", bytes, cudaGetErrorString(e));
-        return FPS_ERR_NOMEM;
+    static std::mutex mu;
+    static cudaMemPool_t pools[64] = {};
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) return nullptr;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!pools[dev]) {
+        cudaMemPoolProps props;
+        memset(&props, 0, sizeof props);
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        if (cudaMemPoolCreate(&pools[dev], &props) != cudaSuccess) { cudaGetLastError(); pools[dev] = nullptr; return nullptr; }
+        unsigned long long keep = ~0ull;
+        cudaMemPoolSetAttribute(pools[dev], cudaMemPoolAttrReleaseThreshold, &keep);
     }
-    p = reinterpret_cast<T *>(q);
-    total += (int64_t)bytes;
-    return FPS_OK;
+    return pools[dev];
 }
+
+static cudaError_t pool_alloc(void **p, size_t bytes, cudaStream_t st)
+{
+    cudaMemPool_t pool = build_pool();
+    if (!pool) return cudaMalloc(p, bytes);
+    return cudaMallocFromPoolAsync(p, bytes, pool, st);
+}
+
+cudaError_t dev_alloc_async(void **p, size_t bytes, cudaStream_t st) { return pool_alloc(p, bytes ? bytes : 4, st); }
+void dev_free_async(void *p, cudaStream_t st)
+{
+    if (!p) return;
+    if (build_pool()) cudaFreeAsync(p, st);
+    else cudaFree(p);
+}
+
+struct Carver {    // hands out 256-byte aligned pieces of one allocation (first pass: sizes only)
+    char *base = nullptr;
+    size_t off = 0;
+    template <class T> T *take(size_t count)
+    {
+        T *p = base ? reinterpret_cast<T *>(base + off) : nullptr;
+        off += ((count ? count : 1) * sizeof(T) + 255) & ~(size_t)255;
+        return p;
+    }
+};
 
 void free_index(DeviceIndex &ix)
 {
-    cudaFree(ix.px); cudaFree(ix.py); cudaFree(ix.pz);
-    cudaFree(ix.porig); cudaFree(ix.pinv); cudaFree(ix.Dp);
-    cudaFree(ix.vgeom); cudaFree(ix.vseg); cudaFree(ix.vstate);
-    cudaFree(ix.K_dev); cudaFree(ix.counters);
+    if (ix.arena) {
+        // stream-ordered: the memory is released after the last sampling kernel enqueued on that stream
+        if (ix.arena_pooled) cudaFreeAsync(ix.arena, ix.last_stream);
+        else cudaFree(ix.arena);
+    }
     free(ix.K_host);
     ix = DeviceIndex();
 }
+
+struct Scratch {
+    unsigned *bbox, *kA, *kB;
+    int *vA, *vB, *table, *bsum, *heads, *rank, *voff, *ntl, *tbase, *Kv;
+};
 
 int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 {
     const int B = ix.B, N = ix.N;
     cudaStream_t st = (cudaStream_t)o.stream;
+    ix.last_stream = st;
     int n_vox = o.n_vox > 0 ? o.n_vox : auto_n_vox(N);
     if (n_vox > 1024) { set_error("n_vox=%d out of range [1,1024]", n_vox); return FPS_ERR_INVALID; }
     int tile_points = o.tile_points == 0 ? 64 : (o.tile_points < 0 ? 0 : o.tile_points);
-    const int vbits = ilog2_ceil((unsigned long long)n_vox * n_vox * n_vox);
+    const int vbits = 3 * ilog2_ceil((unsigned long long)n_vox);
     int sb = tile_points > 0 ? (32 - vbits) / 3 : 0;
     if (sb > 4) sb = 4;
     const int keybits = vbits + 3 * sb;
@@ -493,59 +570,117 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     ix.tile_points = tile_points;
     ix.flags = o.flags;
 
+    // upper bound of the (tiled) voxel count, known before anything runs: no host round-trip is
+    // needed to size the voxel arrays
+    const long long cells = (long long)n_vox * n_vox * n_vox;
+    long long kb = std::min<long long>(N, cells) + (tile_points > 0 ? N / tile_points : 0);
+    kb = std::min<long long>(kb, N);
+    ix.K_cap = (int)((kb + 31) / 32 * 32);
+    ix.G_cap = ix.K_cap / 32;
+
     const size_t BN = (size_t)B * N;
     const int nchunk = (N + RS_CHUNK - 1) / RS_CHUNK;
     const size_t table_n = (size_t)256 * nchunk;       // per cloud
-    DevBuf bbox, kA, kB, vA, vB, table, bsum, heads, rank, voff, ntl, tbase, Kv;
-    if (bbox.alloc(sizeof(unsigned) * B * BBOX_STRIDE) || kA.alloc(4 * BN) || kB.alloc(4 * BN) || vA.alloc(4 * BN) ||
-        vB.alloc(4 * BN) || table.alloc(4 * table_n * B) ||
-        bsum.alloc(4 * (size_t)(scan_tmp_ints((int)std::max((size_t)N, table_n), B))) || heads.alloc(4 * BN) ||
-        rank.alloc(4 * BN) || voff.alloc(4 * BN) || ntl.alloc(4 * BN) || tbase.alloc(4 * BN) || Kv.alloc(4 * B)) {
-        set_error("cudaMalloc of build scratch failed (B=%d, N=%d)", B, N);
+    const bool per_pick = o.flags & FPS_FLAG_PER_PICK;
+
+    Scratch sc;
+    unsigned *meta = nullptr;      // [0] = largest segment, then (persistent arena only)
+    auto carve = [&](Carver &c, bool persistent) {
+        if (persistent) {
+            ix.px = c.take<float>(BN); ix.py = c.take<float>(BN); ix.pz = c.take<float>(BN);
+            ix.porig = c.take<int32_t>(BN); ix.pinv = c.take<int32_t>(BN); ix.Dp = c.take<float>(BN);
+            ix.vgeom = c.take<float4>((size_t)B * ix.K_cap);
+            ix.vseg = c.take<int2>((size_t)B * ix.K_cap);
+            ix.ggeom = c.take<float4>((size_t)B * ix.G_cap);
+            ix.vstate = per_pick ? c.take<uint4>((size_t)B * ix.K_cap) : nullptr;
+            ix.K_dev = c.take<int32_t>(B);
+            ix.counters = c.take<unsigned long long>(NUM_COUNTERS);
+            meta = c.take<unsigned>(8);
+        } else {
+            sc.bbox = c.take<unsigned>((size_t)B * BBOX_STRIDE);
+            sc.kA = c.take<unsigned>(BN); sc.kB = c.take<unsigned>(BN);
+            sc.vA = c.take<int>(BN); sc.vB = c.take<int>(BN);
+            sc.table = c.take<int>(table_n * B);
+            sc.bsum = c.take<int>((size_t)scan_tmp_ints((int)std::max((size_t)N, table_n), B));
+            sc.heads = c.take<int>(BN); sc.rank = c.take<int>(BN); sc.voff = c.take<int>(BN);
+            sc.ntl = c.take<int>(BN); sc.tbase = c.take<int>(BN);
+            sc.Kv = c.take<int>(B);
+        }
+    };
+    Carver sizeP, sizeS;
+    carve(sizeP, true);
+    carve(sizeS, false);
+    void *arena = nullptr, *scratch = nullptr;
+    ix.arena_pooled = build_pool() != nullptr;
+    if (pool_alloc(&arena, sizeP.off, st) != cudaSuccess || pool_alloc(&scratch, sizeS.off, st) != cudaSuccess) {
+        set_error("device allocation of %zu + %zu bytes failed: %s", sizeP.off, sizeS.off, cudaGetErrorString(cudaGetLastError()));
+        if (arena) { if (ix.arena_pooled) cudaFreeAsync(arena, st); else cudaFree(arena); }
         return FPS_ERR_NOMEM;
     }
-    int rc;
-    if ((rc = dev_alloc(ix.K_dev, B, ix.device_bytes)) != FPS_OK) return rc;
+    ix.arena = arena;
+    ix.device_bytes = (int64_t)sizeP.off;
+    Carver cp, cs;
+    cp.base = (char *)arena;
+    cs.base = (char *)scratch;
+    carve(cp, true);
+    carve(cs, false);
+    auto release_scratch = [&]() { if (ix.arena_pooled) cudaFreeAsync(scratch, st); else cudaFree(scratch); };
 
+    int rc;
     g_launches = 0;
     const dim3 gN((N + 255) / 256, B);
-    k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(bbox.as<unsigned>(), B);
-    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, bbox.as<unsigned>());
-    k_keys<<<gN, 256, 0, st>>>(points, N, bbox.as<unsigned>(), n_vox, sb, kA.as<unsigned>(), vA.as<int>());
-    RFPS_CUDA(cudaGetLastError());
+    RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));
+    k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(sc.bbox, B);
+    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, sc.bbox);
+    k_keys<<<gN, 256, 0, st>>>(points, N, sc.bbox, n_vox, sb, sc.kA, sc.vA);
     g_launches += 3;
 
     // a3: LSD radix sort, 8 bits per pass
-    unsigned *kin = kA.as<unsigned>(), *kout = kB.as<unsigned>();
-    int *vin = vA.as<int>(), *vout = vB.as<int>();
+    unsigned *kin = sc.kA, *kout = sc.kB;
+    int *vin = sc.vA, *vout = sc.vB;
     const dim3 gR((nchunk + RS_WARPS - 1) / RS_WARPS, B);
     for (int shift = 0; shift < keybits; shift += 8) {
-        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, N, nchunk, shift, table.as<int>());
-        if ((rc = scan_exclusive(table.as<int>(), table.as<int>(), (int)table_n, (int)table_n, B, nullptr, bsum.as<int>(), st)))
-            return rc;
-        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, N, nchunk, shift, table.as<int>(), kout, vout);
+        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, N, nchunk, shift, sc.table);
+        if ((rc = scan_exclusive(sc.table, sc.table, (int)table_n, (int)table_n, B, nullptr, sc.bsum, st))) { release_scratch(); return rc; }
+        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, N, nchunk, shift, sc.table, kout, vout);
         std::swap(kin, kout);
         std::swap(vin, vout);
         g_launches += 2;
     }
-    RFPS_CUDA(cudaGetLastError());
 
-    // a5: grid voxels -> (tiled) segments
-    k_heads<<<gN, 256, 0, st>>>(kin, N, 3 * sb, heads.as<int>());
-    if ((rc = scan_exclusive(heads.as<int>(), rank.as<int>(), N, N, B, Kv.as<int>(), bsum.as<int>(), st))) return rc;
-    k_voxel_offsets<<<gN, 256, 0, st>>>(heads.as<int>(), rank.as<int>(), N, voff.as<int>());
-    k_ntiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), N, tile_points, ntl.as<int>());
-    if ((rc = scan_exclusive(ntl.as<int>(), tbase.as<int>(), N, N, B, ix.K_dev, bsum.as<int>(), st))) return rc;
-    RFPS_CUDA(cudaGetLastError());
-    g_launches += 3 + 3;   // heads, voxel_offsets, ntiles + tiles, gather, sphere below
+    // a5: grid voxels -> (tiled) segments; a4: gather; a6: spheres
+    k_heads<<<gN, 256, 0, st>>>(kin, N, 3 * sb, sc.heads);
+    if ((rc = scan_exclusive(sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st))) { release_scratch(); return rc; }
+    k_voxel_offsets<<<gN, 256, 0, st>>>(sc.heads, sc.rank, N, sc.voff);
+    k_ntiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, N, tile_points, sc.ntl);
+    if ((rc = scan_exclusive(sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st))) { release_scratch(); return rc; }
+    k_tiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, sc.ntl, sc.tbase, N, ix.K_cap, ix.vseg);
+    k_gather<<<gN, 256, 0, st>>>(points, vin, N, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
+    const int sphere_blocks = std::max(1, std::min((ix.K_cap + 7) / 8, 148 * 8));
+    k_sphere<<<dim3(sphere_blocks, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, N, ix.K_cap, ix.vgeom,
+                                                     reinterpret_cast<int *>(meta));
+    const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, 148 * 8));
+    k_group_sphere<<<dim3(group_blocks, B), 256, 0, st>>>(ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
+    g_launches += 8;
+    if (cudaGetLastError() != cudaSuccess) {
+        set_error("a build kernel failed to launch: %s", cudaGetErrorString(cudaGetLastError()));
+        release_scratch();
+        return FPS_ERR_CUDA;
+    }
 
-    // the one host round-trip of the build: K per cloud + the non-finite flags
+    // the one host round-trip of the build: K per cloud, the non-finite flags, the largest segment
     ix.K_host = (int32_t *)malloc(sizeof(int32_t) * B);
     std::vector<unsigned> hb((size_t)B * BBOX_STRIDE);
-    if (!ix.K_host) { set_error("host malloc failed"); return FPS_ERR_NOMEM; }
-    RFPS_CUDA(cudaMemcpyAsync(ix.K_host, ix.K_dev, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, st));
-    RFPS_CUDA(cudaMemcpyAsync(hb.data(), bbox.p, sizeof(unsigned) * B * BBOX_STRIDE, cudaMemcpyDeviceToHost, st));
-    RFPS_CUDA(cudaStreamSynchronize(st));
+    if (!ix.K_host) { set_error("host malloc failed"); release_scratch(); return FPS_ERR_NOMEM; }
+    cudaError_t e1 = cudaMemcpyAsync(ix.K_host, ix.K_dev, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, st);
+    cudaError_t e2 = cudaMemcpyAsync(hb.data(), sc.bbox, sizeof(unsigned) * B * BBOX_STRIDE, cudaMemcpyDeviceToHost, st);
+    cudaError_t e3 = cudaMemcpyAsync(&ix.max_voxel_points, meta, sizeof(int), cudaMemcpyDeviceToHost, st);
+    release_scratch();
+    cudaError_t e4 = cudaStreamSynchronize(st);
+    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) {
+        set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : (e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3))));
+        return FPS_ERR_CUDA;
+    }
     for (int b = 0; b < B; ++b)
         if (hb[(size_t)b * BBOX_STRIDE + 6]) {
             set_error("cloud %d holds a NaN or infinite coordinate", b);
@@ -557,29 +692,8 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         ix.K_max = std::max(ix.K_max, ix.K_host[b]);
         ix.K_total += ix.K_host[b];
     }
-    ix.K_cap = ix.K_max;
-
-    if ((rc = dev_alloc(ix.px, BN, ix.device_bytes)) || (rc = dev_alloc(ix.py, BN, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.pz, BN, ix.device_bytes)) || (rc = dev_alloc(ix.porig, BN, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.pinv, BN, ix.device_bytes)) || (rc = dev_alloc(ix.Dp, BN, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.vgeom, (size_t)B * ix.K_cap, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.vseg, (size_t)B * ix.K_cap, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.vstate, (size_t)B * ix.K_cap, ix.device_bytes)) ||
-        (rc = dev_alloc(ix.counters, NUM_COUNTERS, ix.device_bytes)))
-        return rc;
-
-    int *maxcnt = reinterpret_cast<int *>(ix.counters);   // borrowed as scratch during the build
-    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
-    k_tiles<<<gN, 256, 0, st>>>(voff.as<int>(), Kv.as<int>(), ntl.as<int>(), tbase.as<int>(), N, ix.K_cap, ix.vseg);
-    k_gather<<<gN, 256, 0, st>>>(points, vin, N, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
-    k_sphere<<<dim3((ix.K_cap + 7) / 8, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, N, ix.K_cap, ix.vgeom,
-                                                          maxcnt);
-    RFPS_CUDA(cudaGetLastError());
-    RFPS_CUDA(cudaMemcpyAsync(&ix.max_voxel_points, maxcnt, sizeof(int), cudaMemcpyDeviceToHost, st));
-    RFPS_CUDA(cudaStreamSynchronize(st));
-    RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
     ix.build_launches = g_launches;
-    return (o.flags & FPS_FLAG_PER_PICK) ? choose_launch_shape(ix, o) : choose_batched_shape(ix, o);
+    return per_pick ? choose_launch_shape(ix, o) : choose_batched_shape(ix, o);
 }
 
 }  // namespace rfps

@@ -46,6 +46,9 @@ struct DeviceIndex {
     int32_t B = 0, N = 0;
     int32_t n_vox = 0, tile_points = 0;
     int32_t K_max = 0, K_cap = 0;       // largest per-cloud K; per-cloud stride of the voxel arrays
+    int32_t G_cap = 0;                  // per-cloud stride of the group array (K_cap / 32)
+    void *arena = nullptr;              // the ONE device allocation behind every pointer below
+    bool arena_pooled = false;          // allocated from the library's stream-ordered pool
     int64_t K_total = 0;
     int32_t max_voxel_points = 0;
     int32_t cluster_size = 0, block_threads = 0, vpt = 0;   // sampling-kernel launch shape
@@ -59,6 +62,7 @@ struct DeviceIndex {
     float *Dp = nullptr;                // Dist_p
     // voxel arrays, [B][K_cap]
     float4 *vgeom = nullptr;
+    float4 *ggeom = nullptr;            // [B][G_cap] spheres around groups of 32 consecutive voxels
     int2 *vseg = nullptr;
     uint4 *vstate = nullptr;
     int32_t *K_dev = nullptr;           // [B]
@@ -71,6 +75,9 @@ struct DeviceIndex {
 
 int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o);
 void free_index(DeviceIndex &ix);
+// stream-ordered device memory from the library's private pool (falls back to cudaMalloc/cudaFree)
+cudaError_t dev_alloc_async(void **p, size_t bytes, cudaStream_t stream);
+void dev_free_async(void *p, cudaStream_t stream);
 int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
                   cudaStream_t stream);
 int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o);

@@ -46,10 +46,10 @@ struct BatchParams {
     const float *px, *py, *pz;
     const int *porig, *pinv;
     float *Dp;
-    const float4 *vgeom;
+    const float4 *vgeom, *ggeom;
     const int2 *vseg;
     const int *K;
-    int N, K_cap, Kc_cap, M, start_idx;
+    int N, K_cap, G_cap, Kc_cap, M, start_idx;     // Kc_cap: voxel slots per CTA (a multiple of 32)
     int *out_idx;
     float *out_mind;
     unsigned long long *counters;
@@ -63,17 +63,18 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
 
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_N };
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, vst, queue, bpick, cand, ctl, wbest, lslot, qn, total;
+    size_t geom, ggeom, vst, queue, bpick, cand, ctl, wbest, lslot, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
     SmemLayout L;
     size_t o = 0;
     L.geom = o;  o += sizeof(float4) * (size_t)Kc_cap;
+    L.ggeom = o; o += sizeof(float4) * (size_t)(Kc_cap / 32);
     L.vst = o;   o += sizeof(uint4) * (size_t)Kc_cap;
     L.bpick = o; o += sizeof(float4) * PB;
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
@@ -225,8 +226,10 @@ __device__ __forceinline__ void local_fps(const float *cX, const float *cY, cons
 }
 
 // ---------------------------------------------------------------------------------------------
-// the kernel: one cluster per cloud; CTA `rank` owns the voxels k = rank + C*kl (round-robin, so
-// that dense regions of the cloud are spread over the CTAs)
+// the kernel: one cluster per cloud.  32 consecutive (Morton-ordered) voxels form a group with its
+// own bounding sphere; CTA `rank` owns the groups g = rank + C*gl (round-robin, so that dense
+// regions of the cloud are spread over the CTAs); local voxel slot kl = 32*gl + l is voxel
+// k = 32*g + l.
 // ---------------------------------------------------------------------------------------------
 template <int CPT, int LW, bool STATS>
 __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, const int flags)
@@ -243,6 +246,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 
     const SmemLayout L = smem_layout(P.Kc_cap, TC, LW);
     float4 *sgeom = reinterpret_cast<float4 *>(smem_raw + L.geom);    // [Kc] {cx, cy, cz, R}
+    float4 *sggeom = reinterpret_cast<float4 *>(smem_raw + L.ggeom);  // [Gc] group spheres
     uint4 *vst = reinterpret_cast<uint4 *>(smem_raw + L.vst);         // [Kc] {Dv bits, ~orig, pos, thr bits}
     float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
     float *cX = reinterpret_cast<float *>(smem_raw + L.cand), *cY = cX + TC, *cZ = cY + TC, *cD = cZ + TC;
@@ -260,18 +264,25 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     const int *__restrict__ porig = P.porig + po;
     float *Dp = P.Dp + po;
     const float4 *__restrict__ vgeom = P.vgeom + vo;
+    const float4 *__restrict__ ggeom = P.ggeom + (size_t)b * P.G_cap;
     const int2 *__restrict__ vseg = P.vseg + vo;
     int *out_idx = P.out_idx + (size_t)b * P.M;
     float *out_mind = P.out_mind + (size_t)b * P.M;
     const int K = P.K[b];
-    const int Kc = K > rank ? (K - rank + C - 1) / C : 0;     // voxels owned by this CTA
+    const int G = (K + 31) / 32;
+    const int Gc = G > rank ? (G - rank + C - 1) / C : 0;     // groups owned by this CTA
+    const int Kc = Gc * 32;                                   // voxel slots of this CTA (some may be empty)
+#define RFPS_VOXEL_OF(kl) ((rank + C * ((kl) >> 5)) * 32 + ((kl) & 31))
 
     // ---- a7: state reset.  Thresholds = NaN: nothing can be pruned by the first pick, which therefore
     // performs the paper's "initial update" (Eq. 13-14).  Dist_p = +inf on this CTA's slice. ----
     for (int kl = tid; kl < Kc; kl += BT) {
-        sgeom[kl] = vgeom[rank + C * kl];
-        vst[kl] = make_uint4(0u, 0u, 0u, F32_NAN_BITS);
+        const int k = RFPS_VOXEL_OF(kl);
+        sgeom[kl] = k < K ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        // empty slot: threshold 0 ("d2 >= 0" always prunes) and key (0,0), below every real key
+        vst[kl] = make_uint4(0u, 0u, 0u, k < K ? F32_NAN_BITS : 0u);
     }
+    for (int gl = tid; gl < Gc; gl += BT) sggeom[gl] = ggeom[rank + C * gl];
     {
         const int chunk = (P.N + C - 1) / C;
         const int p0 = min(P.N, rank * chunk), p1 = min(P.N, p0 + chunk);
@@ -296,7 +307,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned qpar = 0u;
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
-                       c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0;
+                       c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0;
     long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
     cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
 
@@ -307,22 +318,38 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         // =====================================================================================
         for (int sub = 0; sub < nb; sub += 32) {
             const int nsub = min(32, nb - sub);
-            // ---- a9: radius prune (Eq. 25) of the voxels this thread owns against the 32 picks ----
-            for (int base = 0; base < Kc; base += BT) {
-                const int kl = base + tid;
+            // ---- a9: radius prune (Eq. 25), two levels.  One warp per group: lane i tests pick i against
+            // the group sphere (Dist_v := max over the group's voxels); then lane l tests voxel l against
+            // the picks that survived the group test. ----
+            for (int gl = warp; gl < Gc; gl += NW) {
+                const int kl = gl * 32 + lane;
+                const uint4 vs = vst[kl];
+                const float4 gm = sgeom[kl];
+                const bool valid = RFPS_VOXEL_OF(kl) < K;
                 unsigned mask = 0u;
-                if (kl < Kc) {
-                    if (no_prune) mask = nsub == 32 ? FULL : ((1u << nsub) - 1u);
-                    else {
-                        const float4 gm = sgeom[kl];
-                        const float thr = __uint_as_float(vst[kl].w);
-                        for (int i = 0; i < nsub; ++i) {
-                            const float4 s = bpick[sub + i];
-                            const float d2c = d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z);
-                            if (!(d2c >= thr)) mask |= 1u << i;
-                        }
+                if (no_prune) {
+                    mask = valid ? (nsub == 32 ? FULL : ((1u << nsub) - 1u)) : 0u;
+                    if (STATS && valid) c_vtest += nsub;
+                } else {
+                    const float thr = __uint_as_float(vs.w);
+                    const unsigned dvg = __reduce_max_sync(FULL, vs.x);
+                    const bool fresh = __any_sync(FULL, thr != thr);          // a voxel not visited yet (NaN)
+                    const float4 gg = sggeom[gl];
+                    const float thr_g = fresh ? __uint_as_float(F32_NAN_BITS) : prune_threshold(dvg, gg.w);
+                    bool gs = false;
+                    if (lane < nsub) {
+                        const float4 s = bpick[sub + lane];
+                        gs = !(d2_rn(gg.x, gg.y, gg.z, s.x, s.y, s.z) >= thr_g);
                     }
-                    if (STATS) c_vtest += nsub;
+                    unsigned gmask = __ballot_sync(FULL, gs);
+                    if (STATS && lane == 0) c_gtest += nsub;
+                    if (STATS && valid) c_vtest += __popc(gmask);
+                    while (gmask) {
+                        const int i = __ffs(gmask) - 1;
+                        gmask &= gmask - 1u;
+                        const float4 s = bpick[sub + i];
+                        if (!(d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z) >= thr)) mask |= 1u << i;
+                    }
                 }
                 const unsigned bal = __ballot_sync(FULL, mask != 0u);
                 if (bal) {
@@ -340,7 +367,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 const int2 e = queue[qi];
                 const int kl = e.x;
                 const unsigned mask = (unsigned)e.y;
-                const int2 sg = vseg[rank + C * kl];
+                const int2 sg = vseg[RFPS_VOXEL_OF(kl)];
                 const float R = sgeom[kl].w;
                 float bestD = -1.0f;
                 unsigned bestO = 0u;
@@ -450,7 +477,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 const int nq = qn[qpar];
                 if (tid == 0) qn[qpar ^ 1u] = 0;
                 for (int qi = warp; qi < nq; qi += NW) {
-                    const int2 sg = vseg[rank + C * queue[qi].x];
+                    const int2 sg = vseg[RFPS_VOXEL_OF(queue[qi].x)];
                     if (STATS && lane == 0) c_xvox++;
                     for (int p0 = sg.x; p0 < sg.x + sg.y; p0 += 32) {
                         const int p = p0 + lane;
@@ -539,6 +566,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         atomicAdd(P.counters + CNT_EFF, c_eff);
         atomicAdd(P.counters + CNT_XVOX, c_xvox);
         atomicAdd(P.counters + CNT_XPTS, c_xpts);
+        atomicAdd(P.counters + CNT_GTEST, c_gtest);
         if (tid == 0 && rank == 0) {
             atomicAdd(P.counters + CNT_ROUNDS, c_rounds);
             atomicAdd(P.counters + CNT_RETRIES, c_retries);
@@ -551,6 +579,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         }
     }
     cluster_sync_all();   // no CTA may exit while a peer can still read its shared memory
+#undef RFPS_VOXEL_OF
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -597,14 +626,16 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     if (o.block_threads != 0 && o.block_threads != BT) { set_error("block_threads=%d: the batched kernel runs %d threads per CTA", o.block_threads, BT); return FPS_ERR_INVALID; }
     const int K = ix.K_max > 0 ? ix.K_max : 1;
     const int TC = CPT * LW * 32;
-    auto fits = [&](int c) { return smem_layout((K + c - 1) / c, TC, LW).total <= (size_t)kMaxSmem; };
+    const int G = (K + 31) / 32;
+    auto slots = [&](int c) { return 32 * ((G + c - 1) / c); };     // voxel slots per CTA
+    auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= (size_t)kMaxSmem; };
     if (C == 0) {
         C = 1;
         while (C < 16 && (long long)C * 2 * ix.B <= 148 && (long long)ix.N > (long long)C * 2048) C *= 2;
         while (C < 16 && !fits(C)) C *= 2;
         // all B clusters should be resident at once (a cluster lives inside one GPC, so fewer clusters
         // fit than 148 / C suggests); otherwise the clouds run in waves
-        while (C > 1 && fits(C / 2) && max_resident_clusters(C, smem_layout((K + C - 1) / C, TC, LW).total) < std::min(ix.B, 148 / C))
+        while (C > 1 && fits(C / 2) && max_resident_clusters(C, smem_layout(slots(C), TC, LW).total) < std::min(ix.B, 148 / C))
             C /= 2;
     }
     if (!fits(C)) {
@@ -616,7 +647,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     ix.vpt = 0;
     ix.local_warps = LW;
     ix.cand_per_thread = CPT;
-    ix.Kc_cap = (K + C - 1) / C;
+    ix.Kc_cap = slots(C);
     return FPS_OK;
 }
 
@@ -658,9 +689,9 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t
     bp.px = ix.px; bp.py = ix.py; bp.pz = ix.pz;
     bp.porig = ix.porig; bp.pinv = ix.pinv;
     bp.Dp = ix.Dp;
-    bp.vgeom = ix.vgeom; bp.vseg = ix.vseg;
+    bp.vgeom = ix.vgeom; bp.ggeom = ix.ggeom; bp.vseg = ix.vseg;
     bp.K = ix.K_dev;
-    bp.N = ix.N; bp.K_cap = ix.K_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
+    bp.N = ix.N; bp.K_cap = ix.K_cap; bp.G_cap = ix.G_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
     bp.out_idx = out_idx; bp.out_mind = out_mindist;
     bp.counters = ix.counters;
     if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));

@@ -157,11 +157,19 @@ def test_ablations_and_stats_are_bit_identical(rf, flags, kernel):
         assert st["iterations"] == M - 1
         if kernel == "per_pick":
             applied = M - 1                                      # every voxel is tested against every pick
+            assert st["voxel_tests"] == st["K_total"] * applied
         else:
-            # ... except the picks of the last batch, which nothing needs to be updated for
-            applied = st["voxel_tests"] // st["K_total"]
-            assert st["voxel_tests"] == st["K_total"] * applied and M - 1 - 1024 <= applied <= M - 1
-        assert st["voxel_tests"] == st["K_total"] * applied
+            # the picks of the last batch are never applied (nothing needs them); the prune runs on
+            # groups of 32 voxels first, voxels are only tested where their group survived
+            if flags & rf.FPS_FLAG_NO_PRUNE:
+                applied = st["voxel_tests"] // st["K_total"]
+                assert st["voxel_tests"] == st["K_total"] * applied and st["group_tests"] == 0
+            else:
+                G = (st["K_total"] + 31) // 32
+                applied = st["group_tests"] // G
+                assert st["group_tests"] == G * applied
+                assert 0 < st["voxel_tests"] < st["K_total"] * applied
+            assert M - 1 - 1024 <= applied <= M - 1
         if flags & rf.FPS_FLAG_NO_PRUNE:
             if kernel == "per_pick":
                 assert st["voxels_visited"] == st["K_total"] * applied
