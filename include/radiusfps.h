@@ -102,6 +102,10 @@ typedef struct {
                                  by thread 0 of each cloud's first CTA, summed over clouds             */
     int64_t group_tests;      /* (group of 32 voxels, pick) prune tests; voxel_tests then counts only the
                                  pairs whose group survived                                           */
+    int64_t cycles_prune_sum, cycles_visit_sum;   /* APPLY split: prune tests / point visits, SM cycles
+                                 summed over ALL CTAs                                                 */
+    int64_t cycles_prune_max, cycles_visit_max;   /* the same for the slowest CTA                       */
+    int64_t sub_batches;      /* groups of <= 32 picks applied                                        */
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
 } fps_stats;
 

@@ -40,6 +40,8 @@ class fps_stats(ctypes.Structure):
                 ("candidates", ctypes.c_int64), ("extract_voxels", ctypes.c_int64), ("extract_points", ctypes.c_int64),
                 ("cycles_apply", ctypes.c_int64), ("cycles_max", ctypes.c_int64), ("cycles_extract", ctypes.c_int64),
                 ("cycles_local", ctypes.c_int64), ("group_tests", ctypes.c_int64),
+                ("cycles_prune_sum", ctypes.c_int64), ("cycles_visit_sum", ctypes.c_int64),
+                ("cycles_prune_max", ctypes.c_int64), ("cycles_visit_max", ctypes.c_int64), ("sub_batches", ctypes.c_int64),
                 ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
 
     def as_dict(self) -> dict:

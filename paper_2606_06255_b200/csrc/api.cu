@@ -117,6 +117,10 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->cycles_apply = (int64_t)c[11]; out->cycles_max = (int64_t)c[12];
             out->cycles_extract = (int64_t)c[13]; out->cycles_local = (int64_t)c[14];
             out->group_tests = (int64_t)c[15];
+            out->cycles_prune_sum = (int64_t)c[16]; out->cycles_visit_sum = (int64_t)c[17];
+            out->cycles_prune_max = (int64_t)c[18]; out->cycles_visit_max = (int64_t)c[19];
+            out->sub_batches = (int64_t)c[20];
+            if (getenv("RFPS_DEBUG")) fprintf(stderr, "[rfps debug] max phase cycles: scan %llu cluster_sync %llu dsmem %llu\n", c[21], c[22], c[23]);
         }
     }
     return FPS_OK;

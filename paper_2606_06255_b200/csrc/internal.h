@@ -40,7 +40,7 @@ void set_error(const char *fmt, ...);
 //     thr_bits fp32 bits of the prune threshold: the voxel is pruned iff d2(s_j, c_k) >= thr
 //              (sqrt-free squared-domain form of Eq. 25 with fp32 safety margins)
 
-constexpr int NUM_COUNTERS = 16;
+constexpr int NUM_COUNTERS = 32;
 
 struct DeviceIndex {
     int32_t B = 0, N = 0;

@@ -41,6 +41,8 @@ namespace rfps {
 constexpr int BT = 512;        // threads per CTA
 constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
 constexpr int MAX_ATTEMPTS = 4;
+constexpr int SUBW = 4;        // 32-bit mask words per queued voxel
+constexpr int SUBP = 32 * SUBW;   // picks applied between two CTA barriers
 
 struct BatchParams {
     const float *px, *py, *pz;
@@ -57,17 +59,17 @@ struct BatchParams {
 
 struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is the cluster's
     unsigned ccount[MAX_ATTEMPTS];  // candidates found by extraction attempt a (may exceed TC)
-    unsigned best_hi, best_lo, best_pos, pad0;   // this CTA's best voxel key
+    unsigned best_hi, best_lo, pad3, pad0;       // this CTA's best voxel key
     int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
 };
 
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_DBG0, CNT_DBG1, CNT_DBG2, CNT_N };
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, ggeom, vst, queue, bpick, cand, ctl, wbest, lslot, qn, total;
+    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, qkl, qmask, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -75,13 +77,14 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     size_t o = 0;
     L.geom = o;  o += sizeof(float4) * (size_t)Kc_cap;
     L.ggeom = o; o += sizeof(float4) * (size_t)(Kc_cap / 32);
-    L.vst = o;   o += sizeof(uint4) * (size_t)Kc_cap;
+    L.vst = o;   o += sizeof(uint2) * (size_t)Kc_cap;
     L.bpick = o; o += sizeof(float4) * PB;
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
     L.ctl = o;   o += sizeof(Ctl);
     L.wbest = o; o += sizeof(uint4) * 32;
     L.lslot = o; o += sizeof(uint2) * 2 * 8;
-    L.queue = o; o += sizeof(int2) * (size_t)Kc_cap;
+    L.qmask = o; o += sizeof(unsigned) * SUBW * (size_t)Kc_cap;
+    L.qkl = o;   o += sizeof(int) * (size_t)Kc_cap;
     L.qn = o;    o += sizeof(int) * 4;
     L.total = o;
     return L;
@@ -247,15 +250,16 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     const SmemLayout L = smem_layout(P.Kc_cap, TC, LW);
     float4 *sgeom = reinterpret_cast<float4 *>(smem_raw + L.geom);    // [Kc] {cx, cy, cz, R}
     float4 *sggeom = reinterpret_cast<float4 *>(smem_raw + L.ggeom);  // [Gc] group spheres
-    uint4 *vst = reinterpret_cast<uint4 *>(smem_raw + L.vst);         // [Kc] {Dv bits, ~orig, pos, thr bits}
+    uint2 *vst = reinterpret_cast<uint2 *>(smem_raw + L.vst);         // [Kc] voxel key {Dist_v bits, ~orig of the point attaining it}
     float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
     float *cX = reinterpret_cast<float *>(smem_raw + L.cand), *cY = cX + TC, *cZ = cY + TC, *cD = cZ + TC;
     unsigned *cO = reinterpret_cast<unsigned *>(cD + TC);
     Ctl *ctl = reinterpret_cast<Ctl *>(smem_raw + L.ctl);
     uint4 *wbest = reinterpret_cast<uint4 *>(smem_raw + L.wbest);
     uint2 *lslot = reinterpret_cast<uint2 *>(smem_raw + L.lslot);
-    int2 *queue = reinterpret_cast<int2 *>(smem_raw + L.queue);
-    int *qn = reinterpret_cast<int *>(smem_raw + L.qn);
+    int *qkl = reinterpret_cast<int *>(smem_raw + L.qkl);             // [Kc] queued voxel slots
+    unsigned *qmask = reinterpret_cast<unsigned *>(smem_raw + L.qmask);   // [Kc][SUBW] their surviving picks
+    int *qn = reinterpret_cast<int *>(smem_raw + L.qn);               // [0..1] queue length (double-buffered), [2] pop counter
 
     const size_t po = (size_t)b * P.N, vo = (size_t)b * P.K_cap;
     const float *__restrict__ px = P.px + po;
@@ -279,8 +283,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     for (int kl = tid; kl < Kc; kl += BT) {
         const int k = RFPS_VOXEL_OF(kl);
         sgeom[kl] = k < K ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
-        // empty slot: threshold 0 ("d2 >= 0" always prunes) and key (0,0), below every real key
-        vst[kl] = make_uint4(0u, 0u, 0u, k < K ? F32_NAN_BITS : 0u);
+        // not visited yet: Dist_v = NaN, whose prune threshold is NaN ("d2 >= NaN" is false: visit).  Every
+        // voxel is visited by the first pick, so no NaN key survives round 1.  Empty slot: key (0,0), below
+        // every real key, threshold 0 ("d2 >= 0" always prunes)
+        vst[kl] = make_uint2(k < K ? F32_NAN_BITS : 0u, 0u);
     }
     for (int gl = tid; gl < Gc; gl += BT) sggeom[gl] = ggeom[rank + C * gl];
     {
@@ -290,10 +296,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
     }
     if (tid == 0) {
-        qn[0] = qn[1] = 0;
+        qn[0] = qn[1] = qn[2] = 0;
 #pragma unroll
         for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
-        ctl->best_hi = ctl->best_lo = ctl->best_pos = 0u;
+        ctl->best_hi = ctl->best_lo = 0u;
         ctl->nb = 1;
         ctl->j = 1;
         const int p = P.pinv[po + P.start_idx];
@@ -309,105 +315,146 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
                        c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0;
     long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
+    long long dbg0 = 0, dbg1 = 0, dbg2 = 0;
+    long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
     cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
 
     while (j < P.M) {
         if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
         // =====================================================================================
-        // APPLY: the nb picks in bpick[], 32 at a time
+        // APPLY: the nb picks in bpick[], SUBP (= 128) at a time.
+        //   phase A  one warp per group of 32 voxels: lane i tests picks i, i+32, .. against the group
+        //            sphere (Dist_v := max over the group's voxels), then lane l tests voxel l against
+        //            the survivors; voxels with survivors are queued with their pick mask
+        //   phase B  warps pop queued voxels (dynamic) and walk their points once for all surviving picks
         // =====================================================================================
-        for (int sub = 0; sub < nb; sub += 32) {
-            const int nsub = min(32, nb - sub);
-            // ---- a9: radius prune (Eq. 25), two levels.  One warp per group: lane i tests pick i against
-            // the group sphere (Dist_v := max over the group's voxels); then lane l tests voxel l against
-            // the picks that survived the group test. ----
+        for (int sub = 0; sub < nb; sub += SUBP) {
+            const int nsub = min(SUBP, nb - sub);
+            if (STATS && tid == 0) { ta0 = clock64(); n_subs++; }
+            // ---- a9: radius prune (Eq. 25), two levels ----
             for (int gl = warp; gl < Gc; gl += NW) {
                 const int kl = gl * 32 + lane;
-                const uint4 vs = vst[kl];
-                const float4 gm = sgeom[kl];
                 const bool valid = RFPS_VOXEL_OF(kl) < K;
-                unsigned mask = 0u;
+                unsigned mask[SUBW];
+                bool any = false;
                 if (no_prune) {
-                    mask = valid ? (nsub == 32 ? FULL : ((1u << nsub) - 1u)) : 0u;
+#pragma unroll
+                    for (int w = 0; w < SUBW; ++w) {
+                        const int n = min(32, max(0, nsub - 32 * w));
+                        mask[w] = valid ? (n == 32 ? FULL : ((1u << n) - 1u)) : 0u;
+                    }
+                    any = valid;
                     if (STATS && valid) c_vtest += nsub;
                 } else {
-                    const float thr = __uint_as_float(vs.w);
-                    const unsigned dvg = __reduce_max_sync(FULL, vs.x);
-                    const bool fresh = __any_sync(FULL, thr != thr);          // a voxel not visited yet (NaN)
+                    const uint2 vs = vst[kl];
+                    const float4 gm = sgeom[kl];
                     const float4 gg = sggeom[gl];
-                    const float thr_g = fresh ? __uint_as_float(F32_NAN_BITS) : prune_threshold(dvg, gg.w);
-                    bool gs = false;
-                    if (lane < nsub) {
-                        const float4 s = bpick[sub + lane];
-                        gs = !(d2_rn(gg.x, gg.y, gg.z, s.x, s.y, s.z) >= thr_g);
+                    // group threshold from Dist_v := max over the group (NaN bits sort above every real
+                    // value, so a group holding an unvisited voxel is never pruned)
+                    const float thr_g = prune_threshold(__reduce_max_sync(FULL, vs.x), gg.w);
+                    unsigned gmask[SUBW];
+                    unsigned gany = 0u;
+#pragma unroll
+                    for (int w = 0; w < SUBW; ++w) {
+                        bool gs = false;
+                        if (32 * w + lane < nsub) {
+                            const float4 s = bpick[sub + 32 * w + lane];
+                            gs = !(d2_rn(gg.x, gg.y, gg.z, s.x, s.y, s.z) >= thr_g);
+                        }
+                        gmask[w] = __ballot_sync(FULL, gs);
+                        gany |= gmask[w];
+                        mask[w] = 0u;
                     }
-                    unsigned gmask = __ballot_sync(FULL, gs);
+                    if (gany) {
+                        const float thr = prune_threshold(vs.x, gm.w);
+#pragma unroll
+                        for (int w = 0; w < SUBW; ++w) {
+                            unsigned gmw = gmask[w];
+                            if (STATS && valid) c_vtest += __popc(gmw);
+                            while (gmw) {
+                                const int i = __ffs(gmw) - 1;
+                                gmw &= gmw - 1u;
+                                const float4 s = bpick[sub + 32 * w + i];
+                                if (!(d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z) >= thr)) mask[w] |= 1u << i;
+                            }
+                            any |= mask[w] != 0u;
+                        }
+                    }
                     if (STATS && lane == 0) c_gtest += nsub;
-                    if (STATS && valid) c_vtest += __popc(gmask);
-                    while (gmask) {
-                        const int i = __ffs(gmask) - 1;
-                        gmask &= gmask - 1u;
-                        const float4 s = bpick[sub + i];
-                        if (!(d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z) >= thr)) mask |= 1u << i;
-                    }
                 }
-                const unsigned bal = __ballot_sync(FULL, mask != 0u);
+                const unsigned bal = __ballot_sync(FULL, any);
                 if (bal) {
                     int qb = 0;
                     if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
                     qb = __shfl_sync(FULL, qb, 0);
-                    if (mask) queue[qb + __popc(bal & lt)] = make_int2(kl, (int)mask);
+                    if (any) {
+                        const int q = qb + __popc(bal & lt);
+                        qkl[q] = kl;
+#pragma unroll
+                        for (int w = 0; w < SUBW; ++w) qmask[q * SUBW + w] = mask[w];
+                    }
                 }
             }
             __syncthreads();
             const int nq = qn[qpar];
-            if (tid == 0) qn[qpar ^ 1u] = 0;
-            // ---- a10-a12: one warp per surviving voxel: point skip, update, voxel key + threshold ----
-            for (int qi = warp; qi < nq; qi += NW) {
-                const int2 e = queue[qi];
-                const int kl = e.x;
-                const unsigned mask = (unsigned)e.y;
+            if (tid == 0) { qn[qpar ^ 1u] = 0; qn[2] = 0; }
+            if (STATS && tid == 0) { const long long t = clock64(); t_a += t - ta0; ta0 = t; }
+            __syncthreads();
+            // ---- a10-a12: point skip, update, voxel key + threshold; one warp per queued voxel ----
+            for (;;) {
+                int qi = 0;
+                if (lane == 0) qi = atomicAdd(&qn[2], 1);
+                qi = __shfl_sync(FULL, qi, 0);
+                if (qi >= nq) break;
+                const int kl = qkl[qi];
+                unsigned vmask[SUBW];
+#pragma unroll
+                for (int w = 0; w < SUBW; ++w) vmask[w] = qmask[qi * SUBW + w];
                 const int2 sg = vseg[RFPS_VOXEL_OF(kl)];
-                const float R = sgeom[kl].w;
                 float bestD = -1.0f;
                 unsigned bestO = 0u;
-                int bestP = 0;
+                int npk = 0;
+#pragma unroll
+                for (int w = 0; w < SUBW; ++w) npk += __popc(vmask[w]);
                 for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) {
                     const float x = px[p], y = py[p], z = pz[p];
                     const unsigned o = ~(unsigned)porig[p];
                     const float D0 = Dp[p];
                     float D = D0;
-                    unsigned m = mask;
-                    while (m) {
-                        const int i = __ffs(m) - 1;
-                        m &= m - 1u;
-                        const float4 s = bpick[sub + i];
-                        const float dx = __fsub_rn(x, s.x), dy = __fsub_rn(y, s.y), dz = __fsub_rn(z, s.z);
-                        const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                        if (no_skip || !(dx2 >= D || dy2 >= D || dz2 >= D)) {     // Eq. 28, squared domain
-                            const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
-                            if (STATS) c_pcomp++;
-                            if (d < D) {                                          // Eq. 29 / Eq. 2 (strict)
-                                D = d;
-                                if (STATS) c_eff++;
+#pragma unroll
+                    for (int w = 0; w < SUBW; ++w) {
+                        unsigned m = vmask[w];
+                        while (m) {
+                            const int i = __ffs(m) - 1;
+                            m &= m - 1u;
+                            const float4 s = bpick[sub + 32 * w + i];
+                            const float dx = __fsub_rn(x, s.x), dy = __fsub_rn(y, s.y), dz = __fsub_rn(z, s.z);
+                            const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                            if (no_skip || !(dx2 >= D || dy2 >= D || dz2 >= D)) {     // Eq. 28, squared domain
+                                const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                                if (STATS) c_pcomp++;
+                                if (d < D) {                                          // Eq. 29 / Eq. 2 (strict)
+                                    D = d;
+                                    if (STATS) c_eff++;
+                                }
                             }
                         }
                     }
                     if (D < D0) Dp[p] = D;
-                    if (STATS) c_pvisit += __popc(mask);
-                    if (D > bestD || (D == bestD && o > bestO)) { bestD = D; bestO = o; bestP = p; }
+                    if (STATS) c_pvisit += npk;
+                    if (D > bestD || (D == bestD && o > bestO)) { bestD = D; bestO = o; }
                 }
                 const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
                 unsigned mhi, mlo;
-                const int win = warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
-                const int wpos = __shfl_sync(FULL, bestP, win);
+                warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
                 if (lane == 0) {
-                    vst[kl] = make_uint4(mhi, mlo, (unsigned)wpos, __float_as_uint(prune_threshold(mhi, R)));
+                    vst[kl] = make_uint2(mhi, mlo);
                     if (STATS) c_vvisit++;
                 }
             }
             __syncthreads();
             qpar ^= 1u;
+            if (STATS && tid == 0) t_b += clock64() - ta0;
         }
 
         if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_apply += t1 - t0; t0 = t1; }
@@ -415,40 +462,40 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
         // =====================================================================================
         {
-            unsigned bhi = 0u, blo = 0u, bpos = 0u;
+            unsigned bhi = 0u, blo = 0u;
             for (int kl = tid; kl < Kc; kl += BT) {
-                const uint4 s = vst[kl];
-                if (s.x > bhi || (s.x == bhi && s.y > blo)) { bhi = s.x; blo = s.y; bpos = s.z; }
+                const uint2 s = vst[kl];
+                if (s.x > bhi || (s.x == bhi && s.y > blo)) { bhi = s.x; blo = s.y; }
             }
             unsigned mhi, mlo;
-            const int win = warp_argmax_key(bhi, blo, mhi, mlo);
-            const unsigned wpos = __shfl_sync(FULL, bpos, win);
-            if (lane == 0) wbest[warp] = make_uint4(mhi, mlo, wpos, 0u);
+            warp_argmax_key(bhi, blo, mhi, mlo);
+            if (lane == 0) wbest[warp] = make_uint4(mhi, mlo, 0u, 0u);
         }
         __syncthreads();
         if (warp == 0) {
             const uint4 wb = lane < NW ? wbest[lane] : make_uint4(0u, 0u, 0u, 0u);
             unsigned chi, clo;
-            const int win = warp_argmax_key(wb.x, wb.y, chi, clo);
-            const unsigned cpos = __shfl_sync(FULL, wb.z, win);
+            warp_argmax_key(wb.x, wb.y, chi, clo);
             if (lane == 0) {
-                ctl->best_hi = chi; ctl->best_lo = clo; ctl->best_pos = cpos;
+                ctl->best_hi = chi; ctl->best_lo = clo;
                 if (rank == 0) {
 #pragma unroll
                     for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
                 }
             }
         }
+        long long tm1 = 0, tm2 = 0;
+        if (STATS && tid == 0 && rank == 0) tm1 = clock64();
         cluster_sync_all();
-        unsigned ghi, glo, gpos;
+        if (STATS && tid == 0 && rank == 0) tm2 = clock64();
+        unsigned ghi, glo;
         {
             uint4 rb = make_uint4(0u, 0u, 0u, 0u);
             if (lane < C) rb = ld_dsmem_v4(mapa(smem_u32(&ctl->best_hi), (unsigned)lane));
-            const int win = warp_argmax_key(rb.x, rb.y, ghi, glo);
-            gpos = __shfl_sync(FULL, rb.z, win);
+            warp_argmax_key(rb.x, rb.y, ghi, glo);
         }
 
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; dbg0 += tm1 - t0; dbg1 += tm2 - tm1; dbg2 += t1 - tm2; t0 = t1; }
         // =====================================================================================
         // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
         // =====================================================================================
@@ -464,20 +511,25 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[a]), 0u);
                 for (int base = 0; base < Kc; base += BT) {
                     const int kl = base + tid;
-                    const bool hit = kl < Kc && vst[kl].x > tb;
+                    const bool hit = kl < Kc && vst[kl].x > tb;          // empty slots hold 0
                     const unsigned bal = __ballot_sync(FULL, hit);
                     if (bal) {
                         int qb = 0;
                         if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
                         qb = __shfl_sync(FULL, qb, 0);
-                        if (hit) queue[qb + __popc(bal & lt)] = make_int2(kl, 0);
+                        if (hit) qkl[qb + __popc(bal & lt)] = kl;
                     }
                 }
                 __syncthreads();
                 const int nq = qn[qpar];
-                if (tid == 0) qn[qpar ^ 1u] = 0;
-                for (int qi = warp; qi < nq; qi += NW) {
-                    const int2 sg = vseg[RFPS_VOXEL_OF(queue[qi].x)];
+                if (tid == 0) { qn[qpar ^ 1u] = 0; qn[2] = 0; }
+                __syncthreads();
+                for (;;) {
+                    int qi = 0;
+                    if (lane == 0) qi = atomicAdd(&qn[2], 1);
+                    qi = __shfl_sync(FULL, qi, 0);
+                    if (qi >= nq) break;
+                    const int2 sg = vseg[RFPS_VOXEL_OF(qkl[qi])];
                     if (STATS && lane == 0) c_xvox++;
                     for (int p0 = sg.x; p0 < sg.x + sg.y; p0 += 32) {
                         const int p = p0 + lane;
@@ -526,6 +578,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 if (tid == 0) {
                     out_idx[j] = (int)(~glo);
                     out_mind[j] = __uint_as_float(ghi);
+                    const int gpos = P.pinv[po + (size_t)(~glo)];
                     bpick[0] = make_float4(px[gpos], py[gpos], pz[gpos], 0.0f);
                     ctl->nb = 1;
                     ctl->j = j + 1;
@@ -567,7 +620,17 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         atomicAdd(P.counters + CNT_XVOX, c_xvox);
         atomicAdd(P.counters + CNT_XPTS, c_xpts);
         atomicAdd(P.counters + CNT_GTEST, c_gtest);
+        if (tid == 0) {
+            atomicAdd(P.counters + CNT_CYC_A_SUM, (unsigned long long)t_a);
+            atomicAdd(P.counters + CNT_CYC_B_SUM, (unsigned long long)t_b);
+            atomicMax(P.counters + CNT_CYC_A_MAX, (unsigned long long)t_a);
+            atomicMax(P.counters + CNT_CYC_B_MAX, (unsigned long long)t_b);
+        }
         if (tid == 0 && rank == 0) {
+            atomicAdd(P.counters + CNT_SUBS, (unsigned long long)n_subs);
+            atomicAdd(P.counters + CNT_DBG0, (unsigned long long)dbg0);
+            atomicAdd(P.counters + CNT_DBG1, (unsigned long long)dbg1);
+            atomicAdd(P.counters + CNT_DBG2, (unsigned long long)dbg2);
             atomicAdd(P.counters + CNT_ROUNDS, c_rounds);
             atomicAdd(P.counters + CNT_RETRIES, c_retries);
             atomicAdd(P.counters + CNT_SINGLES, c_singles);
