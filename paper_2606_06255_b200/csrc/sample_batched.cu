@@ -69,7 +69,7 @@ enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CN
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, qkl, qmask, qn, total;
+    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, qkl, qmask, qbits, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -85,6 +85,7 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.lslot = o; o += sizeof(uint2) * 2 * 8;
     L.qmask = o; o += sizeof(unsigned) * SUBW * (size_t)Kc_cap;
     L.qkl = o;   o += sizeof(int) * (size_t)Kc_cap;
+    L.qbits = o; o += sizeof(unsigned) * (size_t)(Kc_cap / 32);
     L.qn = o;    o += sizeof(int) * 4;
     L.total = o;
     return L;
@@ -258,7 +259,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     uint4 *wbest = reinterpret_cast<uint4 *>(smem_raw + L.wbest);
     uint2 *lslot = reinterpret_cast<uint2 *>(smem_raw + L.lslot);
     int *qkl = reinterpret_cast<int *>(smem_raw + L.qkl);             // [Kc] queued voxel slots
-    unsigned *qmask = reinterpret_cast<unsigned *>(smem_raw + L.qmask);   // [Kc][SUBW] their surviving picks
+    unsigned *qmask = reinterpret_cast<unsigned *>(smem_raw + L.qmask);   // [Kc][SUBW] surviving picks per voxel slot (zero when not queued)
+    unsigned *qbits = reinterpret_cast<unsigned *>(smem_raw + L.qbits);   // [Gc] voxel-slot-already-queued bits
     int *qn = reinterpret_cast<int *>(smem_raw + L.qn);               // [0..1] queue length (double-buffered), [2] pop counter
 
     const size_t po = (size_t)b * P.N, vo = (size_t)b * P.K_cap;
@@ -288,7 +290,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         // every real key, threshold 0 ("d2 >= 0" always prunes)
         vst[kl] = make_uint2(k < K ? F32_NAN_BITS : 0u, 0u);
     }
-    for (int gl = tid; gl < Gc; gl += BT) sggeom[gl] = ggeom[rank + C * gl];
+    for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[rank + C * gl]; qbits[gl] = 0u; }
+    for (int i = tid; i < Kc * SUBW; i += BT) qmask[i] = 0u;
     {
         const int chunk = (P.N + C - 1) / C;
         const int p0 = min(P.N, rank * chunk), p1 = min(P.N, p0 + chunk);
@@ -331,73 +334,63 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         for (int sub = 0; sub < nb; sub += SUBP) {
             const int nsub = min(SUBP, nb - sub);
             if (STATS && tid == 0) { ta0 = clock64(); n_subs++; }
-            // ---- a9: radius prune (Eq. 25), two levels ----
-            for (int gl = warp; gl < Gc; gl += NW) {
+            // ---- a9: radius prune (Eq. 25), two levels.  Work unit = (group, word of 32 picks), spread over
+            // the warps so that a group whose sphere prunes badly does not serialise on one warp ----
+            const int nw = (nsub + 31) >> 5;
+            for (int u = warp; u < Gc * nw; u += NW) {
+                const int gl = u / nw, w = u - gl * nw;
                 const int kl = gl * 32 + lane;
                 const bool valid = RFPS_VOXEL_OF(kl) < K;
-                unsigned mask[SUBW];
-                bool any = false;
+                const int n = min(32, nsub - 32 * w);
+                unsigned mask = 0u;
                 if (no_prune) {
-#pragma unroll
-                    for (int w = 0; w < SUBW; ++w) {
-                        const int n = min(32, max(0, nsub - 32 * w));
-                        mask[w] = valid ? (n == 32 ? FULL : ((1u << n) - 1u)) : 0u;
-                    }
-                    any = valid;
-                    if (STATS && valid) c_vtest += nsub;
+                    mask = valid ? (n == 32 ? FULL : ((1u << n) - 1u)) : 0u;
+                    if (STATS && valid) c_vtest += n;
                 } else {
                     const uint2 vs = vst[kl];
-                    const float4 gm = sgeom[kl];
                     const float4 gg = sggeom[gl];
                     // group threshold from Dist_v := max over the group (NaN bits sort above every real
                     // value, so a group holding an unvisited voxel is never pruned)
                     const float thr_g = prune_threshold(__reduce_max_sync(FULL, vs.x), gg.w);
-                    unsigned gmask[SUBW];
-                    unsigned gany = 0u;
-#pragma unroll
-                    for (int w = 0; w < SUBW; ++w) {
-                        bool gs = false;
-                        if (32 * w + lane < nsub) {
-                            const float4 s = bpick[sub + 32 * w + lane];
-                            gs = !(d2_rn(gg.x, gg.y, gg.z, s.x, s.y, s.z) >= thr_g);
-                        }
-                        gmask[w] = __ballot_sync(FULL, gs);
-                        gany |= gmask[w];
-                        mask[w] = 0u;
+                    bool gs = false;
+                    if (lane < n) {
+                        const float4 s = bpick[sub + 32 * w + lane];
+                        gs = !(d2_rn(gg.x, gg.y, gg.z, s.x, s.y, s.z) >= thr_g);
                     }
-                    if (gany) {
+                    unsigned gmask = __ballot_sync(FULL, gs);
+                    if (STATS && lane == 0) c_gtest += n;
+                    if (gmask) {
+                        const float4 gm = sgeom[kl];
                         const float thr = prune_threshold(vs.x, gm.w);
-#pragma unroll
-                        for (int w = 0; w < SUBW; ++w) {
-                            unsigned gmw = gmask[w];
-                            if (STATS && valid) c_vtest += __popc(gmw);
-                            while (gmw) {
-                                const int i = __ffs(gmw) - 1;
-                                gmw &= gmw - 1u;
-                                const float4 s = bpick[sub + 32 * w + i];
-                                if (!(d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z) >= thr)) mask[w] |= 1u << i;
-                            }
-                            any |= mask[w] != 0u;
+                        if (STATS && valid) c_vtest += __popc(gmask);
+                        while (gmask) {
+                            const int i = __ffs(gmask) - 1;
+                            gmask &= gmask - 1u;
+                            const float4 s = bpick[sub + 32 * w + i];
+                            if (!(d2_rn(gm.x, gm.y, gm.z, s.x, s.y, s.z) >= thr)) mask |= 1u << i;
                         }
                     }
-                    if (STATS && lane == 0) c_gtest += nsub;
                 }
-                const unsigned bal = __ballot_sync(FULL, any);
+                const unsigned bal = __ballot_sync(FULL, mask != 0u);
                 if (bal) {
-                    int qb = 0;
-                    if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
-                    qb = __shfl_sync(FULL, qb, 0);
-                    if (any) {
-                        const int q = qb + __popc(bal & lt);
-                        qkl[q] = kl;
-#pragma unroll
-                        for (int w = 0; w < SUBW; ++w) qmask[q * SUBW + w] = mask[w];
+                    if (mask) qmask[kl * SUBW + w] = mask;
+                    // the first unit that finds survivors for a voxel queues it (one bit per voxel slot)
+                    unsigned old = 0u;
+                    if (lane == 0) old = atomicOr(&qbits[gl], bal);
+                    old = __shfl_sync(FULL, old, 0);
+                    const unsigned fresh = bal & ~old;
+                    if (fresh) {
+                        int qb = 0;
+                        if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(fresh));
+                        qb = __shfl_sync(FULL, qb, 0);
+                        if (fresh & (1u << lane)) qkl[qb + __popc(fresh & lt)] = kl;
                     }
                 }
             }
             __syncthreads();
             const int nq = qn[qpar];
             if (tid == 0) { qn[qpar ^ 1u] = 0; qn[2] = 0; }
+            for (int gl = tid; gl < Gc; gl += BT) qbits[gl] = 0u;
             if (STATS && tid == 0) { const long long t = clock64(); t_a += t - ta0; ta0 = t; }
             __syncthreads();
             // ---- a10-a12: point skip, update, voxel key + threshold; one warp per queued voxel ----
@@ -408,8 +401,12 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 if (qi >= nq) break;
                 const int kl = qkl[qi];
                 unsigned vmask[SUBW];
-#pragma unroll
-                for (int w = 0; w < SUBW; ++w) vmask[w] = qmask[qi * SUBW + w];
+                {
+                    const uint4 qm = *reinterpret_cast<const uint4 *>(&qmask[kl * SUBW]);
+                    vmask[0] = qm.x; vmask[1] = qm.y; vmask[2] = qm.z; vmask[3] = qm.w;
+                    __syncwarp();
+                    if (lane == 0) *reinterpret_cast<uint4 *>(&qmask[kl * SUBW]) = make_uint4(0u, 0u, 0u, 0u);   // leave it clean
+                }
                 const int2 sg = vseg[RFPS_VOXEL_OF(kl)];
                 float bestD = -1.0f;
                 unsigned bestO = 0u;
