@@ -58,9 +58,11 @@ typedef struct {
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
-    int32_t local_warps;   /* batched kernel: warps running the candidate-set FPS: 0 = choose; 1,2,4,8   */
-    int32_t cand_per_thread; /* batched kernel: candidates per thread (registers): 0 = choose; 4,8,16;
-                              candidate capacity = 32 * local_warps * cand_per_thread                   */
+    int32_t local_warps;   /* batched kernel, local phase: 0 = choose; 16 = hierarchical (all 16 warps hold
+                              candidates, one warp picks from the top <= 128 of them); 1,2,4,8 = flat FPS on
+                              that many warps                                                            */
+    int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2,4 (hierarchical) or 4,8,16
+                              (flat); candidate capacity = 32 * local_warps * cand_per_thread          */
 } fps_build_opts;
 
 enum {
@@ -105,7 +107,9 @@ typedef struct {
     int64_t cycles_prune_sum, cycles_visit_sum;   /* APPLY split: prune tests / point visits, SM cycles
                                  summed over ALL CTAs                                                 */
     int64_t cycles_prune_max, cycles_visit_max;   /* the same for the slowest CTA                       */
-    int64_t sub_batches;      /* groups of <= 32 picks applied                                        */
+    int64_t sub_batches;      /* groups of <= 128 picks applied between two CTA barriers              */
+    int64_t local_subrounds;  /* hierarchical local phase: sub-rounds (one-warp FPS runs)             */
+    int64_t local_fallbacks;  /* ... of which single block-wide argmax picks (first bin overflowed)   */
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
 } fps_stats;
 

@@ -42,6 +42,7 @@ class fps_stats(ctypes.Structure):
                 ("cycles_local", ctypes.c_int64), ("group_tests", ctypes.c_int64),
                 ("cycles_prune_sum", ctypes.c_int64), ("cycles_visit_sum", ctypes.c_int64),
                 ("cycles_prune_max", ctypes.c_int64), ("cycles_visit_max", ctypes.c_int64), ("sub_batches", ctypes.c_int64),
+                ("local_subrounds", ctypes.c_int64), ("local_fallbacks", ctypes.c_int64),
                 ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
 
     def as_dict(self) -> dict:

@@ -65,11 +65,11 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
 
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_DBG0, CNT_DBG1, CNT_DBG2, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_DBG0, CNT_DBG1, CNT_DBG2, CNT_SUBROUNDS, CNT_FALLBACK, CNT_N };
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, qkl, qmask, qbits, qn, total;
+    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -83,6 +83,7 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.ctl = o;   o += sizeof(Ctl);
     L.wbest = o; o += sizeof(uint4) * 32;
     L.lslot = o; o += sizeof(uint2) * 2 * 8;
+    L.hier = o;  o += 3392 + 8 * PB;     // sizeof(HierSmem), checked below
     L.qmask = o; o += sizeof(unsigned) * SUBW * (size_t)Kc_cap;
     L.qkl = o;   o += sizeof(int) * (size_t)Kc_cap;
     L.qbits = o; o += sizeof(unsigned) * (size_t)(Kc_cap / 32);
@@ -230,11 +231,255 @@ __device__ __forceinline__ void local_fps(const float *cX, const float *cY, cons
 }
 
 // ---------------------------------------------------------------------------------------------
+// LOCAL, hierarchical form (the default): the same exact-batching argument applied once more inside
+// the CTA.  All 16 warps keep the candidate set C1 in registers (CPT1 per thread).  A sub-round
+//   (a) finds the block maximum m1,
+//   (b) histograms the live candidates (D > tau) over 64 bins of [tau, m1] with a bin function that
+//       is monotone in D,
+//   (c) takes the longest prefix of bins holding <= T2 = 32*CPT2 candidates (B* bins),
+//   (d) moves those candidates (C2) to shared memory,
+//   (e) lets ONE warp run FPS on C2 in registers -- no barrier, vote or shuffle per pick: two redux
+//       levels and three broadcast loads -- while the maximum stays in the first B* bins, i.e. above
+//       tau2 = the largest live distance left outside C2.  Exact for the same
+//       reason as the outer level: every candidate outside C2 sits in a bin >= B* and can only move
+//       to later bins, so while the restricted maximum is in a bin < B* it is the maximum over C1,
+//       hence (outer argument) over the whole cloud; equal distances share a bin, so ties are
+//       complete inside C2 and go to the lowest original index,
+//   (f) applies the sub-round's picks to all of C1 (all warps, FADD2/FMUL2).
+// If the first bin alone overflows T2 (many equal or nearly equal distances) the sub-round is a
+// single block-wide argmax with the full tie-break.
+// ---------------------------------------------------------------------------------------------
+struct __align__(16) HierSmem {
+    uint4 wb[16];
+    float sD[128], sX[128], sY[128], sZ[128];
+    unsigned sO[128];
+    int hist[64];
+    unsigned wmax[16], wmax2[16];
+    uint2 plist[PB];               // picks of the running sub-round: {slot id in s*, D bits}
+    int cnt2, nb, j, pad;
+};
+
+template <int CPT1, int CPT2>
+__device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY, const float *cZ, const float *cD,
+                                               const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
+                                               const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
+                                               const int tid, unsigned long long &c_subrounds, unsigned long long &c_fallback)
+{
+    static_assert(CPT1 % 2 == 0 && CPT2 >= 1 && CPT2 <= 4, "shape");
+    constexpr int H1 = CPT1 / 2, T2 = 32 * CPT2;
+    const int lane = tid & 31, warp = tid >> 5;
+    const float tau = __uint_as_float(taubits);
+    f32x2 X[H1], Y[H1], Z[H1];
+    float D[CPT1];
+#pragma unroll
+    for (int h = 0; h < H1; ++h) {
+        const int i0 = (2 * h) * BT + tid, i1 = (2 * h + 1) * BT + tid;
+        const bool ok0 = i0 < cnt, ok1 = i1 < cnt;
+        X[h] = pack2(ok0 ? cX[i0] : 0.0f, ok1 ? cX[i1] : 0.0f);
+        Y[h] = pack2(ok0 ? cY[i0] : 0.0f, ok1 ? cY[i1] : 0.0f);
+        Z[h] = pack2(ok0 ? cZ[i0] : 0.0f, ok1 ? cZ[i1] : 0.0f);
+        D[2 * h] = ok0 ? cD[i0] : 0.0f;          // padding: D = 0 is never above tau
+        D[2 * h + 1] = ok1 ? cD[i1] : 0.0f;
+    }
+    int jl = j, nbl = 0, applied = 0;
+    for (;;) {
+        // ---- (a) block maximum ----
+        float m = D[0];
+#pragma unroll
+        for (int c = 1; c < CPT1; ++c) m = fmaxf(m, D[c]);
+        const unsigned wm = __reduce_max_sync(FULL, __float_as_uint(m));
+        if (lane == 0) hs->wmax[warp] = wm;
+        if (tid < 64) hs->hist[tid] = 0;
+        if (tid == 0) hs->cnt2 = 0;
+        __syncthreads();
+        const unsigned m1 = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax[lane] : 0u);
+        if (!(m1 > taubits)) break;
+        const float fm1 = __uint_as_float(m1);
+        const float scale = fminf(__fdiv_rn(64.0f, __fsub_rn(fm1, tau)), FLT_MAX);
+        // bin(d): 0 for d = m1, growing as d falls; monotone because fp32 subtraction and multiplication
+        // by a positive constant are monotone
+#define RFPS_BIN(d) ((int)fminf(__fmul_rn(__fsub_rn(fm1, (d)), scale), 63.0f))
+        // ---- (b) histogram of the live candidates ----
+#pragma unroll
+        for (int c = 0; c < CPT1; ++c)
+            if (D[c] > tau) atomicAdd(&hs->hist[RFPS_BIN(D[c])], 1);
+        __syncthreads();
+        // ---- (c) B* = number of leading bins that together hold <= T2 candidates ----
+        int bstar;
+        {
+            const int h0 = hs->hist[2 * lane], h1 = hs->hist[2 * lane + 1];
+            int incl = h0 + h1;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += t;
+            }
+            const int excl = incl - (h0 + h1);
+            bstar = __popc(__ballot_sync(FULL, excl + h0 <= T2)) + __popc(__ballot_sync(FULL, incl <= T2));
+        }
+        if (bstar == 0) {
+            // ---- fallback: one pick by a block-wide argmax with the full tie-break ----
+            unsigned o = 0u, oi = 0u;
+            if (__float_as_uint(m) == m1) {
+#pragma unroll
+                for (int c = 0; c < CPT1; ++c)
+                    if (D[c] == m) {
+                        const unsigned i = (unsigned)(c * BT + tid);
+                        const unsigned oc = cO[i];
+                        if (oc >= o) { o = oc; oi = i; }
+                    }
+            }
+            const unsigned wo = __reduce_max_sync(FULL, o);
+            const int wl = __ffs(__ballot_sync(FULL, o == wo)) - 1;
+            const unsigned widx = __shfl_sync(FULL, oi, wl);
+            if (lane == 0) hs->wb[warp] = make_uint4(wo, widx, 0u, 0u);
+            __syncthreads();
+            uint4 v = lane < BT / 32 ? hs->wb[lane] : make_uint4(0u, 0u, 0u, 0u);
+            const unsigned go = __reduce_max_sync(FULL, v.x);
+            const unsigned gidx = __shfl_sync(FULL, v.y, __ffs(__ballot_sync(FULL, v.x == go)) - 1);
+            if (tid == 0) {
+                out_idx[jl] = (int)(~go);
+                out_mind[jl] = fm1;
+                bpick[nbl] = make_float4(cX[gidx], cY[gidx], cZ[gidx], 0.0f);
+                c_fallback++;
+            }
+            ++jl;
+            ++nbl;
+            __syncthreads();
+        } else {
+            // ---- (d) C2 -> shared memory; tau2 = the largest live distance left outside C2 (>= tau), so
+            // that C2 = {D > tau2} exactly and the pick loop needs one integer compare to know when to stop ----
+            float exmax = tau;
+#pragma unroll
+            for (int c = 0; c < CPT1; ++c)
+                if (D[c] > tau) {
+                    if (RFPS_BIN(D[c]) < bstar) {
+                        const int sl = atomicAdd(&hs->cnt2, 1);
+                        const int i = c * BT + tid;
+                        hs->sD[sl] = D[c];
+                        hs->sX[sl] = cX[i];
+                        hs->sY[sl] = cY[i];
+                        hs->sZ[sl] = cZ[i];
+                        hs->sO[sl] = cO[i];
+                    } else {
+                        exmax = fmaxf(exmax, D[c]);
+                    }
+                }
+            {
+                const unsigned we = __reduce_max_sync(FULL, __float_as_uint(exmax));
+                if (lane == 0) hs->wmax2[warp] = we;
+            }
+            __syncthreads();
+            // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
+            // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
+            if (warp == 0) {
+                const int n2 = hs->cnt2;
+                const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
+                float x2[CPT2], y2[CPT2], z2[CPT2], d2v[CPT2];
+#pragma unroll
+                for (int c = 0; c < CPT2; ++c) {
+                    const int i = c * 32 + lane;
+                    const bool ok = i < n2;
+                    x2[c] = ok ? hs->sX[i] : 0.0f;
+                    y2[c] = ok ? hs->sY[i] : 0.0f;
+                    z2[c] = ok ? hs->sZ[i] : 0.0f;
+                    d2v[c] = ok ? hs->sD[i] : 0.0f;         // padding never exceeds tau2
+                }
+                // picks are logged as {slot id, D bits}: lane (n & 31) keeps pick n in registers and the warp
+                // writes 32 of them at a time, so the loop itself holds no store and no dependent load
+                const int nb0 = nbl, j0 = jl;
+                unsigned mywid = 0u, myd = 0u;
+                for (;;) {
+                    float bm = d2v[0];
+#pragma unroll
+                    for (int c = 1; c < CPT2; ++c) bm = fmaxf(bm, d2v[c]);
+                    // slot ids (+1) of this lane's candidates at its maximum: largest and smallest
+                    unsigned idmx = 0u, idmn = 0x7fffffffu;
+#pragma unroll
+                    for (int c = 0; c < CPT2; ++c)
+                        if (d2v[c] == bm) { idmx = max(idmx, (unsigned)(c * 32 + lane + 1)); idmn = min(idmn, (unsigned)(c * 32 + lane + 1)); }
+                    const unsigned hi = __float_as_uint(bm);
+                    const unsigned ghi = __reduce_max_sync(FULL, hi);
+                    if (!(ghi > tau2bits)) break;            // restricted max no longer above everything outside C2
+                    const bool top = hi == ghi;
+                    const unsigned gmx = __reduce_max_sync(FULL, top ? idmx : 0u);
+                    const unsigned gmn = __reduce_min_sync(FULL, top ? idmn : 0x7fffffffu);
+                    unsigned wid = gmx - 1u;
+                    if (gmx != gmn) {                        // exact tie: lowest original index wins
+                        unsigned lo = 0u;
+                        if (top) {
+#pragma unroll
+                            for (int c = 0; c < CPT2; ++c)
+                                if (d2v[c] == bm) lo = max(lo, hs->sO[c * 32 + lane]);
+                        }
+                        const unsigned glo = __reduce_max_sync(FULL, lo);
+                        unsigned mine = 0u;
+                        if (top) {
+#pragma unroll
+                            for (int c = 0; c < CPT2; ++c)
+                                if (d2v[c] == bm && hs->sO[c * 32 + lane] == glo) mine = (unsigned)(c * 32 + lane + 1);
+                        }
+                        wid = __reduce_max_sync(FULL, mine) - 1u;
+                    }
+                    const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
+                    const int n = nbl - nb0;
+                    if (lane == (n & 31)) { mywid = wid; myd = ghi; }
+                    ++jl;
+                    ++nbl;
+                    if ((n & 31) == 31) hs->plist[n - 31 + lane] = make_uint2(mywid, myd);
+                    if (jl >= M || nbl >= PB) break;
+#pragma unroll
+                    for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], d2_rn(x2[c], y2[c], z2[c], sx, sy, sz));
+                }
+                {
+                    const int n = nbl - nb0;                 // flush the partial last group, then emit
+                    if ((n & 31) != 0 && lane < (n & 31)) hs->plist[(n & ~31) + lane] = make_uint2(mywid, myd);
+                    __syncwarp();
+                    for (int i = lane; i < n; i += 32) {
+                        const uint2 pk = hs->plist[i];
+                        out_idx[j0 + i] = (int)(~hs->sO[pk.x]);
+                        out_mind[j0 + i] = __uint_as_float(pk.y);
+                        bpick[nb0 + i] = make_float4(hs->sX[pk.x], hs->sY[pk.x], hs->sZ[pk.x], 0.0f);
+                    }
+                }
+                if (lane == 0) { hs->nb = nbl; hs->j = jl; }
+            }
+            __syncthreads();
+            nbl = hs->nb;
+            jl = hs->j;
+        }
+#undef RFPS_BIN
+        c_subrounds++;
+        // ---- (f) the sub-round's picks -> all of C1 ----
+        for (int i = applied; i < nbl; ++i) {
+            const float4 s = bpick[i];
+            const f32x2 SX = pack2(s.x, s.x), SY = pack2(s.y, s.y), SZ = pack2(s.z, s.z);
+#pragma unroll
+            for (int h = 0; h < H1; ++h) {
+                const f32x2 dx = sub2(X[h], SX), dy = sub2(Y[h], SY), dz = sub2(Z[h], SZ);
+                float x0, x1, y0, y1, z0, z1;
+                unpack2(mul2(dx, dx), x0, x1);
+                unpack2(mul2(dy, dy), y0, y1);
+                unpack2(mul2(dz, dz), z0, z1);
+                D[2 * h] = fminf(D[2 * h], __fadd_rn(__fadd_rn(x0, y0), z0));
+                D[2 * h + 1] = fminf(D[2 * h + 1], __fadd_rn(__fadd_rn(x1, y1), z1));
+            }
+        }
+        applied = nbl;
+        if (jl >= M || nbl >= PB) break;
+    }
+    j = jl;
+    nb = nbl;
+}
+
+// ---------------------------------------------------------------------------------------------
 // the kernel: one cluster per cloud.  32 consecutive (Morton-ordered) voxels form a group with its
 // own bounding sphere; CTA `rank` owns the groups g = rank + C*gl (round-robin, so that dense
 // regions of the cloud are spread over the CTAs); local voxel slot kl = 32*gl + l is voxel
 // k = 32*g + l.
 // ---------------------------------------------------------------------------------------------
+static_assert(sizeof(HierSmem) <= 3392 + 8 * PB, "smem_layout reserves this much for HierSmem");
+
 template <int CPT, int LW, bool STATS>
 __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, const int flags)
 {
@@ -258,6 +503,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     Ctl *ctl = reinterpret_cast<Ctl *>(smem_raw + L.ctl);
     uint4 *wbest = reinterpret_cast<uint4 *>(smem_raw + L.wbest);
     uint2 *lslot = reinterpret_cast<uint2 *>(smem_raw + L.lslot);
+    HierSmem *hs = reinterpret_cast<HierSmem *>(smem_raw + L.hier);
     int *qkl = reinterpret_cast<int *>(smem_raw + L.qkl);             // [Kc] queued voxel slots
     unsigned *qmask = reinterpret_cast<unsigned *>(smem_raw + L.qmask);   // [Kc][SUBW] surviving picks per voxel slot (zero when not queued)
     unsigned *qbits = reinterpret_cast<unsigned *>(smem_raw + L.qbits);   // [Gc] voxel-slot-already-queued bits
@@ -316,7 +562,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned qpar = 0u;
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
-                       c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0;
+                       c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0, c_subrounds = 0, c_fallback = 0;
     long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
     long long dbg0 = 0, dbg1 = 0, dbg2 = 0;
     long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
@@ -581,7 +827,17 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     ctl->j = j + 1;
                     if (STATS) c_singles++;
                 }
-            } else if (warp < LW) {
+            } else if constexpr (LW == BT / 32) {
+                int lj = j, lnb = 0;
+                local_fps_hier<CPT, 4>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
+                                       c_subrounds, c_fallback);
+                if (tid == 0) {
+                    ctl->nb = lnb;
+                    ctl->j = lj;
+                    if (STATS) c_cands += (unsigned long long)cnt;
+                }
+            } else if constexpr (LW < BT / 32) {
+              if (warp < LW) {
                 int lj = j, lnb = 0;
                 local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, lslot, bpick, out_idx, out_mind, tid);
                 if (tid == 0) {
@@ -589,6 +845,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     ctl->j = lj;
                     if (STATS) c_cands += (unsigned long long)cnt;
                 }
+              }
             }
         }
         cluster_sync_all();
@@ -625,6 +882,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         }
         if (tid == 0 && rank == 0) {
             atomicAdd(P.counters + CNT_SUBS, (unsigned long long)n_subs);
+            atomicAdd(P.counters + CNT_SUBROUNDS, c_subrounds);
+            atomicAdd(P.counters + CNT_FALLBACK, c_fallback);
             atomicAdd(P.counters + CNT_DBG0, (unsigned long long)dbg0);
             atomicAdd(P.counters + CNT_DBG1, (unsigned long long)dbg1);
             atomicAdd(P.counters + CNT_DBG2, (unsigned long long)dbg2);
@@ -653,7 +912,7 @@ __global__ void k_fps_batched(const BatchParams P, const int flags);
 // how many clusters of `c` CTAs of the default kernel can be resident at once (0 on error)
 static int max_resident_clusters(int c, size_t smem)
 {
-    auto kern = k_fps_batched<8, 4, false>;
+    auto kern = k_fps_batched<2, 16, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
     cudaLaunchConfig_t cfg;
@@ -675,10 +934,13 @@ static int max_resident_clusters(int c, size_t smem)
 
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
 {
-    int LW = o.local_warps > 0 ? o.local_warps : 4;
-    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : 8;
-    if (!((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16))) {
-        set_error("local_warps=%d must be 1,2,4,8 and cand_per_thread=%d must be 4,8,16", LW, CPT);
+    // local_warps = 16: hierarchical local phase (all warps hold candidates, one warp picks);
+    // 1..8: flat local phase on that many warps
+    int LW = o.local_warps > 0 ? o.local_warps : 16;
+    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW == 16 ? 2 : 8);
+    const bool ok_shape = LW == 16 ? (CPT == 2 || CPT == 4) : ((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16));
+    if (!ok_shape) {
+        set_error("local_warps=%d / cand_per_thread=%d: use 16 with 2 or 4 (hierarchical), or 1,2,4,8 with 4,8,16 (flat)", LW, CPT);
         return FPS_ERR_INVALID;
     }
     int C = o.cluster_size;
@@ -759,6 +1021,8 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t
     ix.last_stream = st;
     const int key = ix.cand_per_thread * 100 + ix.local_warps;
     switch (key) {
+        case 216: return launch_batched_s<2, 16>(bp, ix, st);
+        case 416: return launch_batched_s<4, 16>(bp, ix, st);
         case 804: return launch_batched_s<8, 4>(bp, ix, st);
         case 801: return launch_batched_s<8, 1>(bp, ix, st);
         case 802: return launch_batched_s<8, 2>(bp, ix, st);

@@ -42,7 +42,7 @@ def test_struct_sizes_match_header(lib):
     # fps_build_opts: 5 x int32 + pointer (8-aligned) + 2 x int32 = 40 bytes; fps_stats: see header
     from paper_2606_06255_b200 import binding
     assert ctypes.sizeof(binding.fps_build_opts) == 40
-    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8 + 16 * 8 + 2 * 4
+    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8 + 18 * 8 + 2 * 4
 
 
 def test_version_and_error_strings(lib):

@@ -88,14 +88,15 @@ def test_every_cluster_size(rf, name, cluster, kernel):
     assert_same(gi, gm, *ref)
 
 
-@pytest.mark.parametrize("cpt", [4, 8, 16])
-@pytest.mark.parametrize("lw", [1, 2, 4, 8])
-@pytest.mark.parametrize("name", ["room", "lattice", "dups", "clustered"])
+LOCAL_SHAPES = [(16, 2), (16, 4), (4, 8), (1, 8), (2, 8), (8, 8), (4, 4), (8, 4), (4, 16), (8, 16)]
+
+
+@pytest.mark.parametrize("lw,cpt", LOCAL_SHAPES)
+@pytest.mark.parametrize("name", ["room", "lattice", "dups", "clustered", "line"])
 def test_every_local_phase_shape(rf, name, lw, cpt):
-    # candidate capacity 32*lw*cpt from 128 to 4096: different thresholds, batches and tie paths
-    # (lattice: exact ties inside a lane, between lanes and between warps; dups: Dist reaches +0)
-    if (cpt, lw) not in {(8, 4), (8, 1), (8, 2), (8, 8), (4, 4), (4, 8), (16, 4), (16, 8)}:
-        pytest.skip("shape not instantiated")
+    # local_warps = 16: hierarchical local phase (default); 1..8: flat.  Candidate capacity 32*lw*cpt
+    # from 256 to 4096: different thresholds, batches and tie paths (lattice / line: exact ties inside a
+    # lane, between lanes and between warps, first histogram bin overflowing; dups: Dist reaches +0)
     P, M = SMALL[name]()
     ref = oracle.fps(P, M, 0)
     gi, gm, st = run_gpu(rf, P, M, local_warps=lw, cand_per_thread=cpt, flags=rf.FPS_FLAG_STATS)
@@ -104,6 +105,10 @@ def test_every_local_phase_shape(rf, name, lw, cpt):
     assert st["rounds"] >= 1 and st["rounds"] <= M
     if name == "room":
         assert st["rounds"] < M // 8            # batching really happens on ordinary data
+        if lw == 16:
+            assert 0 < st["local_subrounds"] < M // 4 and st["local_fallbacks"] < st["local_subrounds"]
+    if name == "lattice" and lw == 16:
+        assert st["local_fallbacks"] > 0        # many exactly equal distances: the block-wide argmax path ran
 
 
 def test_batched_kernel_degenerates_to_per_pick_rounds_without_batching(rf):
