@@ -121,7 +121,7 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->cycles_prune_max = (int64_t)c[18]; out->cycles_visit_max = (int64_t)c[19];
             out->sub_batches = (int64_t)c[20];
             out->local_subrounds = (int64_t)c[24]; out->local_fallbacks = (int64_t)c[25];
-            if (getenv("RFPS_DEBUG")) fprintf(stderr, "[rfps debug] max phase cycles: scan %llu cluster_sync %llu dsmem %llu\n", c[21], c[22], c[23]);
+            if (getenv("RFPS_DEBUG")) fprintf(stderr, "[rfps debug] local phase cycles (sum over clouds): select %llu pick-loop %llu apply %llu\n", c[21], c[22], c[23]);
         }
     }
     return FPS_OK;

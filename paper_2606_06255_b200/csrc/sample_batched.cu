@@ -41,6 +41,10 @@ namespace rfps {
 constexpr int BT = 512;        // threads per CTA
 constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
 constexpr int MAX_ATTEMPTS = 4;
+#ifndef RFPS_GTARGET
+#define RFPS_GTARGET 0.625f
+#endif
+constexpr float GTARGET = RFPS_GTARGET;   // aim the next extraction at this fraction of the candidate buffer
 constexpr int SUBW = 4;        // 32-bit mask words per queued voxel
 constexpr int SUBP = 32 * SUBW;   // picks applied between two CTA barriers
 
@@ -69,7 +73,7 @@ enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CN
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, ggeom, vst, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
+    size_t geom, ggeom, vst, seg, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -78,6 +82,7 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.geom = o;  o += sizeof(float4) * (size_t)Kc_cap;
     L.ggeom = o; o += sizeof(float4) * (size_t)(Kc_cap / 32);
     L.vst = o;   o += sizeof(uint2) * (size_t)Kc_cap;
+    L.seg = o;   o += sizeof(int2) * (size_t)Kc_cap;
     L.bpick = o; o += sizeof(float4) * PB;
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
     L.ctl = o;   o += sizeof(Ctl);
@@ -263,7 +268,8 @@ template <int CPT1, int CPT2>
 __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY, const float *cZ, const float *cD,
                                                const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
                                                const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
-                                               const int tid, unsigned long long &c_subrounds, unsigned long long &c_fallback)
+                                               const int tid, unsigned long long &c_subrounds, unsigned long long &c_fallback,
+                                               long long &t_sel, long long &t_loop, long long &t_app)
 {
     static_assert(CPT1 % 2 == 0 && CPT2 >= 1 && CPT2 <= 4, "shape");
     constexpr int H1 = CPT1 / 2, T2 = 32 * CPT2;
@@ -282,7 +288,9 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         D[2 * h + 1] = ok1 ? cD[i1] : 0.0f;
     }
     int jl = j, nbl = 0, applied = 0;
+    long long tt0 = 0, tt1 = 0;
     for (;;) {
+        tt0 = clock64();
         // ---- (a) block maximum ----
         float m = D[0];
 #pragma unroll
@@ -370,6 +378,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 if (lane == 0) hs->wmax2[warp] = we;
             }
             __syncthreads();
+            tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1;
             // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
             // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
             if (warp == 0) {
@@ -450,6 +459,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         }
 #undef RFPS_BIN
         c_subrounds++;
+        tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
         // ---- (f) the sub-round's picks -> all of C1 ----
         for (int i = applied; i < nbl; ++i) {
             const float4 s = bpick[i];
@@ -466,6 +476,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             }
         }
         applied = nbl;
+        t_app += clock64() - tt0;
         if (jl >= M || nbl >= PB) break;
     }
     j = jl;
@@ -497,6 +508,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     float4 *sgeom = reinterpret_cast<float4 *>(smem_raw + L.geom);    // [Kc] {cx, cy, cz, R}
     float4 *sggeom = reinterpret_cast<float4 *>(smem_raw + L.ggeom);  // [Gc] group spheres
     uint2 *vst = reinterpret_cast<uint2 *>(smem_raw + L.vst);         // [Kc] voxel key {Dist_v bits, ~orig of the point attaining it}
+    int2 *sseg = reinterpret_cast<int2 *>(smem_raw + L.seg);          // [Kc] {first point, count} of the voxel's segment
     float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
     float *cX = reinterpret_cast<float *>(smem_raw + L.cand), *cY = cX + TC, *cZ = cY + TC, *cD = cZ + TC;
     unsigned *cO = reinterpret_cast<unsigned *>(cD + TC);
@@ -531,6 +543,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     for (int kl = tid; kl < Kc; kl += BT) {
         const int k = RFPS_VOXEL_OF(kl);
         sgeom[kl] = k < K ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        sseg[kl] = k < K ? vseg[k] : make_int2(0, 0);
         // not visited yet: Dist_v = NaN, whose prune threshold is NaN ("d2 >= NaN" is false: visit).  Every
         // voxel is visited by the first pick, so no NaN key survives round 1.  Empty slot: key (0,0), below
         // every real key, threshold 0 ("d2 >= 0" always prunes)
@@ -653,17 +666,21 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     __syncwarp();
                     if (lane == 0) *reinterpret_cast<uint4 *>(&qmask[kl * SUBW]) = make_uint4(0u, 0u, 0u, 0u);   // leave it clean
                 }
-                const int2 sg = vseg[RFPS_VOXEL_OF(kl)];
+                const int2 sg = sseg[kl];
                 float bestD = -1.0f;
                 unsigned bestO = 0u;
                 int npk = 0;
 #pragma unroll
                 for (int w = 0; w < SUBW; ++w) npk += __popc(vmask[w]);
-                for (int p = sg.x + lane; p < sg.x + sg.y; p += 32) {
-                    const float x = px[p], y = py[p], z = pz[p];
-                    const unsigned o = ~(unsigned)porig[p];
-                    const float D0 = Dp[p];
-                    float D = D0;
+                // two chunks of 32 points per step: both chunks' loads are in flight together
+                for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
+                    const int pA = pb + lane, pB = pb + 32 + lane;
+                    const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
+                    float xA = 0.f, yA = 0.f, zA = 0.f, DA0 = -1.0f, xB = 0.f, yB = 0.f, zB = 0.f, DB0 = -1.0f;
+                    unsigned oA = 0u, oB = 0u;
+                    if (inA) { xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; DA0 = Dp[pA]; }
+                    if (inB) { xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; DB0 = Dp[pB]; }
+                    float DA = DA0, DB = DB0;
 #pragma unroll
                     for (int w = 0; w < SUBW; ++w) {
                         unsigned m = vmask[w];
@@ -671,21 +688,38 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                             const int i = __ffs(m) - 1;
                             m &= m - 1u;
                             const float4 s = bpick[sub + 32 * w + i];
-                            const float dx = __fsub_rn(x, s.x), dy = __fsub_rn(y, s.y), dz = __fsub_rn(z, s.z);
-                            const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                            if (no_skip || !(dx2 >= D || dy2 >= D || dz2 >= D)) {     // Eq. 28, squared domain
-                                const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
-                                if (STATS) c_pcomp++;
-                                if (d < D) {                                          // Eq. 29 / Eq. 2 (strict)
-                                    D = d;
-                                    if (STATS) c_eff++;
+                            {
+                                const float dx = __fsub_rn(xA, s.x), dy = __fsub_rn(yA, s.y), dz = __fsub_rn(zA, s.z);
+                                const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                                if (no_skip || !(dx2 >= DA || dy2 >= DA || dz2 >= DA)) {   // Eq. 28, squared domain
+                                    const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                                    if (STATS && inA) c_pcomp++;
+                                    if (d < DA) {                                          // Eq. 29 / Eq. 2 (strict)
+                                        DA = d;
+                                        if (STATS) c_eff++;
+                                    }
+                                }
+                            }
+                            {
+                                const float dx = __fsub_rn(xB, s.x), dy = __fsub_rn(yB, s.y), dz = __fsub_rn(zB, s.z);
+                                const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                                if (no_skip || !(dx2 >= DB || dy2 >= DB || dz2 >= DB)) {
+                                    const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                                    if (STATS && inB) c_pcomp++;
+                                    if (d < DB) {
+                                        DB = d;
+                                        if (STATS) c_eff++;
+                                    }
                                 }
                             }
                         }
                     }
-                    if (D < D0) Dp[p] = D;
-                    if (STATS) c_pvisit += npk;
-                    if (D > bestD || (D == bestD && o > bestO)) { bestD = D; bestO = o; }
+                    if (DA < DA0) Dp[pA] = DA;
+                    if (DB < DB0) Dp[pB] = DB;
+                    if (STATS) c_pvisit += (inA ? npk : 0) + (inB ? npk : 0);
+                    // absent lanes carry D = -1 (< every real distance), so they never become the voxel's key
+                    if (DA > bestD || (DA == bestD && oA > bestO)) { bestD = DA; bestO = oA; }
+                    if (DB > bestD || (DB == bestD && oB > bestO)) { bestD = DB; bestO = oB; }
                 }
                 const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
                 unsigned mhi, mlo;
@@ -738,7 +772,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             warp_argmax_key(rb.x, rb.y, ghi, glo);
         }
 
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; dbg0 += tm1 - t0; dbg1 += tm2 - tm1; dbg2 += t1 - tm2; t0 = t1; }
+        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
         // =====================================================================================
         // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
         // =====================================================================================
@@ -772,7 +806,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     if (lane == 0) qi = atomicAdd(&qn[2], 1);
                     qi = __shfl_sync(FULL, qi, 0);
                     if (qi >= nq) break;
-                    const int2 sg = vseg[RFPS_VOXEL_OF(qkl[qi])];
+                    const int2 sg = sseg[qkl[qi]];
                     if (STATS && lane == 0) c_xvox++;
                     for (int p0 = sg.x; p0 < sg.x + sg.y; p0 += 32) {
                         const int p = p0 + lane;
@@ -803,7 +837,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     cnt = (int)found;
                     taubits = tb;
                     // aim the next round at ~5/8 of the buffer; move by at most 2x per round
-                    const float ratio = fminf(2.0f, fmaxf(0.5f, (0.625f * TC) / (float)max(found, 1u)));
+                    const float ratio = fminf(2.0f, fmaxf(0.5f, (GTARGET * TC) / (float)max(found, 1u)));
                     g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
                     break;
                 }
@@ -830,7 +864,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
                 local_fps_hier<CPT, 4>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
-                                       c_subrounds, c_fallback);
+                                       c_subrounds, c_fallback, dbg0, dbg1, dbg2);
                 if (tid == 0) {
                     ctl->nb = lnb;
                     ctl->j = lj;
