@@ -6,9 +6,11 @@ A "step" is one pass of the WHOLE hot path over one batch of synthetic clouds: f
 persistent fused kernel, all M-1 iterations), inputs already resident in HBM.  Default workload:
 BASELINE.json configs[1] ("C2": B=16 indoor-room-like clouds, N=24000, M=6000).  `e2e` is the same
 metric through fps_sample_host with HOST buffers (H2D + build + sample + D2H inside the timed
-region).  `roofline` is for the dominant kernel (k_fps_sample): algorithmic bytes per launch
-(from the kernel's own counters in a separate, untimed stats run)
-divided by its average launch duration measured with CUDA events on the launching stream.
+region).  `roofline` is for the dominant kernel (k_fps_batched, exact batched picking): algorithmic
+bytes per launch (from the kernel's own counters in a separate,
+untimed stats run) divided by its average launch duration measured with CUDA events on the
+launching stream.  The same run also times the per-pick persistent kernel (the paper's iteration
+structure, FPS_FLAG_PER_PICK) once as an ablation.
 `cpu_baseline` is the CPU oracle timed on this box's host cores (rank 0, N=1 only).
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1..C5] [--impl reference]
@@ -51,6 +53,9 @@ def parse():
     ap.add_argument("--tile-points", type=int, default=0)
     ap.add_argument("--cluster-size", type=int, default=0)
     ap.add_argument("--block-threads", type=int, default=0)
+    ap.add_argument("--local-warps", type=int, default=0)
+    ap.add_argument("--cand-per-thread", type=int, default=0)
+    ap.add_argument("--per-pick", action="store_true", help="time the per-pick persistent kernel instead (ablation)")
     return ap.parse_args()
 
 
@@ -117,16 +122,51 @@ class Clocks:
 # algorithmic bytes (DESIGN.md / SURVEY.md 8(d)) from the kernel's counters
 # ---------------------------------------------------------------------------------------------
 def algorithmic_bytes(st: dict) -> int:
-    """sum over iterations of: 20 B per voxel tested (c_k, r_k, Dist_v) + 8 B per voxel key in the
-    argmax + 16 B per visited point (x, y, z, Dist_p) + 8 B key write-back per visited voxel +
-    4 B per effective Dist_p store + 20 B per iteration (s_j, out_idx, out_mindist)."""
-    return (28 * st["voxel_tests"] + 16 * st["points_visited"] + 8 * st["voxels_visited"] + 4 * st["effective"]
-            + 20 * st["iterations"])
+    """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes", evaluated with the counters of the schedule
+    that ran.  20 B per radius-prune test (centre 12, radius 4, Dist_v 4; group tests and voxel
+    tests alike) + 16 B per (visited point, pick) pair (x, y, z, Dist_p) + 8 B key write-back per
+    voxel visit + 4 B per effective Dist_p store + 8 B per voxel key per argmax (one argmax per
+    pick in the per-pick kernel, one per round in the batched kernel) + 20 B per pick (s_j,
+    out_idx, out_mindist) + batched kernel only: 4 B per point scanned by the candidate extraction
+    and 20 B per candidate moved (x, y, z, Dist_p, index)."""
+    argmaxes = st["rounds"] if st.get("rounds", 0) else st["iterations"]
+    per_cloud_K = st["K_total"] / max(1, st["B"])
+    return int(20 * (st["voxel_tests"] + st.get("group_tests", 0)) + 16 * st["points_visited"] + 8 * st["voxels_visited"]
+               + 4 * st["effective"] + 8 * per_cloud_K * argmaxes + 20 * st["iterations"]
+               + 4 * st.get("extract_points", 0) + 20 * st.get("candidates", 0))
+
+
+def ncu_traffic(workload: str, per_pick: bool):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+    `ncu --set full` capture of this workload (profiles/r01_traffic.csv: workload,kernel,bytes), else None."""
+    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    want = "k_fps_sample" if per_pick else "k_fps_batched"
+    try:
+        for row in open(path).read().splitlines()[1:]:
+            f = [c.strip() for c in row.split(",")]
+            if len(f) >= 3 and f[0] == workload and f[1] == want:
+                return float(f[2])
+    except OSError:
+        pass
+    return None
 
 
 def opts_from(args) -> dict:
     return dict(n_vox=args.n_vox, tile_points=args.tile_points, cluster_size=args.cluster_size,
-                block_threads=args.block_threads)
+                block_threads=args.block_threads, local_warps=args.local_warps, cand_per_thread=args.cand_per_thread,
+                flags=(16 if args.per_pick else 0))
+
+
+GHZ_FALLBACK = 1.965
+
+
+def phase_ms(st: dict, sm_mhz) -> dict:
+    """Per-phase time of the batched kernel (SM cycles seen by thread 0 of each cloud's first CTA,
+    averaged over clouds, converted with the SM clock sampled during the run)."""
+    ghz = (sm_mhz or GHZ_FALLBACK * 1e3) * 1e-3
+    f = lambda k: st.get(k, 0) / max(1, st["B"]) / ghz / 1e6  # noqa: E731
+    return {"apply": f("cycles_apply"), "argmax_and_wait": f("cycles_max"), "extract": f("cycles_extract"),
+            "local": f("cycles_local")}
 
 
 def time_config(rf, torch, w, P_host, steps, warmup, opts, flush):
@@ -157,7 +197,9 @@ def time_config(rf, torch, w, P_host, steps, warmup, opts, flush):
 
 def stats_run(rf, torch, w, P_host, opts):
     Pd = torch.from_numpy(P_host).cuda()
-    ix = rf.fps_index_build(Pd, flags=rf.FPS_FLAG_STATS, **opts)
+    opts = dict(opts)
+    opts["flags"] = opts.get("flags", 0) | rf.FPS_FLAG_STATS
+    ix = rf.fps_index_build(Pd, **opts)
     rf.fps_sample(ix, w.M, w.start_idx)
     torch.cuda.synchronize()
     st = rf.fps_get_stats(ix)
@@ -288,25 +330,41 @@ def main():
             "config": {"workload": f"{w.name}: {w.note}", "B": w.B, "N": w.N, "M": w.M, "start_idx": w.start_idx,
                        "step": "fps_index_build + fps_sample (a1-a13)", "l2": "flushed between iterations (256 MiB fill)",
                        "n_vox": st["n_vox"], "K_max": st["K_max"], "cluster_size": st["cluster_size"],
-                       "block_threads": st["block_threads"], "voxels_per_thread": st["voxels_per_thread"],
+                       "block_threads": st["block_threads"], "local_warps": st["local_warps"],
+                       "cand_per_thread": st["cand_per_thread"],
+                       "kernel": "per-pick persistent (ablation)" if args.per_pick else "exact batched picking",
                        "parallelism": f"replicas x{world}"},
             "ms_per_cloud": total_ms / args.steps / w.B,
             "sample_kernel_ms": float(np.mean(r["kern_ms"])), "index_build_ms": float(np.mean(r["build_ms"])),
             "sample_only_samples_per_s": w.B * w.M / kern_s, "us_per_iteration": kern_s * 1e6 / max(1, w.M - 1),
-            "roofline": {"bound": "hbm", "kernel": "k_fps_sample", "achieved": achieved, "peak": peak, "unit": "GB/s",
+            "roofline": {"bound": "hbm", "kernel": "k_fps_sample" if args.per_pick else "k_fps_batched",
+                         "achieved": achieved, "peak": peak, "unit": "GB/s",
                          "frac": achieved / peak, "frac_of_8000_nominal": achieved / 8000.0, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": alg, "traffic": None,
-                         "note": "latency-bound by construction: M-1 sequentially dependent iterations touching "
-                                 "a few KB each (SURVEY.md 8(d)); working set is L2/L1 resident",
-                         "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9},
-            "counters": {k: st_counts[k] for k in ("iterations", "voxel_tests", "voxels_visited", "points_visited",
-                                                   "points_computed", "effective")},
+                         "algorithmic_bytes_per_launch": alg, "traffic": ncu_traffic(w.name, args.per_pick),
+                         "note": "BASELINE.json asks for the HBM roofline; it is NOT what binds this path: the working "
+                                 "set is L1/L2 resident (see traffic) and the M-1 picks are sequentially dependent, so "
+                                 "the kernel is bound by the latency of its pick chain (DESIGN.md section 8)",
+                         "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9,
+                         "us_per_pick": kern_s * 1e6 / max(1, w.M - 1)},
+            "phases_ms_per_cloud": None if args.per_pick else phase_ms(st_counts, clk.get("sm_mhz")),
+            "counters": {k: st_counts[k] for k in ("iterations", "group_tests", "voxel_tests", "voxels_visited",
+                                                   "points_visited", "points_computed", "effective", "rounds",
+                                                   "extract_retries", "single_picks", "candidates", "extract_points",
+                                                   "sub_batches", "local_subrounds", "local_fallbacks")},
             "e2e": {"value": world * w.B * w.M * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(P.nbytes),
                     "d2h_bytes_per_step": int(oi.numel() * 4 + om.numel() * 4), "ms_per_step": e2e_s / args.steps * 1e3,
                     "api": "fps_sample_host (pinned host buffers)", "matches_device_path": e2e_ok},
             "gpu_launches": (st["build_launches"] + 1) * args.steps,
             "clocks": clk,
         }
+        if world == 1 and not args.per_pick and not args.no_extra_configs:
+            o2 = dict(opts, flags=16, local_warps=0, cand_per_thread=0)
+            r2 = time_config(rf, torch, w, P, 3, 3, o2, flush)
+            line["ablation_per_pick_kernel"] = {
+                "what": "the paper's iteration structure (one cluster-wide argmax exchange per sample) as ONE persistent "
+                        "kernel, FPS_FLAG_PER_PICK; same index, same outputs",
+                "sample_kernel_ms": float(np.median(r2["kern_ms"])),
+                "outputs_identical": bool(torch.equal(r2["out_idx"], r["out_idx"]) and torch.equal(r2["out_mind"], r["out_mind"]))}
         if world == 1 and not args.no_cpu_baseline:
             line["cpu_baseline"] = cpu_oracle_sample(w, P)
         if world == 1 and not args.no_extra_configs:
@@ -327,7 +385,8 @@ def per_config_summary(rf, torch, flush, opts, peak):
         r = time_config(rf, torch, w, P, 5, 3, opts, flush)
         k = float(np.median(r["kern_ms"])) * 1e-3
         alg = algorithmic_bytes(stc)
-        out[name] = {"B": w.B, "N": w.N, "M": w.M, "sample_ms_per_cloud": k * 1e3 / w.B,
+        out[name] = {"B": w.B, "N": w.N, "M": w.M, "sample_ms": k * 1e3, "sample_ms_per_cloud": k * 1e3 / w.B,
+                     "rounds_per_cloud": stc["rounds"] / w.B, "picks_per_round": stc["iterations"] / max(1, stc["rounds"]),
                      "build_plus_sample_ms_per_cloud": float(np.median(r["step_ms"])) / w.B,
                      "samples_per_s": w.B * w.M / k, "us_per_iteration": k * 1e6 / (w.M - 1),
                      "hbm_roofline_frac_measured_peak": alg / k / 1e9 / peak, "hbm_roofline_frac_8000": alg / k / 1e9 / 8000.0,
