@@ -13,19 +13,21 @@
 // one by one, and a voxel may be tested against a pick with a stale (larger) Dist_v because that
 // only makes the prune test of Eq. 25 more conservative.
 //
-// One round, one thread-block cluster per cloud (all CTAs unless noted):
-//   APPLY    the nb picks of the previous batch, 32 at a time: every thread tests the voxels it
-//            owns against the 32 picks (a9, squared-domain Eq. 25 with fp32 margins) and pushes
-//            (voxel, survivor mask) to a queue; warps walk the queued voxels' points (a10 skip,
-//            a11 update) and refresh the voxel key and threshold (a12).
+// One round, one thread-block cluster per cloud (all CTAs unless noted; DESIGN.md section 6):
+//   APPLY    the nb picks of the previous batch, 128 at a time.  Prune (a9, squared-domain Eq. 25 with
+//            fp32 margins) on two levels: a work unit = (group of 32 voxels, 32 picks) tests the picks
+//            against the group sphere, then the group's voxels against the survivors; voxels with
+//            survivors are queued with their pick mask.  Warps pop queued voxels and walk their points
+//            once for all surviving picks (a10 skip, a11 update) and refresh the voxel key (a12).
 //   MAX      CTA argmax of the voxel keys, then cluster argmax over DSMEM (a8).
 //   EXTRACT  tau = Dmax * (1 - g): points with Dist_p > tau are appended to the candidate buffer in
 //            CTA 0's shared memory over DSMEM (atom.shared::cluster + st.shared::cluster).  If more
 //            than TC candidates turn up, tau is raised and the step repeated; if that fails the
 //            batch is the single global argmax (the paper's own per-pick iteration).
-//   LOCAL    (CTA 0, LW warps) register-resident FPS over the <= TC candidates: one named barrier
-//            per pick, no global memory in the loop; stops when the maximum is <= tau, after PB
-//            picks, or at M.  Picks go to out_idx / out_mindist and to the next round's batch.
+//   LOCAL    (CTA 0) FPS restricted to the <= TC candidates, hierarchical by default: all warps hold
+//            the candidates in registers, one warp picks from the top <= 128 of them with no barrier
+//            per pick (local_fps_hier); stops when the maximum is <= tau, after PB picks, or at M.
+//            Picks go to out_idx / out_mindist and to the next round's batch.
 //
 // Arithmetic: d2 only via __fsub_rn/__fmul_rn/__fadd_rn (never FMA); the local phase uses
 // fminf(D, d2), which is value-identical to the strict '<' update for non-NaN operands.
