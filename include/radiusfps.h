@@ -54,7 +54,8 @@ typedef struct {
     int32_t n_vox;         /* voxel bins per axis (Eq. 7); 0 = choose from N; 1..1024   */
     int32_t tile_points;   /* split voxels holding more points than this into tiles with their own
                               bounding sphere; 0 = default, -1 = never split (the paper's layout)      */
-    int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1,2,4,8,16            */
+    int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1..16 (per-pick kernel:
+                              1,2,4,8,16)                                                              */
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */

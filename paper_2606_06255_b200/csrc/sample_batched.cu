@@ -980,7 +980,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         return FPS_ERR_INVALID;
     }
     int C = o.cluster_size;
-    if (C != 0 && C != 1 && C != 2 && C != 4 && C != 8 && C != 16) { set_error("cluster_size=%d must be 0,1,2,4,8 or 16", C); return FPS_ERR_INVALID; }
+    if (C < 0 || C > 16) { set_error("cluster_size=%d must be 0 (choose) or 1..16", C); return FPS_ERR_INVALID; }
     if (o.block_threads != 0 && o.block_threads != BT) { set_error("block_threads=%d: the batched kernel runs %d threads per CTA", o.block_threads, BT); return FPS_ERR_INVALID; }
     const int K = ix.K_max > 0 ? ix.K_max : 1;
     const int TC = CPT * LW * 32;
@@ -988,13 +988,17 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     auto slots = [&](int c) { return 32 * ((G + c - 1) / c); };     // voxel slots per CTA
     auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= (size_t)kMaxSmem; };
     if (C == 0) {
+        // the largest cluster that (a) leaves every CTA >= 1 024 points, (b) holds the voxel state in
+        // shared memory and (c) lets all B clusters be resident at once (a cluster lives inside one
+        // GPC, so fewer clusters fit than 148 / C suggests: 15 of 8, 22 of 6, 7 of 16 on B200);
+        // otherwise the clouds would run in waves
+        const int want = std::min(ix.B, 148);
         C = 1;
-        while (C < 16 && (long long)C * 2 * ix.B <= 148 && (long long)ix.N > (long long)C * 2048) C *= 2;
-        while (C < 16 && !fits(C)) C *= 2;
-        // all B clusters should be resident at once (a cluster lives inside one GPC, so fewer clusters
-        // fit than 148 / C suggests); otherwise the clouds run in waves
-        while (C > 1 && fits(C / 2) && max_resident_clusters(C, smem_layout(slots(C), TC, LW).total) < std::min(ix.B, 148 / C))
-            C /= 2;
+        for (int c = 16; c > 1; --c) {
+            if ((long long)ix.N < 1024ll * c || !fits(c)) continue;
+            if (max_resident_clusters(c, smem_layout(slots(c), TC, LW).total) >= std::min(want, 148 / c)) { C = c; break; }
+        }
+        while (C < 16 && !fits(C)) ++C;
     }
     if (!fits(C)) {
         set_error("K_max=%d voxels do not fit the shared memory of %d CTAs; use a smaller n_vox or a larger tile_points", K, C);

@@ -78,9 +78,11 @@ def test_small_clouds_default_config(rf, name, kernel):
 
 
 @pytest.mark.parametrize("kernel", sorted(KERNELS))
-@pytest.mark.parametrize("cluster", [1, 2, 4, 8, 16])
+@pytest.mark.parametrize("cluster", [1, 2, 3, 4, 6, 7, 8, 13, 16])
 @pytest.mark.parametrize("name", ["room", "lattice", "lidar"])
 def test_every_cluster_size(rf, name, cluster, kernel):
+    if kernel == "per_pick" and cluster not in (1, 2, 4, 8, 16):
+        pytest.skip("the per-pick kernel takes power-of-two clusters")
     P, M = SMALL[name]()
     ref = oracle.fps(P, M, 0)
     gi, gm, st = run_gpu(rf, P, M, cluster_size=cluster, flags=KERNELS[kernel])
@@ -272,7 +274,9 @@ def test_errors(rf):
         rf.fps_index_build(bad)
     assert e.value.status == rf.FPS_ERR_NONFINITE
     with pytest.raises(rf.FpsError):
-        rf.fps_index_build(P, cluster_size=3)
+        rf.fps_index_build(P, cluster_size=17)
+    with pytest.raises(rf.FpsError):
+        rf.fps_index_build(P, cluster_size=3, flags=rf.FPS_FLAG_PER_PICK)
 
 
 # ---------------------------------------------------------------------------------------------
