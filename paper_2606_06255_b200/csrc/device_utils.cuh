@@ -63,6 +63,18 @@ __device__ __forceinline__ unsigned atom_add_dsmem_u32(unsigned addr, unsigned v
     asm volatile("atom.shared::cluster.add.u32 %0, [%1], %2;" : "=r"(old) : "r"(addr), "r"(v) : "memory");
     return old;
 }
+// release store to this CTA's own shared memory / acquire load from a peer's, both at cluster scope:
+// a one-way message channel between CTAs of a cluster without a cluster barrier
+__device__ __forceinline__ void st_release_cluster_u32(unsigned local_addr, unsigned v)
+{
+    asm volatile("st.release.cluster.shared::cta.u32 [%0], %1;" ::"r"(local_addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ unsigned ld_acquire_cluster_u32(unsigned cluster_addr)
+{
+    unsigned v;
+    asm volatile("ld.acquire.cluster.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(cluster_addr) : "memory");
+    return v;
+}
 __device__ __forceinline__ void mbar_init(unsigned bar, unsigned count)
 {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");

@@ -102,8 +102,32 @@ __device__ __forceinline__ unsigned spread3(unsigned v)
     return v;
 }
 
+// Hilbert index of a cell with `b` bits per axis (Skilling's transpose construction, "Programming the
+// Hilbert curve", 2004): undo the excess work of the Gray-code walk, Gray-encode, interleave.
+__device__ __forceinline__ unsigned hilbert3(unsigned x, unsigned y, unsigned z, int b)
+{
+    if (b <= 0) return 0u;
+    unsigned X[3] = {x, y, z};
+    const unsigned M = 1u << (b - 1);
+    for (unsigned Q = M; Q > 1u; Q >>= 1) {
+        const unsigned P = Q - 1u;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            if (X[i] & Q) X[0] ^= P;
+            else { const unsigned t = (X[0] ^ X[i]) & P; X[0] ^= t; X[i] ^= t; }
+        }
+    }
+    X[1] ^= X[0];
+    X[2] ^= X[1];
+    unsigned t = 0u;
+    for (unsigned Q = M; Q > 1u; Q >>= 1)
+        if (X[2] & Q) t ^= Q - 1u;
+    X[0] ^= t; X[1] ^= t; X[2] ^= t;
+    return (spread3(X[0]) << 2) | (spread3(X[1]) << 1) | spread3(X[2]);
+}
+
 __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int N, const unsigned *__restrict__ bbox,
-                                               int n_vox, int sb, unsigned *__restrict__ keys, int *__restrict__ vals)
+                                               int n_vox, int hb, int sb, unsigned *__restrict__ keys, int *__restrict__ vals)
 {
     const int b = blockIdx.y;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -127,10 +151,11 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int
         v[a] = (unsigned)c;
         s[a] = (unsigned)sc;
     }
-    // voxel id: the Morton interleave of (v_x, v_y, v_z) instead of the row-major id of Eq. 31 -- any
-    // bijective id gives the same voxels; Morton order keeps consecutive active voxels spatially
-    // compact, which the sampling kernel's group-level prune relies on
-    unsigned vid = spread3(v[0]) | (spread3(v[1]) << 1) | (spread3(v[2]) << 2);
+    // voxel id: the position of (v_x, v_y, v_z) on a 3-D Hilbert curve instead of the row-major id of
+    // Eq. 31 -- any bijective id gives the same voxels.  Consecutive cells of the curve are face
+    // neighbours (no seams as in Morton order), so 32 consecutive active voxels stay spatially compact,
+    // which the sampling kernel's group-level prune relies on.
+    unsigned vid = hilbert3(v[0], v[1], v[2], hb);
     unsigned sub = sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
     keys[(size_t)b * N + i] = (vid << (3 * sb)) | sub;
     vals[(size_t)b * N + i] = i;
@@ -634,7 +659,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));
     k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(sc.bbox, B);
     k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, sc.bbox);
-    k_keys<<<gN, 256, 0, st>>>(points, N, sc.bbox, n_vox, sb, sc.kA, sc.vA);
+    k_keys<<<gN, 256, 0, st>>>(points, N, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
     g_launches += 3;
 
     // a3: LSD radix sort, 8 bits per pass

@@ -43,6 +43,11 @@ namespace rfps {
 constexpr int BT = 512;        // threads per CTA
 constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
 constexpr int MAX_ATTEMPTS = 4;
+#ifndef RFPS_STREAM_MIN
+#define RFPS_STREAM_MIN 64
+#endif
+constexpr int STREAM_MIN = RFPS_STREAM_MIN;   // workers start on a piece of the running batch once it has this many picks
+constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffffu;
 #ifndef RFPS_GTARGET
 #define RFPS_GTARGET 0.625f
 #endif
@@ -67,6 +72,7 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
     unsigned ccount[MAX_ATTEMPTS];  // candidates found by extraction attempt a (may exceed TC)
     unsigned best_hi, best_lo, pad3, pad0;       // this CTA's best voxel key
     int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
+    unsigned pub, pad4, pad5, pad6; // (CTA 0) picks of the running batch published so far | PUB_DONE | PUB_FINAL
 };
 
 
@@ -75,7 +81,7 @@ enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CN
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
-    size_t geom, ggeom, vst, seg, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
+    size_t geom, ggeom, vst, seg, vthr, gthr, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -85,6 +91,8 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.ggeom = o; o += sizeof(float4) * (size_t)(Kc_cap / 32);
     L.vst = o;   o += sizeof(uint2) * (size_t)Kc_cap;
     L.seg = o;   o += sizeof(int2) * (size_t)Kc_cap;
+    L.vthr = o;  o += sizeof(float) * (size_t)Kc_cap;
+    L.gthr = o;  o += (sizeof(float) * (size_t)(Kc_cap / 32) + 15) & ~(size_t)15;
     L.bpick = o; o += sizeof(float4) * PB;
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
     L.ctl = o;   o += sizeof(Ctl);
@@ -271,7 +279,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                                                const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
                                                const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
                                                const int tid, unsigned long long &c_subrounds, unsigned long long &c_fallback,
-                                               long long &t_sel, long long &t_loop, long long &t_app)
+                                               long long &t_sel, long long &t_loop, long long &t_app, const unsigned pub_addr)
 {
     static_assert(CPT1 % 2 == 0 && CPT2 >= 1 && CPT2 <= 4, "shape");
     constexpr int H1 = CPT1 / 2, T2 = 32 * CPT2;
@@ -397,7 +405,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                     d2v[c] = ok ? hs->sD[i] : 0.0f;         // padding never exceeds tau2
                 }
                 // picks are logged as {slot id, D bits}: lane (n & 31) keeps pick n in registers and the warp
-                // writes 32 of them at a time, so the loop itself holds no store and no dependent load
+                // writes 32 of them at a time, so the loop itself holds no global store and no dependent load
                 const int nb0 = nbl, j0 = jl;
                 unsigned mywid = 0u, myd = 0u;
                 for (;;) {
@@ -461,6 +469,8 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         }
 #undef RFPS_BIN
         c_subrounds++;
+        // the workers may start applying these picks now (bpick was written before the barrier above)
+        if (pub_addr && tid == 0) st_release_cluster_u32(pub_addr, (unsigned)nbl);
         tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
         // ---- (f) the sub-round's picks -> all of C1 ----
         for (int i = applied; i < nbl; ++i) {
@@ -511,6 +521,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     float4 *sggeom = reinterpret_cast<float4 *>(smem_raw + L.ggeom);  // [Gc] group spheres
     uint2 *vst = reinterpret_cast<uint2 *>(smem_raw + L.vst);         // [Kc] voxel key {Dist_v bits, ~orig of the point attaining it}
     int2 *sseg = reinterpret_cast<int2 *>(smem_raw + L.seg);          // [Kc] {first point, count} of the voxel's segment
+    float *svthr = reinterpret_cast<float *>(smem_raw + L.vthr);      // [Kc] prune threshold of the voxel (from its key and radius)
+    float *sgthr = reinterpret_cast<float *>(smem_raw + L.gthr);      // [Gc] prune threshold of the group (from the largest key in it)
     float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
     float *cX = reinterpret_cast<float *>(smem_raw + L.cand), *cY = cX + TC, *cZ = cY + TC, *cD = cZ + TC;
     unsigned *cO = reinterpret_cast<unsigned *>(cD + TC);
@@ -536,9 +548,14 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     float *out_mind = P.out_mind + (size_t)b * P.M;
     const int K = P.K[b];
     const int G = (K + 31) / 32;
-    const int Gc = G > rank ? (G - rank + C - 1) / C : 0;     // groups owned by this CTA
-    const int Kc = Gc * 32;                                   // voxel slots of this CTA (some may be empty)
-#define RFPS_VOXEL_OF(kl) ((rank + C * ((kl) >> 5)) * 32 + ((kl) & 31))
+    // roles: with C > 1 CTA 0 is the PICKER (candidate-set FPS, owns no voxel) and CTAs 1..C-1 are the
+    // WORKERS (own the voxels; apply the picks WHILE the picker is still producing them).  C == 1: both.
+    const bool split = C > 1;
+    const int W = split ? C - 1 : 1, wr = split ? rank - 1 : 0;
+    const bool worker = !split || rank > 0;
+    const int Gc = (worker && G > wr) ? (G - wr + W - 1) / W : 0;   // groups owned by this CTA
+    const int Kc = Gc * 32;                                         // voxel slots of this CTA (some may be empty)
+#define RFPS_VOXEL_OF(kl) ((wr + W * ((kl) >> 5)) * 32 + ((kl) & 31))
 
     // ---- a7: state reset.  Thresholds = NaN: nothing can be pruned by the first pick, which therefore
     // performs the paper's "initial update" (Eq. 13-14).  Dist_p = +inf on this CTA's slice. ----
@@ -550,8 +567,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         // voxel is visited by the first pick, so no NaN key survives round 1.  Empty slot: key (0,0), below
         // every real key, threshold 0 ("d2 >= 0" always prunes)
         vst[kl] = make_uint2(k < K ? F32_NAN_BITS : 0u, 0u);
+        svthr[kl] = k < K ? __uint_as_float(F32_NAN_BITS) : 0.0f;
     }
-    for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[rank + C * gl]; qbits[gl] = 0u; }
+    for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[wr + W * gl]; qbits[gl] = 0u; sgthr[gl] = __uint_as_float(F32_NAN_BITS); }
     for (int i = tid; i < Kc * SUBW; i += BT) qmask[i] = 0u;
     {
         const int chunk = (P.N + C - 1) / C;
@@ -560,7 +578,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
     }
     if (tid == 0) {
-        qn[0] = qn[1] = qn[2] = 0;
+        qn[0] = qn[1] = qn[2] = qn[3] = 0;
+        ctl->pub = 0u;
 #pragma unroll
         for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
         ctl->best_hi = ctl->best_lo = 0u;
@@ -583,17 +602,16 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
     cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
 
-    while (j < P.M) {
-        if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
-        // =====================================================================================
-        // APPLY: the nb picks in bpick[], SUBP (= 128) at a time.
+    // =====================================================================================
+    // APPLY: the picks bpick[lo, hi), SUBP (= 128) at a time (whole CTA; contains CTA barriers).
         //   phase A  one warp per group of 32 voxels: lane i tests picks i, i+32, .. against the group
         //            sphere (Dist_v := max over the group's voxels), then lane l tests voxel l against
         //            the survivors; voxels with survivors are queued with their pick mask
         //   phase B  warps pop queued voxels (dynamic) and walk their points once for all surviving picks
         // =====================================================================================
-        for (int sub = 0; sub < nb; sub += SUBP) {
-            const int nsub = min(SUBP, nb - sub);
+    auto apply_range = [&](const int lo, const int hi) {
+        for (int sub = lo; sub < hi; sub += SUBP) {
+            const int nsub = min(SUBP, hi - sub);
             if (STATS && tid == 0) { ta0 = clock64(); n_subs++; }
             // ---- a9: radius prune (Eq. 25), two levels.  Work unit = (group, word of 32 picks), spread over
             // the warps so that a group whose sphere prunes badly does not serialise on one warp ----
@@ -608,11 +626,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     mask = valid ? (n == 32 ? FULL : ((1u << n) - 1u)) : 0u;
                     if (STATS && valid) c_vtest += n;
                 } else {
-                    const uint2 vs = vst[kl];
+                    // thresholds are kept current by the visits (phase B): group threshold from Dist_v := max
+                    // over the group, voxel threshold from its own Dist_v (NaN = not visited yet: never pruned)
                     const float4 gg = sggeom[gl];
-                    // group threshold from Dist_v := max over the group (NaN bits sort above every real
-                    // value, so a group holding an unvisited voxel is never pruned)
-                    const float thr_g = prune_threshold(__reduce_max_sync(FULL, vs.x), gg.w);
+                    const float thr_g = sgthr[gl];
                     bool gs = false;
                     if (lane < n) {
                         const float4 s = bpick[sub + 32 * w + lane];
@@ -622,7 +639,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     if (STATS && lane == 0) c_gtest += n;
                     if (gmask) {
                         const float4 gm = sgeom[kl];
-                        const float thr = prune_threshold(vs.x, gm.w);
+                        const float thr = svthr[kl];
                         if (STATS && valid) c_vtest += __popc(gmask);
                         while (gmask) {
                             const int i = __ffs(gmask) - 1;
@@ -728,15 +745,28 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
                 if (lane == 0) {
                     vst[kl] = make_uint2(mhi, mlo);
+                    svthr[kl] = prune_threshold(mhi, sgeom[kl].w);
                     if (STATS) c_vvisit++;
+                }
+                __syncwarp();
+                // refresh the group threshold.  A concurrent visit to another voxel of the group may make this
+                // read one stale (larger) key: the threshold then errs on the conservative side
+                {
+                    const int gl = kl >> 5;
+                    const unsigned dvg = __reduce_max_sync(FULL, vst[gl * 32 + lane].x);
+                    if (lane == 0) sgthr[gl] = prune_threshold(dvg, sggeom[gl].w);
                 }
             }
             __syncthreads();
             qpar ^= 1u;
             if (STATS && tid == 0) t_b += clock64() - ta0;
         }
+    };
 
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_apply += t1 - t0; t0 = t1; }
+    apply_range(0, 1);      // the start point: every voxel is visited (the paper's initial update, Eq. 13-14)
+
+    while (j < P.M) {
+        if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
         // =====================================================================================
         // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
         // =====================================================================================
@@ -760,6 +790,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 if (rank == 0) {
 #pragma unroll
                     for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
+                    ctl->pub = 0u;
                 }
             }
         }
@@ -850,7 +881,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 
         if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
         // =====================================================================================
-        // LOCAL (CTA 0): FPS restricted to the candidates; or the single global argmax
+        // LOCAL (CTA 0): FPS restricted to the candidates; or the single global argmax.
+        // With C > 1 the workers apply the picks concurrently, as CTA 0 publishes them.
         // =====================================================================================
         if (rank == 0) {
             if (cnt == 0) {
@@ -866,7 +898,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
                 local_fps_hier<CPT, 4>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
-                                       c_subrounds, c_fallback, dbg0, dbg1, dbg2);
+                                       c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
                     ctl->j = lj;
@@ -884,6 +916,41 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
               }
             }
         }
+        if (split) {
+            if (rank == 0) {
+                __syncthreads();      // ctl->nb / ctl->j and the last picks are written
+                if (tid == 0) st_release_cluster_u32(smem_u32(&ctl->pub), (unsigned)ctl->nb | PUB_DONE | (ctl->j >= P.M ? PUB_FINAL : 0u));
+            } else {
+                // ---- worker: stream the batch out of CTA 0's shared memory and apply it ----
+                const unsigned pub_remote = mapa(smem_u32(&ctl->pub), 0u), src = mapa(smem_u32(bpick), 0u);
+                int applied = 0;
+                for (;;) {
+                    if (tid == 0) {
+                        unsigned v = ld_acquire_cluster_u32(pub_remote);
+                        if (!(v & PUB_DONE) && (int)(v & PUB_COUNT) - applied < STREAM_MIN) { __nanosleep(128); v = ld_acquire_cluster_u32(pub_remote); }
+                        qn[3] = (int)v;
+                    }
+                    __syncthreads();
+                    const unsigned v = (unsigned)qn[3];
+                    __syncthreads();
+                    const int n = (int)(v & PUB_COUNT);
+                    const bool done = v & PUB_DONE;
+                    if (v & PUB_FINAL) break;                 // M reached: nothing needs these picks applied
+                    // whole words of 32 picks, at least STREAM_MIN at a time, until the batch is complete
+                    const int hi = done ? n : (n - applied >= STREAM_MIN ? applied + ((n - applied) & ~31) : applied);
+                    if (hi > applied) {
+                        for (int i = applied + tid; i < hi; i += BT) {
+                            const uint4 q = ld_dsmem_v4(src + 16u * (unsigned)i);
+                            bpick[i] = make_float4(__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), 0.0f);
+                        }
+                        __syncthreads();
+                        apply_range(applied, hi);
+                        applied = hi;
+                    }
+                    if (done && applied == n) break;
+                }
+            }
+        }
         cluster_sync_all();
         if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_local += t1 - t0; }
         {
@@ -891,13 +958,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             nb = (int)r0.x;
             j = (int)r0.y;
         }
-        if (rank != 0 && j < P.M) {
-            const unsigned src = mapa(smem_u32(bpick), 0u);
-            for (int i = tid; i < nb; i += BT) {
-                const uint4 v = ld_dsmem_v4(src + 16u * (unsigned)i);
-                bpick[i] = make_float4(__uint_as_float(v.x), __uint_as_float(v.y), __uint_as_float(v.z), 0.0f);
-            }
-            __syncthreads();
+        if (!split && j < P.M) {
+            if (STATS && tid == 0) t0 = clock64();
+            apply_range(0, nb);
+            if (STATS && tid == 0) t_apply += clock64() - t0;
         }
     }
 
@@ -985,7 +1049,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     const int K = ix.K_max > 0 ? ix.K_max : 1;
     const int TC = CPT * LW * 32;
     const int G = (K + 31) / 32;
-    auto slots = [&](int c) { return 32 * ((G + c - 1) / c); };     // voxel slots per CTA
+    auto slots = [&](int c) { const int w = c > 1 ? c - 1 : 1; return 32 * ((G + w - 1) / w); };   // voxel slots per worker CTA
     auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= (size_t)kMaxSmem; };
     if (C == 0) {
         // the largest cluster that (a) leaves every CTA >= 1 024 points, (b) holds the voxel state in
