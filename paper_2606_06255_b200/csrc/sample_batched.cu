@@ -897,7 +897,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 }
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
-                local_fps_hier<CPT, 4>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
+                local_fps_hier<CPT, 2>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
                                        c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
