@@ -588,7 +588,11 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     ix.last_stream = st;
     int n_vox = o.n_vox > 0 ? o.n_vox : auto_n_vox(N);
     if (n_vox > 1024) { set_error("n_vox=%d out of range [1,1024]", n_vox); return FPS_ERR_INVALID; }
-    int tile_points = o.tile_points == 0 ? 64 : (o.tile_points < 0 ? 0 : o.tile_points);
+    // tiles of <= 64 points by default; for very large clouds the tile grows so that the per-voxel state
+    // of the sampling kernel (60 B per tile, shared memory of <= 15 worker CTAs) still fits
+    int auto_tile = 64;
+    while ((long long)auto_tile * 24000 < N) auto_tile *= 2;
+    int tile_points = o.tile_points == 0 ? auto_tile : (o.tile_points < 0 ? 0 : o.tile_points);
     const int vbits = 3 * ilog2_ceil((unsigned long long)n_vox);
     int sb = tile_points > 0 ? (32 - vbits) / 3 : 0;
     if (sb > 4) sb = 4;
