@@ -78,7 +78,7 @@ enum {
 /* Counters and layout facts, summed over the B clouds (fps_get_stats).  With the batched kernel
  * voxel_tests / points_visited / points_computed count (voxel, pick) and (point, pick) pairs.      */
 typedef struct {
-    int32_t B, N;
+    int32_t B, N;             /* clouds; points per cloud (the largest cloud of a ragged index)       */
     int32_t n_vox;            /* resolution actually used                                             */
     int32_t cluster_size, block_threads, voxels_per_thread;
     int64_t K_total;          /* active (tiled) voxels over all clouds                                */
@@ -147,6 +147,23 @@ fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const
  */
 int fps_sample(fps_index_t *h, int32_t M, int32_t start_idx,
                int32_t *out_idx, float *out_mindist, void *stream);
+
+/*
+ * Ragged batches: clouds of different sizes in one index, and per-cloud sample
+ * counts and start points in one launch.  The paper's workloads are variable-size scenes
+ * (Fig. 1); every cloud is sampled exactly as by fps_index_build + fps_sample on it alone.
+ *
+ *   points     DEVICE fp32 [offsets[B]][3]: the clouds one after the other.
+ *   offsets    HOST int32 [B+1], offsets[0] = 0, strictly increasing: cloud b = points offsets[b] ..
+ *              offsets[b+1]-1.  Read during the call only.
+ *   M          HOST int32 [B], 1 <= M[b] <= N_b.       start_idx  HOST int32 [B] or NULL (= all 0).
+ *   out_idx / out_mindist  DEVICE [sum M[b]]: cloud b's samples start at M[0] + .. + M[b-1]; indices
+ *              are relative to the cloud's own first point.
+ * fps_sample (one M, one start_idx) also works on a ragged index if they fit every cloud.
+ */
+fps_index_t *fps_index_build_ragged(const float *points, const int32_t *offsets, int32_t B, const fps_build_opts *opts);
+int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx,
+                      int32_t *out_idx, float *out_mindist, void *stream);
 
 /* Frees the handle and all device memory it owns.  NULL is allowed. */
 void fps_index_destroy(fps_index_t *h);

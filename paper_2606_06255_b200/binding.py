@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
 FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
 
-EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_sample", "fps_index_destroy", "fps_get_stats",
+EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_index_destroy", "fps_get_stats",
            "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
 
 
@@ -75,6 +75,10 @@ def load() -> ctypes.CDLL:
     lib.fps_index_build_ex.argtypes = [vp, i32, i32, ctypes.POINTER(fps_build_opts)]
     lib.fps_sample.restype = ctypes.c_int
     lib.fps_sample.argtypes = [vp, i32, i32, vp, vp, vp]
+    lib.fps_index_build_ragged.restype = vp
+    lib.fps_index_build_ragged.argtypes = [vp, ctypes.POINTER(i32), i32, ctypes.POINTER(fps_build_opts)]
+    lib.fps_sample_ragged.restype = ctypes.c_int
+    lib.fps_sample_ragged.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), vp, vp, vp]
     lib.fps_index_destroy.restype = None
     lib.fps_index_destroy.argtypes = [vp]
     lib.fps_get_stats.restype = ctypes.c_int
@@ -118,8 +122,9 @@ def _opts(n_vox=0, tile_points=0, cluster_size=0, block_threads=0, flags=0, stre
 class Index:
     """Owner of one ``fps_index_t*``.  ``points``: CUDA float32 [B,N,3] (or [N,3])."""
 
-    def __init__(self, handle: int, B: int, N: int, device: torch.device):
+    def __init__(self, handle: int, B: int, N: int, device: torch.device, offsets: list[int] | None = None):
         self.handle, self.B, self.N, self.device = handle, B, N, device
+        self.offsets = offsets          # ragged index: first point of every cloud (+ total), else None
 
     def sample(self, M: int, start_idx: int = 0, out_idx: torch.Tensor | None = None,
                out_mindist: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
@@ -177,6 +182,66 @@ def fps_sample(index: Index, M: int, start_idx: int = 0, out_idx: torch.Tensor |
     if rc != FPS_OK:
         raise FpsError(rc, fps_last_error())
     return out_idx, out_mindist
+
+
+def fps_index_build_ragged(points: torch.Tensor, offsets, *, n_vox: int = 0, tile_points: int = 0, cluster_size: int = 0,
+                           block_threads: int = 0, flags: int = 0, stream: torch.cuda.Stream | None = None,
+                           local_warps: int = 0, cand_per_thread: int = 0) -> Index:
+    """fps_index_build_ragged: ``points`` CUDA float32 [T,3] holds the clouds one after the other,
+    ``offsets`` (B+1 ints, offsets[0] = 0, offsets[B] = T) says where each starts."""
+    lib = load()
+    if not points.is_cuda or points.dtype != torch.float32 or not points.is_contiguous() or points.dim() != 2 \
+            or points.shape[1] != 3:
+        raise ValueError("points must be a contiguous CUDA float32 tensor [T,3]")
+    off = [int(v) for v in offsets]
+    if len(off) < 2 or off[-1] != points.shape[0]:
+        raise ValueError("offsets must hold B+1 entries and end at the number of points")
+    B = len(off) - 1
+    arr = (ctypes.c_int32 * (B + 1))(*off)
+    with torch.cuda.device(points.device):
+        s = stream if stream is not None else torch.cuda.current_stream()
+        o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, s.cuda_stream, local_warps, cand_per_thread)
+        h = lib.fps_index_build_ragged(points.data_ptr(), arr, B, ctypes.byref(o))
+    if not h:
+        raise FpsError(lib.fps_last_status(), fps_last_error())
+    return Index(h, B, max(off[b + 1] - off[b] for b in range(B)), points.device, off)
+
+
+def fps_sample_ragged(index: Index, M, start_idx=None, out_idx: torch.Tensor | None = None,
+                      out_mindist: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
+    """fps_sample_ragged: per-cloud sample counts ``M`` (B ints) and start points (B ints or None = 0).
+    Returns (out_idx int32 [sum M], out_mindist float32 [sum M], out_offsets list of B+1 ints); cloud b's
+    samples are out[out_offsets[b]:out_offsets[b+1]], indices relative to the cloud's first point."""
+    lib = load()
+    if index.handle is None:
+        raise ValueError("index was destroyed")
+    Ms = [int(v) for v in M]
+    if len(Ms) != index.B:
+        raise ValueError("M must hold one entry per cloud")
+    total = sum(max(m, 0) for m in Ms)
+    marr = (ctypes.c_int32 * index.B)(*Ms)
+    sarr = None
+    if start_idx is not None:
+        ss = [int(v) for v in start_idx]
+        if len(ss) != index.B:
+            raise ValueError("start_idx must hold one entry per cloud")
+        sarr = (ctypes.c_int32 * index.B)(*ss)
+    with torch.cuda.device(index.device):
+        if out_idx is None:
+            out_idx = torch.empty((total,), dtype=torch.int32, device=index.device)
+        if out_mindist is None:
+            out_mindist = torch.empty((total,), dtype=torch.float32, device=index.device)
+        if out_idx.dtype != torch.int32 or out_mindist.dtype != torch.float32 or not out_idx.is_contiguous() \
+                or not out_mindist.is_contiguous() or out_idx.numel() < total or out_mindist.numel() < total:
+            raise ValueError("out_idx must be contiguous int32 [sum M] and out_mindist contiguous float32 [sum M]")
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.fps_sample_ragged(index.handle, marr, sarr, out_idx.data_ptr(), out_mindist.data_ptr(), s.cuda_stream)
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    offs = [0]
+    for m in Ms:
+        offs.append(offs[-1] + m)
+    return out_idx, out_mindist, offs
 
 
 def fps_index_destroy(index: Index) -> None:

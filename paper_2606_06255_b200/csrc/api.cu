@@ -31,13 +31,29 @@ const char *fps_last_error(void) { return rfps::g_err; }
 const char *fps_version(void) { return "radiusfps-b200 0.1 (sm_100a)"; }
 int fps_last_status(void) { return rfps::g_status; }
 
-fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const fps_build_opts *opts)
+// common body of the three build entry points: `offsets` (host, [B+1]) or uniform clouds of N points
+static fps_index_t *build_common(const float *points, int32_t N, int32_t B, const int32_t *offsets, const fps_build_opts *opts)
 {
     rfps::g_err[0] = 0;
     rfps::g_status = FPS_ERR_INVALID;
     if (!points) { set_error("points is NULL"); return nullptr; }
-    if (N < 1 || B < 1) { set_error("N=%d and B=%d must be >= 1", N, B); return nullptr; }
-    if ((long long)N * B > (1ll << 30)) { set_error("B*N=%lld exceeds 2^30", (long long)N * B); return nullptr; }
+    if (B < 1) { set_error("B=%d must be >= 1", B); return nullptr; }
+    long long total = 0;
+    int32_t nmax = 0;
+    if (offsets) {
+        if (offsets[0] != 0) { set_error("offsets[0]=%d must be 0", offsets[0]); return nullptr; }
+        for (int b = 0; b < B; ++b) {
+            const long long nb = (long long)offsets[b + 1] - offsets[b];
+            if (nb < 1) { set_error("cloud %d holds %lld points; every cloud needs >= 1", b, nb); return nullptr; }
+            if (nb > nmax) nmax = (int32_t)nb;
+        }
+        total = offsets[B];
+    } else {
+        if (N < 1) { set_error("N=%d and B=%d must be >= 1", N, B); return nullptr; }
+        total = (long long)N * B;
+        nmax = N;
+    }
+    if (total > (1ll << 30)) { set_error("the batch holds %lld points, more than 2^30", total); return nullptr; }
     fps_build_opts o;
     memset(&o, 0, sizeof o);
     if (opts) o = *opts;
@@ -45,7 +61,17 @@ fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const
     fps_index_t *h = new (std::nothrow) fps_index_t();
     if (!h) { set_error("host allocation failed"); return nullptr; }
     h->ix.B = B;
-    h->ix.N = N;
+    h->ix.N = nmax;
+    h->ix.ragged = offsets != nullptr;
+    h->ix.poff_host = (int32_t *)malloc(sizeof(int32_t) * ((size_t)B + 1));
+    h->ix.rag_host = (int32_t *)malloc(sizeof(int32_t) * 3 * ((size_t)B + 1));
+    if (!h->ix.poff_host || !h->ix.rag_host) {
+        set_error("host allocation failed");
+        free(h->ix.poff_host); free(h->ix.rag_host);
+        delete h;
+        return nullptr;
+    }
+    for (int b = 0; b <= B; ++b) h->ix.poff_host[b] = offsets ? offsets[b] : (int32_t)((long long)b * N);
     int rc = rfps::build_index(h->ix, points, o);
     rfps::g_build_rc = rc;
     rfps::g_status = rc;
@@ -60,6 +86,17 @@ fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const
         return nullptr;
     }
     return h;
+}
+
+fps_index_t *fps_index_build_ex(const float *points, int32_t N, int32_t B, const fps_build_opts *opts)
+{
+    return build_common(points, N, B, nullptr, opts);
+}
+
+fps_index_t *fps_index_build_ragged(const float *points, const int32_t *offsets, int32_t B, const fps_build_opts *opts)
+{
+    if (!offsets) { rfps::g_status = FPS_ERR_INVALID; set_error("offsets is NULL"); return nullptr; }
+    return build_common(points, 0, B, offsets, opts);
 }
 
 fps_index_t *fps_index_build(const float *points, int32_t N, int32_t B)
@@ -77,9 +114,49 @@ int fps_sample(fps_index_t *h, int32_t M, int32_t start_idx, int32_t *out_idx, f
         set_error("start_idx=%d must be in [0, N=%d)", start_idx, h->ix.N);
         return FPS_ERR_INVALID;
     }
+    if (h->ix.ragged) {
+        for (int b = 0; b < h->ix.B; ++b) {
+            const int nb = h->ix.poff_host[b + 1] - h->ix.poff_host[b];
+            if (M > nb || start_idx >= nb) {
+                set_error("cloud %d holds %d points: M=%d / start_idx=%d do not fit (use fps_sample_ragged)", b, nb, M, start_idx);
+                return FPS_ERR_INVALID;
+            }
+        }
+    }
+    const int64_t iters = (int64_t)h->ix.B * (M - 1);
     if (h->ix.flags & FPS_FLAG_PER_PICK)
-        return rfps::launch_sample(h->ix, M, start_idx, out_idx, out_mindist, (cudaStream_t)stream);
-    return rfps::launch_sample_batched(h->ix, M, start_idx, out_idx, out_mindist, (cudaStream_t)stream);
+        return rfps::launch_sample(h->ix, M, start_idx, nullptr, iters, out_idx, out_mindist, (cudaStream_t)stream);
+    return rfps::launch_sample_batched(h->ix, M, start_idx, nullptr, iters, out_idx, out_mindist, (cudaStream_t)stream);
+}
+
+int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx, int32_t *out_idx, float *out_mindist,
+                      void *stream)
+{
+    rfps::g_err[0] = 0;
+    if (!h) { set_error("handle is NULL"); return FPS_ERR_INVALID; }
+    if (!M || !out_idx || !out_mindist) { set_error("NULL argument"); return FPS_ERR_INVALID; }
+    rfps::DeviceIndex &ix = h->ix;
+    const int B = ix.B;
+    int32_t *r = ix.rag_host;                 // [3][B+1]: M_b, start_b, output offsets
+    long long off = 0;
+    int64_t iters = 0;
+    for (int b = 0; b < B; ++b) {
+        const int nb = ix.poff_host[b + 1] - ix.poff_host[b];
+        const int sb = start_idx ? start_idx[b] : 0;
+        if (M[b] < 1 || M[b] > nb) { set_error("M[%d]=%d must be in [1, N_b=%d]", b, M[b], nb); return FPS_ERR_INVALID; }
+        if (sb < 0 || sb >= nb) { set_error("start_idx[%d]=%d must be in [0, N_b=%d)", b, sb, nb); return FPS_ERR_INVALID; }
+        r[b] = M[b];
+        r[(B + 1) + b] = sb;
+        r[2 * (B + 1) + b] = (int32_t)off;
+        off += M[b];
+        iters += M[b] - 1;
+    }
+    r[B] = 0; r[(B + 1) + B] = 0; r[2 * (B + 1) + B] = (int32_t)off;
+    cudaStream_t st = (cudaStream_t)stream;
+    // pageable source: the copy is staged before the call returns, so rag_host can be reused by the next call
+    RFPS_CUDA(cudaMemcpyAsync(ix.rag_dev, r, sizeof(int32_t) * 3 * ((size_t)B + 1), cudaMemcpyHostToDevice, st));
+    if (ix.flags & FPS_FLAG_PER_PICK) return rfps::launch_sample(ix, 0, 0, ix.rag_dev, iters, out_idx, out_mindist, st);
+    return rfps::launch_sample_batched(ix, 0, 0, ix.rag_dev, iters, out_idx, out_mindist, st);
 }
 
 void fps_index_destroy(fps_index_t *h)

@@ -53,10 +53,13 @@ __global__ void k_bbox_init(unsigned *bbox, int B)
     }
 }
 
-__global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, int N, unsigned *bbox)
+// Clouds may differ in size (ragged batches): cloud b holds the points [poff[b], poff[b+1]) of the
+// concatenated arrays.  Every kernel below takes `poff`; grids are sized for the largest cloud.
+__global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, const int *__restrict__ poff, unsigned *bbox)
 {
     const int b = blockIdx.y;
-    const float *P = pts + (size_t)b * N * 3;
+    const int base = poff[b], N = poff[b + 1] - base;
+    const float *P = pts + (size_t)base * 3;
     float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
     bool bad = false;
     for (int i = blockIdx.x * blockDim.x + threadIdx.x; i < N; i += gridDim.x * blockDim.x) {
@@ -126,10 +129,12 @@ __device__ __forceinline__ unsigned hilbert3(unsigned x, unsigned y, unsigned z,
     return (spread3(X[0]) << 2) | (spread3(X[1]) << 1) | spread3(X[2]);
 }
 
-__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int N, const unsigned *__restrict__ bbox,
-                                               int n_vox, int hb, int sb, unsigned *__restrict__ keys, int *__restrict__ vals)
+__global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, const int *__restrict__ poff,
+                                               const unsigned *__restrict__ bbox, int n_vox, int hb, int sb,
+                                               unsigned *__restrict__ keys, int *__restrict__ vals)
 {
     const int b = blockIdx.y;
+    const int base = poff[b], N = poff[b + 1] - base;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const unsigned *bb = bbox + b * BBOX_STRIDE;
@@ -142,7 +147,7 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int
     unsigned v[3], s[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        float t = (pts[((size_t)b * N + i) * 3 + a] - lo[a]) / L;
+        float t = (pts[((size_t)base + i) * 3 + a] - lo[a]) / L;
         float f = floorf(t);
         int c = (int)f;
         c = max(0, min(n_vox - 1, c));
@@ -157,8 +162,8 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, int
     // which the sampling kernel's group-level prune relies on.
     unsigned vid = hilbert3(v[0], v[1], v[2], hb);
     unsigned sub = sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
-    keys[(size_t)b * N + i] = (vid << (3 * sb)) | sub;
-    vals[(size_t)b * N + i] = i;
+    keys[(size_t)base + i] = (vid << (3 * sb)) | sub;
+    vals[(size_t)base + i] = i;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -195,12 +200,14 @@ __device__ __forceinline__ int block_excl_scan(int v, int *total, int *sm /*[33]
     return r;
 }
 
+// `poff` != nullptr: array b is the ragged segment [poff[b], poff[b+1]) (n and stride are ignored)
 __global__ void __launch_bounds__(SCAN_T) k_scan_blocksum(const int *__restrict__ in, int n, int stride, int nblk,
-                                                           int *__restrict__ bsum)
+                                                           int *__restrict__ bsum, const int *__restrict__ poff)
 {
     __shared__ int sm[33];
     const int b = blockIdx.y;
-    const int *src = in + (size_t)b * stride;
+    const int *src = in + (poff ? (size_t)poff[b] : (size_t)b * stride);
+    if (poff) n = poff[b + 1] - poff[b];
     int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     int s = 0;
 #pragma unroll
@@ -229,12 +236,14 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_bsums(int *bsum, int nblk, int 
 }
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ in, int *__restrict__ out, int n, int stride,
-                                                        int nblk, const int *__restrict__ bsum)
+                                                        int nblk, const int *__restrict__ bsum, const int *__restrict__ poff)
 {
     __shared__ int sm[33];
     const int b = blockIdx.y;
-    const int *src = in + (size_t)b * stride;
-    int *dst = out + (size_t)b * stride;
+    const size_t off = poff ? (size_t)poff[b] : (size_t)b * stride;
+    if (poff) n = poff[b + 1] - poff[b];
+    const int *src = in + off;
+    int *dst = out + off;
     int base = blockIdx.x * SCAN_TILE + threadIdx.x * SCAN_ITEMS;
     int v[SCAN_ITEMS], s = 0;
 #pragma unroll
@@ -254,14 +263,15 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ i
 // exclusive scan of B arrays of n ints (per-array stride `stride`); totals[b] (device, may be null)
 static int g_launches = 0;   // kernels launched by the build in progress (host-side bookkeeping only)
 
+// n = length of every array, or (poff given) of the longest one
 static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
-                          cudaStream_t st)
+                          cudaStream_t st, const int *poff = nullptr)
 {
     g_launches += 3;
     const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
-    k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp);
+    k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp, poff);
     k_scan_bsums<<<B, SCAN_T, 0, st>>>(bsum_tmp, nblk, totals);
-    k_scan_apply<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, out, n, stride, nblk, bsum_tmp);
+    k_scan_apply<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, out, n, stride, nblk, bsum_tmp, poff);
     RFPS_CUDA(cudaGetLastError());
     return FPS_OK;
 }
@@ -277,16 +287,17 @@ static inline int scan_tmp_ints(int n, int B) { return ((n + SCAN_TILE - 1) / SC
 // ---------------------------------------------------------------------------------------------
 constexpr int RS_CHUNK = 2048, RS_WARPS = 4;
 
-__global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, int N, int nchunk, int shift,
-                                                               int *__restrict__ table)
+__global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, const int *__restrict__ poff,
+                                                               int nchunk, int shift, int *__restrict__ table)
 {
+    const int pbase = poff[blockIdx.y], N = poff[blockIdx.y + 1] - pbase;
     __shared__ int h[RS_WARPS][256];
     const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int c = blockIdx.x * RS_WARPS + w;
     for (int d = lane; d < 256; d += 32) h[w][d] = 0;
     __syncwarp();
     if (c < nchunk) {
-        const unsigned *k = keys + (size_t)b * N;
+        const unsigned *k = keys + (size_t)pbase;
         const int end = min(N, (c + 1) * RS_CHUNK);
         for (int p = c * RS_CHUNK + lane; p < end; p += 32) atomicAdd(&h[w][(k[p] >> shift) & 255u], 1);
         __syncwarp();
@@ -296,9 +307,11 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__
 }
 
 __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned *__restrict__ keys, const int *__restrict__ vals,
-                                                                  int N, int nchunk, int shift, const int *__restrict__ table,
+                                                                  const int *__restrict__ poff, int nchunk, int shift,
+                                                                  const int *__restrict__ table,
                                                                   unsigned *__restrict__ okeys, int *__restrict__ ovals)
 {
+    const int pbase = poff[blockIdx.y], N = poff[blockIdx.y + 1] - pbase;
     __shared__ int base[RS_WARPS][256];
     const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const int c = blockIdx.x * RS_WARPS + w;
@@ -306,10 +319,10 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
     const int *t = table + (size_t)b * 256 * nchunk;
     for (int d = lane; d < 256; d += 32) base[w][d] = t[(size_t)d * nchunk + c];
     __syncwarp();
-    const unsigned *k = keys + (size_t)b * N;
-    const int *v = vals + (size_t)b * N;
-    unsigned *ok = okeys + (size_t)b * N;
-    int *ov = ovals + (size_t)b * N;
+    const unsigned *k = keys + (size_t)pbase;
+    const int *v = vals + (size_t)pbase;
+    unsigned *ok = okeys + (size_t)pbase;
+    int *ov = ovals + (size_t)pbase;
     const int end = min(N, (c + 1) * RS_CHUNK);
     const unsigned lt = (1u << lane) - 1u;
     for (int p0 = c * RS_CHUNK; p0 < end; p0 += 32) {
@@ -332,55 +345,61 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
 // ---------------------------------------------------------------------------------------------
 // a5: active voxels.  heads[p] = 1 where the grid-voxel id changes; scan -> voxel rank.
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_heads(const unsigned *__restrict__ keys, int N, int subbits, int *__restrict__ heads)
+__global__ void __launch_bounds__(256) k_heads(const unsigned *__restrict__ keys, const int *__restrict__ poff, int subbits,
+                                                int *__restrict__ heads)
 {
     const int b = blockIdx.y;
+    const int base = poff[b], N = poff[b + 1] - base;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
-    const unsigned *k = keys + (size_t)b * N;
-    heads[(size_t)b * N + p] = (p == 0 || (k[p] >> subbits) != (k[p - 1] >> subbits)) ? 1 : 0;
+    const unsigned *k = keys + (size_t)base;
+    heads[(size_t)base + p] = (p == 0 || (k[p] >> subbits) != (k[p - 1] >> subbits)) ? 1 : 0;
 }
 
 // voff[b][rank] = p for every head position p
-__global__ void __launch_bounds__(256) k_voxel_offsets(const int *__restrict__ heads, const int *__restrict__ rank, int N,
-                                                        int *__restrict__ voff)
+__global__ void __launch_bounds__(256) k_voxel_offsets(const int *__restrict__ heads, const int *__restrict__ rank,
+                                                        const int *__restrict__ poff, int *__restrict__ voff)
 {
     const int b = blockIdx.y;
+    const int base = poff[b], N = poff[b + 1] - base;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
-    if (heads[(size_t)b * N + p]) voff[(size_t)b * N + rank[(size_t)b * N + p]] = p;
+    if (heads[(size_t)base + p]) voff[(size_t)base + rank[(size_t)base + p]] = p;
 }
 
 // number of tiles of each grid voxel: ceil(cnt / tile_points) (1 if tiling is off)
-__global__ void __launch_bounds__(256) k_ntiles(const int *__restrict__ voff, const int *__restrict__ Kv, int N, int tile_points,
-                                                 int *__restrict__ ntiles)
+__global__ void __launch_bounds__(256) k_ntiles(const int *__restrict__ voff, const int *__restrict__ Kv,
+                                                 const int *__restrict__ poff, int tile_points, int *__restrict__ ntiles)
 {
     const int b = blockIdx.y;
+    const int base = poff[b], N = poff[b + 1] - base;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= N) return;
     const int kv = Kv[b];
     int nt = 0;
     if (k < kv) {
-        const int off = voff[(size_t)b * N + k];
-        const int cnt = (k + 1 < kv ? voff[(size_t)b * N + k + 1] : N) - off;
+        const int off = voff[(size_t)base + k];
+        const int cnt = (k + 1 < kv ? voff[(size_t)base + k + 1] : N) - off;
         nt = tile_points > 0 ? (cnt + tile_points - 1) / tile_points : 1;
     }
-    ntiles[(size_t)b * N + k] = nt;
+    ntiles[(size_t)base + k] = nt;
 }
 
 // vseg[b][tbase[k] + t] = {off + t*chunk, len}: equal-size tiles of the (Morton-ordered) voxel run
 __global__ void __launch_bounds__(256) k_tiles(const int *__restrict__ voff, const int *__restrict__ Kv, const int *__restrict__ ntiles,
-                                                const int *__restrict__ tbase, int N, int K_cap, int2 *__restrict__ vseg)
+                                                const int *__restrict__ tbase, const int *__restrict__ poff, int K_cap,
+                                                int2 *__restrict__ vseg)
 {
     const int b = blockIdx.y;
+    const int base = poff[b], N = poff[b + 1] - base;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     const int kv = Kv[b];
     if (k >= kv) return;
-    const int off = voff[(size_t)b * N + k];
-    const int cnt = (k + 1 < kv ? voff[(size_t)b * N + k + 1] : N) - off;
-    const int nt = ntiles[(size_t)b * N + k];
+    const int off = voff[(size_t)base + k];
+    const int cnt = (k + 1 < kv ? voff[(size_t)base + k + 1] : N) - off;
+    const int nt = ntiles[(size_t)base + k];
     const int chunk = (cnt + nt - 1) / nt;
-    int2 *dst = vseg + (size_t)b * K_cap + tbase[(size_t)b * N + k];
+    int2 *dst = vseg + (size_t)b * K_cap + tbase[(size_t)base + k];
     for (int t = 0; t < nt; ++t) {
         const int s = t * chunk;
         dst[t] = make_int2(off + s, min(chunk, cnt - s));
@@ -390,14 +409,16 @@ __global__ void __launch_bounds__(256) k_tiles(const int *__restrict__ voff, con
 // ---------------------------------------------------------------------------------------------
 // a4: gather AoS -> sorted SoA (+ permutation and its inverse)
 // ---------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pts, const int *__restrict__ order, int N,
+__global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pts, const int *__restrict__ order,
+                                                 const int *__restrict__ poff,
                                                  float *__restrict__ px, float *__restrict__ py, float *__restrict__ pz,
                                                  int *__restrict__ porig, int *__restrict__ pinv)
 {
     const int b = blockIdx.y;
+    const size_t o = (size_t)poff[b];
+    const int N = poff[b + 1] - poff[b];
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
     if (p >= N) return;
-    const size_t o = (size_t)b * N;
     const int i = order[o + p];
     const float *s = pts + (o + i) * 3;
     px[o + p] = s[0];
@@ -422,12 +443,12 @@ __device__ __forceinline__ float d2_rn(float x, float y, float z, float sx, floa
 
 __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, const float *__restrict__ py,
                                                  const float *__restrict__ pz, const int2 *__restrict__ vseg,
-                                                 const int *__restrict__ K, int N, int K_cap, float4 *__restrict__ vgeom,
-                                                 int *__restrict__ maxcnt)
+                                                 const int *__restrict__ K, const int *__restrict__ poff, int K_cap,
+                                                 float4 *__restrict__ vgeom, int *__restrict__ maxcnt)
 {
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31;
-    const float *x = px + (size_t)b * N, *y = py + (size_t)b * N, *z = pz + (size_t)b * N;
+    const float *x = px + (size_t)poff[b], *y = py + (size_t)poff[b], *z = pz + (size_t)poff[b];
     const int Kb = K[b];
     int local_max = 0;
     for (int k = blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); k < Kb; k += gridDim.x * (blockDim.x >> 5)) {
@@ -573,6 +594,8 @@ void free_index(DeviceIndex &ix)
         else cudaFree(ix.arena);
     }
     free(ix.K_host);
+    free(ix.poff_host);
+    free(ix.rag_host);
     ix = DeviceIndex();
 }
 
@@ -583,7 +606,10 @@ struct Scratch {
 
 int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 {
+    // ix.poff_host[0..B] = first point of every cloud in the concatenated arrays (set by the caller);
+    // N = the largest cloud: grids, the voxel bound and the radix chunks are sized for it
     const int B = ix.B, N = ix.N;
+    const int *ph = ix.poff_host;
     cudaStream_t st = (cudaStream_t)o.stream;
     ix.last_stream = st;
     int n_vox = o.n_vox > 0 ? o.n_vox : auto_n_vox(N);
@@ -609,7 +635,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     ix.K_cap = (int)((kb + 31) / 32 * 32);
     ix.G_cap = ix.K_cap / 32;
 
-    const size_t BN = (size_t)B * N;
+    const size_t BN = (size_t)ph[B];      // all points of the batch
     const int nchunk = (N + RS_CHUNK - 1) / RS_CHUNK;
     const size_t table_n = (size_t)256 * nchunk;       // per cloud
     const bool per_pick = o.flags & FPS_FLAG_PER_PICK;
@@ -625,6 +651,8 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
             ix.ggeom = c.take<float4>((size_t)B * ix.G_cap);
             ix.vstate = per_pick ? c.take<uint4>((size_t)B * ix.K_cap) : nullptr;
             ix.K_dev = c.take<int32_t>(B);
+            ix.poff_dev = c.take<int32_t>(B + 1);
+            ix.rag_dev = c.take<int32_t>(3 * (size_t)(B + 1));
             ix.counters = c.take<unsigned long long>(NUM_COUNTERS);
             meta = c.take<unsigned>(8);
         } else {
@@ -661,9 +689,11 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     g_launches = 0;
     const dim3 gN((N + 255) / 256, B);
     RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));
+    RFPS_CUDA(cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st));
+    const int *poff = ix.poff_dev;
     k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(sc.bbox, B);
-    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, N, sc.bbox);
-    k_keys<<<gN, 256, 0, st>>>(points, N, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
+    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, poff, sc.bbox);
+    k_keys<<<gN, 256, 0, st>>>(points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
     g_launches += 3;
 
     // a3: LSD radix sort, 8 bits per pass
@@ -671,24 +701,24 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     int *vin = sc.vA, *vout = sc.vB;
     const dim3 gR((nchunk + RS_WARPS - 1) / RS_WARPS, B);
     for (int shift = 0; shift < keybits; shift += 8) {
-        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, N, nchunk, shift, sc.table);
+        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, poff, nchunk, shift, sc.table);
         if ((rc = scan_exclusive(sc.table, sc.table, (int)table_n, (int)table_n, B, nullptr, sc.bsum, st))) { release_scratch(); return rc; }
-        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, N, nchunk, shift, sc.table, kout, vout);
+        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, poff, nchunk, shift, sc.table, kout, vout);
         std::swap(kin, kout);
         std::swap(vin, vout);
         g_launches += 2;
     }
 
     // a5: grid voxels -> (tiled) segments; a4: gather; a6: spheres
-    k_heads<<<gN, 256, 0, st>>>(kin, N, 3 * sb, sc.heads);
-    if ((rc = scan_exclusive(sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st))) { release_scratch(); return rc; }
-    k_voxel_offsets<<<gN, 256, 0, st>>>(sc.heads, sc.rank, N, sc.voff);
-    k_ntiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, N, tile_points, sc.ntl);
-    if ((rc = scan_exclusive(sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st))) { release_scratch(); return rc; }
-    k_tiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, sc.ntl, sc.tbase, N, ix.K_cap, ix.vseg);
-    k_gather<<<gN, 256, 0, st>>>(points, vin, N, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
+    k_heads<<<gN, 256, 0, st>>>(kin, poff, 3 * sb, sc.heads);
+    if ((rc = scan_exclusive(sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st, poff))) { release_scratch(); return rc; }
+    k_voxel_offsets<<<gN, 256, 0, st>>>(sc.heads, sc.rank, poff, sc.voff);
+    k_ntiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, poff, tile_points, sc.ntl);
+    if ((rc = scan_exclusive(sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st, poff))) { release_scratch(); return rc; }
+    k_tiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, sc.ntl, sc.tbase, poff, ix.K_cap, ix.vseg);
+    k_gather<<<gN, 256, 0, st>>>(points, vin, poff, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
     const int sphere_blocks = std::max(1, std::min((ix.K_cap + 7) / 8, 148 * 8));
-    k_sphere<<<dim3(sphere_blocks, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, N, ix.K_cap, ix.vgeom,
+    k_sphere<<<dim3(sphere_blocks, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
                                                      reinterpret_cast<int *>(meta));
     const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, 148 * 8));
     k_group_sphere<<<dim3(group_blocks, B), 256, 0, st>>>(ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);

@@ -43,7 +43,12 @@ void set_error(const char *fmt, ...);
 constexpr int NUM_COUNTERS = 32;
 
 struct DeviceIndex {
-    int32_t B = 0, N = 0;
+    int32_t B = 0, N = 0;               // clouds; points of the LARGEST cloud (all clouds, if uniform)
+    bool ragged = false;                // built by fps_index_build_ragged
+    int32_t *poff_host = nullptr;       // [B+1] first point of every cloud in the concatenated arrays (malloc)
+    int32_t *poff_dev = nullptr;        // the same on the device
+    int32_t *rag_dev = nullptr;         // [3][B+1] per-call arguments of fps_sample_ragged
+    int32_t *rag_host = nullptr;        // host staging for them (malloc)
     int32_t n_vox = 0, tile_points = 0;
     int32_t K_max = 0, K_cap = 0;       // largest per-cloud K; per-cloud stride of the voxel arrays
     int32_t G_cap = 0;                  // per-cloud stride of the group array (K_cap / 32)
@@ -78,12 +83,14 @@ void free_index(DeviceIndex &ix);
 // stream-ordered device memory from the library's private pool (falls back to cudaMalloc/cudaFree)
 cudaError_t dev_alloc_async(void **p, size_t bytes, cudaStream_t stream);
 void dev_free_async(void *p, cudaStream_t stream);
-int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
-                  cudaStream_t stream);
+// rag_dev: null for a uniform call (M, start_idx apply to every cloud), else device [3][B+1] =
+// {M_b}, {start_b}, {output offset of cloud b}.  iterations = sum over clouds of (M_b - 1), for the stats.
+int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
+                  int32_t *out_idx, float *out_mindist, cudaStream_t stream);
 int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o);
 // exact batched picking (sample_batched.cu)
-int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
-                          cudaStream_t stream);
+int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
+                          int32_t *out_idx, float *out_mindist, cudaStream_t stream);
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o);
 
 }  // namespace rfps

@@ -62,7 +62,9 @@ struct BatchParams {
     const float4 *vgeom, *ggeom;
     const int2 *vseg;
     const int *K;
-    int N, K_cap, G_cap, Kc_cap, M, start_idx;     // Kc_cap: voxel slots per CTA (a multiple of 32)
+    const int *poff;                               // [B+1] first point of every cloud
+    const int *rag;                                // ragged call: [3][B+1] = M_b, start_b, output offsets; else null
+    int B, K_cap, G_cap, Kc_cap, M, start_idx;     // Kc_cap: voxel slots per CTA (a multiple of 32); M, start_idx: uniform call
     int *out_idx;
     float *out_mind;
     unsigned long long *counters;
@@ -535,7 +537,12 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned *qbits = reinterpret_cast<unsigned *>(smem_raw + L.qbits);   // [Gc] voxel-slot-already-queued bits
     int *qn = reinterpret_cast<int *>(smem_raw + L.qn);               // [0..1] queue length (double-buffered), [2] pop counter
 
-    const size_t po = (size_t)b * P.N, vo = (size_t)b * P.K_cap;
+    // this cloud: points [po, po + Nb), Mb samples from start point startb, outputs at obase
+    const size_t po = (size_t)P.poff[b], vo = (size_t)b * P.K_cap;
+    const int Nb = P.poff[b + 1] - P.poff[b];
+    const int Mb = P.rag ? P.rag[b] : P.M;
+    const int startb = P.rag ? P.rag[(P.B + 1) + b] : P.start_idx;
+    const size_t obase = P.rag ? (size_t)P.rag[2 * (P.B + 1) + b] : (size_t)b * P.M;
     const float *__restrict__ px = P.px + po;
     const float *__restrict__ py = P.py + po;
     const float *__restrict__ pz = P.pz + po;
@@ -544,8 +551,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     const float4 *__restrict__ vgeom = P.vgeom + vo;
     const float4 *__restrict__ ggeom = P.ggeom + (size_t)b * P.G_cap;
     const int2 *__restrict__ vseg = P.vseg + vo;
-    int *out_idx = P.out_idx + (size_t)b * P.M;
-    float *out_mind = P.out_mind + (size_t)b * P.M;
+    int *out_idx = P.out_idx + obase;
+    float *out_mind = P.out_mind + obase;
     const int K = P.K[b];
     const int G = (K + 31) / 32;
     // roles: with C > 1 CTA 0 is the PICKER (candidate-set FPS, owns no voxel) and CTAs 1..C-1 are the
@@ -572,8 +579,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[wr + W * gl]; qbits[gl] = 0u; sgthr[gl] = __uint_as_float(F32_NAN_BITS); }
     for (int i = tid; i < Kc * SUBW; i += BT) qmask[i] = 0u;
     {
-        const int chunk = (P.N + C - 1) / C;
-        const int p0 = min(P.N, rank * chunk), p1 = min(P.N, p0 + chunk);
+        const int chunk = (Nb + C - 1) / C;
+        const int p0 = min(Nb, rank * chunk), p1 = min(Nb, p0 + chunk);
         const float inf = __uint_as_float(F32_INF_BITS);
         for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
     }
@@ -585,10 +592,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         ctl->best_hi = ctl->best_lo = 0u;
         ctl->nb = 1;
         ctl->j = 1;
-        const int p = P.pinv[po + P.start_idx];
+        const int p = P.pinv[po + startb];
         bpick[0] = make_float4(px[p], py[p], pz[p], 0.0f);     // s_0 = the caller's start point
         if (rank == 0) {
-            out_idx[0] = P.start_idx;
+            out_idx[0] = startb;
             out_mind[0] = __uint_as_float(F32_INF_BITS);
         }
     }
@@ -765,7 +772,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 
     apply_range(0, 1);      // the start point: every voxel is visited (the paper's initial update, Eq. 13-14)
 
-    while (j < P.M) {
+    while (j < Mb) {
         if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
         // =====================================================================================
         // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
@@ -897,7 +904,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 }
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
-                local_fps_hier<CPT, 2>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, hs, bpick, out_idx, out_mind, tid,
+                local_fps_hier<CPT, 2>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
                                        c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
@@ -907,7 +914,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             } else if constexpr (LW < BT / 32) {
               if (warp < LW) {
                 int lj = j, lnb = 0;
-                local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, P.M, lslot, bpick, out_idx, out_mind, tid);
+                local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, lslot, bpick, out_idx, out_mind, tid);
                 if (tid == 0) {
                     ctl->nb = lnb;
                     ctl->j = lj;
@@ -919,7 +926,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         if (split) {
             if (rank == 0) {
                 __syncthreads();      // ctl->nb / ctl->j and the last picks are written
-                if (tid == 0) st_release_cluster_u32(smem_u32(&ctl->pub), (unsigned)ctl->nb | PUB_DONE | (ctl->j >= P.M ? PUB_FINAL : 0u));
+                if (tid == 0) st_release_cluster_u32(smem_u32(&ctl->pub), (unsigned)ctl->nb | PUB_DONE | (ctl->j >= Mb ? PUB_FINAL : 0u));
             } else {
                 // ---- worker: stream the batch out of CTA 0's shared memory and apply it ----
                 const unsigned pub_remote = mapa(smem_u32(&ctl->pub), 0u), src = mapa(smem_u32(bpick), 0u);
@@ -958,7 +965,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             nb = (int)r0.x;
             j = (int)r0.y;
         }
-        if (!split && j < P.M) {
+        if (!split && j < Mb) {
             if (STATS && tid == 0) t0 = clock64();
             apply_range(0, nb);
             if (STATS && tid == 0) t_apply += clock64() - t0;
@@ -1108,8 +1115,8 @@ static int launch_batched_s(const BatchParams &bp, const DeviceIndex &ix, cudaSt
                                        : launch_batched_one<CPT, LW, false>(bp, ix, st);
 }
 
-int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist,
-                          cudaStream_t st)
+int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
+                          int32_t *out_idx, float *out_mindist, cudaStream_t st)
 {
     BatchParams bp;
     bp.px = ix.px; bp.py = ix.py; bp.pz = ix.pz;
@@ -1117,11 +1124,12 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t
     bp.Dp = ix.Dp;
     bp.vgeom = ix.vgeom; bp.ggeom = ix.ggeom; bp.vseg = ix.vseg;
     bp.K = ix.K_dev;
-    bp.N = ix.N; bp.K_cap = ix.K_cap; bp.G_cap = ix.G_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
+    bp.poff = ix.poff_dev; bp.rag = rag_dev; bp.B = ix.B;
+    bp.K_cap = ix.K_cap; bp.G_cap = ix.G_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
     bp.out_idx = out_idx; bp.out_mind = out_mindist;
     bp.counters = ix.counters;
     if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
-    ix.last_iterations = (int64_t)ix.B * (M - 1);
+    ix.last_iterations = iterations;
     ix.last_stream = st;
     const int key = ix.cand_per_thread * 100 + ix.local_warps;
     switch (key) {

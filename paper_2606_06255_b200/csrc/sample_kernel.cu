@@ -51,7 +51,9 @@ struct SampleParams {
     const int2 *vseg;
     uint4 *vstate;
     const int *K;
-    int N, K_cap, M, start_idx;
+    const int *poff;              // [B+1] first point of every cloud
+    const int *rag;               // ragged call: [3][B+1] = M_b, start_b, output offsets; else null
+    int B, K_cap, M, start_idx;
     int *out_idx;
     float *out_mind;
     unsigned long long *counters;
@@ -82,7 +84,11 @@ __global__ void __launch_bounds__(TB, 1) k_fps_sample(const SampleParams P, cons
     int *qn = reinterpret_cast<int *>(wbest + 32);                            // [4]
     int *queue = qn + 4;                                                      // [VPT * T]
 
-    const size_t po = (size_t)b * P.N, vo = (size_t)b * P.K_cap;
+    const size_t po = (size_t)P.poff[b], vo = (size_t)b * P.K_cap;
+    const int Nb = P.poff[b + 1] - P.poff[b];
+    const int Mb = P.rag ? P.rag[b] : P.M;
+    const int startb = P.rag ? P.rag[(P.B + 1) + b] : P.start_idx;
+    const size_t obase = P.rag ? (size_t)P.rag[2 * (P.B + 1) + b] : (size_t)b * P.M;
     const float *__restrict__ px = P.px + po;
     const float *__restrict__ py = P.py + po;
     const float *__restrict__ pz = P.pz + po;
@@ -108,8 +114,8 @@ __global__ void __launch_bounds__(TB, 1) k_fps_sample(const SampleParams P, cons
     // ---- a7: state reset.  Dist_p = +inf for the points this CTA owns; thresholds = NaN (nothing can
     // be pruned in iteration 1, which therefore performs the paper's "initial update", Eq. 13-14). ----
     {
-        const int p0 = k0 < K ? vseg[k0].x : P.N;
-        const int p1 = k1 < K ? vseg[k1].x : P.N;
+        const int p0 = k0 < K ? vseg[k0].x : Nb;
+        const int p1 = k1 < K ? vseg[k1].x : Nb;
         const float inf = __uint_as_float(0x7f800000u);
         for (int p = p0 + tid; p < p1; p += T) Dp[p] = inf;
     }
@@ -133,12 +139,12 @@ __global__ void __launch_bounds__(TB, 1) k_fps_sample(const SampleParams P, cons
     // ---- s_0 = the caller's start point ----
     float sx, sy, sz;
     {
-        const int p = P.pinv[po + P.start_idx];
+        const int p = P.pinv[po + startb];
         sx = px[p]; sy = py[p]; sz = pz[p];
     }
     if (rank == 0 && tid == 0) {
-        P.out_idx[(size_t)b * P.M] = P.start_idx;
-        P.out_mind[(size_t)b * P.M] = __uint_as_float(0x7f800000u);
+        P.out_idx[obase] = startb;
+        P.out_mind[obase] = __uint_as_float(0x7f800000u);
     }
     if (CL) {
         if (tid == 0) {
@@ -152,7 +158,7 @@ __global__ void __launch_bounds__(TB, 1) k_fps_sample(const SampleParams P, cons
 
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0;
 
-    for (int j = 1; j < P.M; ++j) {
+    for (int j = 1; j < Mb; ++j) {
         // ================= phase A: radius prune (Eq. 25) over the voxels this thread owns =================
         unsigned pushed = 0u;
 #pragma unroll
@@ -268,8 +274,8 @@ __global__ void __launch_bounds__(TB, 1) k_fps_sample(const SampleParams P, cons
             if (tid == 0) mbar_arrive_expect_tx(smem_u32(&mbar[par]), (unsigned)(C * sizeof(XMsg)));
         }
         if (rank == 0 && tid == 0) {
-            P.out_idx[(size_t)b * P.M + j] = (int)(~glo);
-            P.out_mind[(size_t)b * P.M + j] = __uint_as_float(ghi);
+            P.out_idx[obase + j] = (int)(~glo);
+            P.out_mind[obase + j] = __uint_as_float(ghi);
         }
     }
 
@@ -362,7 +368,8 @@ static int launch_vt(const SampleParams &sp, const DeviceIndex &ix, cudaStream_t
     return stats ? launch_one<VPT, TB, false, true>(sp, ix, st) : launch_one<VPT, TB, false, false>(sp, ix, st);
 }
 
-int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_idx, float *out_mindist, cudaStream_t st)
+int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
+                  int32_t *out_idx, float *out_mindist, cudaStream_t st)
 {
     SampleParams sp;
     sp.px = ix.px; sp.py = ix.py; sp.pz = ix.pz;
@@ -370,11 +377,12 @@ int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, int32_t *out_id
     sp.Dp = ix.Dp;
     sp.vgeom = ix.vgeom; sp.vseg = ix.vseg; sp.vstate = ix.vstate;
     sp.K = ix.K_dev;
-    sp.N = ix.N; sp.K_cap = ix.K_cap; sp.M = M; sp.start_idx = start_idx;
+    sp.poff = ix.poff_dev; sp.rag = rag_dev; sp.B = ix.B;
+    sp.K_cap = ix.K_cap; sp.M = M; sp.start_idx = start_idx;
     sp.out_idx = out_idx; sp.out_mind = out_mindist;
     sp.counters = ix.counters;
     if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
-    ix.last_iterations = (int64_t)ix.B * (M - 1);
+    ix.last_iterations = iterations;
     ix.last_stream = st;
     const bool big = ix.block_threads > 512;
     switch (ix.vpt) {

@@ -252,6 +252,53 @@ def test_batch_of_clouds_and_repeat_calls(rf):
         rf.fps_index_destroy(ix)
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
+def test_ragged_batch_matches_the_oracle_cloud_by_cloud(rf, kernel):
+    # clouds of different sizes, per-cloud M and start point, one index, one launch
+    clouds = [inputs.room(5000, 21), inputs.uniform_cube(1, 22), inputs.lidar(7001, 23, n_azimuth=110),
+              inputs.shuffled_lattice(8, 24), inputs.uniform_cube(33, 25), inputs.clustered(2500, 26),
+              inputs.with_duplicates(900, 27, 200), inputs.uniform_cube(4099, 28)]
+    Ms = [1250, 1, 1800, 512, 33, 600, 450, 1031]
+    starts = [0, 0, 7000, 5, 32, 17, 899, 4098]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])]).astype(np.int64)
+    P = torch.from_numpy(np.ascontiguousarray(np.concatenate(clouds, axis=0))).cuda()
+    ix = rf.fps_index_build_ragged(P, off.tolist(), flags=KERNELS[kernel])
+    try:
+        for ms, ss in ((Ms, starts), ([min(m, 7) for m in Ms], None)):       # the handle is reusable
+            idx, mind, ooff = rf.fps_sample_ragged(ix, ms, ss)
+            torch.cuda.synchronize()
+            idx, mind = idx.cpu().numpy(), mind.cpu().numpy()
+            for b, c in enumerate(clouds):
+                ref_i, ref_m = oracle.fps(c, ms[b], ss[b] if ss else 0)
+                assert_same(idx[ooff[b]:ooff[b + 1]], mind[ooff[b]:ooff[b + 1]], ref_i.reshape(-1), ref_m.reshape(-1))
+        # one M / one start for all clouds also works on a ragged index when they fit ...
+        idx, mind = rf.fps_sample(ix, 1, 0)
+        torch.cuda.synchronize()
+        assert idx.cpu().numpy().reshape(-1).tolist() == [0] * len(clouds)
+        # ... and is refused when they do not (cloud 1 holds a single point)
+        with pytest.raises(rf.FpsError) as e:
+            rf.fps_sample(ix, 2, 0)
+        assert e.value.status == rf.FPS_ERR_INVALID
+        with pytest.raises(rf.FpsError):
+            rf.fps_sample_ragged(ix, [m + 100000 for m in Ms])
+    finally:
+        rf.fps_index_destroy(ix)
+
+
+def test_ragged_index_of_equal_clouds_equals_the_uniform_one(rf):
+    w = inputs.scaled("C2", 3000, 700, B=4)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    Pd = torch.from_numpy(P.reshape(-1, 3)).cuda()
+    ix = rf.fps_index_build_ragged(Pd, [b * w.N for b in range(w.B + 1)])
+    try:
+        idx, mind, _ = rf.fps_sample_ragged(ix, [w.M] * w.B)
+        torch.cuda.synchronize()
+        assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+    finally:
+        rf.fps_index_destroy(ix)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
