@@ -165,8 +165,12 @@ def phase_ms(st: dict, sm_mhz) -> dict:
     averaged over clouds, converted with the SM clock sampled during the run)."""
     ghz = (sm_mhz or GHZ_FALLBACK * 1e3) * 1e-3
     f = lambda k: st.get(k, 0) / max(1, st["B"]) / ghz / 1e6  # noqa: E731
-    return {"apply": f("cycles_apply"), "argmax_and_wait": f("cycles_max"), "extract": f("cycles_extract"),
-            "local": f("cycles_local")}
+    workers = max(1, st["B"] * max(1, st["cluster_size"] - 1))
+    g = lambda k: st.get(k, 0) / workers / ghz / 1e6  # noqa: E731
+    return {"picker_cta": {"argmax": f("cycles_max"), "extract": f("cycles_extract"),
+                           "local_incl_wait_for_workers": f("cycles_local"), "apply_if_single_cta": f("cycles_apply")},
+            "worker_cta_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum")},
+            "note": "with cluster_size > 1 the workers apply the picks while the picker CTA is still producing them"}
 
 
 def time_config(rf, torch, w, P_host, steps, warmup, opts, flush):

@@ -299,6 +299,25 @@ def test_ragged_index_of_equal_clouds_equals_the_uniform_one(rf):
         rf.fps_index_destroy(ix)
 
 
+@pytest.mark.parametrize("cluster", [0, 2, 5])
+def test_repeated_launches_under_load_are_identical(rf, cluster):
+    # the batched kernel passes data between CTAs with release/acquire flags, DSMEM atomics and dynamic work
+    # queues; compute-sanitizer is not available on the GPU pool, so races are hunted by repetition: 16
+    # clouds in flight, 25 launches, every one must equal the oracle bit for bit
+    w = inputs.scaled("C2", 4000, 1000, B=16)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    Pd = torch.from_numpy(P).cuda()
+    ix = rf.fps_index_build(Pd, cluster_size=cluster)
+    try:
+        for _ in range(25):
+            idx, mind = rf.fps_sample(ix, w.M, 0)
+            torch.cuda.synchronize()
+            assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+    finally:
+        rf.fps_index_destroy(ix)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
