@@ -13,7 +13,9 @@
 // one by one, and a voxel may be tested against a pick with a stale (larger) Dist_v because that
 // only makes the prune test of Eq. 25 more conservative.
 //
-// One round, one thread-block cluster per cloud (all CTAs unless noted):
+// One thread-block cluster per cloud.  With more than one CTA, CTA 0 is the PICKER (LOCAL) and CTAs
+// 1..C-1 are the WORKERS (own the voxels: APPLY, MAX, EXTRACT); the workers apply a batch while the
+// picker is still producing it (release/acquire flag + DSMEM copies).  One round:
 //   APPLY    the nb picks of the previous batch, 128 at a time.  Prune (a9, squared-domain Eq. 25 with
 //            fp32 margins) on two levels: a work unit = (group of 32 voxels, 32 picks) tests the picks
 //            against the group sphere, then the group's voxels against the survivors; voxels with

@@ -318,6 +318,43 @@ def test_repeated_launches_under_load_are_identical(rf, cluster):
         rf.fps_index_destroy(ix)
 
 
+@pytest.mark.parametrize("B,N,M,gen", [(100, 2048, 512, "cube"), (300, 1500, 300, "room")])
+def test_many_clouds_more_than_resident_clusters(rf, B, N, M, gen):
+    # B = 300 exceeds the clusters that can be resident at once: the clouds run in waves
+    P = np.stack([(inputs.uniform_cube(N, 100 + b) if gen == "cube" else inputs.room(N, 500 + b)) for b in range(B)])
+    ref = oracle.fps(P, M, 0)
+    gi, gm, _ = run_gpu(rf, P, M)
+    assert_same(gi, gm, *ref)
+
+
+def test_sampling_every_point_of_a_cloud(rf):
+    P = inputs.room(5000, 7)
+    ref = oracle.fps(P, 5000, 3)
+    for kflag in KERNELS.values():
+        gi, gm, _ = run_gpu(rf, P, 5000, 3, flags=kflag)
+        assert_same(gi, gm, *ref)
+        assert sorted(gi.reshape(-1).tolist()) == list(range(5000))
+
+
+def test_three_million_points_tile_size_grows(rf):
+    """Beyond ~1.5 M points the automatic tile size grows so that the voxel state still fits the workers'
+    shared memory; properties that hold at any size + sampled min-distances recomputed from the outputs."""
+    N, M = 3_000_000, 20_000
+    P = inputs.lidar(N, 9, n_beams=128, elev_deg=(-25.0, 15.0), n_azimuth=23439, n_objects=200, max_range=120.0)
+    gi, gm, st = run_gpu(rf, P, M)
+    assert st["max_voxel_points"] > 64 and st["cluster_size"] == 16
+    gi, gm = gi.reshape(-1), gm.reshape(-1)
+    assert gi[0] == 0 and np.isinf(gm[0]) and np.all(gm[1:] <= gm[:-1]) and np.unique(gi).size == M
+    S = P[gi]
+    for j in [1, 2, 100, 5000, M - 1]:
+        d = (S[:j] - S[j]).astype(np.float32)
+        d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
+        assert d2.min().view(np.uint32) == gm[j].view(np.uint32), j
+    d = (P - P[0]).astype(np.float32)
+    d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
+    assert gi[1] == int(np.argmax(d2)) and gm[1].view(np.uint32) == d2.max().view(np.uint32)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
