@@ -62,7 +62,7 @@ typedef struct {
     int32_t local_warps;   /* batched kernel, local phase: 0 = choose; 16 = hierarchical (all 16 warps hold
                               candidates, one warp picks from the top <= 128 of them); 1,2,4,8 = flat FPS on
                               that many warps                                                            */
-    int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2,4 (hierarchical) or 4,8,16
+    int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2,4,8 (hierarchical) or 4,8,16
                               (flat); candidate capacity = 32 * local_warps * cand_per_thread          */
 } fps_build_opts;
 

@@ -825,7 +825,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             const unsigned cX0 = mapa(smem_u32(cX), 0u), cY0 = mapa(smem_u32(cY), 0u), cZ0 = mapa(smem_u32(cZ), 0u),
                            cD0 = mapa(smem_u32(cD), 0u), cO0 = mapa(smem_u32(cO), 0u);
             for (int a = 0; a < MAX_ATTEMPTS; ++a) {
-                const unsigned tb = __float_as_uint(__fmul_rn(Dmax, __fsub_rn(1.0f, g)));
+                // a cloud that fits the candidate buffer whole is taken whole (tau = 0: every point that can
+                // still be picked at a positive distance); the local phase then runs without global rounds
+                const unsigned tb = (a == 0 && Nb <= TC) ? 0u : __float_as_uint(__fmul_rn(Dmax, __fsub_rn(1.0f, g)));
                 if (!(tb < ghi)) break;                      // g too small to separate tau from Dmax
                 const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[a]), 0u);
                 for (int base = 0; base < Kc; base += BT) {
@@ -1046,10 +1048,12 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     // local_warps = 16: hierarchical local phase (all warps hold candidates, one warp picks);
     // 1..8: flat local phase on that many warps
     int LW = o.local_warps > 0 ? o.local_warps : 16;
-    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW == 16 ? 2 : 8);
-    const bool ok_shape = LW == 16 ? (CPT == 2 || CPT == 4) : ((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16));
+    // small clouds are held whole in the picker's registers: 4 candidates per thread up to 2 048 points,
+    // 8 up to 4 096; larger clouds work on the top ~1 024 candidates per round
+    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW == 16 ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : 2))) : 8);
+    const bool ok_shape = LW == 16 ? (CPT == 2 || CPT == 4 || CPT == 8) : ((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16));
     if (!ok_shape) {
-        set_error("local_warps=%d / cand_per_thread=%d: use 16 with 2 or 4 (hierarchical), or 1,2,4,8 with 4,8,16 (flat)", LW, CPT);
+        set_error("local_warps=%d / cand_per_thread=%d: use 16 with 2, 4 or 8 (hierarchical), or 1,2,4,8 with 4,8,16 (flat)", LW, CPT);
         return FPS_ERR_INVALID;
     }
     int C = o.cluster_size;
@@ -1137,6 +1141,7 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
     switch (key) {
         case 216: return launch_batched_s<2, 16>(bp, ix, st);
         case 416: return launch_batched_s<4, 16>(bp, ix, st);
+        case 816: return launch_batched_s<8, 16>(bp, ix, st);
         case 804: return launch_batched_s<8, 4>(bp, ix, st);
         case 801: return launch_batched_s<8, 1>(bp, ix, st);
         case 802: return launch_batched_s<8, 2>(bp, ix, st);

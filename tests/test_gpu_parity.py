@@ -90,7 +90,7 @@ def test_every_cluster_size(rf, name, cluster, kernel):
     assert_same(gi, gm, *ref)
 
 
-LOCAL_SHAPES = [(16, 2), (16, 4), (4, 8), (1, 8), (2, 8), (8, 8), (4, 4), (8, 4), (4, 16), (8, 16)]
+LOCAL_SHAPES = [(16, 2), (16, 4), (16, 8), (4, 8), (1, 8), (2, 8), (8, 8), (4, 4), (8, 4), (4, 16), (8, 16)]
 
 
 @pytest.mark.parametrize("lw,cpt", LOCAL_SHAPES)
