@@ -165,6 +165,15 @@ fps_index_t *fps_index_build_ragged(const float *points, const int32_t *offsets,
 int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx,
                       int32_t *out_idx, float *out_mindist, void *stream);
 
+/*
+ * fps_gather_xyz -- coordinates of sampled points: out_xyz[..][j] = the input point
+ * with original index idx[..][j], read from the index's own sorted copy (the caller's `points` buffer is not
+ * needed any more).  idx: DEVICE int32, out_xyz: DEVICE fp32, 3 floats per sample, same layout as idx:
+ * [B][M] for M >= 1; M = 0 means the ragged layout of the last fps_sample_ragged call on this handle.
+ * An index outside its cloud yields NaN coordinates.  Asynchronous on `stream`.
+ */
+int fps_gather_xyz(fps_index_t *h, const int32_t *idx, int32_t M, float *out_xyz, void *stream);
+
 /* Frees the handle and all device memory it owns.  NULL is allowed. */
 void fps_index_destroy(fps_index_t *h);
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
 FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
 
-EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_index_destroy", "fps_get_stats",
+EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_index_destroy", "fps_get_stats",
            "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
 
 
@@ -79,6 +79,8 @@ def load() -> ctypes.CDLL:
     lib.fps_index_build_ragged.argtypes = [vp, ctypes.POINTER(i32), i32, ctypes.POINTER(fps_build_opts)]
     lib.fps_sample_ragged.restype = ctypes.c_int
     lib.fps_sample_ragged.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), vp, vp, vp]
+    lib.fps_gather_xyz.restype = ctypes.c_int
+    lib.fps_gather_xyz.argtypes = [vp, vp, i32, vp, vp]
     lib.fps_index_destroy.restype = None
     lib.fps_index_destroy.argtypes = [vp]
     lib.fps_get_stats.restype = ctypes.c_int
@@ -242,6 +244,23 @@ def fps_sample_ragged(index: Index, M, start_idx=None, out_idx: torch.Tensor | N
     for m in Ms:
         offs.append(offs[-1] + m)
     return out_idx, out_mindist, offs
+
+
+def fps_gather_xyz(index: Index, idx: torch.Tensor, M: int | None = None, stream: torch.cuda.Stream | None = None):
+    """fps_gather_xyz: coordinates of the sampled points.  ``idx`` int32 [B,M] from fps_sample (M taken from
+    its shape) or the flat tensor of the last fps_sample_ragged call (pass M=0).  Returns float32 [...,3]."""
+    lib = load()
+    if idx.dtype != torch.int32 or not idx.is_cuda or not idx.is_contiguous():
+        raise ValueError("idx must be a contiguous CUDA int32 tensor")
+    if M is None:
+        M = idx.shape[-1] if idx.dim() == 2 else 0
+    with torch.cuda.device(index.device):
+        out = torch.empty(tuple(idx.shape) + (3,), dtype=torch.float32, device=index.device)
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.fps_gather_xyz(index.handle, idx.data_ptr(), int(M), out.data_ptr(), s.cuda_stream)
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return out
 
 
 def fps_index_destroy(index: Index) -> None:

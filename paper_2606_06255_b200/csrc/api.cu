@@ -150,6 +150,7 @@ int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx
         r[2 * (B + 1) + b] = (int32_t)off;
         off += M[b];
         iters += M[b] - 1;
+        if (M[b] > ix.rag_M_max || b == 0) ix.rag_M_max = b == 0 ? M[b] : (M[b] > ix.rag_M_max ? M[b] : ix.rag_M_max);
     }
     r[B] = 0; r[(B + 1) + B] = 0; r[2 * (B + 1) + B] = (int32_t)off;
     cudaStream_t st = (cudaStream_t)stream;
@@ -157,6 +158,18 @@ int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx
     RFPS_CUDA(cudaMemcpyAsync(ix.rag_dev, r, sizeof(int32_t) * 3 * ((size_t)B + 1), cudaMemcpyHostToDevice, st));
     if (ix.flags & FPS_FLAG_PER_PICK) return rfps::launch_sample(ix, 0, 0, ix.rag_dev, iters, out_idx, out_mindist, st);
     return rfps::launch_sample_batched(ix, 0, 0, ix.rag_dev, iters, out_idx, out_mindist, st);
+}
+
+int fps_gather_xyz(fps_index_t *h, const int32_t *idx, int32_t M, float *out_xyz, void *stream)
+{
+    rfps::g_err[0] = 0;
+    if (!h || !idx || !out_xyz) { set_error("NULL argument"); return FPS_ERR_INVALID; }
+    if (M < 0) { set_error("M=%d must be >= 0", M); return FPS_ERR_INVALID; }
+    if (M == 0) {
+        if (h->ix.rag_M_max <= 0) { set_error("M=0 means 'the layout of the last fps_sample_ragged call', but there was none"); return FPS_ERR_INVALID; }
+        return rfps::launch_gather_xyz(h->ix, idx, 0, h->ix.rag_M_max, h->ix.rag_dev, out_xyz, (cudaStream_t)stream);
+    }
+    return rfps::launch_gather_xyz(h->ix, idx, M, M, nullptr, out_xyz, (cudaStream_t)stream);
 }
 
 void fps_index_destroy(fps_index_t *h)

@@ -49,6 +49,7 @@ struct DeviceIndex {
     int32_t *poff_dev = nullptr;        // the same on the device
     int32_t *rag_dev = nullptr;         // [3][B+1] per-call arguments of fps_sample_ragged
     int32_t *rag_host = nullptr;        // host staging for them (malloc)
+    int32_t rag_M_max = 0;              // largest M_b of the last fps_sample_ragged call (0 = none yet)
     int32_t n_vox = 0, tile_points = 0;
     int32_t K_max = 0, K_cap = 0;       // largest per-cloud K; per-cloud stride of the voxel arrays
     int32_t G_cap = 0;                  // per-cloud stride of the group array (K_cap / 32)
@@ -88,6 +89,8 @@ void dev_free_async(void *p, cudaStream_t stream);
 int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
                   int32_t *out_idx, float *out_mindist, cudaStream_t stream);
 int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o);
+int launch_gather_xyz(DeviceIndex &ix, const int32_t *idx, int32_t M, int32_t M_max, const int32_t *rag_dev, float *out_xyz,
+                      cudaStream_t stream);
 // exact batched picking (sample_batched.cu)
 int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
                           int32_t *out_idx, float *out_mindist, cudaStream_t stream);

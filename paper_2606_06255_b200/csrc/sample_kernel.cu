@@ -395,4 +395,38 @@ int launch_sample(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *
     return FPS_ERR_INVALID;
 }
 
+// ---------------------------------------------------------------------------------------------
+// gathered coordinates of the samples (out_xyz).  One thread per sample: original
+// index -> sorted position (pinv) -> SoA coordinates.  rag: layout of the last fps_sample_ragged call.
+// ---------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_gather_xyz(const float *__restrict__ px, const float *__restrict__ py,
+                                                     const float *__restrict__ pz, const int *__restrict__ pinv,
+                                                     const int *__restrict__ poff, const int *__restrict__ rag, int B, int M,
+                                                     const int *__restrict__ idx, float *__restrict__ out_xyz)
+{
+    const int b = blockIdx.y;
+    const int Mb = rag ? rag[b] : M;
+    const size_t obase = rag ? (size_t)rag[2 * (B + 1) + b] : (size_t)b * M;
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    if (j >= Mb) return;
+    const int Nb = poff[b + 1] - poff[b];
+    const int i = idx[obase + j];
+    float x = __uint_as_float(F32_NAN_BITS), y = x, z = x;       // an index outside the cloud gives NaN
+    if (i >= 0 && i < Nb) {
+        const size_t p = (size_t)poff[b] + pinv[(size_t)poff[b] + i];
+        x = px[p]; y = py[p]; z = pz[p];
+    }
+    float *o = out_xyz + 3 * (obase + j);
+    o[0] = x; o[1] = y; o[2] = z;
+}
+
+int launch_gather_xyz(DeviceIndex &ix, const int32_t *idx, int32_t M, int32_t M_max, const int32_t *rag_dev, float *out_xyz,
+                      cudaStream_t st)
+{
+    k_gather_xyz<<<dim3((unsigned)((M_max + 255) / 256), (unsigned)ix.B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.pinv, ix.poff_dev,
+                                                                                      rag_dev, ix.B, M, idx, out_xyz);
+    RFPS_CUDA(cudaGetLastError());
+    return FPS_OK;
+}
+
 }  // namespace rfps

@@ -355,6 +355,32 @@ def test_three_million_points_tile_size_grows(rf):
     assert gi[1] == int(np.argmax(d2)) and gm[1].view(np.uint32) == d2.max().view(np.uint32)
 
 
+def test_gather_xyz_uniform_and_ragged(rf):
+    w = inputs.scaled("C2", 3000, 700, B=3)
+    P = inputs.make_batch(w)
+    ix = rf.fps_index_build(torch.from_numpy(P).cuda())
+    try:
+        idx, _ = rf.fps_sample(ix, w.M, 0)
+        xyz = rf.fps_gather_xyz(ix, idx)
+        torch.cuda.synchronize()
+        gi = idx.cpu().numpy()
+        assert np.array_equal(xyz.cpu().numpy(), np.stack([P[b][gi[b]] for b in range(w.B)]))
+    finally:
+        rf.fps_index_destroy(ix)
+    clouds = [inputs.room(2000, 31), inputs.uniform_cube(17, 32), inputs.lidar(3001, 33, n_azimuth=60)]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])])
+    ix = rf.fps_index_build_ragged(torch.from_numpy(np.concatenate(clouds)).cuda(), off.tolist())
+    try:
+        idx, _, ooff = rf.fps_sample_ragged(ix, [500, 17, 64], [3, 16, 0])
+        xyz = rf.fps_gather_xyz(ix, idx, 0)
+        torch.cuda.synchronize()
+        gi, gx = idx.cpu().numpy(), xyz.cpu().numpy()
+        for b, c in enumerate(clouds):
+            assert np.array_equal(gx[ooff[b]:ooff[b + 1]], c[gi[ooff[b]:ooff[b + 1]]])
+    finally:
+        rf.fps_index_destroy(ix)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
