@@ -151,6 +151,21 @@ def ncu_traffic(workload: str, per_pick: bool):
     return None
 
 
+def latency_report(rf, kern_s, w, sm_mhz) -> dict:
+    """The bound that binds: the M-1 picks of a cloud are sequentially dependent, so `fps_sample` cannot be
+    faster than (M-1) x the dependent chain of one pick.  The floor is MEASURED live: the bare chain on one
+    warp with 1 candidate per lane (fps_pick_chain_cycles; the kernel's pick warp holds 2 per lane).  The
+    clouds of a batch run in parallel, so the achieved figure is kernel time / (M-1) per cloud."""
+    ghz = (sm_mhz or GHZ_FALLBACK * 1e3) * 1e-3
+    floor1 = rf.fps_pick_chain_cycles(1, 8192)
+    floor2 = rf.fps_pick_chain_cycles(2, 8192)
+    achieved = kern_s * ghz * 1e9 / max(1, w.M - 1)
+    return {"bound": "latency", "unit": "SM cycles per pick", "floor": floor1, "floor_2_candidates_per_lane": floor2,
+            "achieved": achieved, "frac": floor1 / achieved,
+            "note": "floor = bare chain update -> lane max -> redux(max D) -> redux(slot id) -> 3 shared loads on one warp, "
+                    "no tie handling, no candidate selection, no global rounds"}
+
+
 def opts_from(args) -> dict:
     return dict(n_vox=args.n_vox, tile_points=args.tile_points, cluster_size=args.cluster_size,
                 block_threads=args.block_threads, local_warps=args.local_warps, cand_per_thread=args.cand_per_thread,
@@ -350,6 +365,7 @@ def main():
                                  "the kernel is bound by the latency of its pick chain (DESIGN.md section 8)",
                          "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9,
                          "us_per_pick": kern_s * 1e6 / max(1, w.M - 1)},
+            "latency": latency_report(rf, kern_s, w, clk.get("sm_mhz")),
             "phases_ms_per_cloud": None if args.per_pick else phase_ms(st_counts, clk.get("sm_mhz")),
             "counters": {k: st_counts[k] for k in ("iterations", "group_tests", "voxel_tests", "voxels_visited",
                                                    "points_visited", "points_computed", "effective", "rounds",

@@ -174,6 +174,15 @@ int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx
  */
 int fps_gather_xyz(fps_index_t *h, const int32_t *idx, int32_t M, float *out_xyz, void *stream);
 
+/*
+ * fps_pick_chain_cycles -- measurement aid, not part of the path: SM cycles per pick of the bare dependent
+ * chain of one pick on one warp (update -> lane max -> redux(max D) -> redux(slot id) -> 3 shared loads)
+ * with cand_per_lane = 1, 2 or 4 candidates per lane, averaged over `iters` picks.  This is the latency
+ * floor of the sequential part of FPS on this GPU; bench.py reports the achieved
+ * cycles per pick against it.  cycles_per_pick: HOST.  Synchronous, default stream.
+ */
+int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_per_pick);
+
 /* Frees the handle and all device memory it owns.  NULL is allowed. */
 void fps_index_destroy(fps_index_t *h);
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
 FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
 
-EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_index_destroy", "fps_get_stats",
+EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_pick_chain_cycles", "fps_index_destroy", "fps_get_stats",
            "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
 
 
@@ -81,6 +81,8 @@ def load() -> ctypes.CDLL:
     lib.fps_sample_ragged.argtypes = [vp, ctypes.POINTER(i32), ctypes.POINTER(i32), vp, vp, vp]
     lib.fps_gather_xyz.restype = ctypes.c_int
     lib.fps_gather_xyz.argtypes = [vp, vp, i32, vp, vp]
+    lib.fps_pick_chain_cycles.restype = ctypes.c_int
+    lib.fps_pick_chain_cycles.argtypes = [i32, i32, ctypes.POINTER(ctypes.c_float)]
     lib.fps_index_destroy.restype = None
     lib.fps_index_destroy.argtypes = [vp]
     lib.fps_get_stats.restype = ctypes.c_int
@@ -261,6 +263,15 @@ def fps_gather_xyz(index: Index, idx: torch.Tensor, M: int | None = None, stream
     if rc != FPS_OK:
         raise FpsError(rc, fps_last_error())
     return out
+
+
+def fps_pick_chain_cycles(cand_per_lane: int = 2, iters: int = 8192) -> float:
+    """fps_pick_chain_cycles: SM cycles per pick of the bare one-warp pick chain (the latency floor)."""
+    out = ctypes.c_float(0.0)
+    rc = load().fps_pick_chain_cycles(int(cand_per_lane), int(iters), ctypes.byref(out))
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return float(out.value)
 
 
 def fps_index_destroy(index: Index) -> None:

@@ -172,6 +172,13 @@ int fps_gather_xyz(fps_index_t *h, const int32_t *idx, int32_t M, float *out_xyz
     return rfps::launch_gather_xyz(h->ix, idx, M, M, nullptr, out_xyz, (cudaStream_t)stream);
 }
 
+int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_per_pick)
+{
+    rfps::g_err[0] = 0;
+    if (!cycles_per_pick || iters < 1) { set_error("bad argument"); return FPS_ERR_INVALID; }
+    return rfps::measure_pick_chain(cand_per_lane, iters, cycles_per_pick);
+}
+
 void fps_index_destroy(fps_index_t *h)
 {
     if (!h) return;

@@ -95,6 +95,7 @@ int launch_gather_xyz(DeviceIndex &ix, const int32_t *idx, int32_t M, int32_t M_
 int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,
                           int32_t *out_idx, float *out_mindist, cudaStream_t stream);
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o);
+int measure_pick_chain(int cand_per_lane, int iters, float *cycles_per_pick);
 
 }  // namespace rfps
 

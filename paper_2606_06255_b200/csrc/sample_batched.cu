@@ -408,11 +408,18 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                     z2[c] = ok ? hs->sZ[i] : 0.0f;
                     d2v[c] = ok ? hs->sD[i] : 0.0f;         // padding never exceeds tau2
                 }
-                // picks are logged as {slot id, D bits}: lane (n & 31) keeps pick n in registers and the warp
-                // writes 32 of them at a time, so the loop itself holds no global store and no dependent load
+                // The picks of the sub-round are logged as {slot id, D bits} in shared memory and emitted after
+                // the loop.  Fast path: KCH picks at a time, speculatively and without a branch in the dependent
+                // chain -- termination (max <= tau2) and exact ties are only recorded; afterwards the prefix of
+                // picks before the first such event is accepted.  Picks computed beyond it are discarded with
+                // the register state (the sub-round ends there, or the chunk is redone pick by pick).
                 const int nb0 = nbl, j0 = jl;
-                unsigned mywid = 0u, myd = 0u;
-                for (;;) {
+#ifndef RFPS_KCH
+#define RFPS_KCH 16
+#endif
+                constexpr int KCH = RFPS_KCH;
+                // one pick, fully checked: returns false when the sub-round is over
+                auto careful_pick = [&]() -> bool {
                     float bm = d2v[0];
 #pragma unroll
                     for (int c = 1; c < CPT2; ++c) bm = fmaxf(bm, d2v[c]);
@@ -423,7 +430,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         if (d2v[c] == bm) { idmx = max(idmx, (unsigned)(c * 32 + lane + 1)); idmn = min(idmn, (unsigned)(c * 32 + lane + 1)); }
                     const unsigned hi = __float_as_uint(bm);
                     const unsigned ghi = __reduce_max_sync(FULL, hi);
-                    if (!(ghi > tau2bits)) break;            // restricted max no longer above everything outside C2
+                    if (!(ghi > tau2bits)) return false;     // restricted max no longer above everything outside C2
                     const bool top = hi == ghi;
                     const unsigned gmx = __reduce_max_sync(FULL, top ? idmx : 0u);
                     const unsigned gmn = __reduce_min_sync(FULL, top ? idmn : 0x7fffffffu);
@@ -445,18 +452,68 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         wid = __reduce_max_sync(FULL, mine) - 1u;
                     }
                     const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
-                    const int n = nbl - nb0;
-                    if (lane == (n & 31)) { mywid = wid; myd = ghi; }
+                    if (lane == 0) hs->plist[nbl - nb0] = make_uint2(wid, ghi);
                     ++jl;
                     ++nbl;
-                    if ((n & 31) == 31) hs->plist[n - 31 + lane] = make_uint2(mywid, myd);
-                    if (jl >= M || nbl >= PB) break;
+                    if (jl >= M || nbl >= PB) return false;
 #pragma unroll
                     for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], d2_rn(x2[c], y2[c], z2[c], sx, sy, sz));
+                    return true;
+                };
+                for (bool go = true; go;) {
+                    if (min(M - jl, PB - nbl) <= KCH) {      // near the end of the output or of the batch buffer
+                        go = careful_pick();
+                        continue;
+                    }
+                    float dsave[CPT2];
+#pragma unroll
+                    for (int c = 0; c < CPT2; ++c) dsave[c] = d2v[c];
+                    unsigned gh[KCH], wd[KCH];
+                    bool over = false, tie = false;          // "max <= tau2 seen" / "exact tie seen before that"
+#pragma unroll
+                    for (int p = 0; p < KCH; ++p) {
+                        float bm = d2v[0];
+#pragma unroll
+                        for (int c = 1; c < CPT2; ++c) bm = fmaxf(bm, d2v[c]);
+                        unsigned idmx = 0u, idmn = 0x7fffffffu;
+#pragma unroll
+                        for (int c = 0; c < CPT2; ++c)
+                            if (d2v[c] == bm) { idmx = max(idmx, (unsigned)(c * 32 + lane + 1)); idmn = min(idmn, (unsigned)(c * 32 + lane + 1)); }
+                        const unsigned hi = __float_as_uint(bm);
+                        const unsigned ghi = __reduce_max_sync(FULL, hi);
+                        const bool top = hi == ghi;
+                        const unsigned gmx = __reduce_max_sync(FULL, top ? idmx : 0u);
+                        const unsigned gmn = __reduce_min_sync(FULL, top ? idmn : 0x7fffffffu);
+                        const unsigned wid = gmx - 1u;       // always a valid slot: some lane is top
+                        over |= !(ghi > tau2bits);
+                        tie |= (gmx != gmn) && !over;
+                        gh[p] = ghi;
+                        wd[p] = wid;
+                        const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
+#pragma unroll
+                        for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], d2_rn(x2[c], y2[c], z2[c], sx, sy, sz));
+                    }
+                    if (tie) {                               // rare: redo this chunk pick by pick
+#pragma unroll
+                        for (int c = 0; c < CPT2; ++c) d2v[c] = dsave[c];
+                        for (int p = 0; p < KCH && go; ++p) go = careful_pick();
+                        continue;
+                    }
+                    int acc = KCH;                           // picks before the first "max <= tau2"
+#pragma unroll
+                    for (int p = KCH - 1; p >= 0; --p)
+                        if (!(gh[p] > tau2bits)) acc = p;
+                    if (lane == 0) {
+#pragma unroll
+                        for (int p = 0; p < KCH; ++p)
+                            if (p < acc) hs->plist[nbl - nb0 + p] = make_uint2(wd[p], gh[p]);
+                    }
+                    jl += acc;
+                    nbl += acc;
+                    go = acc == KCH;
                 }
                 {
-                    const int n = nbl - nb0;                 // flush the partial last group, then emit
-                    if ((n & 31) != 0 && lane < (n & 31)) hs->plist[(n & ~31) + lane] = make_uint2(mywid, myd);
+                    const int n = nbl - nb0;                 // emit the sub-round's picks
                     __syncwarp();
                     for (int i = lane; i < n; i += 32) {
                         const uint2 pk = hs->plist[i];
@@ -1153,6 +1210,71 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
     }
     set_error("unsupported local shape cand_per_thread=%d local_warps=%d", ix.cand_per_thread, ix.local_warps);
     return FPS_ERR_INVALID;
+}
+
+// ---------------------------------------------------------------------------------------------
+// Latency floor of one pick (bench.py "latency": the roofline that actually binds this path).  One warp,
+// 32*CPL candidates in registers, the bare dependent chain of a pick and nothing else:
+//   update (d2, min) -> lane max -> redux.max(D bits) -> redux.max(slot id) -> 3 broadcast shared loads.
+// No tie detection, no termination test, no pick log, no candidate selection, no global round.  A unique
+// per-slot floor is added to the distances so that they never collapse to ties; the arithmetic per pick
+// is that of the real loop.  Returns SM cycles per pick.
+// ---------------------------------------------------------------------------------------------
+template <int CPL>
+__global__ void __launch_bounds__(32, 1) k_pick_chain_floor(const int iters, float *out)
+{
+    __shared__ float sX[32 * CPL], sY[32 * CPL], sZ[32 * CPL];
+    const int lane = threadIdx.x;
+    float x[CPL], y[CPL], z[CPL], d[CPL], fl[CPL];
+#pragma unroll
+    for (int c = 0; c < CPL; ++c) {
+        const int i = c * 32 + lane;
+        x[c] = sX[i] = (float)((i * 37) % 101) * 0.01f;
+        y[c] = sY[i] = (float)((i * 53) % 103) * 0.01f;
+        z[c] = sZ[i] = (float)((i * 71) % 107) * 0.01f;
+        fl[c] = 1.0f + (float)i * 0x1p-10f;
+        d[c] = 4.0f + fl[c];
+    }
+    __syncwarp();
+    unsigned acc = 0u;
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+        float bm = d[0];
+#pragma unroll
+        for (int c = 1; c < CPL; ++c) bm = fmaxf(bm, d[c]);
+        unsigned id = 0u;
+#pragma unroll
+        for (int c = 0; c < CPL; ++c)
+            if (d[c] == bm) id = (unsigned)(c * 32 + lane + 1);
+        const unsigned hi = __float_as_uint(bm);
+        const unsigned ghi = __reduce_max_sync(FULL, hi);
+        const unsigned wid = __reduce_max_sync(FULL, hi == ghi ? id : 0u) - 1u;
+        const float sx = sX[wid], sy = sY[wid], sz = sZ[wid];
+        acc += wid;
+#pragma unroll
+        for (int c = 0; c < CPL; ++c) d[c] = fminf(d[c], __fadd_rn(d2_rn(x[c], y[c], z[c], sx, sy, sz), fl[c]));
+    }
+    const long long t1 = clock64();
+    if (lane == 0) { out[0] = (float)(t1 - t0) / (float)iters; out[1] = (float)acc; }
+}
+
+int measure_pick_chain(int cand_per_lane, int iters, float *cycles_per_pick)
+{
+    float *d = nullptr, h[2] = {0.f, 0.f};
+    RFPS_CUDA(cudaMalloc(&d, 2 * sizeof(float)));
+    for (int rep = 0; rep < 2; ++rep) {      // the first launch warms the instruction cache
+        switch (cand_per_lane) {
+            case 1: k_pick_chain_floor<1><<<1, 32>>>(iters, d); break;
+            case 2: k_pick_chain_floor<2><<<1, 32>>>(iters, d); break;
+            case 4: k_pick_chain_floor<4><<<1, 32>>>(iters, d); break;
+            default: cudaFree(d); set_error("cand_per_lane=%d must be 1, 2 or 4", cand_per_lane); return FPS_ERR_INVALID;
+        }
+    }
+    cudaError_t e = cudaMemcpy(h, d, sizeof h, cudaMemcpyDeviceToHost);
+    cudaFree(d);
+    if (e != cudaSuccess) { set_error("pick-chain measurement failed: %s", cudaGetErrorString(e)); return FPS_ERR_CUDA; }
+    *cycles_per_pick = h[0];
+    return FPS_OK;
 }
 
 }  // namespace rfps

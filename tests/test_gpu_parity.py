@@ -381,6 +381,11 @@ def test_gather_xyz_uniform_and_ragged(rf):
         rf.fps_index_destroy(ix)
 
 
+def test_pick_chain_floor_is_measurable(rf):
+    c1, c4 = rf.fps_pick_chain_cycles(1, 4096), rf.fps_pick_chain_cycles(4, 4096)
+    assert 40.0 < c1 < 1000.0 and c1 < c4 < 2000.0
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
