@@ -533,7 +533,13 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         // the workers may start applying these picks now (bpick was written before the barrier above)
         if (pub_addr && tid == 0) st_release_cluster_u32(pub_addr, (unsigned)nbl);
         tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
-        // ---- (f) the sub-round's picks -> all of C1 ----
+        // ---- (f) the sub-round's picks -> all of C1.  Candidates at or below tau are out of the round for
+        // good; neighbours in the buffer come from the same voxel and tend to die together, so whole
+        // warps drop out of this loop as the round proceeds ----
+        bool live = false;
+#pragma unroll
+        for (int c = 0; c < CPT1; ++c) live |= D[c] > tau;
+        if (__any_sync(FULL, live))
         for (int i = applied; i < nbl; ++i) {
             const float4 s = bpick[i];
             const f32x2 SX = pack2(s.x, s.x), SY = pack2(s.y, s.y), SZ = pack2(s.z, s.z);
@@ -909,24 +915,37 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     if (qi >= nq) break;
                     const int2 sg = sseg[qkl[qi]];
                     if (STATS && lane == 0) c_xvox++;
-                    for (int p0 = sg.x; p0 < sg.x + sg.y; p0 += 32) {
-                        const int p = p0 + lane;
-                        const bool in = p < sg.x + sg.y;
-                        const unsigned db = in ? __float_as_uint(Dp[p]) : 0u;
-                        const bool is = db > tb;
-                        const unsigned bal = __ballot_sync(FULL, is);
-                        if (STATS && in) c_xpts++;
-                        if (bal) {
+                    // two chunks of 32 points per step, everything loaded up front (one memory round trip), one
+                    // slot reservation per step
+                    for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
+                        const int pA = pb + lane, pB = pb + 32 + lane;
+                        const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
+                        unsigned dA = 0u, dB = 0u, oA = 0u, oB = 0u;
+                        float xA = 0.f, yA = 0.f, zA = 0.f, xB = 0.f, yB = 0.f, zB = 0.f;
+                        if (inA) { dA = __float_as_uint(Dp[pA]); xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; }
+                        if (inB) { dB = __float_as_uint(Dp[pB]); xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; }
+                        const bool isA = dA > tb, isB = dB > tb;
+                        const unsigned balA = __ballot_sync(FULL, isA), balB = __ballot_sync(FULL, isB);
+                        if (STATS) c_xpts += (inA ? 1 : 0) + (inB ? 1 : 0);
+                        if (balA | balB) {
                             unsigned cb = 0u;
-                            if (lane == 0) cb = atom_add_dsmem_u32(cnt_addr, (unsigned)__popc(bal));
+                            if (lane == 0) cb = atom_add_dsmem_u32(cnt_addr, (unsigned)(__popc(balA) + __popc(balB)));
                             cb = __shfl_sync(FULL, cb, 0);
-                            const unsigned slot = cb + (unsigned)__popc(bal & lt);
-                            if (is && slot < (unsigned)TC) {
-                                st_dsmem_u32(cX0 + 4u * slot, __float_as_uint(px[p]));
-                                st_dsmem_u32(cY0 + 4u * slot, __float_as_uint(py[p]));
-                                st_dsmem_u32(cZ0 + 4u * slot, __float_as_uint(pz[p]));
-                                st_dsmem_u32(cD0 + 4u * slot, db);
-                                st_dsmem_u32(cO0 + 4u * slot, ~(unsigned)porig[p]);
+                            const unsigned slotA = cb + (unsigned)__popc(balA & lt);
+                            const unsigned slotB = cb + (unsigned)__popc(balA) + (unsigned)__popc(balB & lt);
+                            if (isA && slotA < (unsigned)TC) {
+                                st_dsmem_u32(cX0 + 4u * slotA, __float_as_uint(xA));
+                                st_dsmem_u32(cY0 + 4u * slotA, __float_as_uint(yA));
+                                st_dsmem_u32(cZ0 + 4u * slotA, __float_as_uint(zA));
+                                st_dsmem_u32(cD0 + 4u * slotA, dA);
+                                st_dsmem_u32(cO0 + 4u * slotA, oA);
+                            }
+                            if (isB && slotB < (unsigned)TC) {
+                                st_dsmem_u32(cX0 + 4u * slotB, __float_as_uint(xB));
+                                st_dsmem_u32(cY0 + 4u * slotB, __float_as_uint(yB));
+                                st_dsmem_u32(cZ0 + 4u * slotB, __float_as_uint(zB));
+                                st_dsmem_u32(cD0 + 4u * slotB, dB);
+                                st_dsmem_u32(cO0 + 4u * slotB, oB);
                             }
                         }
                     }
