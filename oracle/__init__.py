@@ -4,6 +4,8 @@ CPU reference programs for exact farthest point sampling (arxiv/paper_2606_06255
 
 * ``fps``         classical O(N*M) FPS, ``oracle/fps_oracle.c`` (Alg. 1; exactness
                   contract PAPER.md:179).  This is THE oracle.
+* ``fps_euclid``  the same with the Euclidean (sqrt) distance of the paper's text, ``oracle/fps_oracle_euclid.c``
+                  (Eq. 1 / Eq. 29): the oracle of the library's FPS_FLAG_EUCLIDEAN mode.
 * ``pruned_fps``  the paper's section-3 CPU RadiusFPS, ``oracle/fps_pruned_cpu.c`` (Eq. 6-30,
                   PAPER.md:187-350); an independent program that must agree with ``fps`` bit for bit.
 
@@ -61,7 +63,7 @@ def _compile(stem: str) -> str:
 
 def build() -> None:
     """Compile both C programs (called by __graft_entry__.build(); building is not using)."""
-    for stem in ("fps_oracle", "fps_pruned_cpu"):
+    for stem in ("fps_oracle", "fps_oracle_euclid", "fps_pruned_cpu"):
         _compile(stem)
 
 
@@ -109,6 +111,24 @@ def fps(points, M: int, start: int = 0, threads: int = 0):
 
 
 fps.threads_used = 1
+
+
+def fps_euclid(points, M: int, start: int = 0, threads: int = 0):
+    """Classical FPS with the Euclidean distance sqrtf(d2) (the paper's literal Eq. 1 / Eq. 29).  Same
+    shapes as ``fps``; ``mindist`` holds distances, not squared distances."""
+    p, single = _as_batch(points)
+    B, N, _ = p.shape
+    fn = _lib("fps_oracle_euclid").oracle_fps_euclid_batch
+    fn.restype = ctypes.c_int
+    fn.argtypes = [_f32p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, _i32p, _f32p,
+                   ctypes.c_int32]
+    idx = np.empty((B, M), dtype=np.int32)
+    mind = np.empty((B, M), dtype=np.float32)
+    r = fn(p.ctypes.data_as(_f32p), B, N, M, start, idx.ctypes.data_as(_i32p), mind.ctypes.data_as(_f32p),
+           threads)
+    if r < 0:
+        raise ValueError(f"oracle_fps_euclid_batch failed with code {r} (N={N}, M={M}, start={start})")
+    return (idx[0], mind[0]) if single else (idx, mind)
 
 
 def pruned_fps(points, M: int, start: int = 0, n_vox: int = 16, *, prune: bool = True, skip: bool = True,

@@ -276,3 +276,72 @@ def test_arithmetic_sensitivity_random_bits():
     _, fmind = cached_fps(P, 512, 0, d2_single_rounding)
     assert not same_bits(mind, rmind)
     assert not same_bits(mind, fmind)
+
+
+# ---------------------------------------------------------------------------------------------
+# 9. the Euclidean oracle (oracle.fps_euclid; the paper's literal Eq. 1 / Eq. 29)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(4))
+@pytest.mark.parametrize("N", [1, 2, 5, 33, 64])
+def test_euclid_brute_force_definition(N, seed):
+    P = inputs.uniform_cube(N, 700 + seed)
+    M = N
+    bi, bm = brute_force_fps(P, M, seed % N, dist=d_sqrt)
+    oi, om = oracle.fps_euclid(P, M, seed % N)
+    assert np.array_equal(oi, bi) and same_bits(om, bm)
+
+
+@pytest.mark.parametrize("name", ["lattice", "line", "corners", "dups"])
+def test_euclid_brute_force_tie_heavy(name):
+    P = {"lattice": inputs.shuffled_lattice(4, 3), "line": inputs.integer_line(33), "corners": inputs.cube_corners(),
+         "dups": inputs.with_duplicates(40, 5, 9)}[name]
+    M = min(P.shape[0], 40)
+    bi, bm = brute_force_fps(P, M, 0, dist=d_sqrt)
+    oi, om = oracle.fps_euclid(P, M, 0)
+    assert np.array_equal(oi, bi) and same_bits(om, bm)
+
+
+def test_euclid_closed_form_line():
+    # integer line 0..8: same bisection as the squared case (PAPER.md:179 tie rule), distances not squared
+    oi, om = oracle.fps_euclid(inputs.integer_line(9), 9, 0)
+    assert oi.tolist() == [0, 8, 4, 2, 6, 1, 3, 5, 7]
+    assert om.tolist() == [np.inf, 8, 4, 2, 2, 1, 1, 1, 1]
+
+
+def test_euclid_equals_sqrt_of_squared_oracle_when_nothing_collapses():
+    # sqrt is monotone, so the two oracles pick the same points unless two different squared maxima round
+    # to the same square root; where the index sequences agree the distances must be sqrt of each other
+    agree = 0
+    for seed in range(6):
+        P = inputs.room(1500, 800 + seed)
+        si, sm = oracle.fps(P, 300, 0)
+        ei, em = oracle.fps_euclid(P, 300, 0)
+        n = 300 if np.array_equal(si, ei) else int(np.argmax(si != ei))
+        assert n >= 2
+        assert same_bits(em[:n], np.sqrt(sm[:n]).astype(F))
+        agree += n == 300
+    assert agree >= 1
+
+
+def test_euclid_differs_from_squared_where_sqrt_collapses_two_maxima():
+    # constructed: origin, A, B with fl(d2(B)) one ulp above fl(d2(A)) but the same correctly rounded
+    # square root.  Squared FPS picks B (larger), Euclidean FPS sees a tie and takes the lower index A.
+    rng = np.random.default_rng(5)
+    found = None
+    for _ in range(200):
+        Q = np.zeros((4000, 3), dtype=F)
+        Q[:, :2] = rng.random((4000, 2), dtype=F) + F(0.5)
+        d2 = d2_stated(Q, np.zeros(3, dtype=F))
+        order = np.argsort(d2, kind="stable")
+        s = d2[order]
+        r = np.sqrt(s).astype(F)
+        hit = np.nonzero((s[1:] > s[:-1]) & (r[1:] == r[:-1]))[0]
+        if hit.size:
+            found = (Q[order[hit[0]]], Q[order[hit[0] + 1]])
+            break
+    assert found is not None
+    P = np.stack([np.zeros(3, dtype=F), found[0], found[1]])
+    si, _ = oracle.fps(P, 2, 0)
+    ei, em = oracle.fps_euclid(P, 2, 0)
+    assert si.tolist() == [0, 2] and ei.tolist() == [0, 1]
+    assert same_bits(em[1:], d_sqrt(P[1:2], P[0]))
