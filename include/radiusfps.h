@@ -71,8 +71,13 @@ enum {
     FPS_FLAG_NO_SKIP  = 2,  /* ablation: no coordinate-wise point skip (Eq. 28 never taken)             */
     FPS_FLAG_STATS    = 4,  /* count voxel tests / visited voxels / visited points / effective updates  */
     FPS_FLAG_NO_BATCH = 8,  /* ablation: every batch of the batched kernel is the single global argmax  */
-    FPS_FLAG_PER_PICK = 16  /* run the per-pick persistent kernel (one cluster-wide exchange per sample,
+    FPS_FLAG_PER_PICK = 16, /* run the per-pick persistent kernel (one cluster-wide exchange per sample,
                                the paper's iteration structure) instead of exact batched picking        */
+    FPS_FLAG_EUCLIDEAN = 32 /* NOT an option that leaves results alone: sample with the Euclidean distance
+                               sqrt_rn(d2), the paper's literal Eq. 1 / Eq. 29, instead of
+                               d2.  out_mindist then holds distances.  In fp32 this is a different function:
+                               maxima that differ in d2 can round to the same square root and tie (lowest
+                               index wins).  Batched kernel with the default local phase only.              */
 };
 
 /* Counters and layout facts, summed over the B clouds (fps_get_stats).  With the batched kernel

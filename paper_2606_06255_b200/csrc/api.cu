@@ -58,6 +58,10 @@ static fps_index_t *build_common(const float *points, int32_t N, int32_t B, cons
     memset(&o, 0, sizeof o);
     if (opts) o = *opts;
     if (o.n_vox < 0 || o.n_vox > 1024) { set_error("n_vox=%d out of range [0,1024]", o.n_vox); return nullptr; }
+    if ((o.flags & FPS_FLAG_EUCLIDEAN) && (o.flags & FPS_FLAG_PER_PICK)) {
+        set_error("FPS_FLAG_EUCLIDEAN is not available with FPS_FLAG_PER_PICK");
+        return nullptr;
+    }
     fps_index_t *h = new (std::nothrow) fps_index_t();
     if (!h) { set_error("host allocation failed"); return nullptr; }
     h->ix.B = B;

@@ -115,6 +115,24 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 // packed fp32x2 arithmetic (sm_100: FADD2 / FMUL2).  Each half is an ordinary IEEE round-to-nearest
 // fp32 operation, so the results are bit-identical to the scalar __f*_rn intrinsics.
 // ---------------------------------------------------------------------------------------------
+// The distance the algorithm works with: the squared fp32 expression d2 (the main path, BASELINE.json), or
+// EUC: its correctly rounded square root, the paper's literal ||p - s|| (Eq. 1 / Eq. 29).
+// Everything else -- min, strict '<', argmax with lowest-index ties, the exact-batching argument -- only
+// needs a distance that is a fixed monotone function of d2, so both modes share all of the code below.
+template <bool EUC>
+__device__ __forceinline__ float distf(const float d2) { return EUC ? __fsqrt_rn(d2) : d2; }
+// prune threshold for the Euclidean mode: Dist_v already is a (rounded) distance, so no square root; the
+// voxel is pruned iff d2(s, c) >= thr.  Then ||p - s|| >= Dv (1 + 3u) for every point p of the voxel, hence
+// fl_d2(p, s) >= Dv^2 and sqrt_rn(fl_d2) >= Dv >= Dist_p[p] (sqrt_rn is monotone, Dv representable).
+__device__ __forceinline__ float prune_threshold_euc(unsigned dv_bits, float R)
+{
+    if (dv_bits == 0u) return 0.0f;
+    const float q = __fadd_rn(__fmul_rn(__uint_as_float(dv_bits), 1.0f + 0x1p-20f), 0x1p-40f);
+    const float a = __fadd_rn(q, R);
+    const float t = __fmul_rn(__fmul_rn(a, a), 1.0f + 0x1p-18f);
+    return (t < __uint_as_float(F32_INF_BITS)) ? t : __uint_as_float(F32_NAN_BITS);
+}
+
 typedef unsigned long long f32x2;
 __device__ __forceinline__ f32x2 pack2(float a, float b)
 {
@@ -278,7 +296,7 @@ struct __align__(16) HierSmem {
     int cnt2, nb, j, pad;
 };
 
-template <int CPT1, int CPT2>
+template <int CPT1, int CPT2, bool EUC>
 __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY, const float *cZ, const float *cD,
                                                const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
                                                const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
@@ -457,7 +475,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                     ++nbl;
                     if (jl >= M || nbl >= PB) return false;
 #pragma unroll
-                    for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], d2_rn(x2[c], y2[c], z2[c], sx, sy, sz));
+                    for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], distf<EUC>(d2_rn(x2[c], y2[c], z2[c], sx, sy, sz)));
                     return true;
                 };
                 for (bool go = true; go;) {
@@ -491,7 +509,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         wd[p] = wid;
                         const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
 #pragma unroll
-                        for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], d2_rn(x2[c], y2[c], z2[c], sx, sy, sz));
+                        for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], distf<EUC>(d2_rn(x2[c], y2[c], z2[c], sx, sy, sz)));
                     }
                     if (tie) {                               // rare: redo this chunk pick by pick
 #pragma unroll
@@ -550,8 +568,8 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 unpack2(mul2(dx, dx), x0, x1);
                 unpack2(mul2(dy, dy), y0, y1);
                 unpack2(mul2(dz, dz), z0, z1);
-                D[2 * h] = fminf(D[2 * h], __fadd_rn(__fadd_rn(x0, y0), z0));
-                D[2 * h + 1] = fminf(D[2 * h + 1], __fadd_rn(__fadd_rn(x1, y1), z1));
+                D[2 * h] = fminf(D[2 * h], distf<EUC>(__fadd_rn(__fadd_rn(x0, y0), z0)));
+                D[2 * h + 1] = fminf(D[2 * h + 1], distf<EUC>(__fadd_rn(__fadd_rn(x1, y1), z1)));
             }
         }
         applied = nbl;
@@ -570,7 +588,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
 // ---------------------------------------------------------------------------------------------
 static_assert(sizeof(HierSmem) <= 3392 + 8 * PB, "smem_layout reserves this much for HierSmem");
 
-template <int CPT, int LW, bool STATS>
+template <int CPT, int LW, bool STATS, bool EUC>
 __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, const int flags)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -782,8 +800,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                             {
                                 const float dx = __fsub_rn(xA, s.x), dy = __fsub_rn(yA, s.y), dz = __fsub_rn(zA, s.z);
                                 const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                                if (no_skip || !(dx2 >= DA || dy2 >= DA || dz2 >= DA)) {   // Eq. 28, squared domain
-                                    const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                                // Eq. 28: squared domain, or literally |dx| >= D in the Euclidean mode (sqrt_rn(fl(dx*dx)) == |dx|)
+                                if (no_skip || !(EUC ? (fabsf(dx) >= DA || fabsf(dy) >= DA || fabsf(dz) >= DA) : (dx2 >= DA || dy2 >= DA || dz2 >= DA))) {
+                                    const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
                                     if (STATS && inA) c_pcomp++;
                                     if (d < DA) {                                          // Eq. 29 / Eq. 2 (strict)
                                         DA = d;
@@ -794,8 +813,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                             {
                                 const float dx = __fsub_rn(xB, s.x), dy = __fsub_rn(yB, s.y), dz = __fsub_rn(zB, s.z);
                                 const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                                if (no_skip || !(dx2 >= DB || dy2 >= DB || dz2 >= DB)) {
-                                    const float d = __fadd_rn(__fadd_rn(dx2, dy2), dz2);
+                                if (no_skip || !(EUC ? (fabsf(dx) >= DB || fabsf(dy) >= DB || fabsf(dz) >= DB) : (dx2 >= DB || dy2 >= DB || dz2 >= DB))) {
+                                    const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
                                     if (STATS && inB) c_pcomp++;
                                     if (d < DB) {
                                         DB = d;
@@ -817,7 +836,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
                 if (lane == 0) {
                     vst[kl] = make_uint2(mhi, mlo);
-                    svthr[kl] = prune_threshold(mhi, sgeom[kl].w);
+                    svthr[kl] = EUC ? prune_threshold_euc(mhi, sgeom[kl].w) : prune_threshold(mhi, sgeom[kl].w);
                     if (STATS) c_vvisit++;
                 }
                 __syncwarp();
@@ -826,7 +845,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 {
                     const int gl = kl >> 5;
                     const unsigned dvg = __reduce_max_sync(FULL, vst[gl * 32 + lane].x);
-                    if (lane == 0) sgthr[gl] = prune_threshold(dvg, sggeom[gl].w);
+                    if (lane == 0) sgthr[gl] = EUC ? prune_threshold_euc(dvg, sggeom[gl].w) : prune_threshold(dvg, sggeom[gl].w);
                 }
             }
             __syncthreads();
@@ -984,14 +1003,14 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 }
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
-                local_fps_hier<CPT, 2>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
+                local_fps_hier<CPT, 2, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
                                        c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
                     ctl->j = lj;
                     if (STATS) c_cands += (unsigned long long)cnt;
                 }
-            } else if constexpr (LW < BT / 32) {
+            } else if constexpr (LW < BT / 32 && !EUC) {
               if (warp < LW) {
                 int lj = j, lnb = 0;
                 local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, lslot, bpick, out_idx, out_mind, tid);
@@ -1093,13 +1112,13 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 // ---------------------------------------------------------------------------------------------
 static const int kMaxSmem = 227 * 1024;
 
-template <int CPT, int LW, bool STATS>
+template <int CPT, int LW, bool STATS, bool EUC>
 __global__ void k_fps_batched(const BatchParams P, const int flags);
 
 // how many clusters of `c` CTAs of the default kernel can be resident at once (0 on error)
 static int max_resident_clusters(int c, size_t smem)
 {
-    auto kern = k_fps_batched<2, 16, false>;
+    auto kern = k_fps_batched<2, 16, false, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
     cudaLaunchConfig_t cfg;
@@ -1128,6 +1147,10 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     // 8 up to 4 096; larger clouds work on the top ~1 024 candidates per round
     int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW == 16 ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : 2))) : 8);
     const bool ok_shape = LW == 16 ? (CPT == 2 || CPT == 4 || CPT == 8) : ((LW == 1 || LW == 2 || LW == 4 || LW == 8) && (CPT == 4 || CPT == 8 || CPT == 16));
+    if ((o.flags & FPS_FLAG_EUCLIDEAN) && LW != 16) {
+        set_error("FPS_FLAG_EUCLIDEAN needs the hierarchical local phase (local_warps = 0 or 16)");
+        return FPS_ERR_INVALID;
+    }
     if (!ok_shape) {
         set_error("local_warps=%d / cand_per_thread=%d: use 16 with 2, 4 or 8 (hierarchical), or 1,2,4,8 with 4,8,16 (flat)", LW, CPT);
         return FPS_ERR_INVALID;
@@ -1166,10 +1189,10 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     return FPS_OK;
 }
 
-template <int CPT, int LW, bool STATS>
+template <int CPT, int LW, bool STATS, bool EUC>
 static int launch_batched_one(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
 {
-    auto kern = k_fps_batched<CPT, LW, STATS>;
+    auto kern = k_fps_batched<CPT, LW, STATS, EUC>;
     const size_t smem = smem_layout(ix.Kc_cap, CPT * LW * 32, LW).total;
     RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (ix.cluster_size > 8) RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
@@ -1193,8 +1216,12 @@ static int launch_batched_one(const BatchParams &bp, const DeviceIndex &ix, cuda
 template <int CPT, int LW>
 static int launch_batched_s(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
 {
-    return (ix.flags & FPS_FLAG_STATS) ? launch_batched_one<CPT, LW, true>(bp, ix, st)
-                                       : launch_batched_one<CPT, LW, false>(bp, ix, st);
+    const bool stats = ix.flags & FPS_FLAG_STATS;
+    if constexpr (LW == BT / 32) {          // the Euclidean mode is built for the hierarchical local phase only
+        if (ix.flags & FPS_FLAG_EUCLIDEAN)
+            return stats ? launch_batched_one<CPT, LW, true, true>(bp, ix, st) : launch_batched_one<CPT, LW, false, true>(bp, ix, st);
+    }
+    return stats ? launch_batched_one<CPT, LW, true, false>(bp, ix, st) : launch_batched_one<CPT, LW, false, false>(bp, ix, st);
 }
 
 int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const int32_t *rag_dev, int64_t iterations,

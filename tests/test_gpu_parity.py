@@ -386,6 +386,61 @@ def test_pick_chain_floor_is_measurable(rf):
     assert 40.0 < c1 < 1000.0 and c1 < c4 < 2000.0
 
 
+# ---------------------------------------------------------------------------------------------
+# Euclidean mode: the paper's literal distance, against its own oracle
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("cluster", [0, 1, 5])
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_euclidean_mode_small_clouds(rf, name, cluster):
+    P, M = SMALL[name]()
+    ref = oracle.fps_euclid(P, M, 0)
+    gi, gm, _ = run_gpu(rf, P, M, flags=rf.FPS_FLAG_EUCLIDEAN, cluster_size=cluster)
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+def test_euclidean_mode_full_size(rf, name):
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    ref = oracle.fps_euclid(P, w.M, w.start_idx)
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx, flags=rf.FPS_FLAG_EUCLIDEAN)
+    assert_same(gi, gm, *ref)
+
+
+def test_euclidean_mode_is_a_different_function_where_sqrt_collapses(rf):
+    # two maxima one ulp apart in d2 with the same correctly rounded square root (found by search, as in
+    # tests/test_oracle_pins.py): the squared mode takes the larger, the Euclidean mode ties -> lower index
+    rng = np.random.default_rng(5)
+    F = np.float32
+    found = None
+    for _ in range(200):
+        Q = np.zeros((4000, 3), dtype=F)
+        Q[:, :2] = rng.random((4000, 2), dtype=F) + F(0.5)
+        d2 = ((Q[:, 0] * Q[:, 0]).astype(F) + (Q[:, 1] * Q[:, 1]).astype(F)).astype(F)
+        order = np.argsort(d2, kind="stable")
+        sd, r = d2[order], np.sqrt(d2[order]).astype(F)
+        hit = np.nonzero((sd[1:] > sd[:-1]) & (r[1:] == r[:-1]))[0]
+        if hit.size:
+            found = (Q[order[hit[0]]], Q[order[hit[0] + 1]])
+            break
+    assert found is not None
+    P = np.stack([np.zeros(3, dtype=F), found[0], found[1]])
+    gi, _, _ = run_gpu(rf, P, 2)
+    assert gi.reshape(-1).tolist() == [0, 2]
+    gi, gm, _ = run_gpu(rf, P, 2, flags=rf.FPS_FLAG_EUCLIDEAN)
+    assert gi.reshape(-1).tolist() == [0, 1]
+    assert_same(gi, gm, *oracle.fps_euclid(P, 2, 0))
+
+
+def test_euclidean_mode_refuses_the_per_pick_kernel(rf):
+    P = torch.from_numpy(inputs.uniform_cube(100, 1)).cuda()
+    with pytest.raises(rf.FpsError) as e:
+        rf.fps_index_build(P, flags=rf.FPS_FLAG_EUCLIDEAN | rf.FPS_FLAG_PER_PICK)
+    assert e.value.status == rf.FPS_ERR_INVALID
+    with pytest.raises(rf.FpsError):
+        rf.fps_index_build(P, flags=rf.FPS_FLAG_EUCLIDEAN, local_warps=4)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
