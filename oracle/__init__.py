@@ -15,7 +15,7 @@ Only ``tests/``, ``__graft_entry__.smoke()`` and ``bench.py``'s CPU legs (``cpu_
 
 Parity pins: tests/test_oracle_pins.py (brute force from Eq. 3, closed forms, M=2 library argmax,
 O(M^2) min-distance recomputation, invariants, metamorphic scaling, arithmetic-sensitivity lattice,
-agreement of ``fps`` with ``pruned_fps``).  Parity with the PAPER'S OWN implementation is unpinned
+agreement of ``fps`` with ``pruned_fps``; section 9 of that file pins ``fps_euclid``).  Parity with the PAPER'S OWN implementation is unpinned
 and unpinnable: the paper publishes no code and prints no worked example.
 """
 from __future__ import annotations
