@@ -311,7 +311,9 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
     float D[CPT1];
 #pragma unroll
     for (int h = 0; h < H1; ++h) {
-        const int i0 = (2 * h) * BT + tid, i1 = (2 * h + 1) * BT + tid;
+        // candidate slots 2t, 2t+1 (then 2*BT + 2t, ...): a buffer that is not full leaves whole warps with
+        // padding only, and those warps drop out of the update loop (f)
+        const int i0 = h * 2 * BT + 2 * tid, i1 = i0 + 1;
         const bool ok0 = i0 < cnt, ok1 = i1 < cnt;
         X[h] = pack2(ok0 ? cX[i0] : 0.0f, ok1 ? cX[i1] : 0.0f);
         Y[h] = pack2(ok0 ? cY[i0] : 0.0f, ok1 ? cY[i1] : 0.0f);
@@ -364,7 +366,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
 #pragma unroll
                 for (int c = 0; c < CPT1; ++c)
                     if (D[c] == m) {
-                        const unsigned i = (unsigned)(c * BT + tid);
+                        const unsigned i = (unsigned)((c >> 1) * 2 * BT + 2 * tid + (c & 1));
                         const unsigned oc = cO[i];
                         if (oc >= o) { o = oc; oi = i; }
                     }
@@ -395,7 +397,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 if (D[c] > tau) {
                     if (RFPS_BIN(D[c]) < bstar) {
                         const int sl = atomicAdd(&hs->cnt2, 1);
-                        const int i = c * BT + tid;
+                        const int i = (c >> 1) * 2 * BT + 2 * tid + (c & 1);
                         hs->sD[sl] = D[c];
                         hs->sX[sl] = cX[i];
                         hs->sY[sl] = cY[i];
