@@ -701,6 +701,83 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         //            the survivors; voxels with survivors are queued with their pick mask
         //   phase B  warps pop queued voxels (dynamic) and walk their points once for all surviving picks
         // =====================================================================================
+    // ---- a10-a12 for one voxel: point skip, update, voxel key + thresholds.  Called by a whole warp; vmask =
+    // the picks bpick[sub + 32*w + i] whose bit i of word w is set ----
+    auto visit = [&](const int kl, const unsigned (&vmask)[SUBW], const int sub) {
+            const int2 sg = sseg[kl];
+            float bestD = -1.0f;
+            unsigned bestO = 0u;
+            int npk = 0;
+#pragma unroll
+            for (int w = 0; w < SUBW; ++w) npk += __popc(vmask[w]);
+            // two chunks of 32 points per step: both chunks' loads are in flight together
+            for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
+                const int pA = pb + lane, pB = pb + 32 + lane;
+                const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
+                float xA = 0.f, yA = 0.f, zA = 0.f, DA0 = -1.0f, xB = 0.f, yB = 0.f, zB = 0.f, DB0 = -1.0f;
+                unsigned oA = 0u, oB = 0u;
+                if (inA) { xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; DA0 = Dp[pA]; }
+                if (inB) { xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; DB0 = Dp[pB]; }
+                float DA = DA0, DB = DB0;
+#pragma unroll
+                for (int w = 0; w < SUBW; ++w) {
+                    unsigned m = vmask[w];
+                    while (m) {
+                        const int i = __ffs(m) - 1;
+                        m &= m - 1u;
+                        const float4 s = bpick[sub + 32 * w + i];
+                        {
+                            const float dx = __fsub_rn(xA, s.x), dy = __fsub_rn(yA, s.y), dz = __fsub_rn(zA, s.z);
+                            const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                            // Eq. 28: squared domain, or literally |dx| >= D in the Euclidean mode (sqrt_rn(fl(dx*dx)) == |dx|)
+                            if (no_skip || !(EUC ? (fabsf(dx) >= DA || fabsf(dy) >= DA || fabsf(dz) >= DA) : (dx2 >= DA || dy2 >= DA || dz2 >= DA))) {
+                                const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
+                                if (STATS && inA) c_pcomp++;
+                                if (d < DA) {                                          // Eq. 29 / Eq. 2 (strict)
+                                    DA = d;
+                                    if (STATS) c_eff++;
+                                }
+                            }
+                        }
+                        {
+                            const float dx = __fsub_rn(xB, s.x), dy = __fsub_rn(yB, s.y), dz = __fsub_rn(zB, s.z);
+                            const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
+                            if (no_skip || !(EUC ? (fabsf(dx) >= DB || fabsf(dy) >= DB || fabsf(dz) >= DB) : (dx2 >= DB || dy2 >= DB || dz2 >= DB))) {
+                                const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
+                                if (STATS && inB) c_pcomp++;
+                                if (d < DB) {
+                                    DB = d;
+                                    if (STATS) c_eff++;
+                                }
+                            }
+                        }
+                    }
+                }
+                if (DA < DA0) Dp[pA] = DA;
+                if (DB < DB0) Dp[pB] = DB;
+                if (STATS) c_pvisit += (inA ? npk : 0) + (inB ? npk : 0);
+                // absent lanes carry D = -1 (< every real distance), so they never become the voxel's key
+                if (DA > bestD || (DA == bestD && oA > bestO)) { bestD = DA; bestO = oA; }
+                if (DB > bestD || (DB == bestD && oB > bestO)) { bestD = DB; bestO = oB; }
+            }
+            const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
+            unsigned mhi, mlo;
+            warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
+            if (lane == 0) {
+                vst[kl] = make_uint2(mhi, mlo);
+                svthr[kl] = EUC ? prune_threshold_euc(mhi, sgeom[kl].w) : prune_threshold(mhi, sgeom[kl].w);
+                if (STATS) c_vvisit++;
+            }
+            __syncwarp();
+            // refresh the group threshold.  A concurrent visit to another voxel of the group may make this
+            // read one stale (larger) key: the threshold then errs on the conservative side
+            {
+                const int gl = kl >> 5;
+                const unsigned dvg = __reduce_max_sync(FULL, vst[gl * 32 + lane].x);
+                if (lane == 0) sgthr[gl] = EUC ? prune_threshold_euc(dvg, sggeom[gl].w) : prune_threshold(dvg, sggeom[gl].w);
+            }
+    };
+
     auto apply_range = [&](const int lo, const int hi) {
         for (int sub = lo; sub < hi; sub += SUBP) {
             const int nsub = min(SUBP, hi - sub);
@@ -777,78 +854,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     __syncwarp();
                     if (lane == 0) *reinterpret_cast<uint4 *>(&qmask[kl * SUBW]) = make_uint4(0u, 0u, 0u, 0u);   // leave it clean
                 }
-                const int2 sg = sseg[kl];
-                float bestD = -1.0f;
-                unsigned bestO = 0u;
-                int npk = 0;
-#pragma unroll
-                for (int w = 0; w < SUBW; ++w) npk += __popc(vmask[w]);
-                // two chunks of 32 points per step: both chunks' loads are in flight together
-                for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
-                    const int pA = pb + lane, pB = pb + 32 + lane;
-                    const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
-                    float xA = 0.f, yA = 0.f, zA = 0.f, DA0 = -1.0f, xB = 0.f, yB = 0.f, zB = 0.f, DB0 = -1.0f;
-                    unsigned oA = 0u, oB = 0u;
-                    if (inA) { xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; DA0 = Dp[pA]; }
-                    if (inB) { xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; DB0 = Dp[pB]; }
-                    float DA = DA0, DB = DB0;
-#pragma unroll
-                    for (int w = 0; w < SUBW; ++w) {
-                        unsigned m = vmask[w];
-                        while (m) {
-                            const int i = __ffs(m) - 1;
-                            m &= m - 1u;
-                            const float4 s = bpick[sub + 32 * w + i];
-                            {
-                                const float dx = __fsub_rn(xA, s.x), dy = __fsub_rn(yA, s.y), dz = __fsub_rn(zA, s.z);
-                                const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                                // Eq. 28: squared domain, or literally |dx| >= D in the Euclidean mode (sqrt_rn(fl(dx*dx)) == |dx|)
-                                if (no_skip || !(EUC ? (fabsf(dx) >= DA || fabsf(dy) >= DA || fabsf(dz) >= DA) : (dx2 >= DA || dy2 >= DA || dz2 >= DA))) {
-                                    const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
-                                    if (STATS && inA) c_pcomp++;
-                                    if (d < DA) {                                          // Eq. 29 / Eq. 2 (strict)
-                                        DA = d;
-                                        if (STATS) c_eff++;
-                                    }
-                                }
-                            }
-                            {
-                                const float dx = __fsub_rn(xB, s.x), dy = __fsub_rn(yB, s.y), dz = __fsub_rn(zB, s.z);
-                                const float dx2 = __fmul_rn(dx, dx), dy2 = __fmul_rn(dy, dy), dz2 = __fmul_rn(dz, dz);
-                                if (no_skip || !(EUC ? (fabsf(dx) >= DB || fabsf(dy) >= DB || fabsf(dz) >= DB) : (dx2 >= DB || dy2 >= DB || dz2 >= DB))) {
-                                    const float d = distf<EUC>(__fadd_rn(__fadd_rn(dx2, dy2), dz2));
-                                    if (STATS && inB) c_pcomp++;
-                                    if (d < DB) {
-                                        DB = d;
-                                        if (STATS) c_eff++;
-                                    }
-                                }
-                            }
-                        }
-                    }
-                    if (DA < DA0) Dp[pA] = DA;
-                    if (DB < DB0) Dp[pB] = DB;
-                    if (STATS) c_pvisit += (inA ? npk : 0) + (inB ? npk : 0);
-                    // absent lanes carry D = -1 (< every real distance), so they never become the voxel's key
-                    if (DA > bestD || (DA == bestD && oA > bestO)) { bestD = DA; bestO = oA; }
-                    if (DB > bestD || (DB == bestD && oB > bestO)) { bestD = DB; bestO = oB; }
-                }
-                const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
-                unsigned mhi, mlo;
-                warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
-                if (lane == 0) {
-                    vst[kl] = make_uint2(mhi, mlo);
-                    svthr[kl] = EUC ? prune_threshold_euc(mhi, sgeom[kl].w) : prune_threshold(mhi, sgeom[kl].w);
-                    if (STATS) c_vvisit++;
-                }
-                __syncwarp();
-                // refresh the group threshold.  A concurrent visit to another voxel of the group may make this
-                // read one stale (larger) key: the threshold then errs on the conservative side
-                {
-                    const int gl = kl >> 5;
-                    const unsigned dvg = __reduce_max_sync(FULL, vst[gl * 32 + lane].x);
-                    if (lane == 0) sgthr[gl] = EUC ? prune_threshold_euc(dvg, sggeom[gl].w) : prune_threshold(dvg, sggeom[gl].w);
-                }
+                visit(kl, vmask, sub);
             }
             __syncthreads();
             qpar ^= 1u;
