@@ -441,6 +441,19 @@ def test_euclidean_mode_refuses_the_per_pick_kernel(rf):
         rf.fps_index_build(P, flags=rf.FPS_FLAG_EUCLIDEAN, local_warps=4)
 
 
+def test_integer_grid_overflowing_ties(rf):
+    # an exact integer grid: thousands of points tie at the maximum, more than the candidate buffer holds, so
+    # extraction attempts overflow, fall back to single global argmax picks, and the local phase takes its
+    # block-wide tie-break path; all of it must still follow the oracle bit for bit
+    g = np.arange(120, dtype=np.float32)
+    P = np.stack(np.meshgrid(g, g, np.zeros(1, dtype=np.float32)), -1).reshape(-1, 3).astype(np.float32)
+    P = np.ascontiguousarray(P[np.random.default_rng(3).permutation(P.shape[0])])
+    ref = oracle.fps(P, 1500, 0)
+    gi, gm, st = run_gpu(rf, P, 1500, flags=rf.FPS_FLAG_STATS)
+    assert_same(gi, gm, *ref)
+    assert st["extract_retries"] > 0 and st["single_picks"] > 0 and st["local_fallbacks"] > 0
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
