@@ -78,16 +78,29 @@ __global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, con
             mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
         }
     bad = __any_sync(0xffffffffu, bad);
-    if ((threadIdx.x & 31) == 0) {
-        unsigned *bb = bbox + b * BBOX_STRIDE;
+    // block level through shared memory, then ONE set of atomics per block (the atomics on a handful of
+    // addresses were most of this kernel's time when every warp issued them)
+    __shared__ float smn[8][3], smx[8][3];
+    __shared__ int sbad;
+    const int w = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    if (threadIdx.x == 0) sbad = 0;
+    __syncthreads();
+    if (lane == 0) {
 #pragma unroll
-        for (int a = 0; a < 3; ++a) {
-            if (mn[a] <= mx[a]) {
-                atomicMin(bb + a, f2ord(mn[a]));
-                atomicMax(bb + 3 + a, f2ord(mx[a]));
-            }
+        for (int a = 0; a < 3; ++a) { smn[w][a] = mn[a]; smx[w][a] = mx[a]; }
+        if (bad) sbad = 1;
+    }
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        const int a = threadIdx.x;
+        float lo = smn[0][a], hi = smx[0][a];
+        for (int i = 1; i < 8; ++i) { lo = fminf(lo, smn[i][a]); hi = fmaxf(hi, smx[i][a]); }
+        unsigned *bb = bbox + b * BBOX_STRIDE;
+        if (lo <= hi) {
+            atomicMin(bb + a, f2ord(lo));
+            atomicMax(bb + 3 + a, f2ord(hi));
         }
-        if (bad) atomicOr(bb + 6, 1u);
+        if (a == 0 && sbad) atomicOr(bb + 6, 1u);
     }
 }
 
@@ -263,10 +276,71 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ i
 // exclusive scan of B arrays of n ints (per-array stride `stride`); totals[b] (device, may be null)
 static int g_launches = 0;   // kernels launched by the build in progress (host-side bookkeeping only)
 
+// short arrays: the whole scan of one array in ONE block (1024 threads x 4 items per step, running carry);
+// one launch instead of three, which is what a build of a small cloud is made of
+constexpr int SCAN1_T = 1024, SCAN1_ITEMS = 4, SCAN1_TILE = SCAN1_T * SCAN1_ITEMS, SCAN1_MAX_N = 32768;
+
+__global__ void __launch_bounds__(SCAN1_T) k_scan_single(const int *__restrict__ in, int *__restrict__ out, int n, int stride,
+                                                         int *__restrict__ totals, const int *__restrict__ poff)
+{
+    __shared__ int wsum[32];
+    __shared__ int carry_s;
+    const int b = blockIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
+    const size_t off = poff ? (size_t)poff[b] : (size_t)b * stride;
+    if (poff) n = poff[b + 1] - poff[b];
+    const int *src = in + off;
+    int *dst = out + off;
+    if (threadIdx.x == 0) carry_s = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += SCAN1_TILE) {
+        const int i0 = base + threadIdx.x * SCAN1_ITEMS;
+        int v[SCAN1_ITEMS], s = 0;
+#pragma unroll
+        for (int i = 0; i < SCAN1_ITEMS; ++i) {
+            v[i] = i0 + i < n ? src[i0 + i] : 0;
+            s += v[i];
+        }
+        int inc = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) wsum[w] = inc;
+        __syncthreads();
+        const int carry = carry_s;
+        if (w == 0) {
+            int ws = wsum[lane], wi = ws;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += t;
+            }
+            wsum[lane] = wi - ws;                      // exclusive warp offsets
+            if (lane == 31) carry_s = carry + wi;      // running total for the next step
+        }
+        __syncthreads();
+        int e = carry + wsum[w] + inc - s;
+#pragma unroll
+        for (int i = 0; i < SCAN1_ITEMS; ++i) {
+            if (i0 + i < n) dst[i0 + i] = e;
+            e += v[i];
+        }
+        __syncthreads();
+    }
+    if (threadIdx.x == 0 && totals) totals[b] = carry_s;
+}
+
 // n = length of every array, or (poff given) of the longest one
 static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
                           cudaStream_t st, const int *poff = nullptr)
 {
+    if (n <= SCAN1_MAX_N) {
+        g_launches += 1;
+        k_scan_single<<<B, SCAN1_T, 0, st>>>(in, out, n, stride, totals, poff);
+        RFPS_CUDA(cudaGetLastError());
+        return FPS_OK;
+    }
     g_launches += 3;
     const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
     k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp, poff);
@@ -285,7 +359,7 @@ static inline int scan_tmp_ints(int n, int B) { return ((n + SCAN_TILE - 1) / SC
 // layout, rounds inside a chunk run in order, lanes inside a round are ranked by lane id
 // (__match_any_sync + popc of lower lanes).
 // ---------------------------------------------------------------------------------------------
-constexpr int RS_CHUNK = 2048, RS_WARPS = 4;
+constexpr int RS_CHUNK = 512, RS_WARPS = 4;    // short chunks: enough warps in flight on small clouds too
 
 __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, const int *__restrict__ poff,
                                                                int nchunk, int shift, int *__restrict__ table)
@@ -692,7 +766,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     RFPS_CUDA(cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st));
     const int *poff = ix.poff_dev;
     k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(sc.bbox, B);
-    k_bbox<<<dim3(std::min((N + 255) / 256, 592), B), 256, 0, st>>>(points, poff, sc.bbox);
+    k_bbox<<<dim3(std::max(1, std::min((N + 4095) / 4096, 148)), B), 256, 0, st>>>(points, poff, sc.bbox);
     k_keys<<<gN, 256, 0, st>>>(points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
     g_launches += 3;
 
