@@ -489,9 +489,14 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
 #pragma unroll
                     for (int c = 0; c < CPT2; ++c) dsave[c] = d2v[c];
                     unsigned gh[KCH], wd[KCH];
+#pragma unroll
+                    for (int p = 0; p < KCH; ++p) { gh[p] = 0u; wd[p] = 0u; }      // not reached = "over"
                     bool over = false, tie = false;          // "max <= tau2 seen" / "exact tie seen before that"
 #pragma unroll
                     for (int p = 0; p < KCH; ++p) {
+                        // one uniform exit test every four picks bounds the speculation past the end of the
+                        // sub-round without putting a branch behind every redux
+                        if ((p & 3) == 0 && p > 0 && over) break;
                         float bm = d2v[0];
 #pragma unroll
                         for (int c = 1; c < CPT2; ++c) bm = fmaxf(bm, d2v[c]);
