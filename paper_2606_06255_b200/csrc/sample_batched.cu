@@ -555,8 +555,10 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         }
 #undef RFPS_BIN
         c_subrounds++;
-        // the workers may start applying these picks now (bpick was written before the barrier above)
-        if (pub_addr && tid == 0) st_release_cluster_u32(pub_addr, (unsigned)nbl);
+        // the workers may start applying these picks now (bpick was written before the barrier above).  The
+        // release costs a fence: it is issued from the last warp, whose candidate slots are padding unless
+        // the buffer is full, so that it overlaps the other warps' update loop instead of delaying the pick warp
+        if (pub_addr && tid == BT - 32) st_release_cluster_u32(pub_addr, (unsigned)nbl);
         tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
         // ---- (f) the sub-round's picks -> all of C1.  Candidates at or below tau are out of the round for
         // good; neighbours in the buffer come from the same voxel and tend to die together, so whole
