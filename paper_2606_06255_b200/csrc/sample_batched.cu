@@ -73,7 +73,8 @@ struct BatchParams {
 };
 
 struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is the cluster's
-    unsigned ccount[MAX_ATTEMPTS];  // candidates found by extraction attempt a (may exceed TC)
+    unsigned ccount[4 * MAX_ATTEMPTS];  // candidates found by an extraction attempt (may exceed TC):
+                                        // [round parity][pass: hung on the previous tau / on the true maximum][attempt]
     unsigned best_hi, best_lo, pad3, pad0;       // this CTA's best voxel key
     int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
     unsigned pub, pad4, pad5, pad6; // (CTA 0) picks of the running batch published so far | PUB_DONE | PUB_FINAL
@@ -680,7 +681,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         qn[0] = qn[1] = qn[2] = qn[3] = 0;
         ctl->pub = 0u;
 #pragma unroll
-        for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
+        for (int a = 0; a < 4 * MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
         ctl->best_hi = ctl->best_lo = 0u;
         ctl->nb = 1;
         ctl->j = 1;
@@ -692,7 +693,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         }
     }
     int nb = 1, j = 1;
-    unsigned qpar = 0u;
+    unsigned qpar = 0u, round_parity = 0u, prev_taubits = 0u;
+    bool prev_tau_valid = false;
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
                        c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0, c_subrounds = 0, c_fallback = 0;
@@ -873,6 +875,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 
     while (j < Mb) {
         if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
+        unsigned ghi = 0u, glo = 0u;
+        bool have_max = false;
+        auto compute_max = [&]() {
         // =====================================================================================
         // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
         // =====================================================================================
@@ -893,40 +898,45 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             warp_argmax_key(wb.x, wb.y, chi, clo);
             if (lane == 0) {
                 ctl->best_hi = chi; ctl->best_lo = clo;
-                if (rank == 0) {
-#pragma unroll
-                    for (int a = 0; a < MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
-                    ctl->pub = 0u;
-                }
             }
         }
-        long long tm1 = 0, tm2 = 0;
-        if (STATS && tid == 0 && rank == 0) tm1 = clock64();
         cluster_sync_all();
-        if (STATS && tid == 0 && rank == 0) tm2 = clock64();
-        unsigned ghi, glo;
         {
             uint4 rb = make_uint4(0u, 0u, 0u, 0u);
             if (lane < C) rb = ld_dsmem_v4(mapa(smem_u32(&ctl->best_hi), (unsigned)lane));
             warp_argmax_key(rb.x, rb.y, ghi, glo);
         }
 
+            have_max = true;
+        };
+        if (tid == 0 && rank == 0) ctl->pub = 0u;      // ordered before the workers' polling by the extraction's barrier
+        const int rp = (int)(round_parity & 1u);
+        round_parity ^= 1u;
+        // A batch that ended on its threshold leaves every point of the cloud <= tau_prev, and the true maximum
+        // just below it: tau can be hung on tau_prev and the cluster-wide argmax (one more cluster barrier) is only
+        // computed when that fails -- no candidate above the new tau, or too many -- or when there is no such
+        // threshold (first round, batch cut short by the buffer).
+        if (!prev_tau_valid) compute_max();
         if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
         // =====================================================================================
         // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
         // =====================================================================================
         int cnt = 0;
         unsigned taubits = ghi;
-        if (!no_batch && ghi > 0u && ghi < F32_INF_BITS) {
-            const float Dmax = __uint_as_float(ghi);
+        for (int pass = have_max ? 1 : 0; pass < 2 && cnt == 0; ++pass) {
+        if (pass == 1 && !have_max) compute_max();
+        const unsigned gref = have_max ? ghi : prev_taubits;
+        taubits = gref;
+        if (!no_batch && gref > 0u && gref < F32_INF_BITS) {
+            const float Dmax = __uint_as_float(gref);
             const unsigned cX0 = mapa(smem_u32(cX), 0u), cY0 = mapa(smem_u32(cY), 0u), cZ0 = mapa(smem_u32(cZ), 0u),
                            cD0 = mapa(smem_u32(cD), 0u), cO0 = mapa(smem_u32(cO), 0u);
             for (int a = 0; a < MAX_ATTEMPTS; ++a) {
                 // a cloud that fits the candidate buffer whole is taken whole (tau = 0: every point that can
                 // still be picked at a positive distance); the local phase then runs without global rounds
                 const unsigned tb = (a == 0 && Nb <= TC) ? 0u : __float_as_uint(__fmul_rn(Dmax, __fsub_rn(1.0f, g)));
-                if (!(tb < ghi)) break;                      // g too small to separate tau from Dmax
-                const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[a]), 0u);
+                if (!(tb < gref)) break;                     // g too small to separate tau from Dmax
+                const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[(rp * 2 + pass) * MAX_ATTEMPTS + a]), 0u);
                 for (int base = 0; base < Kc; base += BT) {
                     const int kl = base + tid;
                     const bool hit = kl < Kc && vst[kl].x > tb;          // empty slots hold 0
@@ -998,6 +1008,12 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 if (STATS && tid == 0 && rank == 0) c_retries++;
                 g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
             }
+        }
+        }
+        if (!have_max) { /* cnt > 0 here: the single-pick path below, which needs the argmax, is not taken */ }
+        if (rank == 0 && tid == 0) {                  // the other parity's counters, for the next round
+#pragma unroll
+            for (int a = 0; a < 2 * MAX_ATTEMPTS; ++a) ctl->ccount[(rp ^ 1) * 2 * MAX_ATTEMPTS + a] = 0u;
         }
 
         if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
@@ -1078,6 +1094,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             const uint4 r0 = ld_dsmem_v4(mapa(smem_u32(&ctl->nb), 0u));
             nb = (int)r0.x;
             j = (int)r0.y;
+            // did the batch end on its threshold (not on the buffer, not on M), and was there one?
+            prev_tau_valid = cnt > 0 && nb < PB && j < Mb && !no_batch;
+            prev_taubits = taubits;
         }
         if (!split && j < Mb) {
             if (STATS && tid == 0) t0 = clock64();
