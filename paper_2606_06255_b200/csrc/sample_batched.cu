@@ -294,7 +294,8 @@ struct __align__(16) HierSmem {
     int hist[64];
     unsigned wmax[16], wmax2[16];
     uint2 plist[PB];               // picks of the running sub-round: {slot id in s*, D bits}
-    int cnt2, nb, j, pad;
+    int cnt2, nb, j;
+    unsigned tau2;
 };
 
 template <int CPT1, int CPT2, bool EUC>
@@ -324,18 +325,24 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
     }
     int jl = j, nbl = 0, applied = 0;
     long long tt0 = 0, tt1 = 0;
+    unsigned bound_bits = 0u;            // an upper bound of every candidate's distance left by the last sub-round
+    bool have_bound = false;
     for (;;) {
         tt0 = clock64();
-        // ---- (a) block maximum ----
+        // ---- (a) block maximum.  After a sub-round that ended on tau2 every candidate is <= tau2, which
+        // serves as the origin of the bins just as well: the reduction and its barrier are skipped ----
         float m = D[0];
 #pragma unroll
         for (int c = 1; c < CPT1; ++c) m = fmaxf(m, D[c]);
-        const unsigned wm = __reduce_max_sync(FULL, __float_as_uint(m));
-        if (lane == 0) hs->wmax[warp] = wm;
-        if (tid < 64) hs->hist[tid] = 0;
-        if (tid == 0) hs->cnt2 = 0;
-        __syncthreads();
-        const unsigned m1 = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax[lane] : 0u);
+        unsigned m1 = bound_bits;
+        if (!have_bound) {
+            const unsigned wm = __reduce_max_sync(FULL, __float_as_uint(m));
+            if (lane == 0) hs->wmax[warp] = wm;
+            if (tid < 64) hs->hist[tid] = 0;
+            if (tid == 0) hs->cnt2 = 0;
+            __syncthreads();
+            m1 = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax[lane] : 0u);
+        }
         if (!(m1 > taubits)) break;
         const float fm1 = __uint_as_float(m1);
         const float scale = fminf(__fdiv_rn(64.0f, __fsub_rn(fm1, tau)), FLT_MAX);
@@ -359,6 +366,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             }
             const int excl = incl - (h0 + h1);
             bstar = __popc(__ballot_sync(FULL, excl + h0 <= T2)) + __popc(__ballot_sync(FULL, incl <= T2));
+            if (__shfl_sync(FULL, incl, 31) == 0) break;      // no live candidate (only possible with a bound as m1)
         }
         if (bstar == 0) {
             // ---- fallback: one pick by a block-wide argmax with the full tie-break ----
@@ -388,6 +396,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             }
             ++jl;
             ++nbl;
+            have_bound = false;          // no tau2 from this path: the next sub-round reduces the maximum again
             __syncthreads();
         } else {
             // ---- (d) C2 -> shared memory; tau2 = the largest live distance left outside C2 (>= tau), so
@@ -413,12 +422,15 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 if (lane == 0) hs->wmax2[warp] = we;
             }
             __syncthreads();
+            if (tid >= BT - 64) hs->hist[tid - (BT - 64)] = 0;      // consumed by every warp in (c): clean for the next sub-round
             tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1;
             // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
             // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
             if (warp == 0) {
                 const int n2 = hs->cnt2;
                 const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
+                __syncwarp();
+                if (lane == 0) { hs->cnt2 = 0; hs->tau2 = tau2bits; }
                 float x2[CPT2], y2[CPT2], z2[CPT2], d2v[CPT2];
 #pragma unroll
                 for (int c = 0; c < CPT2; ++c) {
@@ -553,6 +565,8 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             __syncthreads();
             nbl = hs->nb;
             jl = hs->j;
+            bound_bits = hs->tau2;       // the pick loop stopped at or below tau2, and so did everything outside C2
+            have_bound = true;
         }
 #undef RFPS_BIN
         c_subrounds++;
