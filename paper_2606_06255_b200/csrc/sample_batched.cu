@@ -368,6 +368,13 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             bstar = __popc(__ballot_sync(FULL, excl + h0 <= T2)) + __popc(__ballot_sync(FULL, incl <= T2));
             if (__shfl_sync(FULL, incl, 31) == 0) break;      // no live candidate (only possible with a bound as m1)
         }
+        if (bstar == 0 && have_bound) {
+            // the first bin overflows and m1 is only a bound: redo the sub-round from the true maximum, which
+            // the fallback below needs (all warps have read the histogram before it is cleared again)
+            have_bound = false;
+            __syncthreads();
+            continue;
+        }
         if (bstar == 0) {
             // ---- fallback: one pick by a block-wide argmax with the full tie-break ----
             unsigned o = 0u, oi = 0u;
