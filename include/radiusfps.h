@@ -203,6 +203,33 @@ int fps_get_stats(fps_index_t *h, fps_stats *out);
 int fps_sample_host(const float *points_host, int32_t N, int32_t B, int32_t M, int32_t start_idx,
                     int32_t *out_idx_host, float *out_mindist_host, const fps_build_opts *opts);
 
+/*
+ * fps_build_and_sample -- the one-shot call: index build, sampling and release of
+ * the index for a batch that is sampled once, as the first sampling layer of a network does with every
+ * scene; the build is then on the critical path.  The batch is cut into chunks of
+ * consecutive clouds; the index of chunk k+1 is built on an internal stream while the sampling kernel of
+ * chunk k runs on opts->stream.  Every cloud is sampled exactly as by fps_index_build + fps_sample on it
+ * alone: chunking changes the schedule, never a result.
+ *
+ *   points        DEVICE fp32 [total][3], the clouds one after the other.
+ *   offsets       HOST int32 [B+1] (as fps_index_build_ragged), or NULL: B clouds of N points each.
+ *   M             HOST int32 [B], or NULL: every cloud yields M_all samples.
+ *   start_idx     HOST int32 [B], or NULL: every cloud starts at its point 0.
+ *   out_idx / out_mindist   DEVICE, cloud b's samples start at M[0] + .. + M[b-1] (b * M_all).
+ *   opts          NULL or build options; opts->stream is the stream `points` was produced on and the results
+ *                 are ordered on.
+ *   chunk_clouds  clouds per chunk; 0 or >= B: one chunk (the fastest schedule measured on B200: the
+ *                 sampling time of a chunk is latency-bound and hardly depends on its size).  Smaller
+ *                 chunks bound the device memory of the index (about 100 B per point of one chunk).
+ *
+ * Returns when the last sampling kernel is enqueued (the builds synchronise the internal stream, not
+ * opts->stream).  On a negative return the chunks before the failing one have been enqueued and the rest of
+ * the outputs is untouched.
+ */
+int fps_build_and_sample(const float *points, const int32_t *offsets, int32_t N, int32_t B,
+                         const int32_t *M, int32_t M_all, const int32_t *start_idx,
+                         int32_t *out_idx, float *out_mindist, const fps_build_opts *opts, int32_t chunk_clouds);
+
 /* Thread-local description of the last error on the calling thread ("" if none). */
 const char *fps_last_error(void);
 

@@ -19,7 +19,7 @@ FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG
 FPS_FLAG_EUCLIDEAN = 32
 
 EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_pick_chain_cycles", "fps_index_destroy", "fps_get_stats",
-           "fps_sample_host", "fps_last_error", "fps_last_status", "fps_version"]
+           "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version"]
 
 
 class fps_build_opts(ctypes.Structure):
@@ -90,6 +90,9 @@ def load() -> ctypes.CDLL:
     lib.fps_get_stats.argtypes = [vp, ctypes.POINTER(fps_stats)]
     lib.fps_sample_host.restype = ctypes.c_int
     lib.fps_sample_host.argtypes = [vp, i32, i32, i32, i32, vp, vp, ctypes.POINTER(fps_build_opts)]
+    lib.fps_build_and_sample.restype = ctypes.c_int
+    lib.fps_build_and_sample.argtypes = [vp, ctypes.POINTER(i32), i32, i32, ctypes.POINTER(i32), i32, ctypes.POINTER(i32), vp, vp,
+                                         ctypes.POINTER(fps_build_opts), i32]
     lib.fps_last_error.restype = ctypes.c_char_p
     lib.fps_last_error.argtypes = []
     lib.fps_version.restype = ctypes.c_char_p
@@ -309,3 +312,60 @@ def fps_sample_host(points_host: torch.Tensor, M: int, start_idx: int = 0, *, n_
     if rc != FPS_OK:
         raise FpsError(rc, fps_last_error())
     return out_idx, out_mindist
+
+
+def fps_build_and_sample(points: torch.Tensor, M, *, offsets=None, start_idx=None, chunk_clouds: int = 0, n_vox: int = 0,
+                         tile_points: int = 0, cluster_size: int = 0, block_threads: int = 0, flags: int = 0,
+                         local_warps: int = 0, cand_per_thread: int = 0, out_idx: torch.Tensor | None = None,
+                         out_mindist: torch.Tensor | None = None, stream: torch.cuda.Stream | None = None):
+    """fps_build_and_sample: the one-shot call; the index of chunk k+1 is built while chunk k is sampled.
+    ``points``: CUDA float32 [B,N,3], or [T,3] with ``offsets`` (B+1 ints).  ``M``: one int for all clouds or
+    B ints; ``start_idx``: None (= 0) or B ints.  Returns (out_idx, out_mindist) shaped [B,M] when M is one
+    int, else flat [sum M] plus the list of output offsets.  Results are ordered on ``stream``."""
+    lib = load()
+    if not points.is_cuda:
+        raise ValueError("points must live on a CUDA device")
+    if offsets is None:
+        B, N = _check_points(points)
+        oarr = None
+    else:
+        if points.dtype != torch.float32 or not points.is_contiguous() or points.dim() != 2 or points.shape[1] != 3:
+            raise ValueError("points must be a contiguous CUDA float32 tensor [T,3]")
+        off = [int(v) for v in offsets]
+        if len(off) < 2 or off[-1] != points.shape[0]:
+            raise ValueError("offsets must hold B+1 entries and end at the number of points")
+        B, N = len(off) - 1, 0
+        oarr = (ctypes.c_int32 * (B + 1))(*off)
+    uniform = isinstance(M, int)
+    Ms = [int(M)] * B if uniform else [int(v) for v in M]
+    if len(Ms) != B:
+        raise ValueError("M must be one int or hold one entry per cloud")
+    marr = None if uniform else (ctypes.c_int32 * B)(*Ms)
+    sarr = None
+    if start_idx is not None:
+        ss = [int(v) for v in start_idx]
+        if len(ss) != B:
+            raise ValueError("start_idx must hold one entry per cloud")
+        sarr = (ctypes.c_int32 * B)(*ss)
+    total = sum(max(m, 0) for m in Ms)
+    shape = (B, max(Ms[0], 0)) if uniform else (total,)
+    with torch.cuda.device(points.device):
+        if out_idx is None:
+            out_idx = torch.empty(shape, dtype=torch.int32, device=points.device)
+        if out_mindist is None:
+            out_mindist = torch.empty(shape, dtype=torch.float32, device=points.device)
+        if out_idx.dtype != torch.int32 or out_mindist.dtype != torch.float32 or not out_idx.is_contiguous() \
+                or not out_mindist.is_contiguous() or out_idx.numel() < total or out_mindist.numel() < total:
+            raise ValueError("out_idx must be contiguous int32 and out_mindist contiguous float32, sum M entries each")
+        s = stream if stream is not None else torch.cuda.current_stream()
+        o = _opts(n_vox, tile_points, cluster_size, block_threads, flags, s.cuda_stream, local_warps, cand_per_thread)
+        rc = lib.fps_build_and_sample(points.data_ptr(), oarr, N, B, marr, Ms[0] if uniform else 0, sarr,
+                                      out_idx.data_ptr(), out_mindist.data_ptr(), ctypes.byref(o), int(chunk_clouds))
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    if uniform:
+        return out_idx, out_mindist
+    offs = [0]
+    for m in Ms:
+        offs.append(offs[-1] + m)
+    return out_idx, out_mindist, offs

@@ -1,9 +1,12 @@
 // api.cu -- the C-ABI of include/radiusfps.h: argument validation, error strings, handle lifetime.
 // Every step of the path runs in the kernels of index_build.cu / sample_kernel.cu; there is no CPU
 // fallback anywhere in this library.
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
+#include <vector>
 
 #include "internal.h"
 
@@ -224,6 +227,95 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->local_subrounds = (int64_t)c[24]; out->local_fallbacks = (int64_t)c[25];
             if (getenv("RFPS_DEBUG")) fprintf(stderr, "[rfps debug] local phase cycles (sum over clouds): select %llu pick-loop %llu apply %llu\n", c[21], c[22], c[23]);
         }
+    }
+    return FPS_OK;
+}
+
+// the internal stream the pipelined one-shot call builds on, and the event that orders it behind the
+// caller's stream; one pair per device, created on first use and kept for the life of the process
+static int pipeline_stream(cudaStream_t *bs, cudaEvent_t *ev)
+{
+    static std::mutex mu;
+    static cudaStream_t streams[64] = {};
+    static cudaEvent_t events[64] = {};
+    int dev = 0;
+    RFPS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) { set_error("device ordinal %d out of range", dev); return FPS_ERR_INVALID; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!streams[dev]) {
+        RFPS_CUDA(cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking));
+        RFPS_CUDA(cudaEventCreateWithFlags(&events[dev], cudaEventDisableTiming));
+    }
+    *bs = streams[dev];
+    *ev = events[dev];
+    return FPS_OK;
+}
+
+int fps_build_and_sample(const float *points, const int32_t *offsets, int32_t N, int32_t B, const int32_t *M, int32_t M_all,
+                         const int32_t *start_idx, int32_t *out_idx, float *out_mindist, const fps_build_opts *opts,
+                         int32_t chunk_clouds)
+{
+    rfps::g_err[0] = 0;
+    if (!points || !out_idx || !out_mindist) { set_error("NULL argument"); return FPS_ERR_INVALID; }
+    if (B < 1) { set_error("B=%d must be >= 1", B); return FPS_ERR_INVALID; }
+    if (!offsets && N < 1) { set_error("N=%d must be >= 1 when offsets is NULL", N); return FPS_ERR_INVALID; }
+    if (!M && M_all < 1) { set_error("M_all=%d must be >= 1 when M is NULL", M_all); return FPS_ERR_INVALID; }
+    if (chunk_clouds < 0) { set_error("chunk_clouds=%d must be >= 0", chunk_clouds); return FPS_ERR_INVALID; }
+    if (offsets && offsets[0] != 0) { set_error("offsets[0]=%d must be 0", offsets[0]); return FPS_ERR_INVALID; }
+    fps_build_opts o;
+    memset(&o, 0, sizeof o);
+    if (opts) o = *opts;
+    cudaStream_t us = (cudaStream_t)o.stream;
+    // auto = one chunk: a chunk's sampling time is set by the latency of its longest cloud, not by how many
+    // clouds it holds, and the chunks' sampling kernels run one after the other; measured on B200 the
+    // build that chunking hides never outweighs that.  Chunks are for bounding the
+    // memory of the index (about 100 B per point, held for one chunk at a time)
+    int chunk = chunk_clouds == 0 ? B : chunk_clouds;
+    if (chunk > B) chunk = B;
+    const bool pipelined = chunk < B;
+    cudaStream_t bs = us;
+    cudaEvent_t ev = nullptr;
+    if (pipelined) {
+        int rc = pipeline_stream(&bs, &ev);
+        if (rc != FPS_OK) return rc;
+        // the builds read `points` on the internal stream: order it behind what the caller enqueued
+        RFPS_CUDA(cudaEventRecord(ev, us));
+        RFPS_CUDA(cudaStreamWaitEvent(bs, ev, 0));
+    }
+    o.stream = (void *)bs;
+    std::vector<int32_t> loc;
+    long long out_off = 0;
+    for (int c0 = 0; c0 < B; c0 += chunk) {
+        const int Bk = std::min(chunk, B - c0);
+        const float *pk = points + 3 * (size_t)(offsets ? offsets[c0] : (long long)c0 * N);
+        fps_index_t *h;
+        if (offsets) {
+            loc.resize((size_t)Bk + 1);
+            for (int i = 0; i <= Bk; ++i) loc[i] = offsets[c0 + i] - offsets[c0];
+            h = build_common(pk, 0, Bk, loc.data(), &o);
+        } else {
+            h = build_common(pk, N, Bk, nullptr, &o);
+        }
+        if (!h) return rfps::g_build_rc ? rfps::g_build_rc : FPS_ERR_INVALID;
+        // the index is complete (the build synchronised its stream): sample it on the caller's stream,
+        // behind the previous chunk, while the host goes on to build the next chunk
+        int rc;
+        long long mk = 0;
+        if (!M && !start_idx) {
+            rc = fps_sample(h, M_all, 0, out_idx + out_off, out_mindist + out_off, (void *)us);
+            mk = (long long)M_all * Bk;
+        } else {
+            std::vector<int32_t> mm((size_t)Bk), ss((size_t)Bk);
+            for (int i = 0; i < Bk; ++i) {
+                mm[i] = M ? M[c0 + i] : M_all;
+                ss[i] = start_idx ? start_idx[c0 + i] : 0;
+                mk += mm[i] > 0 ? mm[i] : 0;
+            }
+            rc = fps_sample_ragged(h, mm.data(), ss.data(), out_idx + out_off, out_mindist + out_off, (void *)us);
+        }
+        fps_index_destroy(h);      // stream-ordered behind the sampling kernel just enqueued
+        if (rc != FPS_OK) return rc;
+        out_off += mk;
     }
     return FPS_OK;
 }

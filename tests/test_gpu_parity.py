@@ -299,6 +299,61 @@ def test_ragged_index_of_equal_clouds_equals_the_uniform_one(rf):
         rf.fps_index_destroy(ix)
 
 
+@pytest.mark.parametrize("chunk", [0, 1, 3, 8, 100])
+def test_one_shot_ragged_chunks_match_the_oracle(rf, chunk):
+    # SURVEY 8(f) NEXT-2, second half: build + sample + release in one call, the batch cut into chunks whose
+    # index builds overlap the sampling of the chunk before; the chunking must never change a result
+    clouds = [inputs.room(5000, 21), inputs.uniform_cube(1, 22), inputs.lidar(7001, 23, n_azimuth=110),
+              inputs.shuffled_lattice(8, 24), inputs.uniform_cube(33, 25), inputs.clustered(2500, 26),
+              inputs.with_duplicates(900, 27, 200), inputs.uniform_cube(4099, 28)]
+    Ms = [1250, 1, 1800, 512, 33, 600, 450, 1031]
+    starts = [0, 0, 7000, 5, 32, 17, 899, 4098]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])]).astype(np.int64)
+    P = torch.from_numpy(np.ascontiguousarray(np.concatenate(clouds, axis=0))).cuda()
+    for ms, ss in ((Ms, starts), (Ms, None)):
+        idx, mind, ooff = rf.fps_build_and_sample(P, ms, offsets=off.tolist(), start_idx=ss, chunk_clouds=chunk)
+        torch.cuda.synchronize()
+        idx, mind = idx.cpu().numpy(), mind.cpu().numpy()
+        for b, c in enumerate(clouds):
+            ref_i, ref_m = oracle.fps(c, ms[b], ss[b] if ss else 0)
+            assert_same(idx[ooff[b]:ooff[b + 1]], mind[ooff[b]:ooff[b + 1]], ref_i.reshape(-1), ref_m.reshape(-1))
+    with pytest.raises(rf.FpsError) as e:                    # cloud 1 holds one point: M = 2 cannot fit
+        rf.fps_build_and_sample(P, 2, offsets=off.tolist(), chunk_clouds=chunk)
+    assert e.value.status == rf.FPS_ERR_INVALID
+
+
+@pytest.mark.parametrize("chunk", [0, 5, 16])
+def test_one_shot_uniform_batch_pipelined_on_a_side_stream(rf, chunk):
+    # 40 clouds in one chunk, eight chunks of 5 and chunks of 16 + 16 + 8, inputs produced on a side stream right before the call: the internal
+    # build stream must wait for them, and the results must be ordered on that same stream
+    w = inputs.scaled("C2", 3000, 700, B=40)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    Ph = torch.from_numpy(P).pin_memory()
+    side = torch.cuda.Stream()
+    for _ in range(3):
+        with torch.cuda.stream(side):
+            Pd = torch.empty_like(Ph, device="cuda")
+            Pd.copy_(Ph, non_blocking=True)
+            idx, mind = rf.fps_build_and_sample(Pd, w.M, chunk_clouds=chunk, stream=side)
+            hi = idx.to("cpu", non_blocking=True)
+            hm = mind.to("cpu", non_blocking=True)
+        side.synchronize()
+        assert_same(hi.numpy(), hm.numpy(), *ref)
+
+
+def test_one_shot_rejects_bad_arguments(rf):
+    P = torch.from_numpy(inputs.uniform_cube(100, 1)).cuda()
+    for kw in (dict(M=0), dict(M=101), dict(M=5, chunk_clouds=-1), dict(M=[5, 5]), dict(M=5, start_idx=[100])):
+        with pytest.raises((rf.FpsError, ValueError)):
+            rf.fps_build_and_sample(P, kw.pop("M"), **kw)
+    bad = P.clone()
+    bad[7, 1] = float("nan")
+    with pytest.raises(rf.FpsError) as e:
+        rf.fps_build_and_sample(bad, 5)
+    assert e.value.status == rf.FPS_ERR_NONFINITE
+
+
 @pytest.mark.parametrize("cluster", [0, 2, 5])
 def test_repeated_launches_under_load_are_identical(rf, cluster):
     # the batched kernel passes data between CTAs with release/acquire flags, DSMEM atomics and dynamic work
