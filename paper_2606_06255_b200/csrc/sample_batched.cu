@@ -296,7 +296,9 @@ struct __align__(16) HierSmem {
     uint2 plist[PB];               // picks of the running sub-round: {slot id in s*, D bits}
     int cnt2, nb, j;
     unsigned tau2;
+    int npub;                      // picks of the running sub-round visible in plist (| NP_FINAL: no more will come)
 };
+constexpr int NP_FINAL = 1 << 30;
 
 template <int CPT1, int CPT2, bool EUC>
 __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY, const float *cZ, const float *cD,
@@ -307,7 +309,15 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
 {
     static_assert(CPT1 % 2 == 0 && CPT2 >= 1 && CPT2 <= 4, "shape");
     constexpr int H1 = CPT1 / 2, T2 = 32 * CPT2;
+    // the pick warp is the LAST warp: its own candidate slots are padding unless the buffer is full, so it
+    // rarely has anything to catch up on after its loop, while the other warps follow the picks as they appear
+    constexpr int PW = BT / 32 - 1;
     const int lane = tid & 31, warp = tid >> 5;
+    static_assert(BT == 512, "the slot permutation below is written for 16 warps");
+    // candidate slots are dealt to the warps so that the four warps of the pick warp's scheduler (warp % 4 == 3)
+    // come last: with a buffer that is not nearly full they hold padding only and leave that scheduler alone
+    const int wr = (warp & 3) == 3 ? 12 + (warp >> 2) : 3 * (warp >> 2) + (warp & 3);
+    const int st = 32 * wr + lane;
     const float tau = __uint_as_float(taubits);
     f32x2 X[H1], Y[H1], Z[H1];
     float D[CPT1];
@@ -315,7 +325,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
     for (int h = 0; h < H1; ++h) {
         // candidate slots 2t, 2t+1 (then 2*BT + 2t, ...): a buffer that is not full leaves whole warps with
         // padding only, and those warps drop out of the update loop (f)
-        const int i0 = h * 2 * BT + 2 * tid, i1 = i0 + 1;
+        const int i0 = h * 2 * BT + 2 * st, i1 = i0 + 1;
         const bool ok0 = i0 < cnt, ok1 = i1 < cnt;
         X[h] = pack2(ok0 ? cX[i0] : 0.0f, ok1 ? cX[i1] : 0.0f);
         Y[h] = pack2(ok0 ? cY[i0] : 0.0f, ok1 ? cY[i1] : 0.0f);
@@ -382,7 +392,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
 #pragma unroll
                 for (int c = 0; c < CPT1; ++c)
                     if (D[c] == m) {
-                        const unsigned i = (unsigned)((c >> 1) * 2 * BT + 2 * tid + (c & 1));
+                        const unsigned i = (unsigned)((c >> 1) * 2 * BT + 2 * st + (c & 1));
                         const unsigned oc = cO[i];
                         if (oc >= o) { o = oc; oi = i; }
                     }
@@ -414,7 +424,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 if (D[c] > tau) {
                     if (RFPS_BIN(D[c]) < bstar) {
                         const int sl = atomicAdd(&hs->cnt2, 1);
-                        const int i = (c >> 1) * 2 * BT + 2 * tid + (c & 1);
+                        const int i = (c >> 1) * 2 * BT + 2 * st + (c & 1);
                         hs->sD[sl] = D[c];
                         hs->sX[sl] = cX[i];
                         hs->sY[sl] = cY[i];
@@ -428,12 +438,13 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 const unsigned we = __reduce_max_sync(FULL, __float_as_uint(exmax));
                 if (lane == 0) hs->wmax2[warp] = we;
             }
+            if (tid == 0) hs->npub = 0;
             __syncthreads();
             if (tid >= BT - 64) hs->hist[tid - (BT - 64)] = 0;      // consumed by every warp in (c): clean for the next sub-round
             tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1;
             // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
             // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
-            if (warp == 0) {
+            if (warp == PW) {
                 const int n2 = hs->cnt2;
                 const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
                 __syncwarp();
@@ -492,7 +503,10 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         wid = __reduce_max_sync(FULL, mine) - 1u;
                     }
                     const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
-                    if (lane == 0) hs->plist[nbl - nb0] = make_uint2(wid, ghi);
+                    if (lane == 0) {
+                        hs->plist[nbl - nb0] = make_uint2(wid, ghi);
+                        bpick[nbl] = make_float4(sx, sy, sz, 0.0f);
+                    }
                     ++jl;
                     ++nbl;
                     if (jl >= M || nbl >= PB) return false;
@@ -508,10 +522,8 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                     float dsave[CPT2];
 #pragma unroll
                     for (int c = 0; c < CPT2; ++c) dsave[c] = d2v[c];
-                    unsigned gh[KCH], wd[KCH];
-#pragma unroll
-                    for (int p = 0; p < KCH; ++p) { gh[p] = 0u; wd[p] = 0u; }      // not reached = "over"
                     bool over = false, tie = false;          // "max <= tau2 seen" / "exact tie seen before that"
+                    int acc = 0;                             // picks before the first "max <= tau2"
 #pragma unroll
                     for (int p = 0; p < KCH; ++p) {
                         // one uniform exit test every four picks bounds the speculation past the end of the
@@ -532,9 +544,12 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         const unsigned wid = gmx - 1u;       // always a valid slot: some lane is top
                         over |= !(ghi > tau2bits);
                         tie |= (gmx != gmn) && !over;
-                        gh[p] = ghi;
-                        wd[p] = wid;
+                        acc += over ? 0 : 1;
                         const float sx = hs->sX[wid], sy = hs->sY[wid], sz = hs->sZ[wid];
+                        if (lane == 0) {                     // logged speculatively, off the dependent chain
+                            hs->plist[nbl - nb0 + p] = make_uint2(wid, ghi);
+                            bpick[nbl + p] = make_float4(sx, sy, sz, 0.0f);
+                        }
 #pragma unroll
                         for (int c = 0; c < CPT2; ++c) d2v[c] = fminf(d2v[c], distf<EUC>(d2_rn(x2[c], y2[c], z2[c], sx, sy, sz)));
                     }
@@ -544,18 +559,17 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         for (int p = 0; p < KCH && go; ++p) go = careful_pick();
                         continue;
                     }
-                    int acc = KCH;                           // picks before the first "max <= tau2"
-#pragma unroll
-                    for (int p = KCH - 1; p >= 0; --p)
-                        if (!(gh[p] > tau2bits)) acc = p;
-                    if (lane == 0) {
-#pragma unroll
-                        for (int p = 0; p < KCH; ++p)
-                            if (p < acc) hs->plist[nbl - nb0 + p] = make_uint2(wd[p], gh[p]);
-                    }
                     jl += acc;
                     nbl += acc;
                     go = acc == KCH;
+                    if (lane == 0) {                         // the other warps may apply these picks now
+                        __threadfence_block();
+                        *(volatile int *)&hs->npub = nbl - nb0;
+                    }
+                }
+                if (lane == 0) {
+                    __threadfence_block();
+                    *(volatile int *)&hs->npub = (nbl - nb0) | NP_FINAL;
                 }
                 {
                     const int n = nbl - nb0;                 // emit the sub-round's picks
@@ -564,10 +578,45 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         const uint2 pk = hs->plist[i];
                         out_idx[j0 + i] = (int)(~hs->sO[pk.x]);
                         out_mind[j0 + i] = __uint_as_float(pk.y);
-                        bpick[nb0 + i] = make_float4(hs->sX[pk.x], hs->sY[pk.x], hs->sZ[pk.x], 0.0f);
                     }
                 }
                 if (lane == 0) { hs->nb = nbl; hs->j = jl; }
+            } else {
+                // ---- (f), streamed: the other warps apply the sub-round's picks to their candidates while the
+                // pick warp is still producing them; after the loop only the last few picks are left ----
+                bool live = false;
+#pragma unroll
+                for (int c = 0; c < CPT1; ++c) live |= D[c] > tau;
+                if (__any_sync(FULL, live)) {
+                    int done = 0;
+                    for (;;) {
+                        const int v = *(volatile int *)&hs->npub;
+                        const int n = v & 0xffff;
+                        if (n > done) {
+                            __threadfence_block();
+                            for (int i = done; i < n; ++i) {
+                                const float4 sp = bpick[nbl + i];
+                                const f32x2 SX = pack2(sp.x, sp.x), SY = pack2(sp.y, sp.y), SZ = pack2(sp.z, sp.z);
+#pragma unroll
+                                for (int h = 0; h < H1; ++h) {
+                                    const f32x2 dx = sub2(X[h], SX), dy = sub2(Y[h], SY), dz = sub2(Z[h], SZ);
+                                    float x0, x1, y0, y1, z0, z1;
+                                    unpack2(mul2(dx, dx), x0, x1);
+                                    unpack2(mul2(dy, dy), y0, y1);
+                                    unpack2(mul2(dz, dz), z0, z1);
+                                    D[2 * h] = fminf(D[2 * h], distf<EUC>(__fadd_rn(__fadd_rn(x0, y0), z0)));
+                                    D[2 * h + 1] = fminf(D[2 * h + 1], distf<EUC>(__fadd_rn(__fadd_rn(x1, y1), z1)));
+                                }
+                            }
+                            done = n;
+                        } else if (v & NP_FINAL) {
+                            break;
+                        } else {
+                            __nanosleep(64);
+                        }
+                    }
+                    applied = nbl + done;                    // nbl still is the batch size before this sub-round
+                }
             }
             __syncthreads();
             nbl = hs->nb;
