@@ -54,6 +54,9 @@ constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffff
 #define RFPS_GTARGET 0.625f
 #endif
 constexpr float GTARGET = RFPS_GTARGET;   // aim the next extraction at this fraction of the candidate buffer
+#ifndef RFPS_CPT2
+#define RFPS_CPT2 3
+#endif
 constexpr int SUBW = 4;        // 32-bit mask words per queued voxel
 constexpr int SUBP = 32 * SUBW;   // picks applied between two CTA barriers
 
@@ -1104,7 +1107,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 }
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
-                local_fps_hier<CPT, 2, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
+                local_fps_hier<CPT, RFPS_CPT2, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
                                        c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
