@@ -54,6 +54,9 @@ constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffff
 #define RFPS_GTARGET 0.625f
 #endif
 constexpr float GTARGET = RFPS_GTARGET;   // aim the next extraction at this fraction of the candidate buffer
+#ifndef RFPS_POLL_NS
+#define RFPS_POLL_NS 32
+#endif
 #ifndef RFPS_CPT2
 #define RFPS_CPT2 3
 #endif
@@ -297,8 +300,7 @@ struct __align__(16) HierSmem {
     int hist[64];
     unsigned wmax[16], wmax2[16];
     uint2 plist[PB];               // picks of the running sub-round: {slot id in s*, D bits}
-    int cnt2, nb, j;
-    unsigned tau2;
+    int cnt2;
     int npub;                      // picks of the running sub-round visible in plist (| NP_FINAL: no more will come)
 };
 constexpr int NP_FINAL = 1 << 30;
@@ -443,15 +445,19 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             }
             if (tid == 0) hs->npub = 0;
             __syncthreads();
-            if (tid >= BT - 64) hs->hist[tid - (BT - 64)] = 0;      // consumed by every warp in (c): clean for the next sub-round
+            // every warp is past (c): clean for the next sub-round.  Done by the pick warp, so that it is ordered
+            // before the end-of-loop flag the other warps wait for (no barrier ends the sub-round any more)
+            if (warp == PW) { hs->hist[lane] = 0; hs->hist[32 + lane] = 0; }
+            // tau2 = the largest live distance outside C2: where the pick loop stops, and the bound the next
+            // sub-round hangs its bins on
+            const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
             tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1;
             // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
             // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
             if (warp == PW) {
                 const int n2 = hs->cnt2;
-                const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
                 __syncwarp();
-                if (lane == 0) { hs->cnt2 = 0; hs->tau2 = tau2bits; }
+                if (lane == 0) hs->cnt2 = 0;
                 float x2[CPT2], y2[CPT2], z2[CPT2], d2v[CPT2];
 #pragma unroll
                 for (int c = 0; c < CPT2; ++c) {
@@ -574,6 +580,8 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                     __threadfence_block();
                     *(volatile int *)&hs->npub = (nbl - nb0) | NP_FINAL;
                 }
+                __syncwarp();
+                asm volatile("bar.arrive 1, %0;" ::"n"(BT) : "memory");      // wakes the warps that only wait (below)
                 {
                     const int n = nbl - nb0;                 // emit the sub-round's picks
                     __syncwarp();
@@ -583,21 +591,25 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         out_mind[j0 + i] = __uint_as_float(pk.y);
                     }
                 }
-                if (lane == 0) { hs->nb = nbl; hs->j = jl; }
             } else {
                 // ---- (f), streamed: the other warps apply the sub-round's picks to their candidates while the
                 // pick warp is still producing them; after the loop only the last few picks are left ----
                 bool live = false;
 #pragma unroll
                 for (int c = 0; c < CPT1; ++c) live |= D[c] > tau;
-                if (__any_sync(FULL, live)) {
+                // a warp whose candidates are all dead only needs the final count: it sleeps on a named barrier
+                // that the pick warp and the working warps arrive at without waiting (polling would take issue
+                // slots from the pick warp)
+                const bool wlive = __any_sync(FULL, live);
+                {
                     int done = 0;
+                    if (!wlive) asm volatile("bar.sync 1, %0;" ::"n"(BT) : "memory");
                     for (;;) {
                         const int v = *(volatile int *)&hs->npub;
                         const int n = v & 0xffff;
                         if (n > done) {
                             __threadfence_block();
-                            for (int i = done; i < n; ++i) {
+                            for (int i = done; wlive && i < n; ++i) {
                                 const float4 sp = bpick[nbl + i];
                                 const f32x2 SX = pack2(sp.x, sp.x), SY = pack2(sp.y, sp.y), SZ = pack2(sp.z, sp.z);
 #pragma unroll
@@ -615,23 +627,23 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         } else if (v & NP_FINAL) {
                             break;
                         } else {
-                            __nanosleep(64);
+                            __nanosleep(RFPS_POLL_NS);
                         }
                     }
-                    applied = nbl + done;                    // nbl still is the batch size before this sub-round
+                    if (wlive) asm volatile("bar.arrive 1, %0;" ::"n"(BT) : "memory");
+                    nbl += done;                             // the final count is the sub-round's result: no barrier
+                    jl += done;
+                    applied = nbl;
                 }
             }
-            __syncthreads();
-            nbl = hs->nb;
-            jl = hs->j;
-            bound_bits = hs->tau2;       // the pick loop stopped at or below tau2, and so did everything outside C2
+            bound_bits = tau2bits;       // the pick loop stopped at or below tau2, and so did everything outside C2
             have_bound = true;
         }
 #undef RFPS_BIN
         c_subrounds++;
-        // the workers may start applying these picks now (bpick was written before the barrier above).  The
-        // release costs a fence: it is issued from the last warp, whose candidate slots are padding unless
-        // the buffer is full, so that it overlaps the other warps' update loop instead of delaying the pick warp
+        // the workers may start applying these picks now.  The release is issued by the thread that wrote bpick
+        // (lane 0 of the pick warp; after a barrier on the fallback path); its fence overlaps the other warps'
+        // selection of the next sub-round
         if (pub_addr && tid == BT - 32) st_release_cluster_u32(pub_addr, (unsigned)nbl);
         tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
         // ---- (f) the sub-round's picks -> all of C1.  Candidates at or below tau are out of the round for
