@@ -54,6 +54,12 @@ constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffff
 #define RFPS_GTARGET 0.625f
 #endif
 constexpr float GTARGET = RFPS_GTARGET;   // aim the next extraction at this fraction of the candidate buffer
+#ifndef RFPS_GT_MAX
+#define RFPS_GT_MAX 0.7f
+#define RFPS_GT_UP 1.03f
+#define RFPS_GT_MIN 0.35f
+#define RFPS_GT_DOWN 0.85f
+#endif
 #ifndef RFPS_POLL_NS
 #define RFPS_POLL_NS 32
 #endif
@@ -781,6 +787,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned qpar = 0u, round_parity = 0u, prev_taubits = 0u;
     bool prev_tau_valid = false;
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
+    float gt = GTARGET;              // fraction of the candidate buffer the next extraction aims at; follows the overflow rate
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
                        c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0, c_subrounds = 0, c_fallback = 0;
     long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
@@ -1086,12 +1093,14 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     cnt = (int)found;
                     taubits = tb;
                     // aim the next round at ~5/8 of the buffer; move by at most 2x per round
-                    const float ratio = fminf(2.0f, fmaxf(0.5f, (GTARGET * TC) / (float)max(found, 1u)));
+                    const float ratio = fminf(2.0f, fmaxf(0.5f, (gt * TC) / (float)max(found, 1u)));
                     g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
+                    gt = fminf(RFPS_GT_MAX, gt * RFPS_GT_UP);
                     break;
                 }
                 if (STATS && tid == 0 && rank == 0) c_retries++;
                 g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
+                gt = fmaxf(RFPS_GT_MIN, gt * RFPS_GT_DOWN);
             }
         }
         }
