@@ -241,9 +241,21 @@ def cpu_oracle_sample(w, P_host, budget_s=15.0):
     t = time.perf_counter()
     oracle.fps(P_host[:nb], m, w.start_idx, threads=nb)
     dt = time.perf_counter() - t
-    return {"value": nb * m / dt, "unit": UNIT, "cores": int(oracle.fps.threads_used), "kind": "oracle",
-            "sample": f"first {nb} of {w.B} clouds x first {m} of {w.M} samples, {dt:.1f} s wall, "
-                      f"oracle/fps_oracle.c -O2 one thread per cloud", "ms_per_cloud_extrapolated": dt / m * w.M * 1e3}
+    out = {"value": nb * m / dt, "unit": UNIT, "cores": int(oracle.fps.threads_used), "kind": "oracle",
+           "sample": f"first {nb} of {w.B} clouds x first {m} of {w.M} samples, {dt:.1f} s wall, "
+                     f"oracle/fps_oracle.c -O2 one thread per cloud", "ms_per_cloud_extrapolated": dt / m * w.M * 1e3}
+    # SURVEY 8(d) CPU baseline (2): the plain CPU pruned variant (oracle/fps_pruned_cpu.c, the paper's section 3
+    # algorithm, untuned), same clouds and threading, all M samples (its cost per sample falls as the prune bites,
+    # so a prefix would be biased); its ratio to the oracle is the analogue of the paper's CPU speedups (`:697-705`).
+    t = time.perf_counter()
+    oracle.pruned_fps(P_host[:nb], w.M, w.start_idx, n_vox=16, threads=nb)
+    dtp = time.perf_counter() - t
+    out["pruned_cpu_variant"] = {"value": nb * w.M / dtp, "unit": UNIT, "cores": int(oracle.pruned_fps.threads_used),
+                                 "n_vox": 16, "ms_per_cloud": dtp * 1e3,
+                                 "speedup_over_oracle": (nb * w.M / dtp) / (nb * m / dt),
+                                 "sample": f"first {nb} of {w.B} clouds x all {w.M} samples, {dtp:.2f} s wall, "
+                                           f"oracle/fps_pruned_cpu.c one thread per cloud"}
+    return out
 
 
 def reference_arm(args, rank, world):
