@@ -292,13 +292,26 @@ __global__ void __launch_bounds__(SCAN1_T) k_scan_single(const int *__restrict__
     int *dst = out + off;
     if (threadIdx.x == 0) carry_s = 0;
     __syncthreads();
+    // the steps are serially dependent through the carry: the next step's items are loaded before this
+    // step's barriers so that their memory latency is not on that chain
+    int nx[SCAN1_ITEMS];
+#pragma unroll
+    for (int i = 0; i < SCAN1_ITEMS; ++i) {
+        const int q = threadIdx.x * SCAN1_ITEMS + i;
+        nx[i] = q < n ? src[q] : 0;
+    }
     for (int base = 0; base < n; base += SCAN1_TILE) {
         const int i0 = base + threadIdx.x * SCAN1_ITEMS;
         int v[SCAN1_ITEMS], s = 0;
 #pragma unroll
         for (int i = 0; i < SCAN1_ITEMS; ++i) {
-            v[i] = i0 + i < n ? src[i0 + i] : 0;
+            v[i] = nx[i];
             s += v[i];
+        }
+#pragma unroll
+        for (int i = 0; i < SCAN1_ITEMS; ++i) {
+            const int q = i0 + SCAN1_TILE + i;
+            nx[i] = q < n ? src[q] : 0;
         }
         int inc = s;
 #pragma unroll
@@ -399,20 +412,32 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
     int *ov = ovals + (size_t)pbase;
     const int end = min(N, (c + 1) * RS_CHUNK);
     const unsigned lt = (1u << lane) - 1u;
-    for (int p0 = c * RS_CHUNK; p0 < end; p0 += 32) {
-        const int p = p0 + lane;
+    // the whole chunk is loaded before the ranking loop: its rounds are serially dependent through the
+    // shared counters, and a global load inside each of them would put DRAM/L2 latency on that chain
+    constexpr int R = RS_CHUNK / 32;
+    unsigned key[R];
+    int val[R];
+    const int p0 = c * RS_CHUNK + lane;
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const int p = p0 + 32 * r;
         const bool valid = p < end;
-        unsigned key = valid ? k[p] : 0u;
-        int val = valid ? v[p] : 0;
-        unsigned d = valid ? ((key >> shift) & 255u) : 256u;
-        unsigned peers = __match_any_sync(0xffffffffu, d);
-        int rank = __popc(peers & lt);
+        key[r] = valid ? k[p] : 0u;
+        val[r] = valid ? v[p] : 0;
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r) {
+        const bool valid = p0 + 32 * r < end;
+        if (c * RS_CHUNK + 32 * r >= end) break;          // warp-uniform
+        const unsigned d = valid ? ((key[r] >> shift) & 255u) : 256u;
+        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const int rank = __popc(peers & lt);
         int dst = 0;
         if (valid) dst = base[w][d] + rank;
         __syncwarp();
         if (valid && rank == 0) base[w][d] += __popc(peers);
         __syncwarp();
-        if (valid) { ok[dst] = key; ov[dst] = val; }
+        if (valid) { ok[dst] = key[r]; ov[dst] = val[r]; }
     }
 }
 
