@@ -544,6 +544,13 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         // one uniform exit test every four picks bounds the speculation past the end of the
                         // sub-round without putting a branch behind every redux
                         if ((p & 3) == 0 && p > 0 && over) break;
+                        // half-way publish: the picks before the first "over" or tie stand whatever follows (a tie
+                        // redoes the chunk with the same arithmetic), and what the other warps have not applied when
+                        // the loop ends is on the critical path of the sub-round
+                        if (p == KCH / 2 && !tie && lane == 0) {
+                            __threadfence_block();
+                            *(volatile int *)&hs->npub = nbl - nb0 + p;
+                        }
                         float bm = d2v[0];
 #pragma unroll
                         for (int c = 1; c < CPT2; ++c) bm = fmaxf(bm, d2v[c]);
