@@ -19,6 +19,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <mutex>
+#include <utility>
 #include <vector>
 
 #include "internal.h"
@@ -39,6 +40,33 @@ __device__ __forceinline__ float ord2f(unsigned u)
 }
 
 // ---------------------------------------------------------------------------------------------
+// Programmatic dependent launch: the build is a chain of ~20 short kernels, each depending on the one
+// before it; every kernel lets its successor be scheduled at once (launch_dependents) and then waits for
+// the complete predecessor grid and its memory (wait) before it touches anything, so the order of all
+// memory operations is the stream order, and only the launch latency of the successor is overlapped.
+// ---------------------------------------------------------------------------------------------
+__device__ __forceinline__ void grid_dep_sync()
+{
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+template <typename... P, typename... A>
+static void launch_pdl(void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute at[1];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 1;
+    cudaLaunchKernelEx(&cfg, kern, std::forward<A>(args)...);     // errors surface in the cudaGetLastError checks below
+}
+
+// ---------------------------------------------------------------------------------------------
 // a1: bounding box (Eq. 6) + non-finite detection.  bbox[b] = {minx,miny,minz,maxx,maxy,maxz} as
 // order-preserving uints; bbox[b][6] = non-finite flag.
 // ---------------------------------------------------------------------------------------------
@@ -46,6 +74,7 @@ constexpr int BBOX_STRIDE = 8;
 
 __global__ void k_bbox_init(unsigned *bbox, int B)
 {
+    grid_dep_sync();
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < B * BBOX_STRIDE) {
         int c = i % BBOX_STRIDE;
@@ -57,6 +86,7 @@ __global__ void k_bbox_init(unsigned *bbox, int B)
 // concatenated arrays.  Every kernel below takes `poff`; grids are sized for the largest cloud.
 __global__ void __launch_bounds__(256) k_bbox(const float *__restrict__ pts, const int *__restrict__ poff, unsigned *bbox)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const float *P = pts + (size_t)base * 3;
@@ -146,6 +176,7 @@ __global__ void __launch_bounds__(256) k_keys(const float *__restrict__ pts, con
                                                const unsigned *__restrict__ bbox, int n_vox, int hb, int sb,
                                                unsigned *__restrict__ keys, int *__restrict__ vals)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
@@ -217,6 +248,7 @@ __device__ __forceinline__ int block_excl_scan(int v, int *total, int *sm /*[33]
 __global__ void __launch_bounds__(SCAN_T) k_scan_blocksum(const int *__restrict__ in, int n, int stride, int nblk,
                                                            int *__restrict__ bsum, const int *__restrict__ poff)
 {
+    grid_dep_sync();
     __shared__ int sm[33];
     const int b = blockIdx.y;
     const int *src = in + (poff ? (size_t)poff[b] : (size_t)b * stride);
@@ -233,6 +265,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_blocksum(const int *__restrict_
 
 __global__ void __launch_bounds__(SCAN_T) k_scan_bsums(int *bsum, int nblk, int *totals)
 {
+    grid_dep_sync();
     __shared__ int sm[33];
     const int b = blockIdx.x;
     int *s = bsum + (size_t)b * nblk;
@@ -251,6 +284,7 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_bsums(int *bsum, int nblk, int 
 __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ in, int *__restrict__ out, int n, int stride,
                                                         int nblk, const int *__restrict__ bsum, const int *__restrict__ poff)
 {
+    grid_dep_sync();
     __shared__ int sm[33];
     const int b = blockIdx.y;
     const size_t off = poff ? (size_t)poff[b] : (size_t)b * stride;
@@ -283,6 +317,7 @@ constexpr int SCAN1_T = 1024, SCAN1_ITEMS = 4, SCAN1_TILE = SCAN1_T * SCAN1_ITEM
 __global__ void __launch_bounds__(SCAN1_T) k_scan_single(const int *__restrict__ in, int *__restrict__ out, int n, int stride,
                                                          int *__restrict__ totals, const int *__restrict__ poff)
 {
+    grid_dep_sync();
     __shared__ int wsum[32];
     __shared__ int carry_s;
     const int b = blockIdx.x, lane = threadIdx.x & 31, w = threadIdx.x >> 5;
@@ -350,15 +385,15 @@ static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int
 {
     if (n <= SCAN1_MAX_N) {
         g_launches += 1;
-        k_scan_single<<<B, SCAN1_T, 0, st>>>(in, out, n, stride, totals, poff);
+        launch_pdl(k_scan_single, dim3(B), dim3(SCAN1_T), st, in, out, n, stride, totals, poff);
         RFPS_CUDA(cudaGetLastError());
         return FPS_OK;
     }
     g_launches += 3;
     const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
-    k_scan_blocksum<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, n, stride, nblk, bsum_tmp, poff);
-    k_scan_bsums<<<B, SCAN_T, 0, st>>>(bsum_tmp, nblk, totals);
-    k_scan_apply<<<dim3(nblk, B), SCAN_T, 0, st>>>(in, out, n, stride, nblk, bsum_tmp, poff);
+    launch_pdl(k_scan_blocksum, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, n, stride, nblk, bsum_tmp, poff);
+    launch_pdl(k_scan_bsums, dim3(B), dim3(SCAN_T), st, bsum_tmp, nblk, totals);
+    launch_pdl(k_scan_apply, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, out, n, stride, nblk, bsum_tmp, poff);
     RFPS_CUDA(cudaGetLastError());
     return FPS_OK;
 }
@@ -377,6 +412,7 @@ constexpr int RS_CHUNK = 512, RS_WARPS = 4;    // short chunks: enough warps in 
 __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, const int *__restrict__ poff,
                                                                int nchunk, int shift, int *__restrict__ table)
 {
+    grid_dep_sync();
     const int pbase = poff[blockIdx.y], N = poff[blockIdx.y + 1] - pbase;
     __shared__ int h[RS_WARPS][256];
     const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -398,6 +434,7 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
                                                                   const int *__restrict__ table,
                                                                   unsigned *__restrict__ okeys, int *__restrict__ ovals)
 {
+    grid_dep_sync();
     const int pbase = poff[blockIdx.y], N = poff[blockIdx.y + 1] - pbase;
     __shared__ int base[RS_WARPS][256];
     const int b = blockIdx.y, w = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -447,6 +484,7 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
 __global__ void __launch_bounds__(256) k_heads(const unsigned *__restrict__ keys, const int *__restrict__ poff, int subbits,
                                                 int *__restrict__ heads)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -459,6 +497,7 @@ __global__ void __launch_bounds__(256) k_heads(const unsigned *__restrict__ keys
 __global__ void __launch_bounds__(256) k_voxel_offsets(const int *__restrict__ heads, const int *__restrict__ rank,
                                                         const int *__restrict__ poff, int *__restrict__ voff)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const int p = blockIdx.x * blockDim.x + threadIdx.x;
@@ -470,6 +509,7 @@ __global__ void __launch_bounds__(256) k_voxel_offsets(const int *__restrict__ h
 __global__ void __launch_bounds__(256) k_ntiles(const int *__restrict__ voff, const int *__restrict__ Kv,
                                                  const int *__restrict__ poff, int tile_points, int *__restrict__ ntiles)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -489,6 +529,7 @@ __global__ void __launch_bounds__(256) k_tiles(const int *__restrict__ voff, con
                                                 const int *__restrict__ tbase, const int *__restrict__ poff, int K_cap,
                                                 int2 *__restrict__ vseg)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int base = poff[b], N = poff[b + 1] - base;
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
@@ -513,6 +554,7 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pts, c
                                                  float *__restrict__ px, float *__restrict__ py, float *__restrict__ pz,
                                                  int *__restrict__ porig, int *__restrict__ pinv)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const size_t o = (size_t)poff[b];
     const int N = poff[b + 1] - poff[b];
@@ -545,6 +587,7 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
                                                  const int *__restrict__ K, const int *__restrict__ poff, int K_cap,
                                                  float4 *__restrict__ vgeom, int *__restrict__ maxcnt)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31;
     const float *x = px + (size_t)poff[b], *y = py + (size_t)poff[b], *z = pz + (size_t)poff[b];
@@ -589,6 +632,7 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
 __global__ void __launch_bounds__(256) k_group_sphere(const float4 *__restrict__ vgeom, const int *__restrict__ K, int K_cap,
                                                        int G_cap, float4 *__restrict__ ggeom)
 {
+    grid_dep_sync();
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31;
     const int Kb = K[b];
@@ -790,9 +834,9 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));
     RFPS_CUDA(cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st));
     const int *poff = ix.poff_dev;
-    k_bbox_init<<<(B * BBOX_STRIDE + 255) / 256, 256, 0, st>>>(sc.bbox, B);
-    k_bbox<<<dim3(std::max(1, std::min((N + 4095) / 4096, 148)), B), 256, 0, st>>>(points, poff, sc.bbox);
-    k_keys<<<gN, 256, 0, st>>>(points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
+    launch_pdl(k_bbox_init, dim3((B * BBOX_STRIDE + 255) / 256), dim3(256), st, sc.bbox, B);
+    launch_pdl(k_bbox, dim3(dim3(std::max(1, std::min((N + 4095) / 4096, 148)), B)), dim3(256), st, points, poff, sc.bbox);
+    launch_pdl(k_keys, dim3(gN), dim3(256), st, points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
     g_launches += 3;
 
     // a3: LSD radix sort, 8 bits per pass
@@ -800,27 +844,27 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     int *vin = sc.vA, *vout = sc.vB;
     const dim3 gR((nchunk + RS_WARPS - 1) / RS_WARPS, B);
     for (int shift = 0; shift < keybits; shift += 8) {
-        k_radix_hist<<<gR, RS_WARPS * 32, 0, st>>>(kin, poff, nchunk, shift, sc.table);
+        launch_pdl(k_radix_hist, dim3(gR), dim3(RS_WARPS * 32), st, kin, poff, nchunk, shift, sc.table);
         if ((rc = scan_exclusive(sc.table, sc.table, (int)table_n, (int)table_n, B, nullptr, sc.bsum, st))) { release_scratch(); return rc; }
-        k_radix_scatter<<<gR, RS_WARPS * 32, 0, st>>>(kin, vin, poff, nchunk, shift, sc.table, kout, vout);
+        launch_pdl(k_radix_scatter, dim3(gR), dim3(RS_WARPS * 32), st, kin, vin, poff, nchunk, shift, sc.table, kout, vout);
         std::swap(kin, kout);
         std::swap(vin, vout);
         g_launches += 2;
     }
 
     // a5: grid voxels -> (tiled) segments; a4: gather; a6: spheres
-    k_heads<<<gN, 256, 0, st>>>(kin, poff, 3 * sb, sc.heads);
+    launch_pdl(k_heads, dim3(gN), dim3(256), st, kin, poff, 3 * sb, sc.heads);
     if ((rc = scan_exclusive(sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st, poff))) { release_scratch(); return rc; }
-    k_voxel_offsets<<<gN, 256, 0, st>>>(sc.heads, sc.rank, poff, sc.voff);
-    k_ntiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, poff, tile_points, sc.ntl);
+    launch_pdl(k_voxel_offsets, dim3(gN), dim3(256), st, sc.heads, sc.rank, poff, sc.voff);
+    launch_pdl(k_ntiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, poff, tile_points, sc.ntl);
     if ((rc = scan_exclusive(sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st, poff))) { release_scratch(); return rc; }
-    k_tiles<<<gN, 256, 0, st>>>(sc.voff, sc.Kv, sc.ntl, sc.tbase, poff, ix.K_cap, ix.vseg);
-    k_gather<<<gN, 256, 0, st>>>(points, vin, poff, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
+    launch_pdl(k_tiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, sc.ntl, sc.tbase, poff, ix.K_cap, ix.vseg);
+    launch_pdl(k_gather, dim3(gN), dim3(256), st, points, vin, poff, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
     const int sphere_blocks = std::max(1, std::min((ix.K_cap + 7) / 8, 148 * 8));
-    k_sphere<<<dim3(sphere_blocks, B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
+    launch_pdl(k_sphere, dim3(dim3(sphere_blocks, B)), dim3(256), st, ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
                                                      reinterpret_cast<int *>(meta));
     const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, 148 * 8));
-    k_group_sphere<<<dim3(group_blocks, B), 256, 0, st>>>(ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
+    launch_pdl(k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
     g_launches += 8;
     if (cudaGetLastError() != cudaSuccess) {
         set_error("a build kernel failed to launch: %s", cudaGetErrorString(cudaGetLastError()));
