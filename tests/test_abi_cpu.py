@@ -117,3 +117,21 @@ def test_no_packed_fma_in_the_built_kernels():
         euclid = re.search(r"k_fps_batchedILi\d+ELi\d+ELb[01]ELb1EE", fn) is not None
         if "k_fps_" in fn and not euclid:
             assert ffma <= 48 and fmul > ffma, (fn, ffma, fmul)
+
+
+def test_every_build_kernel_waits_for_its_predecessor_grid():
+    """The index build chains its kernels by programmatic dependent launch: the order of
+    memory operations is the stream order only if EVERY kernel launched that way starts with grid_dep_sync()
+    (griddepcontrol.wait before its first memory access), and no build kernel is launched around launch_pdl."""
+    src = open(os.path.join(ROOT, "paper_2606_06255_b200", "csrc", "index_build.cu")).read()
+    kernels = re.findall(r"__global__\s+void\s+(?:__launch_bounds__\([^)]*\)\s*)?(k_\w+)\s*\(", src)
+    assert len(kernels) >= 16
+    for k in kernels:
+        body = src[re.search(r"__global__\s+void\s+(?:__launch_bounds__\([^)]*\)\s*)?" + k + r"\s*\(", src).end():]
+        first = body[body.index("{") + 1:].lstrip().splitlines()[0].strip()
+        assert first == "grid_dep_sync();", (k, first)
+    assert "<<<" not in src.replace("// ", ""), "a build kernel is launched without launch_pdl"
+    assert set(re.findall(r"launch_pdl\((k_\w+),", src)) == set(kernels)
+    helper = src[src.index("void grid_dep_sync()"):]
+    helper = helper[:helper.index("}")]
+    assert helper.index("griddepcontrol.launch_dependents") < helper.index("griddepcontrol.wait")
