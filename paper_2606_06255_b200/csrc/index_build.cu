@@ -785,6 +785,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 
     Scratch sc;
     unsigned *meta = nullptr;      // [0] = largest segment, then (persistent arena only)
+    unsigned *rb = nullptr;        // the read-back block (persistent arena)
     auto carve = [&](Carver &c, bool persistent) {
         if (persistent) {
             ix.px = c.take<float>(BN); ix.py = c.take<float>(BN); ix.pz = c.take<float>(BN);
@@ -793,13 +794,16 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
             ix.vseg = c.take<int2>((size_t)B * ix.K_cap);
             ix.ggeom = c.take<float4>((size_t)B * ix.G_cap);
             ix.vstate = per_pick ? c.take<uint4>((size_t)B * ix.K_cap) : nullptr;
-            ix.K_dev = c.take<int32_t>(B);
+            // read-back block: K per cloud, meta, the bounding boxes (with the non-finite flags) -- contiguous, so
+            // that the one host round-trip of the build is ONE copy
+            rb = c.take<unsigned>((size_t)B + 8 + (size_t)B * BBOX_STRIDE);
+            ix.K_dev = reinterpret_cast<int32_t *>(rb);
+            meta = rb ? rb + B : nullptr;
+            sc.bbox = rb ? rb + B + 8 : nullptr;
             ix.poff_dev = c.take<int32_t>(B + 1);
             ix.rag_dev = c.take<int32_t>(3 * (size_t)(B + 1));
             ix.counters = c.take<unsigned long long>(NUM_COUNTERS);
-            meta = c.take<unsigned>(8);
         } else {
-            sc.bbox = c.take<unsigned>((size_t)B * BBOX_STRIDE);
             sc.kA = c.take<unsigned>(BN); sc.kB = c.take<unsigned>(BN);
             sc.vA = c.take<int>(BN); sc.vB = c.take<int>(BN);
             sc.table = c.take<int>(table_n * B);
@@ -874,13 +878,18 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 
     // the one host round-trip of the build: K per cloud, the non-finite flags, the largest segment
     ix.K_host = (int32_t *)malloc(sizeof(int32_t) * B);
-    std::vector<unsigned> hb((size_t)B * BBOX_STRIDE);
+    const size_t rb_n = (size_t)B + 8 + (size_t)B * BBOX_STRIDE;
+    std::vector<unsigned> hrb(rb_n);
     if (!ix.K_host) { set_error("host malloc failed"); release_scratch(); return FPS_ERR_NOMEM; }
-    cudaError_t e1 = cudaMemcpyAsync(ix.K_host, ix.K_dev, sizeof(int32_t) * B, cudaMemcpyDeviceToHost, st);
-    cudaError_t e2 = cudaMemcpyAsync(hb.data(), sc.bbox, sizeof(unsigned) * B * BBOX_STRIDE, cudaMemcpyDeviceToHost, st);
-    cudaError_t e3 = cudaMemcpyAsync(&ix.max_voxel_points, meta, sizeof(int), cudaMemcpyDeviceToHost, st);
+    cudaError_t e1 = cudaMemcpyAsync(hrb.data(), rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
+    cudaError_t e2 = cudaSuccess, e3 = cudaSuccess;
     release_scratch();
     cudaError_t e4 = cudaStreamSynchronize(st);
+    if (e1 == cudaSuccess && e4 == cudaSuccess) {
+        memcpy(ix.K_host, hrb.data(), sizeof(int32_t) * B);
+        ix.max_voxel_points = (int)hrb[B];
+    }
+    const unsigned *hb = hrb.data() + B + 8;
     if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) {
         set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : (e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3))));
         return FPS_ERR_CUDA;
