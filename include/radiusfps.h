@@ -25,7 +25,9 @@
  *   - Functions returning int return FPS_OK (0) or a negative fps_status.  fps_last_error()
  *     returns a thread-local, NUL-terminated description of the last failure on this thread.
  *   - A handle holds mutable sampling state (Dist_p, Dist_v): calls on ONE handle must not
- *     overlap; different handles are independent.
+ *     overlap, and one handle is used on ONE stream at a time (fps_index_destroy releases the memory
+ *     stream-ordered behind the last fps_sample / fps_gather_xyz call only); different handles are
+ *     independent, also across host threads.
  */
 #ifndef RADIUSFPS_H
 #define RADIUSFPS_H
@@ -117,6 +119,9 @@ typedef struct {
     int64_t local_subrounds;  /* hierarchical local phase: sub-rounds (one-warp FPS runs)             */
     int64_t local_fallbacks;  /* ... of which single block-wide argmax picks (first bin overflowed)   */
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
+    int64_t cycles_local_select, cycles_local_pick, cycles_local_update;   /* hierarchical local phase, SM cycles
+                                 seen by thread 0 of the picker CTA, summed over clouds: candidate selection /
+                                 the pick loop / applying the picks to the candidates after the loop           */
 } fps_stats;
 
 /*
@@ -188,8 +193,11 @@ int fps_gather_xyz(fps_index_t *h, const int32_t *idx, int32_t M, float *out_xyz
  */
 int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_per_pick);
 
-/* Frees the handle and all device memory it owns.  NULL is allowed. */
+/* Frees the handle and all device memory it owns (stream-ordered behind the last call on the handle).
+ * NULL is allowed.  The memory goes back to a library-private pool that keeps it for the next build;
+ * fps_trim() returns whatever the pool holds unused to the driver. */
 void fps_index_destroy(fps_index_t *h);
+void fps_trim(void);
 
 /* Layout facts and (with FPS_FLAG_STATS) the counters of the last fps_sample; synchronises the
  * stream of that call.  out: host pointer. */
@@ -222,9 +230,11 @@ int fps_sample_host(const float *points_host, int32_t N, int32_t B, int32_t M, i
  *                 sampling time of a chunk is latency-bound and hardly depends on its size).  Smaller
  *                 chunks bound the device memory of the index (about 100 B per point of one chunk).
  *
- * Returns when the last sampling kernel is enqueued (the builds synchronise the internal stream, not
- * opts->stream).  On a negative return the chunks before the failing one have been enqueued and the rest of
- * the outputs is untouched.
+ * Returns when the last sampling kernel is enqueued.  Every index build ends with one small device-to-host
+ * read (voxel counts, non-finite flags) and synchronises the stream it runs on: with several chunks that is
+ * the internal stream, so opts->stream is never waited for; with ONE chunk (the default) the build runs on
+ * opts->stream itself and the call therefore waits for everything enqueued on it before.  On a negative
+ * return the chunks before the failing one have been enqueued and the rest of the outputs is untouched.
  */
 int fps_build_and_sample(const float *points, const int32_t *offsets, int32_t N, int32_t B,
                          const int32_t *M, int32_t M_all, const int32_t *start_idx,

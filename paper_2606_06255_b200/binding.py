@@ -19,7 +19,7 @@ FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG
 FPS_FLAG_EUCLIDEAN = 32
 
 EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_pick_chain_cycles", "fps_index_destroy", "fps_get_stats",
-           "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version"]
+           "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version", "fps_trim"]
 
 
 class fps_build_opts(ctypes.Structure):
@@ -44,7 +44,9 @@ class fps_stats(ctypes.Structure):
                 ("cycles_prune_sum", ctypes.c_int64), ("cycles_visit_sum", ctypes.c_int64),
                 ("cycles_prune_max", ctypes.c_int64), ("cycles_visit_max", ctypes.c_int64), ("sub_batches", ctypes.c_int64),
                 ("local_subrounds", ctypes.c_int64), ("local_fallbacks", ctypes.c_int64),
-                ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32)]
+                ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32),
+                ("cycles_local_select", ctypes.c_int64), ("cycles_local_pick", ctypes.c_int64),
+                ("cycles_local_update", ctypes.c_int64)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -99,6 +101,8 @@ def load() -> ctypes.CDLL:
     lib.fps_version.argtypes = []
     lib.fps_last_status.restype = ctypes.c_int
     lib.fps_last_status.argtypes = []
+    lib.fps_trim.restype = None
+    lib.fps_trim.argtypes = []
     _lib = lib
     return lib
 
@@ -109,6 +113,10 @@ def fps_last_error() -> str:
 
 def fps_version() -> str:
     return load().fps_version().decode()
+
+
+def fps_trim() -> None:
+    load().fps_trim()
 
 
 def _check_points(points: torch.Tensor) -> tuple[int, int]:

@@ -1,48 +1,76 @@
 """In-tree nvcc build of the radiusfps CUDA library for sm_100a.
 
-``python -m paper_2606_06255_b200.build`` (or ``build()``) compiles ``csrc/*.cu`` into
-``paper_2606_06255_b200/libradiusfps.so`` next to this file.  The .so is git-ignored but travels
-to the GPU box with the working tree.  nvcc cross-compiles without a GPU.
+``python -m paper_2606_06255_b200.build`` (or ``build()``) compiles every ``csrc/*.cu`` into an object under
+``paper_2606_06255_b200/_build/`` (in parallel; only the stale ones) and links them into
+``paper_2606_06255_b200/libradiusfps.so`` next to this file.  The .so is git-ignored but travels to the GPU
+box with the working tree.  nvcc cross-compiles without a GPU.
 """
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "_build")
 LIB = os.path.join(HERE, "libradiusfps.so")
-SOURCES = ["api.cu", "index_build.cu", "sample_kernel.cu", "sample_batched.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
     "-O3", "-lineinfo", "-std=c++17",
     "--fmad=false",                      # belt and braces: the kernels use __f*_rn intrinsics anyway
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
     "-I", os.path.join(ROOT, "include"), "-I", CSRC,
 ]
 
 
-def _stale() -> bool:
-    if not os.path.exists(LIB):
+def sources() -> list[str]:
+    return sorted(f for f in os.listdir(CSRC) if f.endswith(".cu"))
+
+
+def _headers() -> list[str]:
+    return [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".h", ".cuh"))] + \
+           [os.path.join(ROOT, "include", "radiusfps.h"), os.path.abspath(__file__)]
+
+
+def _obj(src: str) -> str:
+    return os.path.join(OBJ, os.path.splitext(src)[0] + ".o")
+
+
+def _stale_obj(src: str) -> bool:
+    o = _obj(src)
+    if not os.path.exists(o):
         return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)] + [os.path.join(ROOT, "include", "radiusfps.h"),
-                                                                  os.path.abspath(__file__)]
-    return any(os.path.getmtime(d) > t for d in deps)
+    t = os.path.getmtime(o)
+    return any(os.path.getmtime(d) > t for d in [os.path.join(CSRC, src), *_headers()])
 
 
 def build(force: bool = False, verbose: bool = False, extra: list[str] | None = None) -> str:
-    if not force and not _stale():
-        return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    tmp = LIB + f".tmp{os.getpid()}"
-    cmd = [nvcc, *NVCC_FLAGS, *(extra or []), *[os.path.join(CSRC, s) for s in SOURCES], "-o", tmp]
-    if verbose:
-        print(" ".join(cmd), file=sys.stderr)
-    subprocess.run(cmd, check=True)
-    os.replace(tmp, LIB)
+    os.makedirs(OBJ, exist_ok=True)
+    todo = [s for s in sources() if force or extra or _stale_obj(s)]
+
+    def compile_one(src: str) -> None:
+        tmp = _obj(src) + f".tmp{os.getpid()}"
+        cmd = [nvcc, *NVCC_FLAGS, *(extra or []), "-c", os.path.join(CSRC, src), "-o", tmp]
+        if verbose:
+            print(" ".join(cmd), file=sys.stderr)
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, _obj(src))
+
+    if todo:
+        with ThreadPoolExecutor(max_workers=min(len(todo), os.cpu_count() or 1)) as ex:
+            list(ex.map(compile_one, todo))
+    objs = [_obj(s) for s in sources()]
+    if todo or not os.path.exists(LIB) or any(os.path.getmtime(o) > os.path.getmtime(LIB) for o in objs):
+        tmp = LIB + f".tmp{os.getpid()}"
+        cmd = [nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-shared", *objs, "-o", tmp]
+        if verbose:
+            print(" ".join(cmd), file=sys.stderr)
+        subprocess.run(cmd, check=True)
+        os.replace(tmp, LIB)
     return LIB
 
 

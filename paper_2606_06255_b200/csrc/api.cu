@@ -24,6 +24,24 @@ void set_error(const char *fmt, ...)
     va_end(ap);
 }
 
+const DeviceProps &device_props()
+{
+    static std::mutex mu;
+    static DeviceProps props[64];
+    static bool known[64] = {};
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64) dev = 0;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!known[dev]) {
+        cudaDeviceGetAttribute(&props[dev].sm_count, cudaDevAttrMultiProcessorCount, dev);
+        cudaDeviceGetAttribute(&props[dev].max_smem_optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+        if (props[dev].sm_count <= 0) props[dev].sm_count = 1;
+        known[dev] = true;
+    }
+    return props[dev];
+}
+
 }  // namespace rfps
 
 using rfps::set_error;
@@ -41,6 +59,7 @@ static fps_index_t *build_common(const float *points, int32_t N, int32_t B, cons
     rfps::g_status = FPS_ERR_INVALID;
     if (!points) { set_error("points is NULL"); return nullptr; }
     if (B < 1) { set_error("B=%d must be >= 1", B); return nullptr; }
+    if (B > 65535) { set_error("B=%d: at most 65535 clouds per index (split the batch, or use fps_build_and_sample with chunk_clouds)", B); return nullptr; }
     long long total = 0;
     int32_t nmax = 0;
     if (offsets) {
@@ -144,21 +163,26 @@ int fps_sample_ragged(fps_index_t *h, const int32_t *M, const int32_t *start_idx
     if (!M || !out_idx || !out_mindist) { set_error("NULL argument"); return FPS_ERR_INVALID; }
     rfps::DeviceIndex &ix = h->ix;
     const int B = ix.B;
-    int32_t *r = ix.rag_host;                 // [3][B+1]: M_b, start_b, output offsets
-    long long off = 0;
-    int64_t iters = 0;
+    // validate every cloud before touching the handle's state (rag_host / rag_M_max describe the LAST GOOD call)
     for (int b = 0; b < B; ++b) {
         const int nb = ix.poff_host[b + 1] - ix.poff_host[b];
         const int sb = start_idx ? start_idx[b] : 0;
         if (M[b] < 1 || M[b] > nb) { set_error("M[%d]=%d must be in [1, N_b=%d]", b, M[b], nb); return FPS_ERR_INVALID; }
         if (sb < 0 || sb >= nb) { set_error("start_idx[%d]=%d must be in [0, N_b=%d)", b, sb, nb); return FPS_ERR_INVALID; }
+    }
+    int32_t *r = ix.rag_host;                 // [3][B+1]: M_b, start_b, output offsets
+    long long off = 0;
+    int64_t iters = 0;
+    int32_t mmax = 0;
+    for (int b = 0; b < B; ++b) {
         r[b] = M[b];
-        r[(B + 1) + b] = sb;
+        r[(B + 1) + b] = start_idx ? start_idx[b] : 0;
         r[2 * (B + 1) + b] = (int32_t)off;
         off += M[b];
         iters += M[b] - 1;
-        if (M[b] > ix.rag_M_max || b == 0) ix.rag_M_max = b == 0 ? M[b] : (M[b] > ix.rag_M_max ? M[b] : ix.rag_M_max);
+        mmax = std::max(mmax, M[b]);
     }
+    ix.rag_M_max = mmax;
     r[B] = 0; r[(B + 1) + B] = 0; r[2 * (B + 1) + B] = (int32_t)off;
     cudaStream_t st = (cudaStream_t)stream;
     // pageable source: the copy is staged before the call returns, so rag_host can be reused by the next call
@@ -185,6 +209,8 @@ int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_pe
     if (!cycles_per_pick || iters < 1) { set_error("bad argument"); return FPS_ERR_INVALID; }
     return rfps::measure_pick_chain(cand_per_lane, iters, cycles_per_pick);
 }
+
+void fps_trim(void) { rfps::trim_pool(); }
 
 void fps_index_destroy(fps_index_t *h)
 {
@@ -225,31 +251,25 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->cycles_prune_max = (int64_t)c[18]; out->cycles_visit_max = (int64_t)c[19];
             out->sub_batches = (int64_t)c[20];
             out->local_subrounds = (int64_t)c[24]; out->local_fallbacks = (int64_t)c[25];
-            if (getenv("RFPS_DEBUG")) fprintf(stderr, "[rfps debug] local phase cycles (sum over clouds): select %llu pick-loop %llu apply %llu\n", c[21], c[22], c[23]);
+            out->cycles_local_select = (int64_t)c[21]; out->cycles_local_pick = (int64_t)c[22]; out->cycles_local_update = (int64_t)c[23];
         }
     }
     return FPS_OK;
 }
 
-// the internal stream the pipelined one-shot call builds on, and the event that orders it behind the
-// caller's stream; one pair per device, created on first use and kept for the life of the process
-static int pipeline_stream(cudaStream_t *bs, cudaEvent_t *ev)
-{
-    static std::mutex mu;
-    static cudaStream_t streams[64] = {};
-    static cudaEvent_t events[64] = {};
-    int dev = 0;
-    RFPS_CUDA(cudaGetDevice(&dev));
-    if (dev < 0 || dev >= 64) { set_error("device ordinal %d out of range", dev); return FPS_ERR_INVALID; }
-    std::lock_guard<std::mutex> lock(mu);
-    if (!streams[dev]) {
-        RFPS_CUDA(cudaStreamCreateWithFlags(&streams[dev], cudaStreamNonBlocking));
-        RFPS_CUDA(cudaEventCreateWithFlags(&events[dev], cudaEventDisableTiming));
+// The pipelined one-shot call builds on a stream of its own, ordered behind the caller's stream by an event.
+// Both are created per call and destroyed when the call returns (cudaStreamDestroy / cudaEventDestroy release
+// the objects once the work already enqueued has finished), so two host threads calling at the same time
+// never share a stream or re-record each other's event.
+struct PipelineStream {
+    cudaStream_t bs = nullptr;
+    cudaEvent_t ev = nullptr;
+    ~PipelineStream()
+    {
+        if (ev) cudaEventDestroy(ev);
+        if (bs) cudaStreamDestroy(bs);
     }
-    *bs = streams[dev];
-    *ev = events[dev];
-    return FPS_OK;
-}
+};
 
 int fps_build_and_sample(const float *points, const int32_t *offsets, int32_t N, int32_t B, const int32_t *M, int32_t M_all,
                          const int32_t *start_idx, int32_t *out_idx, float *out_mindist, const fps_build_opts *opts,
@@ -274,13 +294,14 @@ int fps_build_and_sample(const float *points, const int32_t *offsets, int32_t N,
     if (chunk > B) chunk = B;
     const bool pipelined = chunk < B;
     cudaStream_t bs = us;
-    cudaEvent_t ev = nullptr;
+    PipelineStream ps;
     if (pipelined) {
-        int rc = pipeline_stream(&bs, &ev);
-        if (rc != FPS_OK) return rc;
+        RFPS_CUDA(cudaStreamCreateWithFlags(&ps.bs, cudaStreamNonBlocking));
+        RFPS_CUDA(cudaEventCreateWithFlags(&ps.ev, cudaEventDisableTiming));
+        bs = ps.bs;
         // the builds read `points` on the internal stream: order it behind what the caller enqueued
-        RFPS_CUDA(cudaEventRecord(ev, us));
-        RFPS_CUDA(cudaStreamWaitEvent(bs, ev, 0));
+        RFPS_CUDA(cudaEventRecord(ps.ev, us));
+        RFPS_CUDA(cudaStreamWaitEvent(bs, ps.ev, 0));
     }
     o.stream = (void *)bs;
     std::vector<int32_t> loc;

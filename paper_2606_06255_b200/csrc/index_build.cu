@@ -22,6 +22,7 @@
 #include <utility>
 #include <vector>
 
+#include "device_utils.cuh"
 #include "internal.h"
 
 namespace rfps {
@@ -50,8 +51,15 @@ __device__ __forceinline__ void grid_dep_sync()
     asm volatile("griddepcontrol.launch_dependents;");
     asm volatile("griddepcontrol.wait;" ::: "memory");
 }
+// Launch bookkeeping of ONE build (a local of build_index, passed down): kernels launched so far and the first
+// launch error, checked once after the chain has been enqueued.
+struct LaunchLog {
+    int launches = 0;
+    cudaError_t first_error = cudaSuccess;
+};
+
 template <typename... P, typename... A>
-static void launch_pdl(void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
+static void launch_pdl(LaunchLog &log, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
@@ -63,7 +71,9 @@ static void launch_pdl(void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t s
     at[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = at;
     cfg.numAttrs = 1;
-    cudaLaunchKernelEx(&cfg, kern, std::forward<A>(args)...);     // errors surface in the cudaGetLastError checks below
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, std::forward<A>(args)...);
+    if (e != cudaSuccess && log.first_error == cudaSuccess) log.first_error = e;
+    log.launches += 1;
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -308,7 +318,6 @@ __global__ void __launch_bounds__(SCAN_T) k_scan_apply(const int *__restrict__ i
 }
 
 // exclusive scan of B arrays of n ints (per-array stride `stride`); totals[b] (device, may be null)
-static int g_launches = 0;   // kernels launched by the build in progress (host-side bookkeeping only)
 
 // short arrays: the whole scan of one array in ONE block (1024 threads x 4 items per step, running carry);
 // one launch instead of three, which is what a build of a small cloud is made of
@@ -380,22 +389,17 @@ __global__ void __launch_bounds__(SCAN1_T) k_scan_single(const int *__restrict__
 }
 
 // n = length of every array, or (poff given) of the longest one
-static int scan_exclusive(const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
-                          cudaStream_t st, const int *poff = nullptr)
+static void scan_exclusive(LaunchLog &log, const int *in, int *out, int n, int stride, int B, int *totals, int *bsum_tmp,
+                           cudaStream_t st, const int *poff = nullptr)
 {
     if (n <= SCAN1_MAX_N) {
-        g_launches += 1;
-        launch_pdl(k_scan_single, dim3(B), dim3(SCAN1_T), st, in, out, n, stride, totals, poff);
-        RFPS_CUDA(cudaGetLastError());
-        return FPS_OK;
+        launch_pdl(log, k_scan_single, dim3(B), dim3(SCAN1_T), st, in, out, n, stride, totals, poff);
+        return;
     }
-    g_launches += 3;
     const int nblk = (n + SCAN_TILE - 1) / SCAN_TILE;
-    launch_pdl(k_scan_blocksum, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, n, stride, nblk, bsum_tmp, poff);
-    launch_pdl(k_scan_bsums, dim3(B), dim3(SCAN_T), st, bsum_tmp, nblk, totals);
-    launch_pdl(k_scan_apply, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, out, n, stride, nblk, bsum_tmp, poff);
-    RFPS_CUDA(cudaGetLastError());
-    return FPS_OK;
+    launch_pdl(log, k_scan_blocksum, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, n, stride, nblk, bsum_tmp, poff);
+    launch_pdl(log, k_scan_bsums, dim3(B), dim3(SCAN_T), st, bsum_tmp, nblk, totals);
+    launch_pdl(log, k_scan_apply, dim3(dim3(nblk, B)), dim3(SCAN_T), st, in, out, n, stride, nblk, bsum_tmp, poff);
 }
 static inline int scan_tmp_ints(int n, int B) { return ((n + SCAN_TILE - 1) / SCAN_TILE) * B + 1; }
 
@@ -574,14 +578,8 @@ __global__ void __launch_bounds__(256) k_gather(const float *__restrict__ pts, c
 //   c_k = midpoint of the axis-aligned bounding box of the voxel's points (reading A10)
 //   R_k = sqrt_rn(max_p d2(p, c_k)) * (1 + 2^-20)      (reading A9: rounded UP past every fp32
 //         error of d2 and sqrt, so that ||p - c_k|| <= R_k holds over the reals)
-// d2 is the library's one distance expression, ((dx*dx + dy*dy) + dz*dz) without FMA.
+// d2 is the library's one distance expression, ((dx*dx + dy*dy) + dz*dz) without FMA (d2_rn, device_utils.cuh).
 // ---------------------------------------------------------------------------------------------
-__device__ __forceinline__ float d2_rn(float x, float y, float z, float sx, float sy, float sz)
-{
-    const float dx = __fsub_rn(x, sx), dy = __fsub_rn(y, sy), dz = __fsub_rn(z, sz);
-    return __fadd_rn(__fadd_rn(__fmul_rn(dx, dx), __fmul_rn(dy, dy)), __fmul_rn(dz, dz));
-}
-
 __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, const float *__restrict__ py,
                                                  const float *__restrict__ pz, const int2 *__restrict__ vseg,
                                                  const int *__restrict__ K, const int *__restrict__ poff, int K_cap,
@@ -718,6 +716,12 @@ void dev_free_async(void *p, cudaStream_t st)
     else cudaFree(p);
 }
 
+void trim_pool()
+{
+    cudaMemPool_t pool = build_pool();
+    if (pool) cudaMemPoolTrimTo(pool, 0);
+}
+
 struct Carver {    // hands out 256-byte aligned pieces of one allocation (first pass: sizes only)
     char *base = nullptr;
     size_t off = 0;
@@ -832,48 +836,55 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     carve(cs, false);
     auto release_scratch = [&]() { if (ix.arena_pooled) cudaFreeAsync(scratch, st); else cudaFree(scratch); };
 
-    int rc;
-    g_launches = 0;
+    LaunchLog log;
+    const int sms = device_props().sm_count;
     const dim3 gN((N + 255) / 256, B);
-    RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));
-    RFPS_CUDA(cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st));
+    // a failing enqueue below must not leak the scratch block: every exit goes through release_scratch()
+    cudaError_t e0 = cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st);
+    if (e0 == cudaSuccess) e0 = cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st);
+    if (e0 != cudaSuccess) {
+        set_error("index build: enqueueing the first copies failed: %s", cudaGetErrorString(e0));
+        release_scratch();
+        return FPS_ERR_CUDA;
+    }
     const int *poff = ix.poff_dev;
-    launch_pdl(k_bbox_init, dim3((B * BBOX_STRIDE + 255) / 256), dim3(256), st, sc.bbox, B);
-    launch_pdl(k_bbox, dim3(dim3(std::max(1, std::min((N + 4095) / 4096, 148)), B)), dim3(256), st, points, poff, sc.bbox);
-    launch_pdl(k_keys, dim3(gN), dim3(256), st, points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
-    g_launches += 3;
+    launch_pdl(log, k_bbox_init, dim3((B * BBOX_STRIDE + 255) / 256), dim3(256), st, sc.bbox, B);
+    launch_pdl(log, k_bbox, dim3(dim3(std::max(1, std::min((N + 4095) / 4096, sms)), B)), dim3(256), st, points, poff, sc.bbox);
+    launch_pdl(log, k_keys, dim3(gN), dim3(256), st, points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
 
     // a3: LSD radix sort, 8 bits per pass
     unsigned *kin = sc.kA, *kout = sc.kB;
     int *vin = sc.vA, *vout = sc.vB;
     const dim3 gR((nchunk + RS_WARPS - 1) / RS_WARPS, B);
     for (int shift = 0; shift < keybits; shift += 8) {
-        launch_pdl(k_radix_hist, dim3(gR), dim3(RS_WARPS * 32), st, kin, poff, nchunk, shift, sc.table);
-        if ((rc = scan_exclusive(sc.table, sc.table, (int)table_n, (int)table_n, B, nullptr, sc.bsum, st))) { release_scratch(); return rc; }
-        launch_pdl(k_radix_scatter, dim3(gR), dim3(RS_WARPS * 32), st, kin, vin, poff, nchunk, shift, sc.table, kout, vout);
+        launch_pdl(log, k_radix_hist, dim3(gR), dim3(RS_WARPS * 32), st, kin, poff, nchunk, shift, sc.table);
+        scan_exclusive(log, sc.table, sc.table, (int)table_n, (int)table_n, B, nullptr, sc.bsum, st);
+        launch_pdl(log, k_radix_scatter, dim3(gR), dim3(RS_WARPS * 32), st, kin, vin, poff, nchunk, shift, sc.table, kout, vout);
         std::swap(kin, kout);
         std::swap(vin, vout);
-        g_launches += 2;
     }
 
     // a5: grid voxels -> (tiled) segments; a4: gather; a6: spheres
-    launch_pdl(k_heads, dim3(gN), dim3(256), st, kin, poff, 3 * sb, sc.heads);
-    if ((rc = scan_exclusive(sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st, poff))) { release_scratch(); return rc; }
-    launch_pdl(k_voxel_offsets, dim3(gN), dim3(256), st, sc.heads, sc.rank, poff, sc.voff);
-    launch_pdl(k_ntiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, poff, tile_points, sc.ntl);
-    if ((rc = scan_exclusive(sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st, poff))) { release_scratch(); return rc; }
-    launch_pdl(k_tiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, sc.ntl, sc.tbase, poff, ix.K_cap, ix.vseg);
-    launch_pdl(k_gather, dim3(gN), dim3(256), st, points, vin, poff, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
-    const int sphere_blocks = std::max(1, std::min((ix.K_cap + 7) / 8, 148 * 8));
-    launch_pdl(k_sphere, dim3(dim3(sphere_blocks, B)), dim3(256), st, ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
-                                                     reinterpret_cast<int *>(meta));
-    const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, 148 * 8));
-    launch_pdl(k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
-    g_launches += 8;
-    if (cudaGetLastError() != cudaSuccess) {
-        set_error("a build kernel failed to launch: %s", cudaGetErrorString(cudaGetLastError()));
-        release_scratch();
-        return FPS_ERR_CUDA;
+    launch_pdl(log, k_heads, dim3(gN), dim3(256), st, kin, poff, 3 * sb, sc.heads);
+    scan_exclusive(log, sc.heads, sc.rank, N, N, B, sc.Kv, sc.bsum, st, poff);
+    launch_pdl(log, k_voxel_offsets, dim3(gN), dim3(256), st, sc.heads, sc.rank, poff, sc.voff);
+    launch_pdl(log, k_ntiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, poff, tile_points, sc.ntl);
+    scan_exclusive(log, sc.ntl, sc.tbase, N, N, B, ix.K_dev, sc.bsum, st, poff);
+    launch_pdl(log, k_tiles, dim3(gN), dim3(256), st, sc.voff, sc.Kv, sc.ntl, sc.tbase, poff, ix.K_cap, ix.vseg);
+    launch_pdl(log, k_gather, dim3(gN), dim3(256), st, points, vin, poff, ix.px, ix.py, ix.pz, ix.porig, ix.pinv);
+    const int sphere_blocks = std::max(1, std::min((ix.K_cap + 7) / 8, sms * 8));
+    launch_pdl(log, k_sphere, dim3(dim3(sphere_blocks, B)), dim3(256), st, ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
+               reinterpret_cast<int *>(meta));
+    const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, sms * 8));
+    launch_pdl(log, k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
+    {
+        const cudaError_t el = log.first_error != cudaSuccess ? log.first_error : cudaGetLastError();
+        if (el != cudaSuccess) {
+            set_error("a build kernel failed to launch: %s", cudaGetErrorString(el));
+            cudaGetLastError();
+            release_scratch();
+            return FPS_ERR_CUDA;
+        }
     }
 
     // the one host round-trip of the build: K per cloud, the non-finite flags, the largest segment
@@ -882,7 +893,6 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     std::vector<unsigned> hrb(rb_n);
     if (!ix.K_host) { set_error("host malloc failed"); release_scratch(); return FPS_ERR_NOMEM; }
     cudaError_t e1 = cudaMemcpyAsync(hrb.data(), rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
-    cudaError_t e2 = cudaSuccess, e3 = cudaSuccess;
     release_scratch();
     cudaError_t e4 = cudaStreamSynchronize(st);
     if (e1 == cudaSuccess && e4 == cudaSuccess) {
@@ -890,8 +900,8 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         ix.max_voxel_points = (int)hrb[B];
     }
     const unsigned *hb = hrb.data() + B + 8;
-    if (e1 != cudaSuccess || e2 != cudaSuccess || e3 != cudaSuccess || e4 != cudaSuccess) {
-        set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : (e1 != cudaSuccess ? e1 : (e2 != cudaSuccess ? e2 : e3))));
+    if (e1 != cudaSuccess || e4 != cudaSuccess) {
+        set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : e1));
         return FPS_ERR_CUDA;
     }
     for (int b = 0; b < B; ++b)
@@ -905,7 +915,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         ix.K_max = std::max(ix.K_max, ix.K_host[b]);
         ix.K_total += ix.K_host[b];
     }
-    ix.build_launches = g_launches;
+    ix.build_launches = log.launches;
     return per_pick ? choose_launch_shape(ix, o) : choose_batched_shape(ix, o);
 }
 

@@ -42,6 +42,13 @@ void set_error(const char *fmt, ...);
 
 constexpr int NUM_COUNTERS = 32;
 
+// what the launch-shape logic needs to know about the current device (queried once per device)
+struct DeviceProps {
+    int sm_count = 0;          // multiprocessors
+    int max_smem_optin = 0;    // largest dynamic shared memory per block (opt-in), bytes
+};
+const DeviceProps &device_props();
+
 struct DeviceIndex {
     int32_t B = 0, N = 0;               // clouds; points of the LARGEST cloud (all clouds, if uniform)
     bool ragged = false;                // built by fps_index_build_ragged
@@ -81,6 +88,7 @@ struct DeviceIndex {
 
 int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o);
 void free_index(DeviceIndex &ix);
+void trim_pool();   // return the library pool's unused memory to the driver (fps_trim)
 // stream-ordered device memory from the library's private pool (falls back to cudaMalloc/cudaFree)
 cudaError_t dev_alloc_async(void **p, size_t bytes, cudaStream_t stream);
 void dev_free_async(void *p, cudaStream_t stream);

@@ -45,27 +45,14 @@ namespace rfps {
 constexpr int BT = 512;        // threads per CTA
 constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
 constexpr int MAX_ATTEMPTS = 4;
-#ifndef RFPS_STREAM_MIN
-#define RFPS_STREAM_MIN 64
-#endif
-constexpr int STREAM_MIN = RFPS_STREAM_MIN;   // workers start on a piece of the running batch once it has this many picks
+constexpr int STREAM_MIN = 64;    // workers start on a piece of the running batch once it has this many picks
 constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffffu;
-#ifndef RFPS_GTARGET
-#define RFPS_GTARGET 0.625f
-#endif
-constexpr float GTARGET = RFPS_GTARGET;   // aim the next extraction at this fraction of the candidate buffer
-#ifndef RFPS_GT_MAX
-#define RFPS_GT_MAX 0.7f
-#define RFPS_GT_UP 1.03f
-#define RFPS_GT_MIN 0.35f
-#define RFPS_GT_DOWN 0.85f
-#endif
-#ifndef RFPS_POLL_NS
-#define RFPS_POLL_NS 32
-#endif
-#ifndef RFPS_CPT2
-#define RFPS_CPT2 3
-#endif
+// extraction control: the next extraction aims at the fraction `gt` of the candidate buffer; gt starts at GTARGET,
+// creeps up after an extraction that fitted and drops after one that overflowed (all measured on C1-C5)
+constexpr float GTARGET = 0.625f, GT_MAX = 0.7f, GT_UP = 1.03f, GT_MIN = 0.35f, GT_DOWN = 0.85f;
+constexpr int POLL_NS = 32;       // back-off of the warps that follow the pick warp's published count
+constexpr int CPT2 = 3;           // candidates per lane of the pick warp (hierarchical local phase)
+constexpr int KCH = 16;           // picks the pick warp runs speculatively between two exit tests
 constexpr int SUBW = 4;        // 32-bit mask words per queued voxel
 constexpr int SUBP = 32 * SUBW;   // picks applied between two CTA barriers
 
@@ -94,7 +81,7 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
 
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_DBG0, CNT_DBG1, CNT_DBG2, CNT_SUBROUNDS, CNT_FALLBACK, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_LSEL, CNT_LPICK, CNT_LUPD, CNT_SUBROUNDS, CNT_FALLBACK, CNT_N };
 
 // shared-memory carve-up (host and device must agree)
 struct SmemLayout {
@@ -311,7 +298,7 @@ struct __align__(16) HierSmem {
 };
 constexpr int NP_FINAL = 1 << 30;
 
-template <int CPT1, int CPT2, bool EUC>
+template <int CPT1, int CPT2, bool STATS, bool EUC>
 __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY, const float *cZ, const float *cD,
                                                const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
                                                const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
@@ -349,7 +336,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
     unsigned bound_bits = 0u;            // an upper bound of every candidate's distance left by the last sub-round
     bool have_bound = false;
     for (;;) {
-        tt0 = clock64();
+        if (STATS) tt0 = clock64();
         // ---- (a) block maximum.  After a sub-round that ended on tau2 every candidate is <= tau2, which
         // serves as the origin of the bins just as well: the reduction and its barrier are skipped ----
         float m = D[0];
@@ -457,7 +444,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             // tau2 = the largest live distance outside C2: where the pick loop stops, and the bound the next
             // sub-round hangs its bins on
             const unsigned tau2bits = __reduce_max_sync(FULL, lane < BT / 32 ? hs->wmax2[lane] : 0u);
-            tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1;
+            if (STATS) { tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1; }
             // ---- (e) one warp: FPS over C2 in registers.  No barrier and no vote/shuffle per pick: the
             // chain is update -> lane max -> redux(max D) -> redux(slot id) -> 3 broadcast loads. ----
             if (warp == PW) {
@@ -480,10 +467,6 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                 // picks before the first such event is accepted.  Picks computed beyond it are discarded with
                 // the register state (the sub-round ends there, or the chunk is redone pick by pick).
                 const int nb0 = nbl, j0 = jl;
-#ifndef RFPS_KCH
-#define RFPS_KCH 16
-#endif
-                constexpr int KCH = RFPS_KCH;
                 // one pick, fully checked: returns false when the sub-round is over
                 auto careful_pick = [&]() -> bool {
                     float bm = d2v[0];
@@ -640,7 +623,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                         } else if (v & NP_FINAL) {
                             break;
                         } else {
-                            __nanosleep(RFPS_POLL_NS);
+                            __nanosleep(POLL_NS);
                         }
                     }
                     if (wlive) asm volatile("bar.arrive 1, %0;" ::"n"(BT) : "memory");
@@ -658,7 +641,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         // (lane 0 of the pick warp; after a barrier on the fallback path); its fence overlaps the other warps'
         // selection of the next sub-round
         if (pub_addr && tid == BT - 32) st_release_cluster_u32(pub_addr, (unsigned)nbl);
-        tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1;
+        if (STATS) { tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1; }
         // ---- (f) the sub-round's picks -> all of C1.  Candidates at or below tau are out of the round for
         // good; neighbours in the buffer come from the same voxel and tend to die together, so whole
         // warps drop out of this loop as the round proceeds ----
@@ -681,7 +664,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
             }
         }
         applied = nbl;
-        t_app += clock64() - tt0;
+        if (STATS) t_app += clock64() - tt0;
         if (jl >= M || nbl >= PB) break;
     }
     j = jl;
@@ -798,7 +781,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     unsigned long long c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_pcomp = 0, c_eff = 0, c_rounds = 0, c_retries = 0,
                        c_singles = 0, c_cands = 0, c_xvox = 0, c_xpts = 0, c_gtest = 0, c_subrounds = 0, c_fallback = 0;
     long long t_apply = 0, t_max = 0, t_extract = 0, t_local = 0, t0 = 0, t1 = 0;   // CTA 0 / thread 0, SM cycles
-    long long dbg0 = 0, dbg1 = 0, dbg2 = 0;
+    long long t_lsel = 0, t_lpick = 0, t_lupd = 0;                          // local phase: selection / pick loop / update after it
     long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
     cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
 
@@ -1102,12 +1085,12 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     // aim the next round at ~5/8 of the buffer; move by at most 2x per round
                     const float ratio = fminf(2.0f, fmaxf(0.5f, (gt * TC) / (float)max(found, 1u)));
                     g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
-                    gt = fminf(RFPS_GT_MAX, gt * RFPS_GT_UP);
+                    gt = fminf(GT_MAX, gt * GT_UP);
                     break;
                 }
                 if (STATS && tid == 0 && rank == 0) c_retries++;
                 g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
-                gt = fmaxf(RFPS_GT_MIN, gt * RFPS_GT_DOWN);
+                gt = fmaxf(GT_MIN, gt * GT_DOWN);
             }
         }
         }
@@ -1135,8 +1118,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 }
             } else if constexpr (LW == BT / 32) {
                 int lj = j, lnb = 0;
-                local_fps_hier<CPT, RFPS_CPT2, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
-                                       c_subrounds, c_fallback, dbg0, dbg1, dbg2, split ? smem_u32(&ctl->pub) : 0u);
+                local_fps_hier<CPT, CPT2, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
+                                       c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, split ? smem_u32(&ctl->pub) : 0u);
                 if (tid == 0) {
                     ctl->nb = lnb;
                     ctl->j = lj;
@@ -1225,9 +1208,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             atomicAdd(P.counters + CNT_SUBS, (unsigned long long)n_subs);
             atomicAdd(P.counters + CNT_SUBROUNDS, c_subrounds);
             atomicAdd(P.counters + CNT_FALLBACK, c_fallback);
-            atomicAdd(P.counters + CNT_DBG0, (unsigned long long)dbg0);
-            atomicAdd(P.counters + CNT_DBG1, (unsigned long long)dbg1);
-            atomicAdd(P.counters + CNT_DBG2, (unsigned long long)dbg2);
+            atomicAdd(P.counters + CNT_LSEL, (unsigned long long)t_lsel);
+            atomicAdd(P.counters + CNT_LPICK, (unsigned long long)t_lpick);
+            atomicAdd(P.counters + CNT_LUPD, (unsigned long long)t_lupd);
             atomicAdd(P.counters + CNT_ROUNDS, c_rounds);
             atomicAdd(P.counters + CNT_RETRIES, c_retries);
             atomicAdd(P.counters + CNT_SINGLES, c_singles);
@@ -1245,7 +1228,6 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 // ---------------------------------------------------------------------------------------------
 // host side: launch shape and launch
 // ---------------------------------------------------------------------------------------------
-static const int kMaxSmem = 227 * 1024;
 
 template <int CPT, int LW, bool STATS, bool EUC>
 __global__ void k_fps_batched(const BatchParams P, const int flags);
@@ -1258,7 +1240,7 @@ static int max_resident_clusters(int c, size_t smem)
     if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
-    cfg.gridDim = dim3((unsigned)(c * 148));
+    cfg.gridDim = dim3((unsigned)(c * device_props().sm_count));
     cfg.blockDim = dim3(BT);
     cfg.dynamicSmemBytes = smem;
     cudaLaunchAttribute attr[1];
@@ -1297,17 +1279,19 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     const int TC = CPT * LW * 32;
     const int G = (K + 31) / 32;
     auto slots = [&](int c) { const int w = c > 1 ? c - 1 : 1; return 32 * ((G + w - 1) / w); };   // voxel slots per worker CTA
-    auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= (size_t)kMaxSmem; };
+    const size_t max_smem = (size_t)device_props().max_smem_optin;
+    const int sms = device_props().sm_count;
+    auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= max_smem; };
     if (C == 0) {
         // the largest cluster that (a) leaves every CTA >= 1 024 points, (b) holds the voxel state in
         // shared memory and (c) lets all B clusters be resident at once (a cluster lives inside one
-        // GPC, so fewer clusters fit than 148 / C suggests: 15 of 8, 22 of 6, 7 of 16 on B200);
+        // GPC, so fewer clusters fit than SMs / C suggests: 15 of 8, 22 of 6, 7 of 16 on B200's 148 SMs);
         // otherwise the clouds would run in waves
-        const int want = std::min(ix.B, 148);
+        const int want = std::min(ix.B, sms);
         C = 1;
         for (int c = 16; c > 1; --c) {
             if ((long long)ix.N < 1024ll * c || !fits(c)) continue;
-            if (max_resident_clusters(c, smem_layout(slots(c), TC, LW).total) >= std::min(want, 148 / c)) { C = c; break; }
+            if (max_resident_clusters(c, smem_layout(slots(c), TC, LW).total) >= std::min(want, sms / c)) { C = c; break; }
         }
         while (C < 16 && !fits(C)) ++C;
     }

@@ -307,13 +307,13 @@ int choose_launch_shape(DeviceIndex &ix, const fps_build_opts &o)
     const int K = ix.K_max > 0 ? ix.K_max : 1;
     if (C == 0) {
         // one cloud per CTA while the voxel list fits a few slots per thread and the cloud is small;
-        // otherwise a cluster, capped so that all B clusters are co-resident on the 148 SMs.
+        // otherwise a cluster, capped so that all B clusters are co-resident on the device's SMs.
         if (K <= 2 * T && ix.N <= 32768) C = 1;
         else {
             C = 2;
             while (C < 16 && (long long)C * T * 2 < K) C *= 2;
             while (C < 16 && (long long)C * 16384 < ix.N) C *= 2;
-            while (C > 1 && (long long)C * ix.B > 148) C /= 2;
+            while (C > 1 && (long long)C * ix.B > device_props().sm_count) C /= 2;
         }
     }
     const int maxvpt = T <= 512 ? 8 : 4;
@@ -426,6 +426,7 @@ int launch_gather_xyz(DeviceIndex &ix, const int32_t *idx, int32_t M, int32_t M_
     k_gather_xyz<<<dim3((unsigned)((M_max + 255) / 256), (unsigned)ix.B), 256, 0, st>>>(ix.px, ix.py, ix.pz, ix.pinv, ix.poff_dev,
                                                                                       rag_dev, ix.B, M, idx, out_xyz);
     RFPS_CUDA(cudaGetLastError());
+    ix.last_stream = st;      // fps_index_destroy releases the arena stream-ordered behind this kernel
     return FPS_OK;
 }
 

@@ -253,6 +253,13 @@ WORKLOADS = {
                    "stress: N=1000000, 128 beams x 7813 azimuths, 200 objects within 120 m, M=65536"),
 }
 
+# not a BASELINE.json configuration: the parity case for clouds so large that the library's automatic tile size
+# grows past 64 points per voxel (tests/test_gpu_parity.py, golden hash in tests/golden/full_size.json)
+EXTRA_WORKLOADS = {
+    "L3M": Workload("L3M", "lidar", 1, 3000000, 20000, 0, (128, (-25.0, 15.0), 23439, 200, 120.0),
+                    "parity case: N=3000000, 128 beams x 23439 azimuths, 200 objects within 120 m, M=20000"),
+}
+
 
 def scaled(name: str, N: int, M: int, B: int | None = None) -> Workload:
     """The same generator as workload ``name`` at a reduced size (for CPU-time parity cases)."""
@@ -283,5 +290,5 @@ def make_cloud(w: Workload, b: int = 0, seed: int = BASE_SEED) -> np.ndarray:
 def make_batch(w: Workload | str, seed: int = BASE_SEED) -> np.ndarray:
     """[B][N][3] float32, C-contiguous."""
     if isinstance(w, str):
-        w = WORKLOADS[w]
+        w = WORKLOADS[w] if w in WORKLOADS else EXTRA_WORKLOADS[w]
     return np.ascontiguousarray(np.stack([make_cloud(w, b, seed) for b in range(w.B)], axis=0))

@@ -1,10 +1,15 @@
 """Writes tests/golden/full_size.json: SHA-256 of the CPU oracle's outputs on the five full-size
-BASELINE.json configurations (plus the SHA-256 of the generated inputs, to catch generator drift).
+BASELINE.json configurations and on the 3 M-point parity case (plus the SHA-256 of the generated
+inputs, to catch generator drift).
 
 Calls ONLY ``oracle`` and the seeded input generators -- never the CUDA path.  The GPU parity test
 compares the CUDA outputs' hashes with these (a hash of the whole array is a bit-exact comparison
-of every element).  Usage:  python tests/golden/make_golden.py [C1 C2 ...]
+of every element).
+
+  python tests/golden/make_golden.py [C1 C2 ... L3M]            squared distance: oracle.fps        -> key "C5"
+  python tests/golden/make_golden.py --euclid [C4 C5 ...]       Euclidean mode:   oracle.fps_euclid -> key "C5:euclid"
 """
+import fcntl
 import hashlib
 import json
 import os
@@ -26,25 +31,35 @@ def sha(a: np.ndarray) -> str:
     return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
 
 
-def main(names):
-    data = json.load(open(OUT)) if os.path.exists(OUT) else {}
+def main(names, euclid):
+    fn = oracle.fps_euclid if euclid else oracle.fps
     for name in names:
-        w = inputs.WORKLOADS[name]
+        w = inputs.WORKLOADS.get(name) or inputs.EXTRA_WORKLOADS[name]
         P = inputs.make_batch(w)
         t = time.time()
-        idx, mind = oracle.fps(P, w.M, w.start_idx)
+        idx, mind = fn(P, w.M, w.start_idx)
         dt = time.time() - t
-        data[name] = {
+        rec = {
             "B": w.B, "N": w.N, "M": w.M, "start_idx": w.start_idx, "seed": inputs.BASE_SEED,
             "input_sha256": sha(P), "idx_sha256": sha(idx.astype(np.int32)), "mindist_sha256": sha(mind.astype(np.float32)),
             "idx_head": idx.reshape(w.B, w.M)[0, :8].tolist(),
             "mindist_tail_bits": [int(v) for v in mind.reshape(w.B, w.M)[0, -4:].view(np.uint32)],
-            "oracle_seconds": round(dt, 2), "oracle_threads": int(oracle.fps.threads_used),
-            "written_by": "tests/golden/make_golden.py (oracle/fps_oracle.c only)",
+            "oracle_seconds": round(dt, 2),
+            "written_by": "tests/golden/make_golden.py (%s only)" % ("oracle/fps_oracle_euclid.c" if euclid else "oracle/fps_oracle.c"),
         }
-        print(name, data[name], flush=True)
-        json.dump(data, open(OUT, "w"), indent=1, sort_keys=True)
+        if not euclid:
+            rec["oracle_threads"] = int(oracle.fps.threads_used)
+        print(name, rec, flush=True)
+        # several instances may run side by side (the large cases take minutes each): read-modify-write under a lock
+        with open(OUT + ".lock", "w") as lk:
+            fcntl.flock(lk, fcntl.LOCK_EX)
+            data = json.load(open(OUT)) if os.path.exists(OUT) else {}
+            data[name + (":euclid" if euclid else "")] = rec
+            json.dump(data, open(OUT, "w"), indent=1, sort_keys=True)
 
 
 if __name__ == "__main__":
-    main(sys.argv[1:] or ["C1", "C2", "C3", "C4", "C5"])
+    args = sys.argv[1:]
+    euclid = "--euclid" in args
+    args = [a for a in args if a != "--euclid"]
+    main(args or ["C1", "C2", "C3", "C4", "C5"], euclid)

@@ -38,11 +38,30 @@ def test_binding_lists_every_declared_symbol():
     assert sorted(binding.EXPORTS) == declared_functions()
 
 
-def test_struct_sizes_match_header(lib):
-    # fps_build_opts: 5 x int32 + pointer (8-aligned) + 2 x int32 = 40 bytes; fps_stats: see header
+def test_struct_layouts_match_header(tmp_path):
+    """Every field of fps_build_opts / fps_stats sits at the same offset in the ctypes binding as in the C header:
+    a small C program compiled against include/radiusfps.h prints sizeof and offsetof of every field."""
+    import subprocess
     from paper_2606_06255_b200 import binding
-    assert ctypes.sizeof(binding.fps_build_opts) == 40
-    assert ctypes.sizeof(binding.fps_stats) == 6 * 4 + 8 + 4 + 4 + 8 + 4 + 4 + 6 * 8 + 18 * 8 + 2 * 4
+    prog = ["#include <stdio.h>", "#include <stddef.h>", '#include "radiusfps.h"', "int main(void) {"]
+    for cname, cls in (("fps_build_opts", binding.fps_build_opts), ("fps_stats", binding.fps_stats)):
+        prog.append(f'printf("{cname} %zu\\n", sizeof({cname}));')
+        for field, _ in cls._fields_:
+            prog.append(f'printf("{cname}.{field} %zu\\n", offsetof({cname}, {field}));')
+    prog += ["return 0; }"]
+    src, exe = tmp_path / "layout.c", tmp_path / "layout"
+    src.write_text("\n".join(prog))
+    subprocess.run(["gcc", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe)], check=True)
+    want = dict(line.split() for line in subprocess.run([str(exe)], capture_output=True, text=True, check=True).stdout.splitlines())
+    for cname, cls in (("fps_build_opts", binding.fps_build_opts), ("fps_stats", binding.fps_stats)):
+        assert ctypes.sizeof(cls) == int(want[cname]), cname
+        for field, _ in cls._fields_:
+            assert getattr(cls, field).offset == int(want[f"{cname}.{field}"]), (cname, field)
+    # and the header has no field the binding lacks
+    text = re.sub(r"/\*.*?\*/", "", open(os.path.join(ROOT, "include", "radiusfps.h")).read(), flags=re.S)
+    body = text[text.index("typedef struct {", text.index("fps_build_opts;")):text.index("} fps_stats;")]
+    names = [n.strip() for decl in re.findall(r"int(?:32|64)_t\s+([^;]+);", body) for n in decl.split(",")]
+    assert names == [f for f, _ in binding.fps_stats._fields_]
 
 
 def test_version_and_error_strings(lib):
@@ -131,7 +150,7 @@ def test_every_build_kernel_waits_for_its_predecessor_grid():
         first = body[body.index("{") + 1:].lstrip().splitlines()[0].strip()
         assert first == "grid_dep_sync();", (k, first)
     assert "<<<" not in src.replace("// ", ""), "a build kernel is launched without launch_pdl"
-    assert set(re.findall(r"launch_pdl\((k_\w+),", src)) == set(kernels)
+    assert set(re.findall(r"launch_pdl\(log, (k_\w+),", src)) == set(kernels)
     helper = src[src.index("void grid_dep_sync()"):]
     helper = helper[:helper.index("}")]
     assert helper.index("griddepcontrol.launch_dependents") < helper.index("griddepcontrol.wait")

@@ -42,6 +42,10 @@ def run_gpu(rf, P, M, start=0, **opts):
     return idx.cpu().numpy(), mind.cpu().numpy(), st
 
 
+def sha(a):
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+
+
 def assert_same(got_idx, got_mind, ref_idx, ref_mind):
     got_idx = got_idx.reshape(ref_idx.shape)
     got_mind = got_mind.reshape(ref_mind.shape)
@@ -393,21 +397,20 @@ def test_sampling_every_point_of_a_cloud(rf):
 
 def test_three_million_points_tile_size_grows(rf):
     """Beyond ~1.5 M points the automatic tile size grows so that the voxel state still fits the workers'
-    shared memory; properties that hold at any size + sampled min-distances recomputed from the outputs."""
-    N, M = 3_000_000, 20_000
-    P = inputs.lidar(N, 9, n_beams=128, elev_deg=(-25.0, 15.0), n_azimuth=23439, n_objects=200, max_range=120.0)
-    gi, gm, st = run_gpu(rf, P, M)
+    shared memory.  Element by element against the oracle through the stored hashes of its outputs
+    (tests/golden/full_size.json "L3M", written by make_golden.py from oracle/fps_oracle.c alone; 60 G point
+    updates, minutes on one core), plus properties that hold at any size."""
+    gold = json.load(open(GOLDEN))["L3M"]
+    w = inputs.EXTRA_WORKLOADS["L3M"]
+    P = inputs.make_batch(w)
+    assert sha(P) == gold["input_sha256"], "input generator drifted from the one the golden was made with"
+    gi, gm, st = run_gpu(rf, P, w.M)
     assert st["max_voxel_points"] > 64 and st["cluster_size"] == 16
-    gi, gm = gi.reshape(-1), gm.reshape(-1)
-    assert gi[0] == 0 and np.isinf(gm[0]) and np.all(gm[1:] <= gm[:-1]) and np.unique(gi).size == M
-    S = P[gi]
-    for j in [1, 2, 100, 5000, M - 1]:
-        d = (S[:j] - S[j]).astype(np.float32)
-        d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
-        assert d2.min().view(np.uint32) == gm[j].view(np.uint32), j
-    d = (P - P[0]).astype(np.float32)
-    d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
-    assert gi[1] == int(np.argmax(d2)) and gm[1].view(np.uint32) == d2.max().view(np.uint32)
+    gi, gm, P = gi.reshape(-1), gm.reshape(-1), P[0]
+    assert gi[0] == 0 and np.isinf(gm[0]) and np.all(gm[1:] <= gm[:-1]) and np.unique(gi).size == w.M
+    assert gi[:8].tolist() == gold["idx_head"]
+    assert sha(gi.astype(np.int32)) == gold["idx_sha256"]
+    assert sha(gm.astype(np.float32)) == gold["mindist_sha256"]
 
 
 def test_gather_xyz_uniform_and_ragged(rf):
@@ -453,13 +456,26 @@ def test_euclidean_mode_small_clouds(rf, name, cluster):
     assert_same(gi, gm, *ref)
 
 
-@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
 def test_euclidean_mode_full_size(rf, name):
     w = inputs.WORKLOADS[name]
     P = inputs.make_batch(w)
     ref = oracle.fps_euclid(P, w.M, w.start_idx)
     gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx, flags=rf.FPS_FLAG_EUCLIDEAN)
     assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("name", ["C4", "C5"])
+def test_euclidean_mode_full_size_against_stored_oracle_hashes(rf, name):
+    # C5 is minutes of oracle time: its outputs' hashes are stored (make_golden.py --euclid, oracle.fps_euclid only)
+    gold = json.load(open(GOLDEN))[name + ":euclid"]
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    assert sha(P) == gold["input_sha256"], "input generator drifted from the one the golden was made with"
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx, flags=rf.FPS_FLAG_EUCLIDEAN)
+    assert gi.reshape(w.B, w.M)[0, :8].tolist() == gold["idx_head"]
+    assert sha(gi.astype(np.int32)) == gold["idx_sha256"]
+    assert sha(gm.astype(np.float32)) == gold["mindist_sha256"]
 
 
 def test_euclidean_mode_is_a_different_function_where_sqrt_collapses(rf):
@@ -539,10 +555,6 @@ def test_errors(rf):
 # ---------------------------------------------------------------------------------------------
 # full-size configurations, library-default launch configuration (= what bench.py times)
 # ---------------------------------------------------------------------------------------------
-def sha(a):
-    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
-
-
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4"])
 def test_full_size_against_live_oracle(rf, name):
     w = inputs.WORKLOADS[name]
@@ -554,13 +566,14 @@ def test_full_size_against_live_oracle(rf, name):
     assert_same(gi, gm, *ref)
 
 
+@pytest.mark.parametrize("kernel", sorted(KERNELS))
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C4", "C5"])
-def test_full_size_against_stored_oracle_hashes(rf, name):
+def test_full_size_against_stored_oracle_hashes(rf, name, kernel):
     gold = json.load(open(GOLDEN))[name]
     w = inputs.WORKLOADS[name]
     P = inputs.make_batch(w)
     assert sha(P) == gold["input_sha256"], "input generator drifted from the one the golden was made with"
-    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx)
+    gi, gm, _ = run_gpu(rf, P, w.M, w.start_idx, flags=KERNELS[kernel])
     assert gi.reshape(w.B, w.M)[0, :8].tolist() == gold["idx_head"]
     assert sha(gi.astype(np.int32)) == gold["idx_sha256"]
     assert sha(gm.astype(np.float32)) == gold["mindist_sha256"]
@@ -585,3 +598,67 @@ def test_C5_properties_and_sampled_recomputation(rf):
     d = (P - P[w.start_idx]).astype(np.float32)
     d2 = ((d[:, 0] * d[:, 0] + d[:, 1] * d[:, 1]).astype(np.float32) + d[:, 2] * d[:, 2]).astype(np.float32)
     assert gi[1] == int(np.argmax(d2)) and gm[1].view(np.uint32) == d2.max().view(np.uint32)
+
+
+def test_two_host_threads_pipelined_one_shot_calls(rf):
+    """Two host threads call the chunked (pipelined) one-shot entry point at the same time, each on its own
+    stream with its own inputs: every call owns its internal build stream and event, so neither can see the
+    other's ordering.  Each result must equal the oracle."""
+    import threading
+    w = inputs.scaled("C2", 3000, 700, B=12)
+    Ps = [inputs.make_batch(w, seed=4000 + 100 * t) for t in range(2)]
+    refs = [oracle.fps(P, w.M, 0) for P in Ps]
+    errs = []
+
+    def work(t):
+        try:
+            torch.cuda.set_device(0)
+            side = torch.cuda.Stream()
+            Ph = torch.from_numpy(Ps[t]).pin_memory()
+            for _ in range(6):
+                with torch.cuda.stream(side):
+                    Pd = torch.empty_like(Ph, device="cuda")
+                    Pd.copy_(Ph, non_blocking=True)
+                    idx, mind = rf.fps_build_and_sample(Pd, w.M, chunk_clouds=3 + t, stream=side)
+                    hi, hm = idx.to("cpu", non_blocking=True), mind.to("cpu", non_blocking=True)
+                side.synchronize()
+                assert_same(hi.numpy(), hm.numpy(), *refs[t])
+        except BaseException as e:          # noqa: BLE001 -- reported by the main thread
+            errs.append((t, repr(e)))
+
+    th = [threading.Thread(target=work, args=(t,)) for t in range(2)]
+    for t in th:
+        t.start()
+    for t in th:
+        t.join()
+    assert not errs, errs
+
+
+def test_trim_and_rebuild(rf):
+    P = torch.from_numpy(inputs.room(5000, 77)).cuda()
+    ref = oracle.fps(P.cpu().numpy(), 500, 0)
+    for _ in range(2):
+        ix = rf.fps_index_build(P)
+        idx, mind = rf.fps_sample(ix, 500, 0)
+        torch.cuda.synchronize()
+        rf.fps_index_destroy(ix)
+        rf.fps_trim()
+        assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+
+
+def test_bench_replicas_on_two_gpus():
+    """bench.py's world > 1 branch (NCCL init, per-rank seeds, max over ranks of CUDA-event times) on real GPUs.
+    Needs >= 2 devices; the boxes this suite normally runs on have one, so it then SKIPS LOUDLY."""
+    import subprocess
+    import sys
+    if torch.cuda.device_count() < 2:
+        pytest.skip(f"needs >= 2 CUDA devices for torchrun --nproc-per-node 2, found {torch.cuda.device_count()}: "
+                    "the multi-GPU replica path is covered on CPU by tests/test_sharding_gloo.py only")
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    out = subprocess.run([sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2",
+                          "--master-addr", "127.0.0.1", "--master-port", "29533", os.path.join(root, "bench.py"),
+                          "--gpus", "2", "--steps", "3", "--warmup", "3", "--workload", "C1", "--quick"],
+                         capture_output=True, text=True, timeout=600, cwd=root)
+    assert out.returncode == 0, out.stderr[-2000:]
+    line = json.loads([ln for ln in out.stdout.splitlines() if ln.startswith("{")][-1])
+    assert line["n_gpus"] == 2 and line["value"] > 0 and line["scaling"] == "weak"

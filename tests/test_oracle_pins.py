@@ -345,3 +345,21 @@ def test_euclid_differs_from_squared_where_sqrt_collapses_two_maxima():
     ei, em = oracle.fps_euclid(P, 2, 0)
     assert si.tolist() == [0, 2] and ei.tolist() == [0, 1]
     assert same_bits(em[1:], d_sqrt(P[1:2], P[0]))
+
+
+@pytest.mark.parametrize("threads", [1, 2, 0])
+def test_euclid_batch_equals_singles_and_threads(threads):
+    # the batch wrapper oracle_fps_euclid_batch (cloud stride 3N of the input, M of both outputs, OpenMP over
+    # clouds) is pinned to the single-cloud function, which the brute-force tests above pin to Eq. 3; clouds of
+    # three different generators so that a wrong stride cannot land on an identical neighbour
+    N, M = 1500, 200
+    P = np.stack([inputs.room(N, 901), inputs.uniform_cube(N, 902), inputs.clustered(N, 903),
+                  inputs.room(N, 904, dense_half=True), inputs.lidar(N, 905, n_azimuth=24)])
+    idx, mind = oracle.fps_euclid(P, M, 3, threads=threads)
+    assert idx.shape == (5, M) and mind.shape == (5, M)
+    for b in range(P.shape[0]):
+        i1, m1 = oracle.fps_euclid(P[b], M, 3)
+        assert np.array_equal(idx[b], i1) and same_bits(mind[b], m1)
+        bi, bm = brute_force_fps(P[b][:48], 48, 3, dist=d_sqrt)         # and one step further down: Eq. 3 itself
+        oi, om = oracle.fps_euclid(np.stack([P[b][:48]] * 2), 48, 3, threads=threads)
+        assert np.array_equal(oi[1], bi) and same_bits(om[1], bm)
