@@ -3,17 +3,31 @@
 
 A "step" is one pass of the WHOLE hot path over one batch of synthetic clouds: fps_index_build
 (a1-a6: bbox, voxel keys, radix sort, SoA gather, segments, spheres) + fps_sample (a7-a13: the
-persistent fused kernel, all M-1 iterations), inputs already resident in HBM.  Default workload:
-BASELINE.json configs[1] ("C2": B=16 indoor-room-like clouds, N=24000, M=6000).  `e2e` is the same
-metric through fps_sample_host with HOST buffers (H2D + build + sample + D2H inside the timed
-region).  `roofline` is for the dominant kernel (k_fps_batched, exact batched picking): algorithmic
-bytes per launch (from the kernel's own counters in a separate,
-untimed stats run) divided by its average launch duration measured with CUDA events on the
-launching stream.  The same run also times the per-pick persistent kernel (the paper's iteration
-structure, FPS_FLAG_PER_PICK) once as an ablation.
-`cpu_baseline` is the CPU oracle timed on this box's host cores (rank 0, N=1 only).
+persistent fused kernel, all M-1 iterations), inputs already resident in HBM.  Headline workload:
+BASELINE.json configs[1] ("C2": B=16 indoor-room-like clouds, N=24000, M=6000).  The same JSON line
+carries, under "all_configs", the SAME measurement set for every BASELINE.json configuration C1..C5
+(north_star: "ms per cloud, samples/s and achieved fraction of the HBM roofline, alongside the oracle
+timed in the same run" for each config), each with the full --steps.
 
-  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1..C5] [--impl reference]
+  value / ms_per_step   device-resident build + sample, CUDA events, L2 flushed between steps
+  e2e                   the same metric through fps_sample_host with pinned HOST buffers (H2D + build +
+                        sample + D2H inside the timed region)
+  roofline              dominant kernel (k_fps_batched): ALGORITHMIC bytes per launch / its mean launch
+                        duration (CUDA events on the launching stream).  `achieved`/`frac` use SURVEY.md
+                        8(d)'s formula exactly (28 B x K per iteration + 16 B per visited (point, pick) +
+                        8 B per voxel visit + 4 B per effective update + 20 B per pick);
+                        `schedule_*` is the count of the schedule that actually ran (group + voxel tests
+                        that ran, one argmax per round, extraction traffic) -- the smaller, more
+                        conservative figure.  Counters come from a separate untimed stats launch with
+                        identical outputs.  `traffic` = ncu dram bytes per launch (profiles/r02_traffic.csv).
+  latency               the bound that binds: measured cycles per pick of the bare dependent pick chain
+                        (fps_pick_chain_cycles) / achieved cycles per pick
+  cpu_baseline          rank 0, N=1: the CPU oracle as it stands (best of 3 on a bounded prefix), the plain
+                        CPU pruned variant (oracle/fps_pruned_cpu.c) and the tuned CPU RadiusFPS baseline
+                        program (baselines/cpu_radiusfps), threads stated
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C1..C5] [--configs C1,C5] [--quick]
+                  [--impl reference]
   python -m torch.distributed.run --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...
 Multi-GPU: replicas only: every rank runs its own batch (seeds disjoint),
 no data-path collective; time = max over ranks; value = all ranks' samples / that time ("weak").
@@ -21,6 +35,7 @@ no data-path collective; time = max over ranks; value = all ranks' samples / tha
 from __future__ import annotations
 
 import argparse
+import hashlib
 import json
 import os
 import subprocess
@@ -38,6 +53,8 @@ from paper_2606_06255_b200 import inputs, sharding  # noqa: E402
 
 METRIC = "fps_samples_per_s"
 UNIT = "samples/s"
+GHZ_FALLBACK = 1.965
+ALL = ("C1", "C2", "C3", "C4", "C5")
 
 
 def parse():
@@ -46,15 +63,18 @@ def parse():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C2", choices=sorted(inputs.WORKLOADS))
+    ap.add_argument("--configs", default=",".join(ALL), help="configurations of the per-config section (comma list)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--quick", action="store_true", help="headline only: no per-config section, CPU baseline or ablation")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-extra-configs", action="store_true", help="skip the per-config summary (C1..C5)")
+    ap.add_argument("--no-extra-configs", action="store_true", help="skip the per-config section (C1..C5)")
     ap.add_argument("--n-vox", type=int, default=0)
     ap.add_argument("--tile-points", type=int, default=0)
     ap.add_argument("--cluster-size", type=int, default=0)
     ap.add_argument("--block-threads", type=int, default=0)
     ap.add_argument("--local-warps", type=int, default=0)
     ap.add_argument("--cand-per-thread", type=int, default=0)
+    ap.add_argument("--flags", type=int, default=0, help="extra FPS_FLAG_* bits (ablations)")
     ap.add_argument("--per-pick", action="store_true", help="time the per-pick persistent kernel instead (ablation)")
     return ap.parse_args()
 
@@ -63,10 +83,25 @@ def measured_peak():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
         try:
-            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+            return float(json.load(open(p))["hbm_gbs"]), "MEASURED_PEAKS.json hbm_gbs"
         except Exception:
             pass
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def rounded(o, sig=6):
+    """floats to `sig` significant digits: keeps the one JSON line short enough to survive a log tail."""
+    if isinstance(o, float):
+        return float(f"{o:.{sig}g}") if np.isfinite(o) else None
+    if isinstance(o, dict):
+        return {k: rounded(v, sig) for k, v in o.items()}
+    if isinstance(o, (list, tuple)):
+        return [rounded(v, sig) for v in o]
+    if isinstance(o, (np.floating,)):
+        return rounded(float(o), sig)
+    if isinstance(o, (np.integer,)):
+        return int(o)
+    return o
 
 
 # ---------------------------------------------------------------------------------------------
@@ -119,16 +154,24 @@ class Clocks:
 
 
 # ---------------------------------------------------------------------------------------------
-# algorithmic bytes (DESIGN.md / SURVEY.md 8(d)) from the kernel's counters
+# algorithmic bytes from the kernel's counters
 # ---------------------------------------------------------------------------------------------
-def algorithmic_bytes(st: dict) -> int:
-    """SURVEY.md 8(d) / DESIGN.md "Algorithmic bytes", evaluated with the counters of the schedule
-    that ran.  20 B per radius-prune test (centre 12, radius 4, Dist_v 4; group tests and voxel
-    tests alike) + 16 B per (visited point, pick) pair (x, y, z, Dist_p) + 8 B key write-back per
-    voxel visit + 4 B per effective Dist_p store + 8 B per voxel key per argmax (one argmax per
-    pick in the per-pick kernel, one per round in the batched kernel) + 20 B per pick (s_j,
-    out_idx, out_mindist) + batched kernel only: 4 B per point scanned by the candidate extraction
-    and 20 B per candidate moved (x, y, z, Dist_p, index)."""
+def survey_bytes(st: dict) -> int:
+    """SURVEY.md 8(d), exactly: per iteration 20 B x K (prune test: centre 12, radius 4, Dist_v 4, EVERY active
+    voxel) + 8 B x K (argmax over the K keys) + per visited voxel (16 B per point: x, y, z, Dist_p; + 8 B key
+    write-back) + 4 B per effective Dist_p store + 20 B (s_j, out_idx, out_mindist).  With the batched kernel
+    `points_visited` counts (point, pick) pairs, which is what the formula's sum over iterations counts.
+    K_total x (M-1) = sum over clouds of K_b x iterations_b (uniform M)."""
+    iters_per_cloud = st["iterations"] / max(1, st["B"])
+    return int(28 * st["K_total"] * iters_per_cloud + 16 * st["points_visited"] + 8 * st["voxels_visited"]
+               + 4 * st["effective"] + 20 * st["iterations"])
+
+
+def schedule_bytes(st: dict) -> int:
+    """The same per-item costs charged only for the work the schedule that ran actually did: 20 B per radius-prune
+    test that ran (group tests + voxel tests of surviving groups), 8 B x K per ARGMAX that ran (one per round in the
+    batched kernel, one per pick in the per-pick kernel), plus the batched kernel's own terms: 4 B per point scanned
+    by the candidate extraction and 20 B per candidate moved (x, y, z, Dist_p, index)."""
     argmaxes = st["rounds"] if st.get("rounds", 0) else st["iterations"]
     per_cloud_K = st["K_total"] / max(1, st["B"])
     return int(20 * (st["voxel_tests"] + st.get("group_tests", 0)) + 16 * st["points_visited"] + 8 * st["voxels_visited"]
@@ -138,58 +181,85 @@ def algorithmic_bytes(st: dict) -> int:
 
 def ncu_traffic(workload: str, per_pick: bool):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-    `ncu --set full` capture of this workload (profiles/r01_traffic.csv: workload,kernel,bytes), else None."""
-    path = os.path.join(ROOT, "profiles", "r01_traffic.csv")
+    `ncu --set full` capture of this workload (profiles/r02_traffic.csv, else r01_traffic.csv), else None."""
     want = "k_fps_sample" if per_pick else "k_fps_batched"
-    try:
-        for row in open(path).read().splitlines()[1:]:
-            f = [c.strip() for c in row.split(",")]
-            if len(f) >= 3 and f[0] == workload and f[1] == want:
-                return float(f[2])
-    except OSError:
-        pass
+    for fn in ("r02_traffic.csv", "r01_traffic.csv"):
+        try:
+            for row in open(os.path.join(ROOT, "profiles", fn)).read().splitlines()[1:]:
+                f = [c.strip() for c in row.split(",")]
+                if len(f) >= 3 and f[0] == workload and f[1] == want:
+                    return float(f[2])
+        except OSError:
+            pass
     return None
 
 
+def roofline_report(stc, kern_s, w, peak, peak_src, per_pick):
+    sb, cb = survey_bytes(stc), schedule_bytes(stc)
+    ach = sb / kern_s / 1e9
+    return {"bound": "hbm", "kernel": "k_fps_sample" if per_pick else "k_fps_batched", "achieved": ach, "peak": peak,
+            "unit": "GB/s", "frac": ach / peak, "frac_of_8000_nominal": ach / 8000.0, "peak_source": peak_src,
+            "bytes_source": "SURVEY.md 8(d) formula: (28 K + 20) B per iteration + 16 B per visited (point, pick) + "
+                            "8 B per voxel visit + 4 B per effective update",
+            "algorithmic_bytes_per_launch": sb,
+            "schedule_bytes_per_launch": cb, "schedule_achieved": cb / kern_s / 1e9, "schedule_frac": cb / kern_s / 1e9 / peak,
+            "traffic": ncu_traffic(w.name, per_pick),
+            "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9,
+            "note": "not the binding limit: the working set is L2/SMEM resident (see traffic) and the picks are "
+                    "sequentially dependent; see latency"}
+
+
+_floor_cache = {}
+
+
 def latency_report(rf, kern_s, w, sm_mhz) -> dict:
-    """The bound that binds: the M-1 picks of a cloud are sequentially dependent, so `fps_sample` cannot be
-    faster than (M-1) x the dependent chain of one pick.  The floor is MEASURED live: the bare chain on one
-    warp with 1 candidate per lane (fps_pick_chain_cycles; the kernel's pick warp holds 2 per lane).  The
-    clouds of a batch run in parallel, so the achieved figure is kernel time / (M-1) per cloud."""
+    """The M-1 picks of a cloud are sequentially dependent, so `fps_sample` cannot be faster than (M-1) x the
+    dependent chain of one pick.  The floor is MEASURED live: the bare chain on one warp with 1 candidate per
+    lane (fps_pick_chain_cycles).  The clouds of a batch run in parallel: achieved = kernel time / (M-1)."""
     ghz = (sm_mhz or GHZ_FALLBACK * 1e3) * 1e-3
-    floor1 = rf.fps_pick_chain_cycles(1, 8192)
-    floor2 = rf.fps_pick_chain_cycles(2, 8192)
+    if "f" not in _floor_cache:
+        _floor_cache["f"] = rf.fps_pick_chain_cycles(1, 8192)
+    floor1 = _floor_cache["f"]
     achieved = kern_s * ghz * 1e9 / max(1, w.M - 1)
-    return {"bound": "latency", "unit": "SM cycles per pick", "floor": floor1, "floor_2_candidates_per_lane": floor2,
-            "achieved": achieved, "frac": floor1 / achieved,
-            "note": "floor = bare chain update -> lane max -> redux(max D) -> redux(slot id) -> 3 shared loads on one warp, "
-                    "no tie handling, no candidate selection, no global rounds"}
+    return {"bound": "latency", "unit": "SM cycles per pick", "floor": floor1, "achieved": achieved, "frac": floor1 / achieved}
 
 
 def opts_from(args) -> dict:
     return dict(n_vox=args.n_vox, tile_points=args.tile_points, cluster_size=args.cluster_size,
                 block_threads=args.block_threads, local_warps=args.local_warps, cand_per_thread=args.cand_per_thread,
-                flags=(16 if args.per_pick else 0))
-
-
-GHZ_FALLBACK = 1.965
+                flags=(16 if args.per_pick else 0) | args.flags)
 
 
 def phase_ms(st: dict, sm_mhz) -> dict:
-    """Per-phase time of the batched kernel (SM cycles seen by thread 0 of each cloud's first CTA,
-    averaged over clouds, converted with the SM clock sampled during the run)."""
+    """Per-phase time of the batched kernel (SM cycles seen by thread 0 of each cloud's picker CTA, averaged over
+    clouds; workers: averaged over worker CTAs), converted with the SM clock sampled during the run."""
     ghz = (sm_mhz or GHZ_FALLBACK * 1e3) * 1e-3
     f = lambda k: st.get(k, 0) / max(1, st["B"]) / ghz / 1e6  # noqa: E731
     workers = max(1, st["B"] * max(1, st["cluster_size"] - 1))
     g = lambda k: st.get(k, 0) / workers / ghz / 1e6  # noqa: E731
-    return {"picker_cta": {"argmax": f("cycles_max"), "extract": f("cycles_extract"),
-                           "local_incl_wait_for_workers": f("cycles_local"), "apply_if_single_cta": f("cycles_apply")},
-            "worker_cta_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum")},
-            "note": "with cluster_size > 1 the workers apply the picks while the picker CTA is still producing them"}
+    return {"picker": {"argmax": f("cycles_max"), "extract": f("cycles_extract"), "local_incl_wait": f("cycles_local"),
+                       "local_select": f("cycles_local_select"), "local_pick": f("cycles_local_pick"),
+                       "local_update": f("cycles_local_update"), "apply_if_single_cta": f("cycles_apply")},
+            "worker_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum")}}
+
+
+def sha(a) -> str:
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
+
+
+def golden_match(name, out_idx, out_mind):
+    """The timed run's outputs against the stored hashes of the CPU oracle's outputs (tests/golden/full_size.json,
+    written by tests/golden/make_golden.py from oracle/ alone).  None if there is no entry."""
+    try:
+        g = json.load(open(os.path.join(ROOT, "tests", "golden", "full_size.json")))[name]
+    except Exception:
+        return None
+    return bool(sha(out_idx.cpu().numpy().astype(np.int32)) == g["idx_sha256"]
+                and sha(out_mind.cpu().numpy().astype(np.float32)) == g["mindist_sha256"])
 
 
 def time_config(rf, torch, w, P_host, steps, warmup, opts, flush):
-    """Returns dict with per-step ms (whole path), sample-kernel ms, build ms, stats."""
+    """Per-step ms (whole path), sample-kernel ms, build ms, layout stats."""
     Pd = torch.from_numpy(P_host).cuda()
     out_idx = torch.empty((w.B, w.M), dtype=torch.int32, device="cuda")
     out_mind = torch.empty((w.B, w.M), dtype=torch.float32, device="cuda")
@@ -214,6 +284,22 @@ def time_config(rf, torch, w, P_host, steps, warmup, opts, flush):
     return dict(step_ms=step_ms, kern_ms=kern_ms, build_ms=build_ms, stats=st, out_idx=out_idx, out_mind=out_mind)
 
 
+def time_e2e(rf, torch, w, P_host, steps, warmup, opts, barrier):
+    """fps_sample_host with pinned HOST buffers: H2D + build + sample + D2H inside the timed region (wall clock
+    around synchronous calls).  Returns (seconds for `steps` calls, out_idx host tensor)."""
+    Ph = torch.from_numpy(P_host).pin_memory()
+    oi = torch.empty((w.B, w.M), dtype=torch.int32).pin_memory()
+    om = torch.empty((w.B, w.M), dtype=torch.float32).pin_memory()
+    for _ in range(warmup):
+        rf.fps_sample_host(Ph, w.M, w.start_idx, out_idx=oi, out_mindist=om, **opts)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        rf.fps_sample_host(Ph, w.M, w.start_idx, out_idx=oi, out_mindist=om, **opts)
+    torch.cuda.synchronize()
+    return time.perf_counter() - t0, oi
+
+
 def stats_run(rf, torch, w, P_host, opts):
     Pd = torch.from_numpy(P_host).cuda()
     opts = dict(opts)
@@ -226,35 +312,63 @@ def stats_run(rf, torch, w, P_host, opts):
     return st
 
 
-def cpu_oracle_sample(w, P_host, budget_s=15.0):
-    """Times oracle/fps_oracle.c as it stands on a bounded sample of the workload: the first
-    `nb` clouds (one thread per cloud) and the first `m` samples of each, sized from a calibration
-    so that the run takes roughly `budget_s` seconds of wall time.  The oracle's cost per sample is
-    N point updates whatever the iteration, so samples/s on a prefix is unbiased."""
+# ---------------------------------------------------------------------------------------------
+# CPU legs (the only places bench.py executes oracle/; the tuned CPU RadiusFPS is a baseline program)
+# ---------------------------------------------------------------------------------------------
+def cpu_baselines(w, P_host, oracle_budget_s=1.5, repeats=3):
+    """(1) the oracle as it stands on a bounded prefix (first nb clouds, first m samples; its cost per sample is
+    N point updates whatever the iteration, so a prefix is unbiased), best of `repeats`; (2) the plain CPU pruned
+    variant, all M samples (its cost per sample falls as the prune bites: a prefix would be biased), best of
+    `repeats`; (3) the tuned CPU RadiusFPS baseline program over a small n_vox sweep (Fig. 15b), best of `repeats`
+    at the best n_vox.  One thread per cloud up to the core count; B = 1 runs on one thread."""
     import oracle
+    from baselines import cpu_radiusfps as cr
     cores = os.cpu_count() or 1
     nb = min(w.B, cores)
+    oracle.fps(P_host[:1], min(w.M, 9), w.start_idx, threads=1)          # load + page in
     t = time.perf_counter()
-    oracle.fps(P_host[:1], min(w.M, 65), w.start_idx, threads=1)          # calibration: 64 iterations, 1 cloud
-    per_it = (time.perf_counter() - t) / 64
-    m = int(max(2, min(w.M, budget_s / max(per_it, 1e-9))))
-    t = time.perf_counter()
-    oracle.fps(P_host[:nb], m, w.start_idx, threads=nb)
-    dt = time.perf_counter() - t
-    out = {"value": nb * m / dt, "unit": UNIT, "cores": int(oracle.fps.threads_used), "kind": "oracle",
-           "sample": f"first {nb} of {w.B} clouds x first {m} of {w.M} samples, {dt:.1f} s wall, "
-                     f"oracle/fps_oracle.c -O2 one thread per cloud", "ms_per_cloud_extrapolated": dt / m * w.M * 1e3}
-    # SURVEY 8(d) CPU baseline (2): the plain CPU pruned variant (oracle/fps_pruned_cpu.c, the paper's section 3
-    # algorithm, untuned), same clouds and threading, all M samples (its cost per sample falls as the prune bites,
-    # so a prefix would be biased); its ratio to the oracle is the analogue of the paper's CPU speedups (`:697-705`).
-    t = time.perf_counter()
-    oracle.pruned_fps(P_host[:nb], w.M, w.start_idx, n_vox=16, threads=nb)
-    dtp = time.perf_counter() - t
-    out["pruned_cpu_variant"] = {"value": nb * w.M / dtp, "unit": UNIT, "cores": int(oracle.pruned_fps.threads_used),
-                                 "n_vox": 16, "ms_per_cloud": dtp * 1e3,
-                                 "speedup_over_oracle": (nb * w.M / dtp) / (nb * m / dt),
-                                 "sample": f"first {nb} of {w.B} clouds x all {w.M} samples, {dtp:.2f} s wall, "
-                                           f"oracle/fps_pruned_cpu.c one thread per cloud"}
+    oracle.fps(P_host[:1], min(w.M, 33), w.start_idx, threads=1)         # calibration: 32 iterations, 1 cloud
+    per_it = (time.perf_counter() - t) / 32
+    m = int(max(2, min(w.M, oracle_budget_s / max(per_it, 1e-9))))
+    best = 1e30
+    for _ in range(repeats):
+        t = time.perf_counter()
+        oracle.fps(P_host[:nb], m, w.start_idx, threads=nb)
+        best = min(best, time.perf_counter() - t)
+    thr = int(oracle.fps.threads_used)
+    ov = nb * m / best
+    out = {"value": ov, "unit": UNIT, "cores": thr, "kind": "oracle",
+           "sample": f"oracle/fps_oracle.c as it stands: first {nb} of {w.B} clouds x first {m} of {w.M} samples, one thread "
+                     f"per cloud, best of {repeats} ({best:.2f} s)", "ms_per_cloud_extrapolated": best / m * w.M * 1e3}
+    nv_plain = 16 if w.N <= 30000 else (32 if w.N <= 200000 else 64)     # plain variant: no tiling of dense voxels
+    bestp = 1e30
+    for _ in range(repeats if w.N <= 30000 else 1):
+        t = time.perf_counter()
+        oracle.pruned_fps(P_host[:nb], w.M, w.start_idx, n_vox=nv_plain, threads=nb)
+        bestp = min(bestp, time.perf_counter() - t)
+    out["pruned_cpu_variant"] = {"value": nb * w.M / bestp, "cores": int(oracle.pruned_fps.threads_used), "n_vox": nv_plain,
+                                 "ms_per_cloud": bestp * 1e3, "speedup_over_oracle": (nb * w.M / bestp) / ov,
+                                 "what": "oracle/fps_pruned_cpu.c (plain, untuned cross-check), all M samples"}
+    auto = round((w.N / 8.0) ** (1.0 / 3.0))
+    sweep = {}
+    for nv in (8, 12, 16, 24, 32, 48, 64, 96, 128, 192, 256):           # ascending; stop once the time turns up
+        if nv / auto < 0.5 or (sweep and (nv / auto > 5.5 or sweep[max(sweep)] > 1.15 * min(sweep.values()))):
+            continue
+        t = time.perf_counter()
+        cr.fps(P_host[:nb], w.M, w.start_idx, nv, threads=nb)
+        sweep[nv] = time.perf_counter() - t
+    nvb = min(sweep, key=sweep.get)
+    bestt = sweep[nvb]
+    for _ in range(repeats - 1):
+        t = time.perf_counter()
+        cr.fps(P_host[:nb], w.M, w.start_idx, nvb, threads=nb)
+        bestt = min(bestt, time.perf_counter() - t)
+    out["tuned_cpu_radiusfps"] = {"value": nb * w.M / bestt, "cores": int(cr.fps.threads_used), "n_vox": nvb,
+                                  "ms_per_cloud": bestt * 1e3, "speedup_over_oracle": (nb * w.M / bestt) / ov,
+                                  "n_vox_sweep_ms": {str(k): v * 1e3 for k, v in sweep.items()},
+                                  "what": "baselines/cpu_radiusfps (SoA, two-level sqrt-free prune, SIMD visits, OpenMP over "
+                                          "clouds), all M samples; the paper reports 46-186x for its CPU RadiusFPS on its own "
+                                          "data and CPU (PAPER.md:697-705)"}
     return out
 
 
@@ -267,9 +381,10 @@ def reference_arm(args, rank, world):
     import oracle
     cores = os.cpu_count() or 1
     nb = min(w.B, cores)
+    oracle.fps(P[:1], min(w.M, 9), w.start_idx, threads=1)
     t = time.perf_counter()
-    oracle.fps(P[:1], min(w.M, 65), w.start_idx, threads=1)
-    per_it = (time.perf_counter() - t) / 64
+    oracle.fps(P[:1], min(w.M, 33), w.start_idx, threads=1)
+    per_it = (time.perf_counter() - t) / 32
     total_steps = args.steps + args.warmup
     m = int(max(2, min(w.M, (120.0 / total_steps) / max(per_it, 1e-9))))   # whole run within ~2 minutes
     times = []
@@ -288,7 +403,42 @@ def reference_arm(args, rank, world):
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": int(oracle.fps.threads_used), "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
-    print(json.dumps(line), flush=True)
+    print(json.dumps(rounded(line)), flush=True)
+
+
+def config_entry(rf, torch, name, flush, opts, peak, peak_src, steps, warmup, sm_mhz, with_cpu, per_pick):
+    """The full measurement set for one BASELINE.json configuration (north_star / BASELINE.md section 5.4)."""
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    stc = stats_run(rf, torch, w, P, opts)
+    r = time_config(rf, torch, w, P, steps, warmup, opts, flush)
+    e2e_s, oi = time_e2e(rf, torch, w, P, steps, warmup, opts, torch.cuda.synchronize)
+    k = float(np.mean(r["kern_ms"])) * 1e-3
+    step = float(np.mean(r["step_ms"]))
+    roof = roofline_report(stc, k, w, peak, peak_src, per_pick)
+    for drop in ("peak_source", "bytes_source", "note", "kernel", "bound", "unit"):
+        roof.pop(drop, None)
+    lat = latency_report(rf, k, w, sm_mhz)
+    out = {"B": w.B, "N": w.N, "M": w.M, "n_vox": stc["n_vox"], "K_max": stc["K_max"], "cluster_size": stc["cluster_size"],
+           "steps": steps, "ms_per_step": step, "ms_per_cloud": step / w.B, "samples_per_s": w.B * w.M / (step * 1e-3),
+           "sample_kernel_ms": k * 1e3, "index_build_ms": float(np.mean(r["build_ms"])),
+           "sample_only_samples_per_s": w.B * w.M / k,
+           "e2e": {"value": w.B * w.M * steps / e2e_s, "ms_per_step": e2e_s / steps * 1e3, "h2d_bytes_per_step": int(P.nbytes),
+                   "d2h_bytes_per_step": int(2 * 4 * w.B * w.M)},
+           "roofline": roof, "latency": {"achieved": lat["achieved"], "floor": lat["floor"], "frac": lat["frac"]},
+           "rounds_per_cloud": stc["rounds"] / w.B, "picks_per_round": stc["iterations"] / max(1, stc["rounds"]),
+           "points_visited_per_iter": stc["points_visited"] / stc["iterations"],
+           "voxels_visited_per_iter": stc["voxels_visited"] / stc["iterations"],
+           "device_bytes": stc["device_bytes"],
+           "equals_oracle_hash": golden_match(name, r["out_idx"], r["out_mind"]),
+           "e2e_equals_device_path": bool(np.array_equal(oi.numpy(), r["out_idx"].cpu().numpy()))}
+    if with_cpu:
+        c = cpu_baselines(w, P)
+        out["cpu"] = {"oracle": {"value": c["value"], "cores": c["cores"], "sample": c["sample"]},
+                      "pruned_plain": {k2: c["pruned_cpu_variant"][k2] for k2 in ("value", "cores", "n_vox", "speedup_over_oracle")},
+                      "tuned_radiusfps": {k2: c["tuned_cpu_radiusfps"][k2] for k2 in ("value", "cores", "n_vox", "speedup_over_oracle", "ms_per_cloud")}}
+        out["_cpu_full"] = c
+    return out
 
 
 def main():
@@ -335,25 +485,15 @@ def main():
     value = world * w.B * w.M * args.steps / (total_ms * 1e-3)
 
     # end to end through the host entry point: pinned host buffers, copies inside the timed region
-    Ph = torch.from_numpy(P).pin_memory()
-    oi = torch.empty((w.B, w.M), dtype=torch.int32).pin_memory()
-    om = torch.empty((w.B, w.M), dtype=torch.float32).pin_memory()
-    for _ in range(args.warmup):
-        rf.fps_sample_host(Ph, w.M, w.start_idx, out_idx=oi, out_mindist=om, **opts)
-    barrier()
-    t0 = time.perf_counter()
-    for i in range(args.steps):
-        rf.fps_sample_host(Ph, w.M, w.start_idx, out_idx=oi, out_mindist=om, **opts)
-    torch.cuda.synchronize()
-    e2e_s = sharding.max_over_ranks(time.perf_counter() - t0, dist if world > 1 else None)
+    e2e_local, oi = time_e2e(rf, torch, w, P, args.steps, args.warmup, opts, barrier)
+    e2e_s = sharding.max_over_ranks(e2e_local, dist if world > 1 else None)
     e2e_ok = bool(np.array_equal(oi.numpy(), r["out_idx"].cpu().numpy()))
 
     if rank == 0:
         peak, peak_src = measured_peak()
         kern_s = float(np.mean(r["kern_ms"])) * 1e-3
-        alg = algorithmic_bytes(st_counts)
-        achieved = alg / kern_s / 1e9
         st = r["stats"]
+        extra = world == 1 and not args.quick
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": total_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -366,66 +506,44 @@ def main():
                        "kernel": "per-pick persistent (ablation)" if args.per_pick else "exact batched picking",
                        "parallelism": f"replicas x{world}"},
             "ms_per_cloud": total_ms / args.steps / w.B,
-            "sample_kernel_ms": float(np.mean(r["kern_ms"])), "index_build_ms": float(np.mean(r["build_ms"])),
-            "sample_only_samples_per_s": w.B * w.M / kern_s, "us_per_iteration": kern_s * 1e6 / max(1, w.M - 1),
-            "roofline": {"bound": "hbm", "kernel": "k_fps_sample" if args.per_pick else "k_fps_batched",
-                         "achieved": achieved, "peak": peak, "unit": "GB/s",
-                         "frac": achieved / peak, "frac_of_8000_nominal": achieved / 8000.0, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": alg, "traffic": ncu_traffic(w.name, args.per_pick),
-                         "note": "BASELINE.json asks for the HBM roofline; it is NOT what binds this path: the working "
-                                 "set is L1/L2 resident (see traffic) and the M-1 picks are sequentially dependent, so "
-                                 "the kernel is bound by the latency of its pick chain (DESIGN.md section 8)",
-                         "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9,
-                         "us_per_pick": kern_s * 1e6 / max(1, w.M - 1)},
+            "sample_kernel_ms": kern_s * 1e3, "index_build_ms": float(np.mean(r["build_ms"])),
+            "sample_only_samples_per_s": w.B * w.M / kern_s, "us_per_pick": kern_s * 1e6 / max(1, w.M - 1),
+            "roofline": roofline_report(st_counts, kern_s, w, peak, peak_src, args.per_pick),
             "latency": latency_report(rf, kern_s, w, clk.get("sm_mhz")),
-            "phases_ms_per_cloud": None if args.per_pick else phase_ms(st_counts, clk.get("sm_mhz")),
-            "counters": {k: st_counts[k] for k in ("iterations", "group_tests", "voxel_tests", "voxels_visited",
-                                                   "points_visited", "points_computed", "effective", "rounds",
-                                                   "extract_retries", "single_picks", "candidates", "extract_points",
-                                                   "sub_batches", "local_subrounds", "local_fallbacks")},
             "e2e": {"value": world * w.B * w.M * args.steps / e2e_s, "unit": UNIT, "h2d_bytes_per_step": int(P.nbytes),
-                    "d2h_bytes_per_step": int(oi.numel() * 4 + om.numel() * 4), "ms_per_step": e2e_s / args.steps * 1e3,
+                    "d2h_bytes_per_step": int(oi.numel() * 4 * 2), "ms_per_step": e2e_s / args.steps * 1e3,
                     "api": "fps_sample_host (pinned host buffers)", "matches_device_path": e2e_ok},
             "gpu_launches": (st["build_launches"] + 1) * args.steps,
             "clocks": clk,
+            "equals_oracle_hash": golden_match(w.name, r["out_idx"], r["out_mind"]) if seed == inputs.BASE_SEED else None,
+            "phases_ms_per_cloud": None if args.per_pick else phase_ms(st_counts, clk.get("sm_mhz")),
+            "counters": {k: st_counts[k] for k in ("iterations", "K_total", "group_tests", "voxel_tests", "voxels_visited",
+                                                   "points_visited", "points_computed", "effective", "rounds",
+                                                   "extract_retries", "single_picks", "candidates", "extract_points",
+                                                   "sub_batches", "local_subrounds", "local_fallbacks")},
         }
-        if world == 1 and not args.per_pick and not args.no_extra_configs:
+        if extra and not args.per_pick:
             o2 = dict(opts, flags=16, local_warps=0, cand_per_thread=0)
             r2 = time_config(rf, torch, w, P, 3, 3, o2, flush)
             line["ablation_per_pick_kernel"] = {
-                "what": "the paper's iteration structure (one cluster-wide argmax exchange per sample) as ONE persistent "
-                        "kernel, FPS_FLAG_PER_PICK; same index, same outputs",
+                "what": "the paper's iteration structure (one cluster-wide argmax exchange per sample) as one persistent kernel",
                 "sample_kernel_ms": float(np.median(r2["kern_ms"])),
                 "outputs_identical": bool(torch.equal(r2["out_idx"], r["out_idx"]) and torch.equal(r2["out_mind"], r["out_mind"]))}
-        if world == 1 and not args.no_cpu_baseline:
-            line["cpu_baseline"] = cpu_oracle_sample(w, P)
-        if world == 1 and not args.no_extra_configs:
-            line["all_configs"] = per_config_summary(rf, torch, flush, opts, peak)
-        print(json.dumps(line), flush=True)
+        if extra and not args.no_extra_configs:
+            allc = {}
+            for name in [c for c in args.configs.split(",") if c]:
+                allc[name] = config_entry(rf, torch, name, flush, opts, peak, peak_src, args.steps, args.warmup,
+                                          clk.get("sm_mhz"), not args.no_cpu_baseline, args.per_pick)
+            if w.name in allc and "_cpu_full" in allc[w.name]:
+                line["cpu_baseline"] = allc[w.name]["_cpu_full"]
+            for e in allc.values():
+                e.pop("_cpu_full", None)
+            line["all_configs"] = allc
+        if world == 1 and not args.quick and not args.no_cpu_baseline and "cpu_baseline" not in line:
+            line["cpu_baseline"] = cpu_baselines(w, P)
+        print(json.dumps(rounded(line)), flush=True)
     if world > 1:
         dist.destroy_process_group()
-
-
-def per_config_summary(rf, torch, flush, opts, peak):
-    """north_star asks for ms/cloud + roofline fraction on each of the five configs: short runs
-    (3 warm-up + 5 timed), same protocol, reported inside the one JSON line."""
-    out = {}
-    for name in ("C1", "C2", "C3", "C4", "C5"):
-        w = inputs.WORKLOADS[name]
-        P = inputs.make_batch(w)
-        stc = stats_run(rf, torch, w, P, opts)
-        r = time_config(rf, torch, w, P, 5, 3, opts, flush)
-        k = float(np.median(r["kern_ms"])) * 1e-3
-        alg = algorithmic_bytes(stc)
-        out[name] = {"B": w.B, "N": w.N, "M": w.M, "sample_ms": k * 1e3, "sample_ms_per_cloud": k * 1e3 / w.B,
-                     "rounds_per_cloud": stc["rounds"] / w.B, "picks_per_round": stc["iterations"] / max(1, stc["rounds"]),
-                     "build_plus_sample_ms_per_cloud": float(np.median(r["step_ms"])) / w.B,
-                     "samples_per_s": w.B * w.M / k, "us_per_iteration": k * 1e6 / (w.M - 1),
-                     "hbm_roofline_frac_measured_peak": alg / k / 1e9 / peak, "hbm_roofline_frac_8000": alg / k / 1e9 / 8000.0,
-                     "n_vox": stc["n_vox"], "K_max": stc["K_max"], "cluster_size": stc["cluster_size"],
-                     "points_visited_per_iter": stc["points_visited"] / stc["iterations"],
-                     "voxels_visited_per_iter": stc["voxels_visited"] / stc["iterations"]}
-    return out
 
 
 if __name__ == "__main__":
