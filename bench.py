@@ -239,7 +239,8 @@ def phase_ms(st: dict, sm_mhz) -> dict:
     g = lambda k: st.get(k, 0) / workers / ghz / 1e6  # noqa: E731
     return {"picker": {"argmax": f("cycles_max"), "extract": f("cycles_extract"), "local_incl_wait": f("cycles_local"),
                        "local_select": f("cycles_local_select"), "local_pick": f("cycles_local_pick"),
-                       "local_update": f("cycles_local_update"), "apply_if_single_cta": f("cycles_apply")},
+                       "local_update": f("cycles_local_update"), "local_pairs": f("cycles_local_pairs"),
+                       "local_publish": f("cycles_local_publish"), "apply_if_single_cta": f("cycles_apply")},
             "worker_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum")}}
 
 

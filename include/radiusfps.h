@@ -61,11 +61,12 @@ typedef struct {
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
-    int32_t local_warps;   /* batched kernel, local phase: 0 = choose; 16 = hierarchical (all 16 warps hold
-                              candidates, one warp picks from the top <= 128 of them); 1,2,4,8 = flat FPS on
-                              that many warps                                                            */
-    int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2,4,8 (hierarchical) or 4,8,16
-                              (flat); candidate capacity = 32 * local_warps * cand_per_thread          */
+    int32_t local_warps;   /* batched kernel, local phase: 0 = choose; 32 = parallel resolution (all 16 warps hold
+                              candidates, the top <= 64 are resolved into picks per step; the default);
+                              16 = hierarchical (all 16 warps hold candidates, one warp picks sequentially from the
+                              top <= 96 of them); 4, 1, 8 = flat FPS on that many warps                          */
+    int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2, 4, 8 with local_warps 32 / 16
+                              (capacity 512 * cand_per_thread); flat shapes: 8 with 4 or 1 warps, 16 with 8        */
 } fps_build_opts;
 
 enum {
@@ -121,7 +122,10 @@ typedef struct {
     int32_t local_warps, cand_per_thread;   /* local-phase shape actually used                        */
     int64_t cycles_local_select, cycles_local_pick, cycles_local_update;   /* hierarchical local phase, SM cycles
                                  seen by thread 0 of the picker CTA, summed over clouds: candidate selection /
-                                 the pick loop / applying the picks to the candidates after the loop           */
+                                 the pick loop (parallel resolution: all pairs + resolving) / applying the picks
+                                 to the candidates after it                                                    */
+    int64_t cycles_local_pairs, cycles_local_publish;   /* parallel resolution: the all-pairs part of cycles_local_pick;
+                                 publishing a step's picks to the workers (release at cluster scope)          */
 } fps_stats;
 
 /*

@@ -12,7 +12,8 @@ import os
 import torch
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libradiusfps.so")
+# RADIUSFPS_LIB: another build of the same library (kernel experiments); the default is the in-tree build
+LIB_PATH = os.environ.get("RADIUSFPS_LIB") or os.path.join(_HERE, "libradiusfps.so")
 
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
 FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
@@ -46,7 +47,8 @@ class fps_stats(ctypes.Structure):
                 ("local_subrounds", ctypes.c_int64), ("local_fallbacks", ctypes.c_int64),
                 ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32),
                 ("cycles_local_select", ctypes.c_int64), ("cycles_local_pick", ctypes.c_int64),
-                ("cycles_local_update", ctypes.c_int64)]
+                ("cycles_local_update", ctypes.c_int64), ("cycles_local_pairs", ctypes.c_int64),
+                ("cycles_local_publish", ctypes.c_int64)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

@@ -1,0 +1,31 @@
+// sb_inst_2_32.cu -- k_fps_batched with 2 candidates per thread and local-phase shape 32 (one translation
+// unit per shape so that the shapes compile in parallel; the kernel is sample_batched.cuh)
+#include "sample_batched.cuh"
+
+namespace rfps {
+
+int launch_batched_2_32(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st) { return launch_batched_s<2, 32>(bp, ix, st); }
+
+int batched_max_resident_clusters(int c, size_t smem)
+{
+    auto kern = k_fps_batched<2, 32, false, false>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
+    cudaLaunchConfig_t cfg;
+    memset(&cfg, 0, sizeof cfg);
+    cfg.gridDim = dim3((unsigned)(c * device_props().sm_count));
+    cfg.blockDim = dim3(BT);
+    cfg.dynamicSmemBytes = smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = (unsigned)c;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int n = 0;
+    if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return n;
+}
+
+}  // namespace rfps
