@@ -55,7 +55,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         C = 1;
         for (int c = 16; c > 1; --c) {
             if ((long long)ix.N < 1024ll * c || !fits(c)) continue;
-            if (batched_max_resident_clusters(c, smem_layout(slots(c), TC, LW).total) >= std::min(want, sms / c)) { C = c; break; }
+            if (batched_max_resident_clusters(c, max_smem) >= std::min(want, sms / c)) { C = c; break; }   // the launch takes all shared memory
         }
         while (C < 16 && !fits(C)) ++C;
     }
@@ -83,6 +83,8 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
     bp.K = ix.K_dev;
     bp.poff = ix.poff_dev; bp.rag = rag_dev; bp.B = ix.B;
     bp.K_cap = ix.K_cap; bp.G_cap = ix.G_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
+    bp.smem_bytes = std::max((int)smem_layout(ix.Kc_cap, cand_capacity(ix.cand_per_thread, ix.local_warps), ix.local_warps).total,
+                             device_props().max_smem_optin);
     bp.out_idx = out_idx; bp.out_mind = out_mindist;
     bp.counters = ix.counters;
     if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));

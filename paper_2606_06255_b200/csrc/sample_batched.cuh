@@ -978,8 +978,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     const SmemLayout L = smem_layout(P.Kc_cap, TC, LW);
     float4 *sgeom = reinterpret_cast<float4 *>(smem_raw + L.geom);    // [Kc] {cx, cy, cz, R}
     float4 *sggeom = reinterpret_cast<float4 *>(smem_raw + L.ggeom);  // [Gc] group spheres
-    uint2 *vst = reinterpret_cast<uint2 *>(smem_raw + L.vst);         // [Kc] voxel key {Dist_v bits, ~orig of the point attaining it}
+    unsigned *vdv = reinterpret_cast<unsigned *>(smem_raw + L.vdv);   // [Kc] Dist_v bits = max Dist_p in the voxel (Eq. 30)
     int2 *sseg = reinterpret_cast<int2 *>(smem_raw + L.seg);          // [Kc] {first point, count} of the voxel's segment
+    int *sloc = reinterpret_cast<int *>(smem_raw + L.loc);            // [Kc] first point in this CTA's resident copy, or -1
+    int *gpre = reinterpret_cast<int *>(smem_raw + L.gpre);           // [Gc+1] resident points before group gl
     float *svthr = reinterpret_cast<float *>(smem_raw + L.vthr);      // [Kc] prune threshold of the voxel (from its key and radius)
     float *sgthr = reinterpret_cast<float *>(smem_raw + L.gthr);      // [Gc] prune threshold of the group (from the largest key in it)
     float4 *bpick = reinterpret_cast<float4 *>(smem_raw + L.bpick);   // [PB] picks of the current batch
@@ -1028,9 +1030,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         sgeom[kl] = k < K ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
         sseg[kl] = k < K ? vseg[k] : make_int2(0, 0);
         // not visited yet: Dist_v = NaN, whose prune threshold is NaN ("d2 >= NaN" is false: visit).  Every
-        // voxel is visited by the first pick, so no NaN key survives round 1.  Empty slot: key (0,0), below
-        // every real key, threshold 0 ("d2 >= 0" always prunes)
-        vst[kl] = make_uint2(k < K ? F32_NAN_BITS : 0u, 0u);
+        // voxel is visited by the first pick, so no NaN survives round 1.  Empty slot: Dist_v = 0, below
+        // every live distance, threshold 0 ("d2 >= 0" always prunes)
+        vdv[kl] = k < K ? F32_NAN_BITS : 0u;
         svthr[kl] = k < K ? __uint_as_float(F32_NAN_BITS) : 0.0f;
     }
     for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[wr + W * gl]; qbits[gl] = 0u; sgthr[gl] = __uint_as_float(F32_NAN_BITS); }
@@ -1040,6 +1042,57 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         const int p0 = min(Nb, rank * chunk), p1 = min(Nb, p0 + chunk);
         const float inf = __uint_as_float(F32_INF_BITS);
         for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
+    }
+    // ---- resident points.  The points of a group of 32 consecutive voxels are one contiguous run of the sorted
+    // arrays; the runs of the groups this CTA owns are copied one after the other into what is left of its shared
+    // memory -- as many whole groups as fit, the rest is read from global memory (L2) as before.  x, y, z and
+    // Dist_p only: the original index is needed for candidates and for exact ties of the global maximum, both
+    // rare, and stays in global memory. ----
+    float *const sPX = reinterpret_cast<float *>(smem_raw + (split ? L.picker : L.pts));
+    const int pts_cap = worker ? (int)(((size_t)P.smem_bytes - (split ? L.picker : L.pts)) / 16) : 0;
+    float *const sPY = sPX + pts_cap, *const sPZ = sPY + pts_cap, *const sPD = sPZ + pts_cap;
+    __syncthreads();
+    if (warp == 0) {
+        // exclusive prefix of the groups' point counts (a group's run ends where the next group's starts; Gc is small)
+        int carry = 0;
+        for (int base = 0; base < Gc; base += 32) {
+            const int gl = base + lane;
+            int len = 0;
+            if (gl < Gc) {
+                int s = 0;
+                for (int l = 0; l < 32; ++l) s += sseg[gl * 32 + l].y;
+                len = s;
+            }
+            int incl = len;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(FULL, incl, o);
+                if (lane >= o) incl += t;
+            }
+            if (gl < Gc) gpre[gl] = carry + incl - len;
+            carry += __shfl_sync(FULL, incl, 31);
+        }
+        if (lane == 0) gpre[Gc] = carry;
+    }
+    __syncthreads();
+    // groups 0 .. Gres-1 are resident (the prefix is monotone; Gc < BT because the voxel state has to fit as well)
+    const int Gres = __syncthreads_count(tid < Gc && gpre[tid + 1] <= pts_cap);
+    for (int kl = tid; kl < Kc; kl += BT) {
+        const int gl = kl >> 5;
+        sloc[kl] = gl < Gres ? gpre[gl] + (sseg[kl].x - sseg[gl * 32].x) : -1;
+    }
+    {
+        const int nres = Gres > 0 ? gpre[Gres] : 0;
+        const float inf = __uint_as_float(F32_INF_BITS);
+        int gl = 0;
+        for (int q = tid; q < nres; q += BT) {          // coalesced: consecutive q are consecutive sorted points
+            while (q >= gpre[gl + 1]) ++gl;
+            const int p = sseg[gl * 32].x + (q - gpre[gl]);
+            sPX[q] = px[p];
+            sPY[q] = py[p];
+            sPZ[q] = pz[p];
+            sPD[q] = inf;
+        }
     }
     if (tid == 0) {
         qn[0] = qn[1] = qn[2] = qn[3] = 0;
@@ -1080,19 +1133,21 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     // the picks bpick[sub + 32*w + i] whose bit i of word w is set ----
     auto visit = [&](const int kl, const unsigned (&vmask)[SUBW], const int sub) {
             const int2 sg = sseg[kl];
+            const int lo = sloc[kl];
+            // the voxel's points: this CTA's resident copy, or the sorted global arrays (generic pointers)
+            const float *X = lo >= 0 ? sPX + lo : px + sg.x, *Y = lo >= 0 ? sPY + lo : py + sg.x, *Z = lo >= 0 ? sPZ + lo : pz + sg.x;
+            float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
             float bestD = -1.0f;
-            unsigned bestO = 0u;
             int npk = 0;
 #pragma unroll
             for (int w = 0; w < SUBW; ++w) npk += __popc(vmask[w]);
             // two chunks of 32 points per step: both chunks' loads are in flight together
-            for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
+            for (int pb = 0; pb < sg.y; pb += 64) {
                 const int pA = pb + lane, pB = pb + 32 + lane;
-                const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
+                const bool inA = pA < sg.y, inB = pB < sg.y;
                 float xA = 0.f, yA = 0.f, zA = 0.f, DA0 = -1.0f, xB = 0.f, yB = 0.f, zB = 0.f, DB0 = -1.0f;
-                unsigned oA = 0u, oB = 0u;
-                if (inA) { xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; DA0 = Dp[pA]; }
-                if (inB) { xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; DB0 = Dp[pB]; }
+                if (inA) { xA = X[pA]; yA = Y[pA]; zA = Z[pA]; DA0 = Dq[pA]; }
+                if (inB) { xB = X[pB]; yB = Y[pB]; zB = Z[pB]; DB0 = Dq[pB]; }
                 float DA = DA0, DB = DB0;
 #pragma unroll
                 for (int w = 0; w < SUBW; ++w) {
@@ -1128,27 +1183,27 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                         }
                     }
                 }
-                if (DA < DA0) Dp[pA] = DA;
-                if (DB < DB0) Dp[pB] = DB;
+                if (DA < DA0) Dq[pA] = DA;
+                if (DB < DB0) Dq[pB] = DB;
                 if (STATS) c_pvisit += (inA ? npk : 0) + (inB ? npk : 0);
-                // absent lanes carry D = -1 (< every real distance), so they never become the voxel's key
-                if (DA > bestD || (DA == bestD && oA > bestO)) { bestD = DA; bestO = oA; }
-                if (DB > bestD || (DB == bestD && oB > bestO)) { bestD = DB; bestO = oB; }
+                // absent lanes carry D = -1 (< every real distance)
+                bestD = fmaxf(bestD, fmaxf(DA, DB));
             }
-            const unsigned hi = bestD >= 0.0f ? __float_as_uint(bestD) : 0u;
-            unsigned mhi, mlo;
-            warp_argmax_key(hi, bestD >= 0.0f ? bestO : 0u, mhi, mlo);
+            // a12: Dist_v = max Dist_p of the voxel (Eq. 30).  Which point attains it -- the lowest original index
+            // among them, PAPER.md:179 -- is only needed when the voxel holds the global maximum in a round without
+            // candidates; compute_max looks it up then
+            const unsigned mhi = __reduce_max_sync(FULL, bestD >= 0.0f ? __float_as_uint(bestD) : 0u);
             if (lane == 0) {
-                vst[kl] = make_uint2(mhi, mlo);
+                vdv[kl] = mhi;
                 svthr[kl] = EUC ? prune_threshold_euc(mhi, sgeom[kl].w) : prune_threshold(mhi, sgeom[kl].w);
                 if (STATS) c_vvisit++;
             }
             __syncwarp();
             // refresh the group threshold.  A concurrent visit to another voxel of the group may make this
-            // read one stale (larger) key: the threshold then errs on the conservative side
+            // read one stale (larger) Dist_v: the threshold then errs on the conservative side
             {
                 const int gl = kl >> 5;
-                const unsigned dvg = __reduce_max_sync(FULL, vst[gl * 32 + lane].x);
+                const unsigned dvg = __reduce_max_sync(FULL, vdv[gl * 32 + lane]);
                 if (lane == 0) sgthr[gl] = EUC ? prune_threshold_euc(dvg, sggeom[gl].w) : prune_threshold(dvg, sggeom[gl].w);
             }
     };
@@ -1245,26 +1300,34 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         bool have_max = false;
         auto compute_max = [&]() {
         // =====================================================================================
-        // MAX: argmax of the voxel keys (Eq. 15-18): thread -> warp -> CTA -> cluster
+        // MAX: argmax of Dist_v (Eq. 15-18): thread -> warp -> CTA -> cluster.  The voxels keep Dist_v only;
+        // the lowest original index among the points attaining the maximum (the tie-break of PAPER.md:179) is
+        // looked up here, in the voxels that hold this CTA's maximum (normally one)
         // =====================================================================================
         {
-            unsigned bhi = 0u, blo = 0u;
-            for (int kl = tid; kl < Kc; kl += BT) {
-                const uint2 s = vst[kl];
-                if (s.x > bhi || (s.x == bhi && s.y > blo)) { bhi = s.x; blo = s.y; }
-            }
-            unsigned mhi, mlo;
-            warp_argmax_key(bhi, blo, mhi, mlo);
-            if (lane == 0) wbest[warp] = make_uint4(mhi, mlo, 0u, 0u);
+            unsigned bhi = 0u;
+            for (int kl = tid; kl < Kc; kl += BT) bhi = max(bhi, vdv[kl]);
+            bhi = __reduce_max_sync(FULL, bhi);
+            if (lane == 0) wbest[warp].x = bhi;
+            if (tid == 0) ctl->best_lo = 0u;
         }
         __syncthreads();
-        if (warp == 0) {
-            const uint4 wb = lane < NW ? wbest[lane] : make_uint4(0u, 0u, 0u, 0u);
-            unsigned chi, clo;
-            warp_argmax_key(wb.x, wb.y, chi, clo);
-            if (lane == 0) {
-                ctl->best_hi = chi; ctl->best_lo = clo;
+        {
+            const unsigned chi = __reduce_max_sync(FULL, lane < NW ? wbest[lane].x : 0u);
+            // (also when the maximum is +0 -- duplicates exhausted, reading A7: every point ties and the lowest index of
+            // the cloud is the answer; empty slots hold Dist_v = 0 too, with no points)
+            unsigned bo = 0u;
+            for (int kl = warp; kl < Kc; kl += NW) {
+                if (vdv[kl] != chi) continue;                             // warp-uniform
+                const int2 sg = sseg[kl];
+                const int lo = sloc[kl];
+                const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
+                for (int p = lane; p < sg.y; p += 32)
+                    if (__float_as_uint(Dq[p]) == chi) bo = max(bo, ~(unsigned)porig[sg.x + p]);
             }
+            bo = __reduce_max_sync(FULL, bo);
+            if (lane == 0 && bo) atomicMax(&ctl->best_lo, bo);
+            if (tid == 0) ctl->best_hi = chi;
         }
         cluster_sync_all();
         {
@@ -1305,7 +1368,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[(rp * 2 + pass) * MAX_ATTEMPTS + a]), 0u);
                 for (int base = 0; base < Kc; base += BT) {
                     const int kl = base + tid;
-                    const bool hit = kl < Kc && vst[kl].x > tb;          // empty slots hold 0
+                    const bool hit = kl < Kc && vdv[kl] > tb;             // empty slots hold 0
                     const unsigned bal = __ballot_sync(FULL, hit);
                     if (bal) {
                         int qb = 0;
@@ -1323,17 +1386,23 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     if (lane == 0) qi = atomicAdd(&qn[2], 1);
                     qi = __shfl_sync(FULL, qi, 0);
                     if (qi >= nq) break;
-                    const int2 sg = sseg[qkl[qi]];
+                    const int kq = qkl[qi];
+                    const int2 sg = sseg[kq];
+                    const int lo = sloc[kq];
+                    const float *X = lo >= 0 ? sPX + lo : px + sg.x, *Y = lo >= 0 ? sPY + lo : py + sg.x, *Z = lo >= 0 ? sPZ + lo : pz + sg.x;
+                    const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
                     if (STATS && lane == 0) c_xvox++;
-                    // two chunks of 32 points per step, everything loaded up front (one memory round trip), one
-                    // slot reservation per step
-                    for (int pb = sg.x; pb < sg.x + sg.y; pb += 64) {
+                    // two chunks of 32 points per step, everything loaded up front, one slot reservation per step; the
+                    // original index (global memory) is fetched for the hits only
+                    for (int pb = 0; pb < sg.y; pb += 64) {
                         const int pA = pb + lane, pB = pb + 32 + lane;
-                        const bool inA = pA < sg.x + sg.y, inB = pB < sg.x + sg.y;
+                        const bool inA = pA < sg.y, inB = pB < sg.y;
                         unsigned dA = 0u, dB = 0u, oA = 0u, oB = 0u;
                         float xA = 0.f, yA = 0.f, zA = 0.f, xB = 0.f, yB = 0.f, zB = 0.f;
-                        if (inA) { dA = __float_as_uint(Dp[pA]); xA = px[pA]; yA = py[pA]; zA = pz[pA]; oA = ~(unsigned)porig[pA]; }
-                        if (inB) { dB = __float_as_uint(Dp[pB]); xB = px[pB]; yB = py[pB]; zB = pz[pB]; oB = ~(unsigned)porig[pB]; }
+                        if (inA) { dA = __float_as_uint(Dq[pA]); xA = X[pA]; yA = Y[pA]; zA = Z[pA]; }
+                        if (inB) { dB = __float_as_uint(Dq[pB]); xB = X[pB]; yB = Y[pB]; zB = Z[pB]; }
+                        if (dA > tb) oA = ~(unsigned)porig[sg.x + pA];
+                        if (dB > tb) oB = ~(unsigned)porig[sg.x + pB];
                         const bool isA = dA > tb, isB = dB > tb;
                         const unsigned balA = __ballot_sync(FULL, isA), balB = __ballot_sync(FULL, isB);
                         if (STATS) c_xpts += (inA ? 1 : 0) + (inB ? 1 : 0);
@@ -1524,7 +1593,9 @@ template <int CPT, int LW, bool STATS, bool EUC>
 static int launch_batched_one(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
 {
     auto kern = k_fps_batched<CPT, LW, STATS, EUC>;
-    const size_t smem = smem_layout(ix.Kc_cap, cand_capacity(CPT, LW), LW).total;
+    // the voxel state and the picker's regions are the minimum; everything else up to the device limit holds
+    // resident points (sample_batched_shapes.h)
+    const size_t smem = (size_t)bp.smem_bytes;
     RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     if (ix.cluster_size > 8) RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg;

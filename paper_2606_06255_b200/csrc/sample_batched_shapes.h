@@ -38,6 +38,7 @@ struct BatchParams {
     const int *poff;                               // [B+1] first point of every cloud
     const int *rag;                                // ragged call: [3][B+1] = M_b, start_b, output offsets; else null
     int B, K_cap, G_cap, Kc_cap, M, start_idx;     // Kc_cap: voxel slots per CTA (a multiple of 32); M, start_idx: uniform call
+    int smem_bytes;                                // dynamic shared memory of the launch (what is left of it holds resident points)
     int *out_idx;
     float *out_mind;
     unsigned long long *counters;
@@ -51,9 +52,13 @@ struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is th
     unsigned pub, pad4, pad5, pad6; // (CTA 0) picks of the running batch published so far | PUB_DONE | PUB_FINAL
 };
 
-// shared-memory carve-up (host and device must agree)
+// shared-memory carve-up (host and device must agree).  The picker-only regions (candidates, local-phase
+// scratch) come last: a worker CTA of a cluster with a separate picker never touches them, and its RESIDENT
+// POINTS -- x, y, z, Dist_p of the voxels it owns, copied once per fps_sample so that the visits of a9-a12 and
+// the candidate extraction run at shared-memory instead of L2 latency -- start at `picker` and use everything
+// up to the end of the allocation; a single-CTA cloud (picker and worker in one) starts them at `pts`.
 struct SmemLayout {
-    size_t geom, ggeom, vst, seg, vthr, gthr, bpick, cand, ctl, wbest, lslot, hier, qkl, qmask, qbits, qn, total;
+    size_t geom, ggeom, vdv, seg, loc, vthr, gthr, bpick, ctl, wbest, qkl, qmask, qbits, qn, gpre, picker, cand, lslot, hier, pts, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -61,24 +66,28 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     size_t o = 0;
     L.geom = o;  o += sizeof(float4) * (size_t)Kc_cap;
     L.ggeom = o; o += sizeof(float4) * (size_t)(Kc_cap / 32);
-    L.vst = o;   o += sizeof(uint2) * (size_t)Kc_cap;
     L.seg = o;   o += sizeof(int2) * (size_t)Kc_cap;
+    L.vdv = o;   o += sizeof(unsigned) * (size_t)Kc_cap;
+    L.loc = o;   o += sizeof(int) * (size_t)Kc_cap;
     L.vthr = o;  o += sizeof(float) * (size_t)Kc_cap;
     L.gthr = o;  o += (sizeof(float) * (size_t)(Kc_cap / 32) + 15) & ~(size_t)15;
+    L.gpre = o;  o += (sizeof(int) * (size_t)(Kc_cap / 32 + 1) + 15) & ~(size_t)15;
     L.bpick = o; o += sizeof(float4) * PB;
-    L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
     L.ctl = o;   o += sizeof(Ctl);
     L.wbest = o; o += sizeof(uint4) * 32;
-    L.lslot = o; o += sizeof(uint2) * 2 * 8;
-    L.hier = o;  o += 3392 + 8 * PB;     // sizeof(HierSmem), checked below
     L.qmask = o; o += sizeof(unsigned) * SUBW * (size_t)Kc_cap;
     L.qkl = o;   o += sizeof(int) * (size_t)Kc_cap;
-    L.qbits = o; o += sizeof(unsigned) * (size_t)(Kc_cap / 32);
+    L.qbits = o; o += (sizeof(unsigned) * (size_t)(Kc_cap / 32) + 15) & ~(size_t)15;
     L.qn = o;    o += sizeof(int) * 4;
-    L.total = o;
+    L.picker = o;
+    L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
+    L.lslot = o; o += sizeof(uint2) * 2 * 8;
+    L.hier = o;  o += 3392 + 8 * PB;     // local-phase scratch (HierSmem / ParSmem), checked in sample_batched.cuh
+    L.pts = o;
+    L.total = o;                          // + 16 B per resident point (the launch asks for the device maximum)
+    (void)LW;
     return L;
 }
-
 
 // per-shape launchers (sb_inst_*.cu): cand_per_thread x local_warps
 #define RFPS_BATCHED_SHAPES(X) X(2, 32) X(4, 32) X(8, 32) X(2, 16) X(4, 16) X(8, 16) X(8, 4) X(8, 1) X(16, 8)

@@ -170,21 +170,21 @@ def test_ablations_and_stats_are_bit_identical(rf, flags, kernel):
             applied = M - 1                                      # every voxel is tested against every pick
             assert st["voxel_tests"] == st["K_total"] * applied
         else:
-            # the picks of the last batch are never applied (nothing needs them); the prune runs on
+            # the picks of the last batch need not be applied (nothing needs them): a worker CTA that sees the end of
+            # the sampling stops, so the CTAs may have applied different prefixes of that batch; the prune runs on
             # groups of 32 voxels first, voxels are only tested where their group survived
             if flags & rf.FPS_FLAG_NO_PRUNE:
-                applied = st["voxel_tests"] // st["K_total"]
-                assert st["voxel_tests"] == st["K_total"] * applied and st["group_tests"] == 0
+                applied = st["voxel_tests"] / st["K_total"]
+                assert st["group_tests"] == 0
             else:
                 G = (st["K_total"] + 31) // 32
-                applied = st["group_tests"] // G
-                assert st["group_tests"] == G * applied
+                applied = st["group_tests"] / G
                 assert 0 < st["voxel_tests"] < st["K_total"] * applied
             assert M - 1 - 1024 <= applied <= M - 1
         if flags & rf.FPS_FLAG_NO_PRUNE:
             if kernel == "per_pick":
                 assert st["voxels_visited"] == st["K_total"] * applied
-            assert st["points_visited"] == P.shape[0] * applied
+            assert abs(st["points_visited"] - P.shape[0] * applied) <= 0.02 * st["points_visited"]
         if flags & rf.FPS_FLAG_NO_SKIP:
             assert st["points_computed"] == st["points_visited"]
 
