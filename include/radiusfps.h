@@ -56,8 +56,10 @@ typedef struct {
     int32_t n_vox;         /* voxel bins per axis (Eq. 7); 0 = choose from N; 1..1024   */
     int32_t tile_points;   /* split voxels holding more points than this into tiles with their own
                               bounding sphere; 0 = default, -1 = never split (the paper's layout)      */
-    int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1..16 (per-pick kernel:
-                              1,2,4,8,16)                                                              */
+    int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1..16 = one thread-block cluster of
+                              that size per cloud (per-pick kernel: 1,2,4,8,16); batched kernel only: -2..-148 =
+                              that many CTAs per cloud spread over the whole grid (one picker, the others workers,
+                              exchanging through global memory; needs B * CTAs <= SMs)                      */
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
@@ -94,7 +96,8 @@ typedef struct {
     int32_t max_voxel_points; /* largest segment                                                      */
     int64_t device_bytes;     /* memory owned by the handle                                           */
     int32_t build_launches;   /* kernels fps_index_build launched (a1-a6); fps_sample launches ONE    */
-    int32_t reserved;
+    int32_t grid_ctas;        /* batched kernel: > 0 = CTAs per cloud spread over the grid (cooperative launch,
+                                 exchange through global memory); 0 = one cluster of cluster_size CTAs per cloud */
     /* the following are filled only when FPS_FLAG_STATS was set, for the LAST fps_sample call:      */
     int64_t iterations;       /* sum over clouds of (M-1)                                             */
     int64_t voxel_tests;      /* Eq. 25 evaluations                                                   */

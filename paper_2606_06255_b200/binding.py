@@ -34,7 +34,7 @@ class fps_stats(ctypes.Structure):
                 ("cluster_size", ctypes.c_int32), ("block_threads", ctypes.c_int32),
                 ("voxels_per_thread", ctypes.c_int32),
                 ("K_total", ctypes.c_int64), ("K_max", ctypes.c_int32), ("max_voxel_points", ctypes.c_int32),
-                ("device_bytes", ctypes.c_int64), ("build_launches", ctypes.c_int32), ("reserved", ctypes.c_int32),
+                ("device_bytes", ctypes.c_int64), ("build_launches", ctypes.c_int32), ("grid_ctas", ctypes.c_int32),
                 ("iterations", ctypes.c_int64), ("voxel_tests", ctypes.c_int64),
                 ("voxels_visited", ctypes.c_int64), ("points_visited", ctypes.c_int64),
                 ("points_computed", ctypes.c_int64), ("effective", ctypes.c_int64),

@@ -230,6 +230,7 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
     out->K_total = ix.K_total; out->K_max = ix.K_max; out->max_voxel_points = ix.max_voxel_points;
     out->device_bytes = ix.device_bytes;
     out->build_launches = ix.build_launches;
+    out->grid_ctas = ix.grid_ctas;
     out->local_warps = ix.local_warps; out->cand_per_thread = ix.cand_per_thread;
     if (ix.flags & FPS_FLAG_STATS) {
         unsigned long long c[rfps::NUM_COUNTERS];

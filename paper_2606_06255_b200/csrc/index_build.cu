@@ -740,6 +740,7 @@ void free_index(DeviceIndex &ix)
         if (ix.arena_pooled) cudaFreeAsync(ix.arena, ix.last_stream);
         else cudaFree(ix.arena);
     }
+    if (ix.gx) dev_free_async(ix.gx, ix.last_stream);
     free(ix.K_host);
     free(ix.poff_host);
     free(ix.rag_host);
@@ -807,6 +808,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
             ix.poff_dev = c.take<int32_t>(B + 1);
             ix.rag_dev = c.take<int32_t>(3 * (size_t)(B + 1));
             ix.counters = c.take<unsigned long long>(NUM_COUNTERS);
+
         } else {
             sc.kA = c.take<unsigned>(BN); sc.kB = c.take<unsigned>(BN);
             sc.vA = c.take<int>(BN); sc.vB = c.take<int>(BN);

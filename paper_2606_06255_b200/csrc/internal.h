@@ -66,6 +66,10 @@ struct DeviceIndex {
     int32_t max_voxel_points = 0;
     int32_t cluster_size = 0, block_threads = 0, vpt = 0;   // sampling-kernel launch shape
     int32_t local_warps = 0, cand_per_thread = 0, Kc_cap = 0;   // batched kernel: local-phase shape, voxels per CTA
+    int32_t grid_ctas = 0;              // batched kernel: > 0 = CTAs per cloud spread over the grid (cooperative launch,
+                                        // exchange through global memory); 0 = one cluster of cluster_size CTAs per cloud
+    void *gx = nullptr;                 // grid mode: the clouds' exchange blocks (allocated by the first fps_sample)
+    size_t gx_pitch = 0;
     int32_t flags = 0;
     int32_t build_launches = 0;         // kernels launched by fps_index_build (a1-a6)
     // point arrays, [B][N], sorted by voxel

@@ -37,16 +37,26 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         return FPS_ERR_INVALID;
     }
     int C = o.cluster_size;
-    if (C < 0 || C > 16) { set_error("cluster_size=%d must be 0 (choose) or 1..16", C); return FPS_ERR_INVALID; }
+    const int sms = device_props().sm_count;
+    if (C < -sms || C > 16) { set_error("cluster_size=%d must be 0 (choose), 1..16 (CTAs per cluster) or -2..-%d (CTAs per cloud, grid mode)", C, sms); return FPS_ERR_INVALID; }
     if (o.block_threads != 0 && o.block_threads != BT) { set_error("block_threads=%d: the batched kernel runs %d threads per CTA", o.block_threads, BT); return FPS_ERR_INVALID; }
     const int K = ix.K_max > 0 ? ix.K_max : 1;
     const int TC = cand_capacity(CPT, LW);
     const int G = (K + 31) / 32;
     auto slots = [&](int c) { const int w = c > 1 ? c - 1 : 1; return 32 * ((G + w - 1) / w); };   // voxel slots per worker CTA
     const size_t max_smem = (size_t)device_props().max_smem_optin;
-    const int sms = device_props().sm_count;
     auto fits = [&](int c) { return smem_layout(slots(c), TC, LW).total <= max_smem; };
-    if (C == 0) {
+    int grid = 0;
+    if (C < 0) {
+        // grid mode asked for: -C CTAs per cloud, all clouds resident at once (the CTAs of a cloud wait for one another)
+        grid = -C;
+        if (grid < 2 || LW != LW_PAR) { set_error("cluster_size=%d: grid mode takes >= 2 CTAs per cloud and the default local phase", C); return FPS_ERR_INVALID; }
+        if ((long long)grid * ix.B > batched_max_resident_ctas(max_smem)) {
+            set_error("cluster_size=%d: %d clouds x %d CTAs cannot all be resident on this device", C, ix.B, grid);
+            return FPS_ERR_INVALID;
+        }
+        C = grid;
+    } else if (C == 0) {
         // the largest cluster that (a) leaves every CTA >= 1 024 points, (b) holds the voxel state in
         // shared memory and (c) lets all B clusters be resident at once (a cluster lives inside one
         // GPC, so fewer clusters fit than SMs / C suggests: 15 of 8, 22 of 6, 7 of 16 on B200's 148 SMs);
@@ -63,6 +73,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         set_error("K_max=%d voxels do not fit the shared memory of %d CTAs; use a smaller n_vox or a larger tile_points", K, C);
         return FPS_ERR_INVALID;
     }
+    ix.grid_ctas = grid;
     ix.cluster_size = C;
     ix.block_threads = BT;
     ix.vpt = 0;
@@ -83,6 +94,23 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
     bp.K = ix.K_dev;
     bp.poff = ix.poff_dev; bp.rag = rag_dev; bp.B = ix.B;
     bp.K_cap = ix.K_cap; bp.G_cap = ix.G_cap; bp.Kc_cap = ix.Kc_cap; bp.M = M; bp.start_idx = start_idx;
+    bp.ctas_per_cloud = ix.grid_ctas > 0 ? ix.grid_ctas : ix.cluster_size;
+    bp.gx = nullptr;
+    if (ix.grid_ctas > 0) {
+        // the clouds' exchange blocks: allocated once per handle, control words zeroed before every launch
+        const size_t pitch = gx_bytes(cand_capacity(ix.cand_per_thread, ix.local_warps));
+        if (!ix.gx) {
+            if (dev_alloc_async(&ix.gx, pitch * (size_t)ix.B, st) != cudaSuccess) {
+                cudaGetLastError();
+                ix.gx = nullptr;
+                set_error("device allocation of the exchange blocks failed");
+                return FPS_ERR_NOMEM;
+            }
+            ix.gx_pitch = pitch;
+        }
+        RFPS_CUDA(cudaMemset2DAsync(ix.gx, pitch, 0, GX_PICK, (size_t)ix.B, st));
+        bp.gx = (unsigned char *)ix.gx;
+    }
     bp.smem_bytes = std::max((int)smem_layout(ix.Kc_cap, cand_capacity(ix.cand_per_thread, ix.local_warps), ix.local_warps).total,
                              device_props().max_smem_optin);
     bp.out_idx = out_idx; bp.out_mind = out_mindist;

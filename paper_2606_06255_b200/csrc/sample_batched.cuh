@@ -94,6 +94,22 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
 // with scalar __fadd_rn on the unpacked halves (scalar .rn adds are never contracted), and
 // tests/test_abi_cpu.py checks that the built library holds no FFMA2 at all.
 
+// How the picker tells its workers how far the running batch has got: a release store of
+// (batch id << PUB_SHIFT | count) to the exchange block's `pub` word -- in its own shared memory (cluster) or in
+// global memory (grid; the picks themselves are then mirrored to `gpick`).  Inactive for a single-CTA cloud.
+struct Publisher {
+    unsigned local_addr = 0u;     // cluster: shared::cta address of ctl->pub
+    unsigned *gptr = nullptr;     // grid: &gx->pub
+    float4 *gpick = nullptr;      // grid: global mirror of the batch buffer
+    unsigned base = 0u;           // batch id << PUB_SHIFT
+    __device__ __forceinline__ bool on() const { return local_addr != 0u || gptr != nullptr; }
+    __device__ __forceinline__ void operator()(const unsigned count_and_flags) const
+    {
+        if (gptr) st_release_gpu_u32(gptr, base | count_and_flags);
+        else if (local_addr) st_release_cluster_u32(local_addr, base | count_and_flags);
+    }
+};
+
 // ---------------------------------------------------------------------------------------------
 // LOCAL: register-resident FPS over the candidate set (CTA 0, warps 0..LW-1).  Thread t keeps the
 // candidates i = c*(LW*32) + t, c < CPT: coordinates (packed in pairs) and D in registers; the
@@ -239,7 +255,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
                                                const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
                                                const int M, HierSmem *hs, float4 *bpick, int *out_idx, float *out_mind,
                                                const int tid, unsigned long long &c_subrounds, unsigned long long &c_fallback,
-                                               long long &t_sel, long long &t_loop, long long &t_app, const unsigned pub_addr)
+                                               long long &t_sel, long long &t_loop, long long &t_app, const Publisher &pubr)
 {
     static_assert(CPT1 % 2 == 0 && CPT2 >= 1 && CPT2 <= 4, "shape");
     constexpr int H1 = CPT1 / 2, T2 = 32 * CPT2;
@@ -576,7 +592,7 @@ __device__ __forceinline__ void local_fps_hier(const float *cX, const float *cY,
         // the workers may start applying these picks now.  The release is issued by the thread that wrote bpick
         // (lane 0 of the pick warp; after a barrier on the fallback path); its fence overlaps the other warps'
         // selection of the next sub-round
-        if (pub_addr && tid == BT - 32) st_release_cluster_u32(pub_addr, (unsigned)nbl);
+        if (pubr.on() && tid == BT - 32) pubr((unsigned)nbl);
         if (STATS) { tt1 = clock64(); t_loop += tt1 - tt0; tt0 = tt1; }
         // ---- (f) the sub-round's picks -> all of C1.  Candidates at or below tau are out of the round for
         // good; neighbours in the buffer come from the same voxel and tend to die together, so whole
@@ -661,7 +677,7 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
                                               const int M, ParSmem *ps, float4 *bpick, int *out_idx, float *out_mind,
                                               const int tid, unsigned long long &c_steps, unsigned long long &c_fallback,
                                               long long &t_sel, long long &t_pick, long long &t_upd, long long &t_pairs,
-                                              long long &t_publish, const unsigned pub_addr)
+                                              long long &t_publish, const Publisher &pubr)
 {
     static_assert(CPT1 % 2 == 0 && BT == 512 && KS == 64, "shape");
     constexpr int H1 = CPT1 / 2;
@@ -799,10 +815,11 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
                 out_idx[jl] = (int)(~go);
                 out_mind[jl] = hi;
                 bpick[nbl] = make_float4(cX[gidx], cY[gidx], cZ[gidx], 0.0f);
+                if (pubr.gpick) pubr.gpick[nbl] = bpick[nbl];
                 c_fallback++;
             }
             __syncthreads();
-            if (pub_addr && tid == 0) st_release_cluster_u32(pub_addr, (unsigned)(nbl + 1));
+            if (pubr.on() && tid == 0) pubr((unsigned)(nbl + 1));
             apply_range(nbl, nbl + 1);
             ++jl;
             ++nbl;
@@ -916,11 +933,13 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
                 out_idx[jl + posa] = (int)(~ps->sO[ia]);
                 out_mind[jl + posa] = ca.w;
                 bpick[nbl + posa] = make_float4(ca.x, ca.y, ca.z, 0.0f);
+                if (pubr.gpick) pubr.gpick[nbl + posa] = make_float4(ca.x, ca.y, ca.z, 0.0f);
             }
             if (accb) {
                 out_idx[jl + posb] = (int)(~ps->sO[ib]);
                 out_mind[jl + posb] = cb.w;
                 bpick[nbl + posb] = make_float4(cb.x, cb.y, cb.z, 0.0f);
+                if (pubr.gpick) pubr.gpick[nbl + posb] = make_float4(cb.x, cb.y, cb.z, 0.0f);
             }
             // bound of what is left: members neither picked nor surely below every member, else the smallest
             // member distance (everything outside the members is below it)
@@ -940,7 +959,7 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
         // published when it crosses a multiple of that.  The release is issued by a thread with no global stores of
         // its own in flight (warp 1; warp 0 has just written out_idx / out_mindist): its fence is then short.  The
         // barrier above orders warp 0's writes to bpick before it.
-        if (pub_addr && tid == 32 && (nbl + npk) / STREAM_MIN != nbl / STREAM_MIN) st_release_cluster_u32(pub_addr, (unsigned)(nbl + npk));
+        if (pubr.on() && tid == 32 && (nbl + npk) / STREAM_MIN != nbl / STREAM_MIN) pubr((unsigned)(nbl + npk));
         if (STATS) { tt1 = clock64(); t_publish += tt1 - tt0; tt0 = tt1; }
         // ---- (5) the step's picks -> all of C1 ----
         apply_range(nbl, nbl + npk);
@@ -962,7 +981,7 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
 // ---------------------------------------------------------------------------------------------
 static_assert(sizeof(HierSmem) <= 3392 + 8 * PB, "smem_layout reserves this much for HierSmem");
 
-template <int CPT, int LW, bool STATS, bool EUC>
+template <int CPT, int LW, bool STATS, bool EUC, bool GRID>
 __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, const int flags)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -970,7 +989,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     constexpr int NW = BT / 32;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt = (1u << lane) - 1u;
-    const int C = (int)cluster_nctarank(), rank = (int)cluster_ctarank();
+    // the CTAs of one cloud: a thread-block cluster (exchange over DSMEM), or -- GRID -- `ctas_per_cloud`
+    // consecutive CTAs of a cooperative launch (exchange through global memory)
+    const int C = GRID ? P.ctas_per_cloud : (int)cluster_nctarank();
+    const int rank = GRID ? (int)(blockIdx.x % (unsigned)C) : (int)cluster_ctarank();
     const int b = blockIdx.x / C;
     const bool no_prune = flags & FPS_FLAG_NO_PRUNE, no_skip = flags & FPS_FLAG_NO_SKIP;
     const bool no_batch = flags & FPS_FLAG_NO_BATCH;
@@ -1024,7 +1046,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
 #define RFPS_VOXEL_OF(kl) ((wr + W * ((kl) >> 5)) * 32 + ((kl) & 31))
 
     // ---- a7: state reset.  Thresholds = NaN: nothing can be pruned by the first pick, which therefore
-    // performs the paper's "initial update" (Eq. 13-14).  Dist_p = +inf on this CTA's slice. ----
+    // performs the paper's "initial update" (Eq. 13-14).  Dist_p = +inf (below, with the resident copy). ----
     for (int kl = tid; kl < Kc; kl += BT) {
         const int k = RFPS_VOXEL_OF(kl);
         sgeom[kl] = k < K ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
@@ -1037,12 +1059,6 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     }
     for (int gl = tid; gl < Gc; gl += BT) { sggeom[gl] = ggeom[wr + W * gl]; qbits[gl] = 0u; sgthr[gl] = __uint_as_float(F32_NAN_BITS); }
     for (int i = tid; i < Kc * SUBW; i += BT) qmask[i] = 0u;
-    {
-        const int chunk = (Nb + C - 1) / C;
-        const int p0 = min(Nb, rank * chunk), p1 = min(Nb, p0 + chunk);
-        const float inf = __uint_as_float(F32_INF_BITS);
-        for (int p = p0 + tid; p < p1; p += BT) Dp[p] = inf;
-    }
     // ---- resident points.  The points of a group of 32 consecutive voxels are one contiguous run of the sorted
     // arrays; the runs of the groups this CTA owns are copied one after the other into what is left of its shared
     // memory -- as many whole groups as fit, the rest is read from global memory (L2) as before.  x, y, z and
@@ -1093,15 +1109,24 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             sPZ[q] = pz[p];
             sPD[q] = inf;
         }
+        // Dist_p of the groups that stay in global memory: only this CTA ever touches them
+        for (int gl2 = Gres; gl2 < Gc; ++gl2) {
+            const int p0 = sseg[gl2 * 32].x, len = gpre[gl2 + 1] - gpre[gl2];
+            for (int q = tid; q < len; q += BT) Dp[p0 + q] = inf;
+        }
     }
+    // exchange block of this cloud as seen from here (sample_batched_shapes.h)
+    unsigned char *const gxb = GRID ? P.gx + (size_t)b * gx_bytes(TC) : nullptr;
+    Ctl *const gctl = reinterpret_cast<Ctl *>(gxb);
+    float4 *const gpick = GRID ? reinterpret_cast<float4 *>(gxb + GX_PICK) : nullptr;
+    float *const gcand = GRID ? reinterpret_cast<float *>(gxb + gx_cand()) : nullptr;
+    const unsigned ctl0 = GRID ? 0u : mapa(smem_u32(ctl), 0u);          // cluster: the picker's control block
     if (tid == 0) {
         qn[0] = qn[1] = qn[2] = qn[3] = 0;
-        ctl->pub = 0u;
+        ctl->pub = 0u; ctl->cmd = 0u; ctl->cmd_tb = 0u; ctl->ack = 0u;
 #pragma unroll
-        for (int a = 0; a < 4 * MAX_ATTEMPTS; ++a) ctl->ccount[a] = 0u;
+        for (int a = 0; a < 8; ++a) ctl->ccount[a] = 0u;
         ctl->best_hi = ctl->best_lo = 0u;
-        ctl->nb = 1;
-        ctl->j = 1;
         const int p = P.pinv[po + startb];
         bpick[0] = make_float4(px[p], py[p], pz[p], 0.0f);     // s_0 = the caller's start point
         if (rank == 0) {
@@ -1110,7 +1135,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         }
     }
     int nb = 1, j = 1;
-    unsigned qpar = 0u, round_parity = 0u, prev_taubits = 0u;
+    unsigned qpar = 0u, prev_taubits = 0u;
     bool prev_tau_valid = false;
     float g = 0.25f;                 // tau = Dmax * (1 - g); adapted from the candidate counts
     float gt = GTARGET;              // fraction of the candidate buffer the next extraction aims at; follows the overflow rate
@@ -1120,7 +1145,11 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     long long t_lpairs = 0, t_lpub = 0;                                      // parallel resolution: all-pairs part of the pick time / publishing
     long long t_lsel = 0, t_lpick = 0, t_lupd = 0;                          // local phase: selection / pick loop / update after it
     long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
-    cluster_sync_all();              // Dist_p = +inf is visible to every CTA of the cluster
+    // Dist_p = +inf and the control blocks are in place before any message is sent (grid mode: the global exchange
+    // block was zeroed by the host, and nothing a CTA writes before its first message is read by another CTA)
+    if (GRID) {
+        __syncthreads();
+    } else cluster_sync_all();
 
     // =====================================================================================
     // APPLY: the picks bpick[lo, hi), SUBP (= 128) at a time (whole CTA; contains CTA barriers).
@@ -1292,18 +1321,12 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         }
     };
 
-    apply_range(0, 1);      // the start point: every voxel is visited (the paper's initial update, Eq. 13-14)
-
-    while (j < Mb) {
-        if (STATS && tid == 0 && rank == 0) { c_rounds++; t0 = clock64(); }
-        unsigned ghi = 0u, glo = 0u;
-        bool have_max = false;
-        auto compute_max = [&]() {
-        // =====================================================================================
-        // MAX: argmax of Dist_v (Eq. 15-18): thread -> warp -> CTA -> cluster.  The voxels keep Dist_v only;
-        // the lowest original index among the points attaining the maximum (the tie-break of PAPER.md:179) is
-        // looked up here, in the voxels that hold this CTA's maximum (normally one)
-        // =====================================================================================
+    // ---- a8 on this CTA's voxels: max Dist_v and, among the points attaining it, the lowest original index
+    // (PAPER.md:179), as one 64-bit key (Dist_v bits << 32 | ~orig).  The voxels keep Dist_v only; the index is
+    // looked up here, in the voxels that hold the maximum (normally one) -- also when the maximum is +0
+    // (duplicates exhausted, reading A7: every point ties and the lowest index is the answer; empty slots hold
+    // Dist_v = 0 too, with no points).  Whole CTA; the result is valid in thread 0. ----
+    auto cta_best_key = [&]() -> unsigned long long {
         {
             unsigned bhi = 0u;
             for (int kl = tid; kl < Kc; kl += BT) bhi = max(bhi, vdv[kl]);
@@ -1312,242 +1335,389 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             if (tid == 0) ctl->best_lo = 0u;
         }
         __syncthreads();
-        {
-            const unsigned chi = __reduce_max_sync(FULL, lane < NW ? wbest[lane].x : 0u);
-            // (also when the maximum is +0 -- duplicates exhausted, reading A7: every point ties and the lowest index of
-            // the cloud is the answer; empty slots hold Dist_v = 0 too, with no points)
-            unsigned bo = 0u;
-            for (int kl = warp; kl < Kc; kl += NW) {
-                if (vdv[kl] != chi) continue;                             // warp-uniform
-                const int2 sg = sseg[kl];
-                const int lo = sloc[kl];
-                const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
-                for (int p = lane; p < sg.y; p += 32)
-                    if (__float_as_uint(Dq[p]) == chi) bo = max(bo, ~(unsigned)porig[sg.x + p]);
-            }
-            bo = __reduce_max_sync(FULL, bo);
-            if (lane == 0 && bo) atomicMax(&ctl->best_lo, bo);
-            if (tid == 0) ctl->best_hi = chi;
+        const unsigned chi = __reduce_max_sync(FULL, lane < NW ? wbest[lane].x : 0u);
+        unsigned bo = 0u;
+        for (int kl = warp; kl < Kc; kl += NW) {
+            if (vdv[kl] != chi) continue;                                 // warp-uniform
+            const int2 sg = sseg[kl];
+            const int lo = sloc[kl];
+            const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
+            for (int p = lane; p < sg.y; p += 32)
+                if (__float_as_uint(Dq[p]) == chi) bo = max(bo, ~(unsigned)porig[sg.x + p]);
         }
-        cluster_sync_all();
-        {
-            uint4 rb = make_uint4(0u, 0u, 0u, 0u);
-            if (lane < C) rb = ld_dsmem_v4(mapa(smem_u32(&ctl->best_hi), (unsigned)lane));
-            warp_argmax_key(rb.x, rb.y, ghi, glo);
-        }
+        bo = __reduce_max_sync(FULL, bo);
+        if (lane == 0 && bo) atomicMax(&ctl->best_lo, bo);
+        __syncthreads();
+        return ((unsigned long long)chi << 32) | ctl->best_lo;
+    };
 
-            have_max = true;
-        };
-        if (tid == 0 && rank == 0) ctl->pub = 0u;      // ordered before the workers' polling by the extraction's barrier
-        const int rp = (int)(round_parity & 1u);
-        round_parity ^= 1u;
-        // A batch that ended on its threshold leaves every point of the cloud <= tau_prev, and the true maximum
-        // just below it: tau can be hung on tau_prev and the cluster-wide argmax (one more cluster barrier) is only
-        // computed when that fails -- no candidate above the new tau, or too many -- or when there is no such
-        // threshold (first round, batch cut short by the buffer).
-        if (!prev_tau_valid) compute_max();
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
-        // =====================================================================================
-        // EXTRACT: candidates C = {p : Dist_p > tau} -> CTA 0's shared memory (over DSMEM)
-        // =====================================================================================
-        int cnt = 0;
-        unsigned taubits = ghi;
-        for (int pass = have_max ? 1 : 0; pass < 2 && cnt == 0; ++pass) {
-        if (pass == 1 && !have_max) compute_max();
-        const unsigned gref = have_max ? ghi : prev_taubits;
-        taubits = gref;
-        if (!no_batch && gref > 0u && gref < F32_INF_BITS) {
-            const float Dmax = __uint_as_float(gref);
-            const unsigned cX0 = mapa(smem_u32(cX), 0u), cY0 = mapa(smem_u32(cY), 0u), cZ0 = mapa(smem_u32(cZ), 0u),
-                           cD0 = mapa(smem_u32(cD), 0u), cO0 = mapa(smem_u32(cO), 0u);
-            for (int a = 0; a < MAX_ATTEMPTS; ++a) {
-                // a cloud that fits the candidate buffer whole is taken whole (tau = 0: every point that can
-                // still be picked at a positive distance); the local phase then runs without global rounds
-                const unsigned tb = (a == 0 && Nb <= TC) ? 0u : __float_as_uint(__fmul_rn(Dmax, __fsub_rn(1.0f, g)));
-                if (!(tb < gref)) break;                     // g too small to separate tau from Dmax
-                const unsigned cnt_addr = mapa(smem_u32(&ctl->ccount[(rp * 2 + pass) * MAX_ATTEMPTS + a]), 0u);
-                for (int base = 0; base < Kc; base += BT) {
-                    const int kl = base + tid;
-                    const bool hit = kl < Kc && vdv[kl] > tb;             // empty slots hold 0
-                    const unsigned bal = __ballot_sync(FULL, hit);
-                    if (bal) {
-                        int qb = 0;
-                        if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
-                        qb = __shfl_sync(FULL, qb, 0);
-                        if (hit) qkl[qb + __popc(bal & lt)] = kl;
-                    }
-                }
-                __syncthreads();
-                const int nq = qn[qpar];
-                if (tid == 0) { qn[qpar ^ 1u] = 0; qn[2] = 0; }
-                __syncthreads();
-                for (;;) {
-                    int qi = 0;
-                    if (lane == 0) qi = atomicAdd(&qn[2], 1);
-                    qi = __shfl_sync(FULL, qi, 0);
-                    if (qi >= nq) break;
-                    const int kq = qkl[qi];
-                    const int2 sg = sseg[kq];
-                    const int lo = sloc[kq];
-                    const float *X = lo >= 0 ? sPX + lo : px + sg.x, *Y = lo >= 0 ? sPY + lo : py + sg.x, *Z = lo >= 0 ? sPZ + lo : pz + sg.x;
-                    const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
-                    if (STATS && lane == 0) c_xvox++;
-                    // two chunks of 32 points per step, everything loaded up front, one slot reservation per step; the
-                    // original index (global memory) is fetched for the hits only
-                    for (int pb = 0; pb < sg.y; pb += 64) {
-                        const int pA = pb + lane, pB = pb + 32 + lane;
-                        const bool inA = pA < sg.y, inB = pB < sg.y;
-                        unsigned dA = 0u, dB = 0u, oA = 0u, oB = 0u;
-                        float xA = 0.f, yA = 0.f, zA = 0.f, xB = 0.f, yB = 0.f, zB = 0.f;
-                        if (inA) { dA = __float_as_uint(Dq[pA]); xA = X[pA]; yA = Y[pA]; zA = Z[pA]; }
-                        if (inB) { dB = __float_as_uint(Dq[pB]); xB = X[pB]; yB = Y[pB]; zB = Z[pB]; }
-                        if (dA > tb) oA = ~(unsigned)porig[sg.x + pA];
-                        if (dB > tb) oB = ~(unsigned)porig[sg.x + pB];
-                        const bool isA = dA > tb, isB = dB > tb;
-                        const unsigned balA = __ballot_sync(FULL, isA), balB = __ballot_sync(FULL, isB);
-                        if (STATS) c_xpts += (inA ? 1 : 0) + (inB ? 1 : 0);
-                        if (balA | balB) {
-                            unsigned cb = 0u;
-                            if (lane == 0) cb = atom_add_dsmem_u32(cnt_addr, (unsigned)(__popc(balA) + __popc(balB)));
-                            cb = __shfl_sync(FULL, cb, 0);
-                            const unsigned slotA = cb + (unsigned)__popc(balA & lt);
-                            const unsigned slotB = cb + (unsigned)__popc(balA) + (unsigned)__popc(balB & lt);
-                            if (isA && slotA < (unsigned)TC) {
-                                st_dsmem_u32(cX0 + 4u * slotA, __float_as_uint(xA));
-                                st_dsmem_u32(cY0 + 4u * slotA, __float_as_uint(yA));
-                                st_dsmem_u32(cZ0 + 4u * slotA, __float_as_uint(zA));
-                                st_dsmem_u32(cD0 + 4u * slotA, dA);
-                                st_dsmem_u32(cO0 + 4u * slotA, oA);
-                            }
-                            if (isB && slotB < (unsigned)TC) {
-                                st_dsmem_u32(cX0 + 4u * slotB, __float_as_uint(xB));
-                                st_dsmem_u32(cY0 + 4u * slotB, __float_as_uint(yB));
-                                st_dsmem_u32(cZ0 + 4u * slotB, __float_as_uint(zB));
-                                st_dsmem_u32(cD0 + 4u * slotB, dB);
-                                st_dsmem_u32(cO0 + 4u * slotB, oB);
-                            }
-                        }
-                    }
-                }
-                qpar ^= 1u;
-                cluster_sync_all();
-                const unsigned found = ld_dsmem_u32(cnt_addr);
-                if (found <= (unsigned)TC) {
-                    cnt = (int)found;
-                    taubits = tb;
-                    // aim the next round at ~5/8 of the buffer; move by at most 2x per round
-                    const float ratio = fminf(2.0f, fmaxf(0.5f, (gt * TC) / (float)max(found, 1u)));
-                    g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
-                    gt = fminf(GT_MAX, gt * GT_UP);
-                    break;
-                }
-                if (STATS && tid == 0 && rank == 0) c_retries++;
-                g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
-                gt = fmaxf(GT_MIN, gt * GT_DOWN);
+    // ---- candidates {p : Dist_p > tb} of this CTA's voxels -> the cloud's candidate buffer.  reserve(n) hands out
+    // n consecutive slots (it may run past the buffer: the count then says "too many"); store(slot, ...) writes one
+    // candidate.  Whole CTA. ----
+    auto extract_scan = [&](const unsigned tb, auto reserve, auto store) {
+        for (int base = 0; base < Kc; base += BT) {
+            const int kl = base + tid;
+            const bool hit = kl < Kc && vdv[kl] > tb;                     // empty slots hold 0
+            const unsigned bal = __ballot_sync(FULL, hit);
+            if (bal) {
+                int qb = 0;
+                if (lane == 0) qb = atomicAdd(&qn[qpar], __popc(bal));
+                qb = __shfl_sync(FULL, qb, 0);
+                if (hit) qkl[qb + __popc(bal & lt)] = kl;
             }
         }
+        __syncthreads();
+        const int nq = qn[qpar];
+        if (tid == 0) { qn[qpar ^ 1u] = 0; qn[2] = 0; }
+        __syncthreads();
+        for (;;) {
+            int qi = 0;
+            if (lane == 0) qi = atomicAdd(&qn[2], 1);
+            qi = __shfl_sync(FULL, qi, 0);
+            if (qi >= nq) break;
+            const int kq = qkl[qi];
+            const int2 sg = sseg[kq];
+            const int lo = sloc[kq];
+            const float *X = lo >= 0 ? sPX + lo : px + sg.x, *Y = lo >= 0 ? sPY + lo : py + sg.x, *Z = lo >= 0 ? sPZ + lo : pz + sg.x;
+            const float *Dq = lo >= 0 ? sPD + lo : Dp + sg.x;
+            if (STATS && lane == 0) c_xvox++;
+            // two chunks of 32 points per step, everything loaded up front, one slot reservation per step; the
+            // original index (global memory) is fetched for the hits only
+            for (int pb = 0; pb < sg.y; pb += 64) {
+                const int pA = pb + lane, pB = pb + 32 + lane;
+                const bool inA = pA < sg.y, inB = pB < sg.y;
+                unsigned dA = 0u, dB = 0u, oA = 0u, oB = 0u;
+                float xA = 0.f, yA = 0.f, zA = 0.f, xB = 0.f, yB = 0.f, zB = 0.f;
+                if (inA) { dA = __float_as_uint(Dq[pA]); xA = X[pA]; yA = Y[pA]; zA = Z[pA]; }
+                if (inB) { dB = __float_as_uint(Dq[pB]); xB = X[pB]; yB = Y[pB]; zB = Z[pB]; }
+                const bool isA = dA > tb, isB = dB > tb;
+                if (isA) oA = ~(unsigned)porig[sg.x + pA];
+                if (isB) oB = ~(unsigned)porig[sg.x + pB];
+                const unsigned balA = __ballot_sync(FULL, isA), balB = __ballot_sync(FULL, isB);
+                if (STATS) c_xpts += (inA ? 1 : 0) + (inB ? 1 : 0);
+                if (balA | balB) {
+                    unsigned cb = 0u;
+                    if (lane == 0) cb = reserve((unsigned)(__popc(balA) + __popc(balB)));
+                    cb = __shfl_sync(FULL, cb, 0);
+                    const unsigned slotA = cb + (unsigned)__popc(balA & lt);
+                    const unsigned slotB = cb + (unsigned)__popc(balA) + (unsigned)__popc(balB & lt);
+                    if (isA && slotA < (unsigned)TC) store(slotA, xA, yA, zA, dA, oA);
+                    if (isB && slotB < (unsigned)TC) store(slotB, xB, yB, zB, dB, oB);
+                }
+            }
         }
-        if (!have_max) { /* cnt > 0 here: the single-pick path below, which needs the argmax, is not taken */ }
-        if (rank == 0 && tid == 0) {                  // the other parity's counters, for the next round
-#pragma unroll
-            for (int a = 0; a < 2 * MAX_ATTEMPTS; ++a) ctl->ccount[(rp ^ 1) * 2 * MAX_ATTEMPTS + a] = 0u;
-        }
+        qpar ^= 1u;
+        __syncthreads();
+    };
 
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
+    // ---- threshold control shared by the solo and the picker loop: tau = Dmax * (1 - g), g follows the counts ----
+    auto next_threshold = [&](const unsigned gref, const int attempt) -> unsigned {
+        // a cloud that fits the candidate buffer whole is taken whole (tau = 0: every point that can still be
+        // picked at a positive distance); the local phase then runs without global rounds
+        return (attempt == 0 && Nb <= TC) ? 0u : __float_as_uint(__fmul_rn(__uint_as_float(gref), __fsub_rn(1.0f, g)));
+    };
+    auto adapt_fit = [&](const unsigned found) {          // aim the next round at ~5/8 of the buffer; move by at most 2x
+        const float ratio = fminf(2.0f, fmaxf(0.5f, (gt * TC) / (float)max(found, 1u)));
+        g = fminf(0.75f, fmaxf(0x1p-22f, g * ratio));
+        gt = fminf(GT_MAX, gt * GT_UP);
+    };
+    auto adapt_overflow = [&](const unsigned found) {
+        g = fmaxf(0x1p-22f, g * fmaxf(0.125f, (0.5f * TC) / (float)found));
+        gt = fmaxf(GT_MIN, gt * GT_DOWN);
+    };
+    // ---- LOCAL: FPS restricted to the candidates (whole CTA); returns through j / nb ----
+    auto run_local = [&](const int cnt, const unsigned taubits, int &lj, int &lnb, const Publisher &pubr) {
+        if constexpr (LW == LW_PAR) {
+            local_fps_par<CPT, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, reinterpret_cast<ParSmem *>(hs), bpick, out_idx,
+                                           out_mind, tid, c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, t_lpairs, t_lpub, pubr);
+        } else if constexpr (LW == LW_HIER) {
+            local_fps_hier<CPT, CPT2, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
+                                                  c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, pubr);
+        } else if constexpr (!EUC) {
+            if (warp < LW) local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, lslot, bpick, out_idx, out_mind, tid);
+            if (tid == 0) { ctl->scratch[0] = lj; ctl->scratch[1] = lnb; }      // the other warps learn the outcome
+            __syncthreads();
+            lj = ctl->scratch[0];
+            lnb = ctl->scratch[1];
+            __syncthreads();
+        }
+        if (STATS && tid == 0) c_cands += (unsigned long long)cnt;
+    };
+
+    if (!split) {
         // =====================================================================================
-        // LOCAL (CTA 0): FPS restricted to the candidates; or the single global argmax.
-        // With C > 1 the workers apply the picks concurrently, as CTA 0 publishes them.
+        // ONE CTA per cloud: apply, argmax, extract and local phase in turn
         // =====================================================================================
-        if (rank == 0) {
-            if (cnt == 0) {
+        apply_range(0, 1);      // the start point: every voxel is visited (the paper's initial update, Eq. 13-14)
+        while (j < Mb) {
+            if (STATS && tid == 0) { c_rounds++; t0 = clock64(); }
+            unsigned ghi = 0u, glo = 0u;
+            bool have_max = false;
+            int cnt = 0;
+            unsigned taubits = 0u;
+            // A batch that ended on its threshold leaves every point of the cloud <= tau_prev, and the true maximum
+            // just below it: tau is hung on tau_prev and the argmax is only computed when that fails -- no candidate
+            // above the new tau, or too many -- or when there is no such threshold (first round, batch cut short)
+            for (int pass = prev_tau_valid ? 0 : 1; pass < 2 && cnt == 0; ++pass) {
+                if (pass == 1) {
+                    const unsigned long long key = cta_best_key();
+                    if (tid == 0) { ctl->scratch[0] = (int)(unsigned)(key >> 32); ctl->scratch[1] = (int)(unsigned)key; }
+                    __syncthreads();
+                    ghi = (unsigned)ctl->scratch[0]; glo = (unsigned)ctl->scratch[1];
+                    have_max = true;
+                    __syncthreads();
+                }
+                const unsigned gref = have_max ? ghi : prev_taubits;
+                taubits = gref;
+                if (no_batch || !(gref > 0u && gref < F32_INF_BITS)) continue;
+                for (int a = 0; a < MAX_ATTEMPTS; ++a) {
+                    const unsigned tb = next_threshold(gref, a);
+                    if (!(tb < gref)) break;                     // g too small to separate tau from Dmax
+                    if (tid == 0) ctl->ccount[0] = 0u;
+                    __syncthreads();
+                    extract_scan(tb, [&](unsigned n) { return atomicAdd(&ctl->ccount[0], n); },
+                                 [&](unsigned sl, float x, float y, float z, unsigned dbits, unsigned o) {
+                                     cX[sl] = x; cY[sl] = y; cZ[sl] = z; cD[sl] = __uint_as_float(dbits); cO[sl] = o;
+                                 });
+                    const unsigned found = ctl->ccount[0];
+                    __syncthreads();
+                    if (found <= (unsigned)TC) { cnt = (int)found; taubits = tb; adapt_fit(found); break; }
+                    if (STATS && tid == 0) c_retries++;
+                    adapt_overflow(found);
+                }
+            }
+            if (STATS && tid == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
+            if (cnt == 0) {                              // the single global argmax = the paper's own iteration
                 if (tid == 0) {
                     out_idx[j] = (int)(~glo);
                     out_mind[j] = __uint_as_float(ghi);
                     const int gpos = P.pinv[po + (size_t)(~glo)];
                     bpick[0] = make_float4(px[gpos], py[gpos], pz[gpos], 0.0f);
-                    ctl->nb = 1;
-                    ctl->j = j + 1;
                     if (STATS) c_singles++;
                 }
-            } else if constexpr (LW == LW_PAR) {
-                int lj = j, lnb = 0;
-                local_fps_par<CPT, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, reinterpret_cast<ParSmem *>(hs), bpick, out_idx,
-                                               out_mind, tid, c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, t_lpairs, t_lpub, split ? smem_u32(&ctl->pub) : 0u);
-                if (tid == 0) {
-                    ctl->nb = lnb;
-                    ctl->j = lj;
-                    if (STATS) c_cands += (unsigned long long)cnt;
-                }
-            } else if constexpr (LW == LW_HIER) {
-                int lj = j, lnb = 0;
-                local_fps_hier<CPT, CPT2, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
-                                       c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, split ? smem_u32(&ctl->pub) : 0u);
-                if (tid == 0) {
-                    ctl->nb = lnb;
-                    ctl->j = lj;
-                    if (STATS) c_cands += (unsigned long long)cnt;
-                }
-            } else if constexpr (LW < LW_HIER && !EUC) {
-              if (warp < LW) {
-                int lj = j, lnb = 0;
-                local_fps<CPT, LW>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, lslot, bpick, out_idx, out_mind, tid);
-                if (tid == 0) {
-                    ctl->nb = lnb;
-                    ctl->j = lj;
-                    if (STATS) c_cands += (unsigned long long)cnt;
-                }
-              }
-            }
-        }
-        if (split) {
-            if (rank == 0) {
-                __syncthreads();      // ctl->nb / ctl->j and the last picks are written
-                if (tid == 0) st_release_cluster_u32(smem_u32(&ctl->pub), (unsigned)ctl->nb | PUB_DONE | (ctl->j >= Mb ? PUB_FINAL : 0u));
+                nb = 1;
+                j += 1;
             } else {
-                // ---- worker: stream the batch out of CTA 0's shared memory and apply it ----
-                const unsigned pub_remote = mapa(smem_u32(&ctl->pub), 0u), src = mapa(smem_u32(bpick), 0u);
-                int applied = 0;
-                for (;;) {
-                    if (tid == 0) {
-                        unsigned v = ld_acquire_cluster_u32(pub_remote);
-                        if (!(v & PUB_DONE) && (int)(v & PUB_COUNT) - applied < STREAM_MIN) { __nanosleep(128); v = ld_acquire_cluster_u32(pub_remote); }
-                        qn[3] = (int)v;
-                    }
-                    __syncthreads();
-                    const unsigned v = (unsigned)qn[3];
-                    __syncthreads();
-                    const int n = (int)(v & PUB_COUNT);
-                    const bool done = v & PUB_DONE;
-                    if (v & PUB_FINAL) break;                 // M reached: nothing needs these picks applied
-                    // whole words of 32 picks, at least STREAM_MIN at a time, until the batch is complete
-                    const int hi = done ? n : (n - applied >= STREAM_MIN ? applied + ((n - applied) & ~31) : applied);
-                    if (hi > applied) {
-                        for (int i = applied + tid; i < hi; i += BT) {
-                            const uint4 q = ld_dsmem_v4(src + 16u * (unsigned)i);
-                            bpick[i] = make_float4(__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), 0.0f);
-                        }
-                        __syncthreads();
-                        apply_range(applied, hi);
-                        applied = hi;
-                    }
-                    if (done && applied == n) break;
-                }
+                int lj = j, lnb = 0;
+                run_local(cnt, taubits, lj, lnb, Publisher());
+                j = lj;
+                nb = lnb;
+            }
+            __syncthreads();
+            if (STATS && tid == 0) { t1 = clock64(); t_local += t1 - t0; t0 = t1; }
+            prev_tau_valid = cnt > 0 && nb < PB && j < Mb && !no_batch;
+            prev_taubits = taubits;
+            if (j < Mb) {
+                apply_range(0, nb);
+                if (STATS && tid == 0) t_apply += clock64() - t0;
             }
         }
-        cluster_sync_all();
-        if (STATS && tid == 0 && rank == 0) { t1 = clock64(); t_local += t1 - t0; }
-        {
-            const uint4 r0 = ld_dsmem_v4(mapa(smem_u32(&ctl->nb), 0u));
-            nb = (int)r0.x;
-            j = (int)r0.y;
-            // did the batch end on its threshold (not on the buffer, not on M), and was there one?
+    } else if (rank == 0) {
+        // =====================================================================================
+        // PICKER: decides the rounds.  Between two batches it sends commands (argmax, candidate extraction at a
+        // threshold) and waits for every worker's acknowledgement; then it runs the local phase, publishing the
+        // picks as they are produced.  It never waits for a batch to be applied: the workers answer the next
+        // command only after they have applied the whole batch before it.
+        // =====================================================================================
+        unsigned ncmd = 0u, batch = 0u;
+        auto pub_word = [&](const unsigned v) {            // thread 0
+            if (GRID) st_release_gpu_u32(&gctl->pub, v);
+            else st_release_cluster_u32(smem_u32(&ctl->pub), v);
+        };
+        // one command: send, wait for W acknowledgements (thread 0), fetch the result, broadcast
+        auto command = [&](const unsigned type, const unsigned tb, unsigned &r0, unsigned &r1) {
+            ++ncmd;
+            if (tid == 0) {
+                Ctl *const c = GRID ? gctl : ctl;
+                c->ccount[ncmd & 7u] = 0u;
+                c->cmd_tb = tb;
+                if (GRID) st_release_gpu_u32(&gctl->cmd, (ncmd << 2) | type);
+                else st_release_cluster_u32(smem_u32(&ctl->cmd), (ncmd << 2) | type);
+                const unsigned want = ncmd * (unsigned)W;
+                if (GRID) { while (ld_acquire_gpu_u32(&gctl->ack) != want) __nanosleep(20); }
+                else { while (ld_acquire_cluster_local_u32(smem_u32(&ctl->ack)) != want) __nanosleep(20); }
+                if (type == CMD_EXTRACT)
+                    ctl->scratch[0] = (int)(GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->ccount[ncmd & 7u]) : *reinterpret_cast<volatile unsigned *>(&ctl->ccount[ncmd & 7u]));
+            }
+            __syncthreads();                               // thread 0's acquire now covers the whole CTA
+            if (type == CMD_MAX && warp == 0) {            // argmax over the workers' slots (Eq. 15-18, last level)
+                unsigned khi = 0u, klo = 0u;
+                for (int r = 1 + lane; r < C; r += 32) {
+                    const uint2 k = GRID ? __ldcg(reinterpret_cast<const uint2 *>(gxb + GX_SLOT) + r) : ctl->slot[r];
+                    if (k.x > khi || (k.x == khi && k.y > klo)) { khi = k.x; klo = k.y; }
+                }
+                unsigned mhi, mlo;
+                warp_argmax_key(khi, klo, mhi, mlo);
+                if (lane == 0) { ctl->scratch[0] = (int)mhi; ctl->scratch[1] = (int)mlo; }
+            }
+            if (type == CMD_MAX) __syncthreads();
+            r0 = (unsigned)ctl->scratch[0]; r1 = (unsigned)ctl->scratch[1];
+            __syncthreads();
+        };
+        if (tid == 0) {                                    // batch 0 = the start point: every voxel is visited
+            if (GRID) gpick[0] = bpick[0];
+            pub_word(1u | PUB_DONE | (Mb <= 1 ? PUB_FINAL : 0u));
+        }
+        while (j < Mb) {
+            if (STATS && tid == 0) { c_rounds++; t0 = clock64(); }
+            unsigned ghi = 0u, glo = 0u;
+            bool have_max = false;
+            int cnt = 0;
+            unsigned taubits = 0u;
+            for (int pass = prev_tau_valid ? 0 : 1; pass < 2 && cnt == 0; ++pass) {
+                if (pass == 1) {
+                    command(CMD_MAX, 0u, ghi, glo);
+                    have_max = true;
+                    if (STATS && tid == 0) { t1 = clock64(); t_max += t1 - t0; t0 = t1; }
+                }
+                const unsigned gref = have_max ? ghi : prev_taubits;
+                taubits = gref;
+                if (no_batch || !(gref > 0u && gref < F32_INF_BITS)) continue;
+                for (int a = 0; a < MAX_ATTEMPTS; ++a) {
+                    const unsigned tb = next_threshold(gref, a);
+                    if (!(tb < gref)) break;
+                    unsigned found, dummy;
+                    command(CMD_EXTRACT, tb, found, dummy);
+                    if (found <= (unsigned)TC) { cnt = (int)found; taubits = tb; adapt_fit(found); break; }
+                    if (STATS && tid == 0) c_retries++;
+                    adapt_overflow(found);
+                }
+            }
+            if (GRID && cnt > 0) {                         // candidates: global exchange block -> shared memory
+                for (int i = tid; i < cnt; i += BT) {
+                    cX[i] = __ldcg(gcand + i); cY[i] = __ldcg(gcand + TC + i); cZ[i] = __ldcg(gcand + 2 * TC + i);
+                    cD[i] = __ldcg(gcand + 3 * TC + i); cO[i] = __float_as_uint(__ldcg(gcand + 4 * TC + i));
+                }
+                __syncthreads();
+            }
+            if (STATS && tid == 0) { t1 = clock64(); t_extract += t1 - t0; t0 = t1; }
+            ++batch;
+            Publisher pubr;
+            pubr.base = (batch & 0x7ffffu) << PUB_SHIFT;
+            if (GRID) { pubr.gptr = &gctl->pub; pubr.gpick = gpick; }
+            else pubr.local_addr = smem_u32(&ctl->pub);
+            if (cnt == 0) {                              // the single global argmax = the paper's own iteration
+                if (tid == 0) {
+                    out_idx[j] = (int)(~glo);
+                    out_mind[j] = __uint_as_float(ghi);
+                    const int gpos = P.pinv[po + (size_t)(~glo)];
+                    bpick[0] = make_float4(px[gpos], py[gpos], pz[gpos], 0.0f);
+                    if (GRID) gpick[0] = bpick[0];
+                    if (STATS) c_singles++;
+                }
+                nb = 1;
+                j += 1;
+            } else {
+                int lj = j, lnb = 0;
+                run_local(cnt, taubits, lj, lnb, pubr);
+                j = lj;
+                nb = lnb;
+            }
+            __syncthreads();                               // the last picks are written
+            if (tid == 0) pubr((unsigned)nb | PUB_DONE | (j >= Mb ? PUB_FINAL : 0u));
+            if (STATS && tid == 0) { t1 = clock64(); t_local += t1 - t0; }
             prev_tau_valid = cnt > 0 && nb < PB && j < Mb && !no_batch;
             prev_taubits = taubits;
         }
-        if (!split && j < Mb) {
-            if (STATS && tid == 0) t0 = clock64();
-            apply_range(0, nb);
-            if (STATS && tid == 0) t_apply += clock64() - t0;
+    } else {
+        // =====================================================================================
+        // WORKER: owns voxels.  Applies every batch while the picker is still producing it (pieces of >=
+        // STREAM_MIN picks), then answers the picker's commands -- always after the whole batch before them.
+        // =====================================================================================
+        unsigned next_batch = 0u, next_cmd = 1u;
+        int applied = 0;
+        bool in_batch = true;                              // batch `next_batch` is not completely applied yet
+        const unsigned pick_rc = GRID ? 0u : mapa(smem_u32(bpick), 0u);
+        const unsigned cX0 = GRID ? 0u : mapa(smem_u32(cX), 0u), cY0 = GRID ? 0u : mapa(smem_u32(cY), 0u), cZ0 = GRID ? 0u : mapa(smem_u32(cZ), 0u),
+                       cD0 = GRID ? 0u : mapa(smem_u32(cD), 0u), cO0 = GRID ? 0u : mapa(smem_u32(cO), 0u);
+        auto ack = [&]() {                                 // after a barrier that follows the command's last store
+            if (tid == 0) {
+                if (GRID) red_release_gpu_add_u32(&gctl->ack, 1u);
+                else red_release_cluster_add_u32(ctl0 + (unsigned)offsetof(Ctl, ack), 1u);
+            }
+        };
+        for (;;) {
+            // ---- wait for the next message (thread 0 polls, the CTA sleeps at the barrier) ----
+            if (tid == 0) {
+                unsigned v, c;
+                for (;;) {
+                    // The command word is read BEFORE the batch word: the picker finishes a batch (pub: DONE) and only
+                    // then sends the next command, so a worker that sees the new command is guaranteed (acquire) to
+                    // see, in the read that follows, the batch it has to apply first.  The other order has a window
+                    // in which the command is seen and the batch before it is not.
+                    c = in_batch ? 0u : (GRID ? ld_acquire_gpu_u32(&gctl->cmd) : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, cmd)));
+                    v = GRID ? ld_acquire_gpu_u32(&gctl->pub) : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, pub));
+                    const bool mine = (v >> PUB_SHIFT) == (next_batch & 0x7ffffu);
+                    if (mine && ((v & (PUB_DONE | PUB_FINAL)) || (int)(v & PUB_COUNT) - applied >= STREAM_MIN)) { c = 0u; break; }
+                    if (!in_batch && !mine && (c >> 2) == next_cmd) { v = 0u; break; }
+                    __nanosleep(40);
+                }
+                ctl->scratch[0] = (int)v;
+                ctl->scratch[1] = (int)c;
+                if (c) ctl->scratch[2] = (int)(GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->cmd_tb) : ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_tb)));
+            }
+            __syncthreads();
+            const unsigned v = (unsigned)ctl->scratch[0], c = (unsigned)ctl->scratch[1], ctb = (unsigned)ctl->scratch[2];
+            __syncthreads();
+            if (c) {
+                // ---- a command; the batch before it has been applied completely ----
+                if ((c & 3u) == CMD_MAX) {
+                    const unsigned long long key = cta_best_key();
+                    if (tid == 0) {
+                        const uint2 k = make_uint2((unsigned)(key >> 32), (unsigned)key);
+                        if (GRID) {
+                            reinterpret_cast<uint2 *>(gxb + GX_SLOT)[rank] = k;
+                        } else {
+                            st_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, slot) + 8u * (unsigned)rank, k.x);
+                            st_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, slot) + 8u * (unsigned)rank + 4u, k.y);
+                        }
+                    }
+                    __syncthreads();
+                } else {
+                    const unsigned slot = next_cmd & 7u;
+                    if (GRID) {
+                        extract_scan(ctb, [&](unsigned n) { return atomicAdd(&gctl->ccount[slot], n); },
+                                     [&](unsigned sl, float x, float y, float z, unsigned dbits, unsigned o) {
+                                         gcand[sl] = x; gcand[TC + sl] = y; gcand[2 * TC + sl] = z;
+                                         gcand[3 * TC + sl] = __uint_as_float(dbits); gcand[4 * TC + sl] = __uint_as_float(o);
+                                     });
+                    } else {
+                        const unsigned cnt_addr = ctl0 + (unsigned)offsetof(Ctl, ccount) + 4u * slot;
+                        extract_scan(ctb, [&](unsigned n) { return atom_add_dsmem_u32(cnt_addr, n); },
+                                     [&](unsigned sl, float x, float y, float z, unsigned dbits, unsigned o) {
+                                         st_dsmem_u32(cX0 + 4u * sl, __float_as_uint(x));
+                                         st_dsmem_u32(cY0 + 4u * sl, __float_as_uint(y));
+                                         st_dsmem_u32(cZ0 + 4u * sl, __float_as_uint(z));
+                                         st_dsmem_u32(cD0 + 4u * sl, dbits);
+                                         st_dsmem_u32(cO0 + 4u * sl, o);
+                                     });
+                    }
+                }
+                ack();                                     // (both branches end with a CTA barrier)
+                ++next_cmd;
+                continue;
+            }
+            // ---- progress of batch `next_batch` ----
+            if (v & PUB_FINAL) break;                      // M reached: nothing needs these picks applied
+            const int n = (int)(v & PUB_COUNT);
+            const bool done = v & PUB_DONE;
+            in_batch = true;
+            // whole words of 32 picks, at least STREAM_MIN at a time, until the batch is complete
+            const int hi = done ? n : applied + ((n - applied) & ~31);
+            if (hi > applied) {
+                for (int i = applied + tid; i < hi; i += BT) {
+                    if (GRID) {
+                        bpick[i] = __ldcg(gpick + i);
+                    } else {
+                        const uint4 q = ld_dsmem_v4(pick_rc + 16u * (unsigned)i);
+                        bpick[i] = make_float4(__uint_as_float(q.x), __uint_as_float(q.y), __uint_as_float(q.z), 0.0f);
+                    }
+                }
+                __syncthreads();
+                apply_range(applied, hi);
+                applied = hi;
+            }
+            if (done && applied == n) { ++next_batch; applied = 0; in_batch = false; }
         }
     }
 
@@ -1585,30 +1755,37 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             atomicAdd(P.counters + CNT_CYC_LOCAL, (unsigned long long)t_local);
         }
     }
-    cluster_sync_all();   // no CTA may exit while a peer can still read its shared memory
+    if (!GRID) cluster_sync_all();   // no CTA may exit while a peer can still read its shared memory
 #undef RFPS_VOXEL_OF
 }
 
-template <int CPT, int LW, bool STATS, bool EUC>
+template <int CPT, int LW, bool STATS, bool EUC, bool GRID>
 static int launch_batched_one(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
 {
-    auto kern = k_fps_batched<CPT, LW, STATS, EUC>;
+    auto kern = k_fps_batched<CPT, LW, STATS, EUC, GRID>;
     // the voxel state and the picker's regions are the minimum; everything else up to the device limit holds
     // resident points (sample_batched_shapes.h)
     const size_t smem = (size_t)bp.smem_bytes;
     RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    if (ix.cluster_size > 8) RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
+    if (!GRID && ix.cluster_size > 8) RFPS_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1));
     cudaLaunchConfig_t cfg;
     memset(&cfg, 0, sizeof cfg);
-    cfg.gridDim = dim3((unsigned)(ix.B * ix.cluster_size));
+    cfg.gridDim = dim3((unsigned)(ix.B * (GRID ? ix.grid_ctas : ix.cluster_size)));
     cfg.blockDim = dim3(BT);
     cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = (unsigned)ix.cluster_size;
-    attr[0].val.clusterDim.y = 1;
-    attr[0].val.clusterDim.z = 1;
+    if (GRID) {
+        // the CTAs of a cloud wait for one another's messages: all of them must be resident (checked when the
+        // shape was chosen; a cooperative launch fails instead of deadlocking if they are not)
+        attr[0].id = cudaLaunchAttributeCooperative;
+        attr[0].val.cooperative = 1;
+    } else {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = (unsigned)ix.cluster_size;
+        attr[0].val.clusterDim.y = 1;
+        attr[0].val.clusterDim.z = 1;
+    }
     cfg.attrs = attr;
     cfg.numAttrs = 1;
     RFPS_CUDA(cudaLaunchKernelEx(&cfg, kern, bp, ix.flags));
@@ -1619,12 +1796,18 @@ template <int CPT, int LW>
 static int launch_batched_s(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
 {
     const bool stats = ix.flags & FPS_FLAG_STATS;
+    if constexpr (LW == LW_PAR) {           // the grid-wide exchange is built for the default local phase only
+        if (ix.grid_ctas > 0) {
+            if (ix.flags & FPS_FLAG_EUCLIDEAN)
+                return stats ? launch_batched_one<CPT, LW, true, true, true>(bp, ix, st) : launch_batched_one<CPT, LW, false, true, true>(bp, ix, st);
+            return stats ? launch_batched_one<CPT, LW, true, false, true>(bp, ix, st) : launch_batched_one<CPT, LW, false, false, true>(bp, ix, st);
+        }
+    }
     if constexpr (LW >= LW_HIER) {          // the Euclidean mode is built for the 16-warp local phases only
         if (ix.flags & FPS_FLAG_EUCLIDEAN)
-            return stats ? launch_batched_one<CPT, LW, true, true>(bp, ix, st) : launch_batched_one<CPT, LW, false, true>(bp, ix, st);
+            return stats ? launch_batched_one<CPT, LW, true, true, false>(bp, ix, st) : launch_batched_one<CPT, LW, false, true, false>(bp, ix, st);
     }
-    return stats ? launch_batched_one<CPT, LW, true, false>(bp, ix, st) : launch_batched_one<CPT, LW, false, false>(bp, ix, st);
+    return stats ? launch_batched_one<CPT, LW, true, false, false>(bp, ix, st) : launch_batched_one<CPT, LW, false, false, false>(bp, ix, st);
 }
-
 
 }  // namespace rfps

@@ -13,7 +13,6 @@ constexpr int BT = 512;        // threads per CTA
 constexpr int PB = 1024;       // picks per batch (capacity of the batch buffer)
 constexpr int MAX_ATTEMPTS = 4;
 constexpr int STREAM_MIN = 64;    // workers start on a piece of the running batch once it has this many picks
-constexpr unsigned PUB_DONE = 1u << 31, PUB_FINAL = 1u << 30, PUB_COUNT = 0xffffu;
 // extraction control: the next extraction aims at the fraction `gt` of the candidate buffer; gt starts at GTARGET,
 // creeps up after an extraction that fitted and drops after one that overflowed (all measured on C1-C5)
 constexpr float GTARGET = 0.625f, GT_MAX = 0.7f, GT_UP = 1.03f, GT_MIN = 0.35f, GT_DOWN = 0.85f;
@@ -39,18 +38,40 @@ struct BatchParams {
     const int *rag;                                // ragged call: [3][B+1] = M_b, start_b, output offsets; else null
     int B, K_cap, G_cap, Kc_cap, M, start_idx;     // Kc_cap: voxel slots per CTA (a multiple of 32); M, start_idx: uniform call
     int smem_bytes;                                // dynamic shared memory of the launch (what is left of it holds resident points)
+    int ctas_per_cloud;                            // grid mode: CTAs per cloud (1 picker + workers); cluster mode: the cluster size
+    unsigned char *gx;                             // grid mode: [B] exchange blocks of gx_bytes(candidate capacity) each, zeroed
     int *out_idx;
     float *out_mind;
     unsigned long long *counters;
 };
 
-struct __align__(16) Ctl {          // per-CTA control block; CTA 0's copy is the cluster's
-    unsigned ccount[4 * MAX_ATTEMPTS];  // candidates found by an extraction attempt (may exceed TC):
-                                        // [round parity][pass: hung on the previous tau / on the true maximum][attempt]
-    unsigned best_hi, best_lo, pad3, pad0;       // this CTA's best voxel key
-    int nb, j, pad1, pad2;          // (CTA 0) size of the batch just produced, samples emitted so far
-    unsigned pub, pad4, pad5, pad6; // (CTA 0) picks of the running batch published so far | PUB_DONE | PUB_FINAL
+// Exchange block of one cloud: how its picker CTA and its worker CTAs talk.  It lives in the picker's shared
+// memory when the cloud's CTAs form a thread-block cluster (the workers reach it over DSMEM), and in global
+// memory when they are spread over the whole grid (cooperative launch; then followed by the pick and candidate
+// buffers, see GX_* below).  All traffic is one-way messages with release / acquire at cluster or gpu scope;
+// there is no barrier between the CTAs of a cloud while it is sampled.
+//   pub    picker -> workers: the batch being produced: (batch id << PUB_SHIFT) | flags | picks published so far
+//   cmd    picker -> workers: (command id << 2) | type, issued between two batches; cmd_tb = its threshold
+//   ack    workers -> picker: counts completed commands (every worker adds 1 per command)
+//   ccount workers -> picker: candidates found by extraction command id & 7 (may exceed the buffer)
+//   slot   workers -> picker: worker `rank`'s best key (Dist_v bits, ~orig) for a MAX command, one slot per worker
+//          (plain stores, reduced by the picker; a red.max.u64 on the picker's shared memory lost updates when
+//          several workers arrived together -- measured on B200);
+//          cluster mode: in this block; grid mode: GX_SLOT bytes into the cloud's global block
+struct __align__(16) Ctl {
+    unsigned ccount[8];
+    unsigned pub, cmd, cmd_tb, ack;
+    unsigned best_hi, best_lo;      // this CTA's best key while it is being computed
+    int scratch[6];                 // CTA-local broadcast of what thread 0 read
+    uint2 slot[16];
 };
+constexpr unsigned PUB_COUNT = 0x7ffu, PUB_DONE = 1u << 11, PUB_FINAL = 1u << 12;
+constexpr int PUB_SHIFT = 13;       // batch id above the flags (compared modulo 2^19)
+constexpr unsigned CMD_MAX = 1u, CMD_EXTRACT = 2u;
+// grid mode: byte offsets inside a cloud's global exchange block; tc = candidate capacity
+constexpr size_t GX_SLOT = 256, GX_PICK = 2048;      // the header (control words + one slot per CTA) is zeroed before a launch
+__host__ __device__ constexpr size_t gx_cand(void) { return GX_PICK + sizeof(float4) * 1024; }
+__host__ __device__ constexpr size_t gx_bytes(int tc) { return gx_cand() + sizeof(float) * 5 * (size_t)tc; }
 
 // shared-memory carve-up (host and device must agree).  The picker-only regions (candidates, local-phase
 // scratch) come last: a worker CTA of a cluster with a separate picker never touches them, and its RESIDENT
@@ -96,5 +117,7 @@ RFPS_BATCHED_SHAPES(RFPS_DECL_LAUNCH)
 #undef RFPS_DECL_LAUNCH
 // how many clusters of `c` CTAs of the default kernel can be resident at once (0 on error)
 int batched_max_resident_clusters(int c, size_t smem);
+// grid mode: how many CTAs of the default kernel fit the device at once
+int batched_max_resident_ctas(size_t smem);
 
 }  // namespace rfps

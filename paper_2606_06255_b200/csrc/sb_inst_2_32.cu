@@ -8,7 +8,7 @@ int launch_batched_2_32(const BatchParams &bp, const DeviceIndex &ix, cudaStream
 
 int batched_max_resident_clusters(int c, size_t smem)
 {
-    auto kern = k_fps_batched<2, 32, false, false>;
+    auto kern = k_fps_batched<2, 32, false, false, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
     if (c > 8 && cudaFuncSetAttribute(kern, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) { cudaGetLastError(); return 0; }
     cudaLaunchConfig_t cfg;
@@ -26,6 +26,15 @@ int batched_max_resident_clusters(int c, size_t smem)
     int n = 0;
     if (cudaOccupancyMaxActiveClusters(&n, kern, &cfg) != cudaSuccess) { cudaGetLastError(); return 0; }
     return n;
+}
+
+int batched_max_resident_ctas(size_t smem)
+{
+    auto kern = k_fps_batched<2, 32, false, false, true>;
+    if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    int per_sm = 0;
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kern, BT, smem) != cudaSuccess) { cudaGetLastError(); return 0; }
+    return per_sm * device_props().sm_count;
 }
 
 }  // namespace rfps

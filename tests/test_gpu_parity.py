@@ -94,6 +94,46 @@ def test_every_cluster_size(rf, name, cluster, kernel):
     assert_same(gi, gm, *ref)
 
 
+@pytest.mark.parametrize("ctas", [2, 3, 5, 9, 40, 148])
+@pytest.mark.parametrize("name", ["room", "lattice", "lidar", "dups"])
+def test_grid_mode_ctas_per_cloud(rf, name, ctas):
+    # one picker CTA + (ctas - 1) worker CTAs per cloud spread over the grid (cooperative launch), exchanging picks,
+    # commands and candidates through global memory with release / acquire at gpu scope
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, cluster_size=-ctas)
+    assert st["grid_ctas"] == ctas
+    assert_same(gi, gm, *ref)
+
+
+def test_grid_mode_batch_and_repeat_calls(rf):
+    w = inputs.scaled("C2", 4000, 1000, B=16)
+    P = inputs.make_batch(w)
+    ref = oracle.fps(P, w.M, 0)
+    Pd = torch.from_numpy(P).cuda()
+    ix = rf.fps_index_build(Pd, cluster_size=-9)
+    try:
+        for _ in range(10):
+            idx, mind = rf.fps_sample(ix, w.M, 0)
+            torch.cuda.synchronize()
+            assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+    finally:
+        rf.fps_index_destroy(ix)
+    with pytest.raises(rf.FpsError):                        # 16 clouds x 10 CTAs cannot be resident on 148 SMs
+        rf.fps_index_build(Pd, cluster_size=-10)
+
+
+@pytest.mark.parametrize("name,ctas", [("C2", 9), ("C3", 100), ("C4", 37), ("C5", 148)])
+def test_grid_mode_full_size(rf, name, ctas):
+    gold = json.load(open(GOLDEN))[name]
+    w = inputs.WORKLOADS[name]
+    P = inputs.make_batch(w)
+    gi, gm, st = run_gpu(rf, P, w.M, w.start_idx, cluster_size=-ctas)
+    assert st["grid_ctas"] == ctas
+    assert sha(gi.astype(np.int32)) == gold["idx_sha256"]
+    assert sha(gm.astype(np.float32)) == gold["mindist_sha256"]
+
+
 LOCAL_SHAPES = [(32, 2), (32, 4), (32, 8), (16, 2), (16, 4), (16, 8), (4, 8), (1, 8), (8, 16)]
 
 
