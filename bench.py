@@ -241,7 +241,9 @@ def phase_ms(st: dict, sm_mhz) -> dict:
                        "local_select": f("cycles_local_select"), "local_pick": f("cycles_local_pick"),
                        "local_update": f("cycles_local_update"), "local_pairs": f("cycles_local_pairs"),
                        "local_publish": f("cycles_local_publish"), "apply_if_single_cta": f("cycles_apply")},
-            "worker_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum")}}
+            "worker_avg": {"prune_tests": g("cycles_prune_sum"), "point_visits": g("cycles_visit_sum"),
+                           "tail_after_done": g("cycles_worker_tail"), "extract_scan": g("cycles_worker_extract"),
+                           "idle": g("cycles_worker_idle"), "pieces": st.get("worker_pieces", 0) / workers}}
 
 
 def sha(a) -> str:

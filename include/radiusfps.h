@@ -129,6 +129,10 @@ typedef struct {
                                  to the candidates after it                                                    */
     int64_t cycles_local_pairs, cycles_local_publish;   /* parallel resolution: the all-pairs part of cycles_local_pick;
                                  publishing a step's picks to the workers (release at cluster scope)          */
+    int64_t cycles_worker_tail, cycles_worker_extract, cycles_worker_idle;   /* worker CTAs, thread 0, summed over all
+                                 workers: applying what is left of a batch once it is declared complete / the candidate
+                                 extraction scans / waiting for the next message                              */
+    int64_t worker_pieces;    /* pieces of <= 128 picks applied, summed over all workers                       */
 } fps_stats;
 
 /*

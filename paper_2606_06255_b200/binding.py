@@ -48,7 +48,9 @@ class fps_stats(ctypes.Structure):
                 ("local_warps", ctypes.c_int32), ("cand_per_thread", ctypes.c_int32),
                 ("cycles_local_select", ctypes.c_int64), ("cycles_local_pick", ctypes.c_int64),
                 ("cycles_local_update", ctypes.c_int64), ("cycles_local_pairs", ctypes.c_int64),
-                ("cycles_local_publish", ctypes.c_int64)]
+                ("cycles_local_publish", ctypes.c_int64), ("cycles_worker_tail", ctypes.c_int64),
+                ("cycles_worker_extract", ctypes.c_int64), ("cycles_worker_idle", ctypes.c_int64),
+                ("worker_pieces", ctypes.c_int64)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

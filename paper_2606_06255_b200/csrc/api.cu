@@ -254,6 +254,8 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
             out->local_subrounds = (int64_t)c[24]; out->local_fallbacks = (int64_t)c[25];
             out->cycles_local_select = (int64_t)c[21]; out->cycles_local_pick = (int64_t)c[22]; out->cycles_local_update = (int64_t)c[23];
             out->cycles_local_pairs = (int64_t)c[26]; out->cycles_local_publish = (int64_t)c[27];
+            out->cycles_worker_tail = (int64_t)c[28]; out->cycles_worker_extract = (int64_t)c[29];
+            out->cycles_worker_idle = (int64_t)c[30]; out->worker_pieces = (int64_t)c[31];
         }
     }
     return FPS_OK;

@@ -45,7 +45,7 @@
 namespace rfps {
 
 enum { CNT_VTEST = 0, CNT_VVISIT, CNT_PVISIT, CNT_PCOMP, CNT_EFF, CNT_ROUNDS, CNT_RETRIES, CNT_SINGLES, CNT_CANDS,
-       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_LSEL, CNT_LPICK, CNT_LUPD, CNT_SUBROUNDS, CNT_FALLBACK, CNT_LPAIRS, CNT_LPUB, CNT_N };
+       CNT_XVOX, CNT_XPTS, CNT_CYC_APPLY, CNT_CYC_MAX, CNT_CYC_EXTRACT, CNT_CYC_LOCAL, CNT_GTEST, CNT_CYC_A_SUM, CNT_CYC_B_SUM, CNT_CYC_A_MAX, CNT_CYC_B_MAX, CNT_SUBS, CNT_LSEL, CNT_LPICK, CNT_LUPD, CNT_SUBROUNDS, CNT_FALLBACK, CNT_LPAIRS, CNT_LPUB, CNT_W_TAIL, CNT_W_XSCAN, CNT_W_IDLE, CNT_W_PIECES, CNT_N };
 
 // ---------------------------------------------------------------------------------------------
 // packed fp32x2 arithmetic (sm_100: FADD2 / FMUL2).  Each half is an ordinary IEEE round-to-nearest
@@ -1205,6 +1205,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     long long t_lpairs = 0, t_lpub = 0;                                      // parallel resolution: all-pairs part of the pick time / publishing
     long long t_lsel = 0, t_lpick = 0, t_lupd = 0;                          // local phase: selection / pick loop / update after it
     long long t_a = 0, t_b = 0, ta0 = 0, n_subs = 0;                        // every CTA / thread 0
+    long long t_wtail = 0, t_wx = 0, t_widle = 0, tw0 = 0;                  // workers / thread 0: applying what is left when a batch is
+                                                                            // declared complete, extraction scans, waiting for messages
     // Dist_p = +inf and the control blocks are in place before any message is sent (grid mode: the global exchange
     // block was zeroed by the host, and nothing a CTA writes before its first message is read by another CTA)
     if (GRID) {
@@ -1709,6 +1711,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         for (;;) {
             // ---- wait for the next message (thread 0 polls, the CTA sleeps at the barrier) ----
             if (tid == 0) {
+                if (STATS) tw0 = clock64();
                 unsigned v, c;
                 for (;;) {
                     // The command word is read BEFORE the batch word: the picker finishes a batch (pub: DONE) and only
@@ -1726,6 +1729,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     }
                     __nanosleep(40);
                 }
+                if (STATS) t_widle += clock64() - tw0;
                 ctl->scratch[0] = (int)v;
                 ctl->scratch[1] = (int)c;
                 if (c) ctl->scratch[2] = (int)(GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->cmd_tb) : ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_tb)));
@@ -1749,6 +1753,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     __syncthreads();
                 } else {
                     const unsigned slot = next_cmd & 7u;
+                    if (STATS && tid == 0) tw0 = clock64();
                     if (GRID) {
                         extract_scan(ctb, [&](unsigned n) { return atomicAdd(&gctl->ccount[slot], n); },
                                      [&](unsigned sl, float x, float y, float z, unsigned dbits, unsigned o) {
@@ -1767,6 +1772,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                                      });
                     }
                 }
+                if (STATS && tid == 0 && (c & 3u) == CMD_EXTRACT) t_wx += clock64() - tw0;
                 ack();                                     // (both branches end with a CTA barrier)
                 ++next_cmd;
                 continue;
@@ -1779,6 +1785,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             // whole words of 32 picks, at least STREAM_MIN at a time, until the batch is complete
             const int hi = done ? n : applied + ((n - applied) & ~31);
             if (hi > applied) {
+                if (STATS && tid == 0) tw0 = clock64();
                 for (int i = applied + tid; i < hi; i += BT) {
                     if (GRID) {
                         bpick[i] = __ldcg(gpick + i);
@@ -1790,6 +1797,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                 __syncthreads();
                 apply_range(applied, hi);
                 applied = hi;
+                if (STATS && tid == 0 && done) t_wtail += clock64() - tw0;
             }
             if (done && applied == n) { ++next_batch; applied = 0; in_batch = false; }
         }
@@ -1809,6 +1817,10 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             atomicAdd(P.counters + CNT_CYC_B_SUM, (unsigned long long)t_b);
             atomicMax(P.counters + CNT_CYC_A_MAX, (unsigned long long)t_a);
             atomicMax(P.counters + CNT_CYC_B_MAX, (unsigned long long)t_b);
+            atomicAdd(P.counters + CNT_W_TAIL, (unsigned long long)t_wtail);
+            atomicAdd(P.counters + CNT_W_XSCAN, (unsigned long long)t_wx);
+            atomicAdd(P.counters + CNT_W_IDLE, (unsigned long long)t_widle);
+            if (split && rank > 0) atomicAdd(P.counters + CNT_W_PIECES, (unsigned long long)n_subs);
         }
         if (tid == 0 && rank == 0) {
             atomicAdd(P.counters + CNT_SUBS, (unsigned long long)n_subs);
