@@ -22,7 +22,9 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
     // sequential pick warp, 15 warps following its picks) measures fastest; larger clouds work on the top ~1 024
     // candidates per round with the parallel resolution
     const bool whole = ix.N <= 4096;
-    int LW = o.local_warps > 0 ? o.local_warps : (whole && ix.N > 1024 && o.cluster_size >= 0 ? LW_HIER : LW_PAR);   // (grid mode: parallel resolution only)
+    // (grid mode: parallel resolution only; Euclidean mode: the parallel resolution applies picks in the squared domain
+    // and takes one square root per candidate and step, the hierarchical phase one per candidate and pick)
+    int LW = o.local_warps > 0 ? o.local_warps : (whole && ix.N > 1024 && o.cluster_size >= 0 && !(o.flags & FPS_FLAG_EUCLIDEAN) ? LW_HIER : LW_PAR);
     int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW >= LW_HIER ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : 2))) : (LW == 8 ? 16 : 8));
     bool ok_shape = false;
 #define RFPS_OK(C_, L_) ok_shape |= (CPT == C_ && LW == L_);

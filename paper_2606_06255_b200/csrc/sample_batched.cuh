@@ -689,6 +689,12 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
     // only, and those warps drop out of the update loop
     f32x2 X[H1], Y[H1], Z[H1];
     float D[CPT1];
+    // Euclidean mode: sqrt_rn is monotone, so min_k sqrt_rn(d2_k) == sqrt_rn(min_k d2_k): the picks of a step are
+    // applied in the squared domain (M2 = the smallest d2 since the last fold) and folded into D -- which holds
+    // distances -- once per step, instead of one correctly rounded square root per (candidate, pick) pair
+    float M2[EUC ? CPT1 : 1];
+#pragma unroll
+    for (int c = 0; c < (EUC ? CPT1 : 1); ++c) M2[c] = __uint_as_float(F32_INF_BITS);
 #pragma unroll
     for (int h = 0; h < H1; ++h) {
         const int i0 = h * 2 * BT + 2 * tid, i1 = i0 + 1;
@@ -733,8 +739,13 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
             unpack2(mul2(dx, dx), x0, x1);
             unpack2(mul2(dy, dy), y0, y1);
             unpack2(mul2(dz, dz), z0, z1);
-            D[2 * h] = fminf(D[2 * h], distf<EUC>(__fadd_rn(__fadd_rn(x0, y0), z0)));
-            D[2 * h + 1] = fminf(D[2 * h + 1], distf<EUC>(__fadd_rn(__fadd_rn(x1, y1), z1)));
+            if (EUC) {       // squared domain; folded into D at the top of the next step (one square root per step)
+                M2[2 * h] = fminf(M2[2 * h], __fadd_rn(__fadd_rn(x0, y0), z0));
+                M2[2 * h + 1] = fminf(M2[2 * h + 1], __fadd_rn(__fadd_rn(x1, y1), z1));
+            } else {
+                D[2 * h] = fminf(D[2 * h], __fadd_rn(__fadd_rn(x0, y0), z0));
+                D[2 * h + 1] = fminf(D[2 * h + 1], __fadd_rn(__fadd_rn(x1, y1), z1));
+            }
         }
     };
     auto apply_range = [&](const int lo, const int hi_) {
@@ -748,6 +759,13 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
         if (!(hibits > taubits)) break;                      // nothing above tau is left: the candidates no longer decide
         if (STATS) tt0 = clock64();
         hp ^= 1;
+        if (EUC) {
+#pragma unroll
+            for (int c = 0; c < CPT1; ++c) {
+                D[c] = fminf(D[c], __fsqrt_rn(M2[c]));
+                M2[c] = __uint_as_float(F32_INF_BITS);
+            }
+        }
         const float hi = __uint_as_float(hibits);
         const float scale = fminf(__fdiv_rn(32.0f, __fsub_rn(hi, blo)), FLT_MAX);
         // bin(d): 0 for d = hi, growing as d falls; monotone because fp32 subtraction and multiplication by a
