@@ -18,6 +18,7 @@ LIB_PATH = os.environ.get("RADIUSFPS_LIB") or os.path.join(_HERE, "libradiusfps.
 FPS_OK, FPS_ERR_INVALID, FPS_ERR_CUDA, FPS_ERR_NONFINITE, FPS_ERR_NOMEM = 0, -1, -2, -3, -4
 FPS_FLAG_NO_PRUNE, FPS_FLAG_NO_SKIP, FPS_FLAG_STATS, FPS_FLAG_NO_BATCH, FPS_FLAG_PER_PICK = 1, 2, 4, 8, 16
 FPS_FLAG_EUCLIDEAN = 32
+FPS_FLAG_CHAIN_BUILD = 64
 
 EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_pick_chain_cycles", "fps_index_destroy", "fps_get_stats",
            "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version", "fps_trim"]

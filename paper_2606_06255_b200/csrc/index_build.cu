@@ -59,12 +59,21 @@ struct LaunchLog {
 };
 
 template <typename... P, typename... A>
+static void launch_pdl_smem(LaunchLog &log, size_t smem, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args);
+
+template <typename... P, typename... A>
 static void launch_pdl(LaunchLog &log, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
+{
+    launch_pdl_smem(log, 0, kern, grid, block, st, std::forward<A>(args)...);
+}
+
+template <typename... P, typename... A>
+static void launch_pdl_smem(LaunchLog &log, size_t smem, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
 {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = grid;
     cfg.blockDim = block;
-    cfg.dynamicSmemBytes = 0;
+    cfg.dynamicSmemBytes = smem;
     cfg.stream = st;
     cudaLaunchAttribute at[1];
     at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
@@ -411,7 +420,22 @@ static inline int scan_tmp_ints(int n, int B) { return ((n + SCAN_TILE - 1) / SC
 // layout, rounds inside a chunk run in order, lanes inside a round are ranked by lane id
 // (__match_any_sync + popc of lower lanes).
 // ---------------------------------------------------------------------------------------------
-constexpr int RS_CHUNK = 512, RS_WARPS = 4;    // short chunks: enough warps in flight on small clouds too
+constexpr int RS_CHUNK = 512, RS_WARPS = 4;
+
+// the lanes of the warp that hold the same 8-bit digit as this one (valid lanes only): eight ballots, one per bit.
+// (`__match_any_sync` does the same in one instruction, but measured several hundred cycles per call on B200: the
+// ranking loop below is a chain of them.)
+__device__ __forceinline__ unsigned same_digit_lanes(const unsigned d, const bool valid)
+{
+    unsigned peers = __ballot_sync(0xffffffffu, valid);
+#pragma unroll
+    for (int bit = 0; bit < 8; ++bit) {
+        const bool one = (d >> bit) & 1u;
+        const unsigned bal = __ballot_sync(0xffffffffu, one);
+        peers &= one ? bal : ~bal;
+    }
+    return peers;
+}    // short chunks: enough warps in flight on small clouds too
 
 __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_hist(const unsigned *__restrict__ keys, const int *__restrict__ poff,
                                                                int nchunk, int shift, int *__restrict__ table)
@@ -471,7 +495,7 @@ __global__ void __launch_bounds__(RS_WARPS * 32) k_radix_scatter(const unsigned 
         const bool valid = p0 + 32 * r < end;
         if (c * RS_CHUNK + 32 * r >= end) break;          // warp-uniform
         const unsigned d = valid ? ((key[r] >> shift) & 255u) : 256u;
-        const unsigned peers = __match_any_sync(0xffffffffu, d);
+        const unsigned peers = same_digit_lanes(d, valid);
         const int rank = __popc(peers & lt);
         int dst = 0;
         if (valid) dst = base[w][d] + rank;
@@ -654,6 +678,332 @@ __global__ void __launch_bounds__(256) k_group_sphere(const float4 *__restrict__
         if (in) r = __fmul_rn(__fadd_rn(__fmul_rn(__fsqrt_rn(d2_rn(v.x, v.y, v.z, cx, cy, cz)), 1.0f + 0x1p-20f), v.w), 1.0f + 0x1p-20f);
         for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
         if (lane == 0) ggeom[(size_t)b * G_cap + g] = make_float4(cx, cy, cz, r);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------
+// Single-launch build for small clouds (N <= FUSED_MAX_N = 8 192): ONE CTA of 1 024 threads per cloud runs a1-a6 back
+// to back -- bbox, keys, the LSD radix passes, segments, tiles, gather, spheres, group spheres -- with CTA barriers
+// where the 22-kernel chain has kernel boundaries, and with every intermediate array (keys, values, digit table,
+// ranks, offsets, tile counts: 16 B per point + 1 KB per chunk) in SHARED memory, so that a phase costs a barrier and
+// a few hundred cycles instead of a kernel boundary (~4.7 us) or an L2 round trip.  Same arithmetic, same stable
+// sort, same output arrays as the chain (the sampler cannot tell which path built an index).  Measured: a first
+// version with the scratch in global memory took 63 us for 4 096 points and 264 us for 24 000 on its one SM -- slower
+// than the chain for C2-sized clouds, which therefore keep the chain.
+// ---------------------------------------------------------------------------------------------
+constexpr int FUSED_T = 1024, FUSED_MAX_N = 8192;
+constexpr int FUSED_CHUNK = 256;     // keys per warp and radix pass: 4 096 points keep 16 of the 32 warps busy, 8 192 all of them
+static inline size_t fused_smem_bytes(int N) { return (size_t)16 * N + (size_t)1024 * (((N + FUSED_CHUNK - 1) / FUSED_CHUNK) | 1); }
+
+struct FusedArgs {
+    const float *pts;
+    const int *poff;
+    unsigned *bbox;                 // [B][8] (the non-finite flag is what the host reads)
+    int n_vox, hb, sb, keybits, tile_points, K_cap, G_cap, Nmax;
+    float *px, *py, *pz;
+    int *porig, *pinv;
+    int2 *vseg;
+    float4 *vgeom, *ggeom;
+    int *K_dev;
+    int *maxcnt;                    // meta[0]
+};
+
+// exclusive scan of n ints by the whole CTA: tiles of 4 096 with a running carry; returns the total
+__device__ int cta_scan_excl(const int *in, int *out, const int n, int *sm /*[34]*/)
+{
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    if (tid == 0) sm[33] = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += FUSED_T * 4) {
+        const int i0 = base + tid * 4;
+        int v[4], s = 0;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { v[i] = i0 + i < n ? in[i0 + i] : 0; s += v[i]; }
+        int inc = s;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int t = __shfl_up_sync(0xffffffffu, inc, o);
+            if (lane >= o) inc += t;
+        }
+        if (lane == 31) sm[w] = inc;
+        __syncthreads();
+        const int carry = sm[33];
+        if (w == 0) {
+            const int ws = sm[lane];
+            int wi = ws;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int t = __shfl_up_sync(0xffffffffu, wi, o);
+                if (lane >= o) wi += t;
+            }
+            sm[lane] = wi - ws;
+            if (lane == 31) sm[32] = carry + wi;
+        }
+        __syncthreads();
+        int e = carry + sm[w] + inc - s;
+#pragma unroll
+        for (int i = 0; i < 4; ++i) { if (i0 + i < n) out[i0 + i] = e; e += v[i]; }
+        __syncthreads();
+        if (tid == 0) sm[33] = sm[32];
+        __syncthreads();
+    }
+    return sm[33];
+}
+
+__global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
+{
+    grid_dep_sync();
+    extern __shared__ __align__(16) unsigned char fsm[];
+    __shared__ int hist[FUSED_T / 32][256];          // per-warp digit counters / bases of the radix passes
+    __shared__ float red[FUSED_T / 32][6];
+    __shared__ int sm[34];
+    __shared__ float bb[8];
+    __shared__ int sbad, skv, sK;
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, NWF = FUSED_T / 32;
+    const int b = blockIdx.x;
+    const int base = A.poff[b], N = A.poff[b + 1] - base;
+    const float *P = A.pts + (size_t)base * 3;
+    // ---- a1: bounding box + non-finite flag ----
+    {
+        float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+        bool bad = false;
+        for (int i = tid; i < N; i += FUSED_T) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float v = P[3 * (size_t)i + a];
+                bad |= !(fabsf(v) <= FLT_MAX);
+                mn[a] = fminf(mn[a], v);
+                mx[a] = fmaxf(mx[a], v);
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            for (int o = 16; o > 0; o >>= 1) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+            }
+        bad = __any_sync(0xffffffffu, bad);
+        if (tid == 0) sbad = 0;
+        __syncthreads();
+        if (lane == 0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { red[w][a] = mn[a]; red[w][3 + a] = mx[a]; }
+            if (bad) sbad = 1;
+        }
+        __syncthreads();
+        if (tid < 3) {
+            float lo = red[0][tid], hi = red[0][3 + tid];
+            for (int i = 1; i < NWF; ++i) { lo = fminf(lo, red[i][tid]); hi = fmaxf(hi, red[i][3 + tid]); }
+            bb[tid] = lo; bb[3 + tid] = hi;
+            unsigned *g = A.bbox + b * BBOX_STRIDE;
+            g[tid] = f2ord(lo); g[3 + tid] = f2ord(hi);
+            if (tid == 0) g[6] = sbad ? 1u : 0u;
+        }
+        __syncthreads();
+    }
+    // shared-memory scratch, sized for the largest cloud of the batch: two key and two value buffers, the digit table
+    unsigned *kin = reinterpret_cast<unsigned *>(fsm), *kout = kin + A.Nmax;
+    int *vin = reinterpret_cast<int *>(kout + A.Nmax), *vout = vin + A.Nmax;
+    int *const table = vout + A.Nmax;                              // digit-major [256][nchunk]
+    // ---- a2: sort keys (Eq. 8: floor, then clamp; Hilbert voxel id + Morton sub-cell bits) ----
+    {
+        const float E = fmaxf(fmaxf(bb[3] - bb[0], bb[4] - bb[1]), bb[5] - bb[2]);
+        float L = (1.0f + 1e-3f) * E / (float)A.n_vox;
+        if (!(L > 0.0f)) L = 1.0f;
+        const float invsub = (float)(1 << A.sb);
+        for (int i = tid; i < N; i += FUSED_T) {
+            unsigned v[3], s[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float t = (P[3 * (size_t)i + a] - bb[a]) / L;
+                int c = (int)floorf(t);
+                c = max(0, min(A.n_vox - 1, c));
+                int sc = (int)floorf((t - (float)c) * invsub);
+                sc = max(0, min((1 << A.sb) - 1, sc));
+                v[a] = (unsigned)c;
+                s[a] = (unsigned)sc;
+            }
+            const unsigned vid = hilbert3(v[0], v[1], v[2], A.hb);
+            const unsigned sub = A.sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
+            kin[i] = (vid << (3 * A.sb)) | sub;
+            vin[i] = i;
+        }
+        __syncthreads();
+    }
+    // ---- a3: stable LSD radix sort, 8 bits per pass; a warp owns chunks of FUSED_CHUNK keys ----
+    {
+        const int nchunk = (N + FUSED_CHUNK - 1) / FUSED_CHUNK;
+        const int ts = nchunk | 1;        // odd row stride of the digit table: a warp's 32 digits hit 32 banks
+        const unsigned lt = (1u << lane) - 1u;
+        for (int shift = 0; shift < A.keybits; shift += 8) {
+            if (ts != nchunk && tid < 256) table[tid * ts + nchunk] = 0;      // the pad column counts nothing (the scan below runs over it)
+            for (int c0 = 0; c0 < nchunk; c0 += NWF) {
+                const int c = c0 + w;
+                for (int d = lane; d < 256; d += 32) hist[w][d] = 0;
+                __syncwarp();
+                if (c < nchunk) {
+                    const int end = min(N, (c + 1) * FUSED_CHUNK);
+                    unsigned kr[FUSED_CHUNK / 32];              // the whole chunk first: one memory round trip, not 16
+#pragma unroll
+                    for (int r = 0; r < FUSED_CHUNK / 32; ++r) { const int p = c * FUSED_CHUNK + 32 * r + lane; kr[r] = p < end ? kin[p] : 0u; }
+#pragma unroll
+                    for (int r = 0; r < FUSED_CHUNK / 32; ++r)
+                        if (c * FUSED_CHUNK + 32 * r + lane < end) atomicAdd(&hist[w][(kr[r] >> shift) & 255u], 1);
+                    __syncwarp();
+                    for (int d = lane; d < 256; d += 32) table[d * ts + c] = hist[w][d];
+                }
+                __syncwarp();
+            }
+            __syncthreads();
+            cta_scan_excl(table, table, 256 * ts, sm);
+            for (int c0 = 0; c0 < nchunk; c0 += NWF) {
+                const int c = c0 + w;
+                if (c < nchunk) {
+                    for (int d = lane; d < 256; d += 32) hist[w][d] = table[d * ts + c];
+                    __syncwarp();
+                    const int end = min(N, (c + 1) * FUSED_CHUNK);
+                    // the chunk is loaded before the ranking loop, whose rounds are serially dependent through the
+                    // shared counters: a global load inside each of them would put L2 latency on that chain
+                    unsigned kr[FUSED_CHUNK / 32];
+                    int vr[FUSED_CHUNK / 32];
+#pragma unroll
+                    for (int r = 0; r < FUSED_CHUNK / 32; ++r) {
+                        const int p = c * FUSED_CHUNK + 32 * r + lane;
+                        kr[r] = p < end ? kin[p] : 0u;
+                        vr[r] = p < end ? vin[p] : 0;
+                    }
+#pragma unroll
+                    for (int r = 0; r < FUSED_CHUNK / 32; ++r) {
+                        if (c * FUSED_CHUNK + 32 * r >= end) break;      // warp-uniform
+                        const bool valid = c * FUSED_CHUNK + 32 * r + lane < end;
+                        const unsigned key = kr[r];
+                        const int val = vr[r];
+                        const unsigned d = valid ? ((key >> shift) & 255u) : 256u;
+                        const unsigned peers = same_digit_lanes(d, valid);
+                        const int rk = __popc(peers & lt);
+                        int dst = 0;
+                        if (valid) dst = hist[w][d] + rk;
+                        __syncwarp();
+                        if (valid && rk == 0) hist[w][d] += __popc(peers);
+                        __syncwarp();
+                        if (valid) { kout[dst] = key; vout[dst] = val; }
+                    }
+                }
+                __syncwarp();
+            }
+            __syncthreads();
+            unsigned *tk = kin; kin = kout; kout = tk;
+            int *tv = vin; vin = vout; vout = tv;
+        }
+    }
+    // ---- a5: grid voxels (heads -> rank -> offsets), tiles (ntiles -> base -> segments) ----
+    // the sort's spare buffers are reused: heads -> F1, rank -> F2, then voff -> F1 (the head flags are recomputed from
+    // the keys), tile counts and their scan -> F2 (in place; a voxel's tile count is recomputed from its length)
+    int *const F1 = reinterpret_cast<int *>(kout), *const F2 = vout;
+    const int subbits = 3 * A.sb;
+    for (int p = tid; p < N; p += FUSED_T) F1[p] = (p == 0 || (kin[p] >> subbits) != (kin[p - 1] >> subbits)) ? 1 : 0;
+    __syncthreads();
+    {
+        const int kvt = cta_scan_excl(F1, F2, N, sm);
+        if (tid == 0) skv = kvt;
+    }
+    __syncthreads();
+    const int kv = skv;
+    int *const voff = F1;
+    for (int p = tid; p < N; p += FUSED_T)
+        if (p == 0 || (kin[p] >> subbits) != (kin[p - 1] >> subbits)) voff[F2[p]] = p;
+    __syncthreads();
+    auto tiles_of = [&](const int cnt) { return A.tile_points > 0 ? (cnt + A.tile_points - 1) / A.tile_points : 1; };
+    for (int k = tid; k < N; k += FUSED_T) {
+        int nt = 0;
+        if (k < kv) nt = tiles_of((k + 1 < kv ? voff[k + 1] : N) - voff[k]);
+        F2[k] = nt;
+    }
+    __syncthreads();
+    {
+        const int Kt = cta_scan_excl(F2, F2, N, sm);
+        if (tid == 0) { sK = Kt; A.K_dev[b] = Kt; }
+    }
+    __syncthreads();
+    const int K = sK;
+    const int *const tbase = F2;
+    int2 *vseg = A.vseg + (size_t)b * A.K_cap;
+    for (int k = tid; k < kv; k += FUSED_T) {
+        const int off = voff[k];
+        const int cnt = (k + 1 < kv ? voff[k + 1] : N) - off;
+        const int nt = tiles_of(cnt);
+        const int chunk = (cnt + nt - 1) / nt;
+        int2 *dst = vseg + tbase[k];
+        for (int t = 0; t < nt; ++t) dst[t] = make_int2(off + t * chunk, min(chunk, cnt - t * chunk));
+    }
+    // ---- a4: gather AoS -> sorted SoA (+ permutation and its inverse) ----
+    float *px = A.px + base, *py = A.py + base, *pz = A.pz + base;
+    int *porig = A.porig + base, *pinv = A.pinv + base;
+    for (int p = tid; p < N; p += FUSED_T) {
+        const int i = vin[p];
+        const float *s = P + 3 * (size_t)i;
+        px[p] = s[0]; py[p] = s[1]; pz[p] = s[2];
+        porig[p] = i;
+        pinv[i] = p;
+    }
+    __syncthreads();
+    // ---- a6: tight bounding sphere per (tiled) voxel, 8 lanes per voxel (small clouds have small voxels: a whole
+    // warp per voxel spends its time in shuffles); then the group spheres ----
+    float4 *vgeom = A.vgeom + (size_t)b * A.K_cap;
+    int local_max = 0;
+    {
+        const int sub = lane & 7, grp = (w << 2) | (lane >> 3), NG = NWF * 4;
+        for (int k0 = 0; k0 < K; k0 += NG) {
+            const int k = k0 + grp;
+            const int2 sg = k < K ? vseg[k] : make_int2(0, 0);
+            float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) {
+                mn[0] = fminf(mn[0], px[p]); mx[0] = fmaxf(mx[0], px[p]);
+                mn[1] = fminf(mn[1], py[p]); mx[1] = fmaxf(mx[1], py[p]);
+                mn[2] = fminf(mn[2], pz[p]); mx[2] = fmaxf(mx[2], pz[p]);
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                for (int o = 4; o > 0; o >>= 1) {
+                    mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                    mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+                }
+            const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+            const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+            const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+            float r2 = 0.0f;
+            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) r2 = fmaxf(r2, d2_rn(px[p], py[p], pz[p], cx, cy, cz));
+            for (int o = 4; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+            if (sub == 0 && k < K) {
+                vgeom[k] = make_float4(cx, cy, cz, __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f));
+                local_max = max(local_max, sg.y);
+            }
+        }
+    }
+    local_max = __reduce_max_sync(0xffffffffu, local_max);
+    if (lane == 0 && local_max > 0) atomicMax(A.maxcnt, local_max);
+    __syncthreads();
+    float4 *ggeom = A.ggeom + (size_t)b * A.G_cap;
+    const int G = (K + 31) / 32;
+    for (int g = w; g < G; g += NWF) {
+        const int k = g * 32 + lane;
+        const bool in = k < K;
+        const float4 v = in ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float mn[3] = {in ? v.x - v.w : FLT_MAX, in ? v.y - v.w : FLT_MAX, in ? v.z - v.w : FLT_MAX};
+        float mx[3] = {in ? v.x + v.w : -FLT_MAX, in ? v.y + v.w : -FLT_MAX, in ? v.z + v.w : -FLT_MAX};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            for (int o = 16; o > 0; o >>= 1) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+            }
+        const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+        const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+        const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+        float r = 0.0f;
+        if (in) r = __fmul_rn(__fadd_rn(__fmul_rn(__fsqrt_rn(d2_rn(v.x, v.y, v.z, cx, cy, cz)), 1.0f + 0x1p-20f), v.w), 1.0f + 0x1p-20f);
+        for (int o = 16; o > 0; o >>= 1) r = fmaxf(r, __shfl_xor_sync(0xffffffffu, r, o));
+        if (lane == 0) ggeom[g] = make_float4(cx, cy, cz, r);
     }
 }
 
@@ -850,6 +1200,22 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         return FPS_ERR_CUDA;
     }
     const int *poff = ix.poff_dev;
+    if (N <= FUSED_MAX_N && !(o.flags & FPS_FLAG_CHAIN_BUILD)) {
+        // small clouds: the whole build in ONE launch, one CTA per cloud (k_build_fused)
+        FusedArgs fa;
+        fa.pts = points; fa.poff = poff; fa.bbox = sc.bbox;
+        fa.n_vox = n_vox; fa.hb = vbits / 3; fa.sb = sb; fa.keybits = keybits; fa.tile_points = tile_points;
+        fa.K_cap = ix.K_cap; fa.G_cap = ix.G_cap; fa.Nmax = N;
+        fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
+        fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
+        fa.maxcnt = reinterpret_cast<int *>(meta);
+        if (cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)) != cudaSuccess) {
+            set_error("cudaFuncSetAttribute(k_build_fused) failed: %s", cudaGetErrorString(cudaGetLastError()));
+            release_scratch();
+            return FPS_ERR_CUDA;
+        }
+        launch_pdl_smem(log, fused_smem_bytes(N), k_build_fused, dim3(B), dim3(FUSED_T), st, fa);
+    } else {
     launch_pdl(log, k_bbox_init, dim3((B * BBOX_STRIDE + 255) / 256), dim3(256), st, sc.bbox, B);
     launch_pdl(log, k_bbox, dim3(dim3(std::max(1, std::min((N + 4095) / 4096, sms)), B)), dim3(256), st, points, poff, sc.bbox);
     launch_pdl(log, k_keys, dim3(gN), dim3(256), st, points, poff, sc.bbox, n_vox, vbits / 3, sb, sc.kA, sc.vA);
@@ -879,6 +1245,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
                reinterpret_cast<int *>(meta));
     const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, sms * 8));
     launch_pdl(log, k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
+    }
     {
         const cudaError_t el = log.first_error != cudaSuccess ? log.first_error : cudaGetLastError();
         if (el != cudaSuccess) {

@@ -1,12 +1,28 @@
 // sb_inst_2_32.cu -- k_fps_batched with 2 candidates per thread and local-phase shape 32 (one translation
 // unit per shape so that the shapes compile in parallel; the kernel is sample_batched.cuh)
+#include <mutex>
+
 #include "sample_batched.cuh"
 
 namespace rfps {
 
 int launch_batched_2_32(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st) { return launch_batched_s<2, 32>(bp, ix, st); }
 
+// (asked for every index build; the answer depends on the device, the cluster size and the shared memory only)
+static int resident_clusters_uncached(int c, size_t smem);
 int batched_max_resident_clusters(int c, size_t smem)
+{
+    static std::mutex mu;
+    static int cache[64][17];
+    static size_t cache_smem[64][17];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    if (dev < 0 || dev >= 64 || c < 1 || c > 16) return resident_clusters_uncached(c, smem);
+    std::lock_guard<std::mutex> lock(mu);
+    if (cache_smem[dev][c] != smem || cache[dev][c] == 0) { cache[dev][c] = resident_clusters_uncached(c, smem); cache_smem[dev][c] = smem; }
+    return cache[dev][c];
+}
+static int resident_clusters_uncached(int c, size_t smem)
 {
     auto kern = k_fps_batched<2, 32, false, false, false>;
     if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return 0; }

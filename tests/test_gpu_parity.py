@@ -187,6 +187,40 @@ def test_result_independent_of_tiling(rf, name, tile):
     assert_same(gi, gm, *ref)
 
 
+@pytest.mark.parametrize("name", sorted(SMALL))
+def test_single_launch_build_equals_the_kernel_chain(rf, name):
+    # clouds of <= 32 768 points are indexed by ONE kernel launch (one CTA per cloud); FPS_FLAG_CHAIN_BUILD forces the
+    # chain of ~22 kernels that larger clouds take: same voxels, same tiles, same samples
+    P, M = SMALL[name]()
+    ref = oracle.fps(P, M, 0)
+    a = run_gpu(rf, P, M, n_vox=8)
+    b = run_gpu(rf, P, M, n_vox=8, flags=rf.FPS_FLAG_CHAIN_BUILD)
+    assert a[2]["build_launches"] == 1 and b[2]["build_launches"] > 10
+    for key in ("K_total", "K_max", "max_voxel_points", "n_vox"):
+        assert a[2][key] == b[2][key], key
+    assert_same(a[0], a[1], *ref)
+    assert_same(b[0], b[1], *ref)
+
+
+def test_single_launch_build_ragged_batch(rf):
+    clouds = [inputs.room(5000, 21), inputs.uniform_cube(1, 22), inputs.lidar(7001, 23, n_azimuth=110),
+              inputs.shuffled_lattice(8, 24), inputs.uniform_cube(33, 25), inputs.clustered(2500, 26)]
+    Ms = [1250, 1, 1800, 512, 33, 600]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])]).astype(np.int64)
+    P = torch.from_numpy(np.ascontiguousarray(np.concatenate(clouds, axis=0))).cuda()
+    for flags in (0, rf.FPS_FLAG_CHAIN_BUILD):
+        ix = rf.fps_index_build_ragged(P, off.tolist(), flags=flags)
+        try:
+            idx, mind, ooff = rf.fps_sample_ragged(ix, Ms)
+            torch.cuda.synchronize()
+            idx, mind = idx.cpu().numpy(), mind.cpu().numpy()
+            for b, c in enumerate(clouds):
+                ref_i, ref_m = oracle.fps(c, Ms[b], 0)
+                assert_same(idx[ooff[b]:ooff[b + 1]], mind[ooff[b]:ooff[b + 1]], ref_i.reshape(-1), ref_m.reshape(-1))
+        finally:
+            rf.fps_index_destroy(ix)
+
+
 @pytest.mark.parametrize("threads", [64, 128, 256, 1024])
 def test_block_sizes(rf, threads):
     P, M = SMALL["room"]()
