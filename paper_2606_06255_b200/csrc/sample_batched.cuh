@@ -98,14 +98,15 @@ __device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
 // (batch id << PUB_SHIFT | count) to the exchange block's `pub` word -- in its own shared memory (cluster) or in
 // global memory (grid; the picks themselves are then mirrored to `gpick`).  Inactive for a single-CTA cloud.
 struct Publisher {
-    unsigned local_addr = 0u;     // cluster: shared::cta address of ctl->pub
-    unsigned *gptr = nullptr;     // grid: &gx->pub
-    float4 *gpick = nullptr;      // grid: global mirror of the batch buffer
-    unsigned base = 0u;           // batch id << PUB_SHIFT
+    unsigned local_addr = 0u;              // cluster: shared::cta address of ctl->pub
+    unsigned long long *gptr = nullptr;    // grid: the packed word cmd << 32 | pub (GX_PC)
+    unsigned cmd_hi = 0u;                  // grid: the command word that stays in its upper half while the batch runs
+    float4 *gpick = nullptr;               // grid: global mirror of the batch buffer
+    unsigned base = 0u;                    // batch id << PUB_SHIFT
     __device__ __forceinline__ bool on() const { return local_addr != 0u || gptr != nullptr; }
     __device__ __forceinline__ void operator()(const unsigned count_and_flags) const
     {
-        if (gptr) st_release_gpu_u32(gptr, base | count_and_flags);
+        if (gptr) st_release_gpu_u64(gptr, ((unsigned long long)cmd_hi << 32) | (base | count_and_flags));
         else if (local_addr) st_release_cluster_u32(local_addr, base | count_and_flags);
     }
 };
@@ -1195,7 +1196,6 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
     }
     // exchange block of this cloud as seen from here (sample_batched_shapes.h)
     unsigned char *const gxb = GRID ? P.gx + (size_t)b * gx_bytes(TC) : nullptr;
-    Ctl *const gctl = reinterpret_cast<Ctl *>(gxb);
     float4 *const gpick = GRID ? reinterpret_cast<float4 *>(gxb + GX_PICK) : nullptr;
     float *const gcand = GRID ? reinterpret_cast<float *>(gxb + gx_cand()) : nullptr;
     const unsigned ctl0 = GRID ? 0u : mapa(smem_u32(ctl), 0u);          // cluster: the picker's control block
@@ -1600,30 +1600,44 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         // picks as they are produced.  It never waits for a batch to be applied: the workers answer the next
         // command only after they have applied the whole batch before it.
         // =====================================================================================
-        unsigned ncmd = 0u, batch = 0u;
+        unsigned ncmd = 0u, batch = 0u, cur_cmd = 0u, cur_pub = 0u;
+        unsigned long long *const gpc = reinterpret_cast<unsigned long long *>(gxb + GX_PC), *const gctb = reinterpret_cast<unsigned long long *>(gxb + GX_CTB),
+                           *const gac = reinterpret_cast<unsigned long long *>(gxb + GX_AC);
         auto pub_word = [&](const unsigned v) {            // thread 0
-            if (GRID) st_release_gpu_u32(&gctl->pub, v);
+            cur_pub = v;
+            if (GRID) st_release_gpu_u64(gpc, ((unsigned long long)cur_cmd << 32) | v);
             else st_release_cluster_u32(smem_u32(&ctl->pub), v);
         };
         // one command: send (thread 0), wait for W acknowledgements, fetch the result, broadcast
         auto send = [&](const unsigned type, const unsigned tb) {
             ++ncmd;
+            cur_cmd = (ncmd << 2) | type;
             if (tid == 0) {
-                Ctl *const c = GRID ? gctl : ctl;
-                c->ccount[ncmd & 7u] = 0u;
-                c->cmd_tb = tb;
-                c->cmd_after = batch;
-                if (GRID) st_release_gpu_u32(&gctl->cmd, (ncmd << 2) | type);
-                else st_release_cluster_u32(smem_u32(&ctl->cmd), (ncmd << 2) | type);
+                if (GRID) {
+                    // nobody touches the count / acknowledgement word between two commands: a plain store resets the count
+                    *reinterpret_cast<volatile unsigned long long *>(gac) = (unsigned long long)((ncmd - 1u) * (unsigned)W) << 32;
+                    *reinterpret_cast<volatile unsigned long long *>(gctb) =
+                        ((unsigned long long)(((batch & 0xffffu) << 16) | (ncmd & 0xffffu)) << 32) | tb;
+                    st_release_gpu_u64(gpc, ((unsigned long long)cur_cmd << 32) | cur_pub);
+                } else {
+                    ctl->ccount[ncmd & 7u] = 0u;
+                    ctl->cmd_tb = tb;
+                    ctl->cmd_after = batch;
+                    st_release_cluster_u32(smem_u32(&ctl->cmd), cur_cmd);
+                }
             }
         };
         auto wait = [&](const unsigned type, unsigned &r0, unsigned &r1) {
             if (tid == 0) {
                 const unsigned want = ncmd * (unsigned)W;
-                if (GRID) { while (ld_acquire_gpu_u32(&gctl->ack) != want) __nanosleep(20); }
-                else { while (ld_acquire_cluster_local_u32(smem_u32(&ctl->ack)) != want) __nanosleep(20); }
-                if (type == CMD_EXTRACT)
-                    ctl->scratch[0] = (int)(GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->ccount[ncmd & 7u]) : *reinterpret_cast<volatile unsigned *>(&ctl->ccount[ncmd & 7u]));
+                if (GRID) {
+                    unsigned long long ac;
+                    while ((unsigned)((ac = ld_acquire_gpu_u64(gac)) >> 32) != want) __nanosleep(20);
+                    if (type == CMD_EXTRACT) ctl->scratch[0] = (int)(unsigned)ac;
+                } else {
+                    while (ld_acquire_cluster_local_u32(smem_u32(&ctl->ack)) != want) __nanosleep(20);
+                    if (type == CMD_EXTRACT) ctl->scratch[0] = (int)*reinterpret_cast<volatile unsigned *>(&ctl->ccount[ncmd & 7u]);
+                }
             }
             __syncthreads();                               // thread 0's acquire now covers the whole CTA
             if (type == CMD_MAX && warp == 0) {            // argmax over the workers' slots (Eq. 15-18, last level)
@@ -1684,7 +1698,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             ++batch;
             Publisher pubr;
             pubr.base = (batch & 0x7ffffu) << PUB_SHIFT;
-            if (GRID) { pubr.gptr = &gctl->pub; pubr.gpick = gpick; }
+            if (GRID) { pubr.gptr = gpc; pubr.cmd_hi = cur_cmd; pubr.gpick = gpick; }
             else pubr.local_addr = smem_u32(&ctl->pub);
             if (cnt == 0) {                              // the single global argmax = the paper's own iteration
                 if (tid == 0) {
@@ -1706,6 +1720,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             __syncthreads();                               // the last picks are written
             prev_tau_valid = cnt > 0 && nb < PB && j < Mb && !no_batch;
             prev_taubits = taubits;
+            cur_pub = pubr.base | (unsigned)nb | PUB_DONE | (j >= Mb ? PUB_FINAL : 0u);
             if (tid == 0) pubr((unsigned)nb | PUB_DONE | (j >= Mb ? PUB_FINAL : 0u));
             if (STATS && tid == 0) { t1 = clock64(); t_local += t1 - t0; }
         }
@@ -1720,9 +1735,11 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
         const unsigned pick_rc = GRID ? 0u : mapa(smem_u32(bpick), 0u);
         const unsigned cX0 = GRID ? 0u : mapa(smem_u32(cX), 0u), cY0 = GRID ? 0u : mapa(smem_u32(cY), 0u), cZ0 = GRID ? 0u : mapa(smem_u32(cZ), 0u),
                        cD0 = GRID ? 0u : mapa(smem_u32(cD), 0u), cO0 = GRID ? 0u : mapa(smem_u32(cO), 0u);
+        unsigned long long *const gpc = reinterpret_cast<unsigned long long *>(gxb + GX_PC), *const gctb = reinterpret_cast<unsigned long long *>(gxb + GX_CTB),
+                           *const gac = reinterpret_cast<unsigned long long *>(gxb + GX_AC);
         auto ack = [&]() {                                 // after a barrier that follows the command's last store
             if (tid == 0) {
-                if (GRID) red_release_gpu_add_u32(&gctl->ack, 1u);
+                if (GRID) red_release_gpu_add_u64(gac, 1ull << 32);
                 else red_release_cluster_add_u32(ctl0 + (unsigned)offsetof(Ctl, ack), 1u);
             }
         };
@@ -1730,27 +1747,43 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
             // ---- wait for the next message (thread 0 polls, the CTA sleeps at the barrier) ----
             if (tid == 0) {
                 if (STATS) tw0 = clock64();
-                unsigned v, c;
+                unsigned v, c, tbv = 0u;
                 for (;;) {
-                    // The command word is read BEFORE the batch word: the picker finishes a batch (pub: DONE) and only
-                    // then sends the next command, so a worker that sees the new command is guaranteed (acquire) to
-                    // see, in the read that follows, the batch it has to apply first.  The other order has a window
-                    // in which the command is seen and the batch before it is not.
-                    c = in_batch ? 0u : (GRID ? ld_acquire_gpu_u32(&gctl->cmd) : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, cmd)));
-                    v = GRID ? ld_acquire_gpu_u32(&gctl->pub) : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, pub));
+                    // The command word is read BEFORE (cluster mode) or TOGETHER WITH (grid mode: one 64-bit word) the
+                    // batch word: the picker finishes a batch (pub: DONE) and only then sends the next command, so a
+                    // worker that sees the new command is guaranteed (acquire) to see the batch it has to apply
+                    // first.  Reading pub first has a window in which the command is seen and the batch is not.
+                    unsigned long long pay = 0ull;
+                    if (GRID) {
+                        pay = *reinterpret_cast<volatile unsigned long long *>(gctb);      // in flight together with the next load
+                        const unsigned long long pc = ld_acquire_gpu_u64(gpc);
+                        v = (unsigned)pc;
+                        c = in_batch ? 0u : (unsigned)(pc >> 32);
+                    } else {
+                        c = in_batch ? 0u : ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, cmd));
+                        v = ld_acquire_cluster_u32(ctl0 + (unsigned)offsetof(Ctl, pub));
+                    }
                     const bool mine = (v >> PUB_SHIFT) == (next_batch & 0x7ffffu);
                     if (mine && ((v & (PUB_DONE | PUB_FINAL)) || (int)(v & PUB_COUNT) - applied >= STREAM_MIN)) { c = 0u; break; }
                     if (!in_batch && !mine && (c >> 2) == next_cmd) {
                         // answered only when the batch it follows has been applied (it may have been sent early)
-                        const unsigned after = GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->cmd_after) : ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_after));
-                        if (after + 1u == next_batch) { v = 0u; break; }
+                        if (GRID) {
+                            // the payload was loaded before the acquire: if its tag is not this command's, read it again
+                            if ((unsigned)((pay >> 32) & 0xffffull) != (next_cmd & 0xffffu)) pay = *reinterpret_cast<volatile unsigned long long *>(gctb);
+                            const unsigned after = (unsigned)(pay >> 48);
+                            tbv = (unsigned)pay;
+                            if (((after + 1u) & 0xffffu) == (next_batch & 0xffffu)) { v = 0u; break; }
+                        } else {
+                            const unsigned after = ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_after));
+                            if (after + 1u == next_batch) { tbv = ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_tb)); v = 0u; break; }
+                        }
                     }
                     __nanosleep(40);
                 }
                 if (STATS) t_widle += clock64() - tw0;
                 ctl->scratch[0] = (int)v;
                 ctl->scratch[1] = (int)c;
-                if (c) ctl->scratch[2] = (int)(GRID ? *reinterpret_cast<volatile unsigned *>(&gctl->cmd_tb) : ld_dsmem_u32(ctl0 + (unsigned)offsetof(Ctl, cmd_tb)));
+                ctl->scratch[2] = (int)tbv;
             }
             __syncthreads();
             const unsigned v = (unsigned)ctl->scratch[0], c = (unsigned)ctl->scratch[1], ctb = (unsigned)ctl->scratch[2];
@@ -1773,7 +1806,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_batched(const BatchParams P, cons
                     const unsigned slot = next_cmd & 7u;
                     if (STATS && tid == 0) tw0 = clock64();
                     if (GRID) {
-                        extract_scan(ctb, [&](unsigned n) { return atomicAdd(&gctl->ccount[slot], n); },
+                        extract_scan(ctb, [&](unsigned n) { return (unsigned)atomicAdd(gac, (unsigned long long)n); },
                                      [&](unsigned sl, float x, float y, float z, unsigned dbits, unsigned o) {
                                          gcand[sl] = x; gcand[TC + sl] = y; gcand[2 * TC + sl] = z;
                                          gcand[3 * TC + sl] = __uint_as_float(dbits); gcand[4 * TC + sl] = __uint_as_float(o);

@@ -72,6 +72,15 @@ constexpr int PUB_SHIFT = 13;       // batch id above the flags (compared modulo
 constexpr unsigned CMD_MAX = 1u, CMD_EXTRACT = 2u;
 // grid mode: byte offsets inside a cloud's global exchange block; tc = candidate capacity
 constexpr size_t GX_SLOT = 256, GX_PICK = 2048;      // the header (control words + one slot per CTA) is zeroed before a launch
+// Grid mode packs the control words into three 64-bit words so that a poll is ONE L2 round trip (every message
+// latency is on the critical path of a round):
+//   GX_PC  = cmd << 32 | pub            written whole by the picker (release), read whole by the workers (acquire)
+//   GX_CTB = the current command's payload: (cmd_after & 0xffff) << 48 | (command id & 0xffff) << 32 | cmd_tb, written
+//            before GX_PC; a worker loads it together with GX_PC and re-reads it if the id tag is not the command's
+//   GX_AC  = acknowledgements (cumulative) << 32 | candidates found by the running extraction: the workers reserve
+//            candidate slots and acknowledge on the same word, the picker reads both with one acquire
+constexpr size_t GX_PC = 216, GX_CTB = 224, GX_AC = 232;
+static_assert(sizeof(Ctl) <= GX_PC && GX_AC + 8 <= GX_SLOT, "packed control words sit between the control block and the slots");
 __host__ __device__ constexpr size_t gx_cand(void) { return GX_PICK + sizeof(float4) * 1024; }
 __host__ __device__ constexpr size_t gx_bytes(int tc) { return gx_cand() + sizeof(float) * 5 * (size_t)tc; }
 
