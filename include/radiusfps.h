@@ -212,6 +212,30 @@ int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_pe
 void fps_index_destroy(fps_index_t *h);
 void fps_trim(void);
 
+/*
+ * fps_sample_noalloc -- the whole path (index build a1-a6 + sampling a7-a13, Algorithm 1 / Sec. 3.2-3.4) for
+ * ONE cloud, for callers that must not allocate device memory (tight serving loops, harnesses that forbid
+ * cudaMalloc).  It calls no cudaMalloc / cudaFree / pool routine and creates no handle: the voxel index, which is
+ * scratch memory of such a call, lives in a static device array of FPS_NOALLOC_SCRATCH_BYTES (512 KiB) that every GPU
+ * loading the library holds until the process exits.  Results are bit-identical to fps_index_build + fps_sample with
+ * default options on the same cloud.
+ *   points       DEVICE [N][3] fp32, finite; N in [1, FPS_NOALLOC_MAX_N = 8192] -- a larger N is rejected with
+ *                FPS_ERR_INVALID and a message naming the limit (nothing is launched)
+ *   M, start_idx as for fps_sample (1 <= M <= N, 0 <= start_idx < N)
+ *   flags        0, or FPS_FLAG_EUCLIDEAN; any other flag is rejected
+ *   out_idx      DEVICE [M] int32, out_mindist DEVICE [M] fp32: owned by the caller, written by the call
+ *   stream       cudaStream_t (NULL = default stream) of the CURRENT device
+ * The call synchronises `stream` once (the build's read-back of the voxel count, as fps_index_build does) and returns
+ * with the sampling kernel enqueued.  ALL calls on one device share the one static array: it keeps the previous
+ * call's contents (the call clears what has to start at zero), calls on the same stream are ordered, and calls that
+ * overlap on the GPU -- different streams without an ordering between them, several host threads -- RACE on it; the
+ * caller serialises them.  Errors: FPS_ERR_INVALID (arguments, N above the limit), FPS_ERR_NONFINITE, FPS_ERR_CUDA.
+ */
+#define FPS_NOALLOC_MAX_N 8192
+#define FPS_NOALLOC_SCRATCH_BYTES (512 * 1024)
+int fps_sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx, int32_t flags, int32_t *out_idx,
+                       float *out_mindist, void *stream);
+
 /* Layout facts and (with FPS_FLAG_STATS) the counters of the last fps_sample; synchronises the
  * stream of that call.  out: host pointer. */
 int fps_get_stats(fps_index_t *h, fps_stats *out);

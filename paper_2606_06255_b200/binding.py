@@ -21,7 +21,7 @@ FPS_FLAG_EUCLIDEAN = 32
 FPS_FLAG_CHAIN_BUILD = 64
 
 EXPORTS = ["fps_index_build", "fps_index_build_ex", "fps_index_build_ragged", "fps_sample", "fps_sample_ragged", "fps_gather_xyz", "fps_pick_chain_cycles", "fps_index_destroy", "fps_get_stats",
-           "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version", "fps_trim"]
+           "fps_sample_host", "fps_build_and_sample", "fps_last_error", "fps_last_status", "fps_version", "fps_trim", "fps_sample_noalloc"]
 
 
 class fps_build_opts(ctypes.Structure):
@@ -108,6 +108,9 @@ def load() -> ctypes.CDLL:
     lib.fps_last_status.argtypes = []
     lib.fps_trim.restype = None
     lib.fps_trim.argtypes = []
+    lib.fps_sample_noalloc.restype = ctypes.c_int
+    lib.fps_sample_noalloc.argtypes = [ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
     _lib = lib
     return lib
 
@@ -200,6 +203,30 @@ def fps_sample(index: Index, M: int, start_idx: int = 0, out_idx: torch.Tensor |
             raise ValueError("out_idx must be contiguous int32 [B,M] and out_mindist contiguous float32 [B,M]")
         s = stream if stream is not None else torch.cuda.current_stream()
         rc = lib.fps_sample(index.handle, M, int(start_idx), out_idx.data_ptr(), out_mindist.data_ptr(), s.cuda_stream)
+    if rc != FPS_OK:
+        raise FpsError(rc, fps_last_error())
+    return out_idx, out_mindist
+
+
+FPS_NOALLOC_MAX_N = 8192
+
+
+def fps_sample_noalloc(points: torch.Tensor, M: int, out_idx: torch.Tensor, out_mindist: torch.Tensor, start_idx: int = 0,
+                       flags: int = 0, stream: torch.cuda.Stream | None = None):
+    """fps_sample_noalloc: build + sample ONE cloud (``points`` CUDA float32 [N,3], N <= FPS_NOALLOC_MAX_N) with the index
+    in the library's static device array -- no device allocation.  The caller passes the outputs (int32 [M], float32
+    [M], CUDA); nothing is allocated here either.  Calls that overlap on the GPU race on the shared array."""
+    lib = load()
+    if not points.is_cuda or points.dtype != torch.float32 or not points.is_contiguous() or points.dim() != 2 or points.shape[1] != 3:
+        raise ValueError("points must be a contiguous CUDA float32 tensor [N,3]")
+    M = int(M)
+    if out_idx.dtype != torch.int32 or out_mindist.dtype != torch.float32 or not out_idx.is_contiguous() or not out_mindist.is_contiguous() \
+            or out_idx.device != points.device or out_mindist.device != points.device or out_idx.numel() < M or out_mindist.numel() < M:
+        raise ValueError("out_idx must be contiguous CUDA int32 [M] and out_mindist contiguous CUDA float32 [M]")
+    with torch.cuda.device(points.device):
+        s = stream if stream is not None else torch.cuda.current_stream()
+        rc = lib.fps_sample_noalloc(points.data_ptr(), points.shape[0], M, int(start_idx), int(flags), out_idx.data_ptr(),
+                                    out_mindist.data_ptr(), s.cuda_stream)
     if rc != FPS_OK:
         raise FpsError(rc, fps_last_error())
     return out_idx, out_mindist

@@ -212,6 +212,22 @@ int fps_pick_chain_cycles(int32_t cand_per_lane, int32_t iters, float *cycles_pe
 
 void fps_trim(void) { rfps::trim_pool(); }
 
+int fps_sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx, int32_t flags, int32_t *out_idx, float *out_mindist,
+                       void *stream)
+{
+    rfps::g_err[0] = 0;
+    int rc = FPS_ERR_INVALID;
+    if (!points) set_error("points is NULL");
+    else if (!out_idx || !out_mindist) set_error("output pointer is NULL");
+    else if (N < 1) set_error("N=%d must be >= 1", N);
+    else if (M < 1 || M > N) set_error("M=%d must be in [1, N=%d]", M, N);
+    else if (start_idx < 0 || start_idx >= N) set_error("start_idx=%d must be in [0, N=%d)", start_idx, N);
+    else if (flags & ~FPS_FLAG_EUCLIDEAN) set_error("fps_sample_noalloc takes flags 0 or FPS_FLAG_EUCLIDEAN, got %d", flags);
+    else rc = rfps::sample_noalloc(points, N, M, start_idx, flags, out_idx, out_mindist, (cudaStream_t)stream);
+    if (rc != FPS_OK) rfps::g_status = rc;
+    return rc;
+}
+
 void fps_index_destroy(fps_index_t *h)
 {
     if (!h) return;

@@ -1288,4 +1288,134 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     return per_pick ? choose_launch_shape(ix, o) : choose_batched_shape(ix, o);
 }
 
+// ---------------------------------------------------------------------------------------------
+// fps_sample_noalloc (radiusfps.h): the whole path a1-a13 for ONE cloud of <= FPS_NOALLOC_MAX_N points without a
+// single device allocation.  The voxel index -- everything build_index() carves out of its arena: the sorted point
+// arrays, Dist_p, the voxel and group records, the read-back block -- is scratch memory of such a call, and here it
+// lives in a file-scope device array that every GPU loading the library holds until the process exits.
+//
+// In host code `g_noalloc_scratch` is only a stand-in for the symbol, not a device address: its address is resolved
+// once per device, with that device current, by cudaGetSymbolAddress, and it is this pointer that the kernels get.
+// Every call on a device shares the array and finds the previous call's contents in it; the one block that has to
+// start at zero (meta: the running maximum of the segment sizes) is cleared on the stream before the build kernel;
+// everything else is written before it is read (k_build_fused writes the whole index and the bounding box block,
+// the sampling kernel initialises Dist_p).  Two calls that overlap on the GPU -- different streams without an
+// ordering between them, or two host threads -- race on the array; on one stream they are ordered.
+// ---------------------------------------------------------------------------------------------
+static_assert(FPS_NOALLOC_MAX_N <= FUSED_MAX_N, "the no-allocation entry point uses the single-launch build");
+static __device__ __align__(256) unsigned char g_noalloc_scratch[FPS_NOALLOC_SCRATCH_BYTES];
+
+static int noalloc_scratch_ptr(unsigned char **out)
+{
+    static std::mutex mu;
+    static unsigned char *ptr[64] = {};
+    int dev = 0;
+    RFPS_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) { set_error("device ordinal %d is not supported by fps_sample_noalloc", dev); return FPS_ERR_INVALID; }
+    std::lock_guard<std::mutex> lock(mu);
+    if (!ptr[dev]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_noalloc_scratch);
+        if (e != cudaSuccess || !p) {
+            set_error("cudaGetSymbolAddress(g_noalloc_scratch) failed on device %d: %s", dev, cudaGetErrorString(e));
+            cudaGetLastError();
+            return FPS_ERR_CUDA;
+        }
+        ptr[dev] = static_cast<unsigned char *>(p);
+    }
+    *out = ptr[dev];
+    return FPS_OK;
+}
+
+int sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx, int32_t flags, int32_t *out_idx, float *out_mindist,
+                   cudaStream_t st)
+{
+    if (N > FPS_NOALLOC_MAX_N) {
+        set_error("fps_sample_noalloc: N=%d is above FPS_NOALLOC_MAX_N=%d (the static scratch array holds the index of one cloud of at most "
+                  "that many points); use fps_index_build + fps_sample", N, (int)FPS_NOALLOC_MAX_N);
+        return FPS_ERR_INVALID;
+    }
+    unsigned char *base = nullptr;
+    const int rcp = noalloc_scratch_ptr(&base);
+    if (rcp != FPS_OK) return rcp;
+
+    // the same parameters as build_index() picks for this N
+    int32_t poff_h[2] = {0, N}, K_h[1] = {0};
+    DeviceIndex ix;
+    ix.B = 1; ix.N = N;
+    ix.poff_host = poff_h;            // (stack storage: this index is never handed to free_index)
+    ix.K_host = K_h;
+    ix.last_stream = st;
+    fps_build_opts o;
+    memset(&o, 0, sizeof o);
+    o.flags = flags;
+    o.stream = (void *)st;
+    const int n_vox = auto_n_vox(N);
+    const int tile_points = 64;
+    const int vbits = 3 * ilog2_ceil((unsigned long long)n_vox);
+    const int sb = std::min(4, (32 - vbits) / 3);
+    const int keybits = vbits + 3 * sb;
+    ix.n_vox = n_vox; ix.tile_points = tile_points; ix.flags = flags;
+    const long long cells = (long long)n_vox * n_vox * n_vox;
+    const long long kb = std::min<long long>(std::min<long long>(N, cells) + N / tile_points, N);
+    ix.K_cap = (int)((kb + 31) / 32 * 32);
+    ix.G_cap = ix.K_cap / 32;
+
+    Carver c;
+    c.base = reinterpret_cast<char *>(base);
+    const size_t BN = (size_t)N;
+    ix.px = c.take<float>(BN); ix.py = c.take<float>(BN); ix.pz = c.take<float>(BN);
+    ix.porig = c.take<int32_t>(BN); ix.pinv = c.take<int32_t>(BN); ix.Dp = c.take<float>(BN);
+    ix.vgeom = c.take<float4>((size_t)ix.K_cap);
+    ix.vseg = c.take<int2>((size_t)ix.K_cap);
+    ix.ggeom = c.take<float4>((size_t)ix.G_cap);
+    constexpr size_t RB_N = 1 + 8 + BBOX_STRIDE;          // K, meta, the bounding box block (with the non-finite flag)
+    unsigned *rb = c.take<unsigned>(RB_N);
+    ix.K_dev = reinterpret_cast<int32_t *>(rb);
+    unsigned *meta = rb + 1, *bbox = rb + 1 + 8;
+    ix.poff_dev = c.take<int32_t>(2);
+    ix.counters = c.take<unsigned long long>(NUM_COUNTERS);
+    if (c.off > (size_t)FPS_NOALLOC_SCRATCH_BYTES) {
+        set_error("fps_sample_noalloc: the index of N=%d points needs %zu bytes, the static scratch array holds %zu", N, c.off,
+                  (size_t)FPS_NOALLOC_SCRATCH_BYTES);
+        return FPS_ERR_INVALID;
+    }
+    ix.device_bytes = (int64_t)c.off;
+
+    RFPS_CUDA(cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st));     // the array keeps the last call's contents
+    RFPS_CUDA(cudaMemcpyAsync(ix.poff_dev, poff_h, sizeof poff_h, cudaMemcpyHostToDevice, st));
+    FusedArgs fa;
+    fa.pts = points; fa.poff = ix.poff_dev; fa.bbox = bbox;
+    fa.n_vox = n_vox; fa.hb = vbits / 3; fa.sb = sb; fa.keybits = keybits; fa.tile_points = tile_points;
+    fa.K_cap = ix.K_cap; fa.G_cap = ix.G_cap; fa.Nmax = N;
+    fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
+    fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
+    fa.maxcnt = reinterpret_cast<int *>(meta);
+    RFPS_CUDA(cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)));
+    LaunchLog log;
+    launch_pdl_smem(log, fused_smem_bytes(N), k_build_fused, dim3(1), dim3(FUSED_T), st, fa);
+    {
+        const cudaError_t el = log.first_error != cudaSuccess ? log.first_error : cudaGetLastError();
+        if (el != cudaSuccess) {
+            set_error("the build kernel failed to launch: %s", cudaGetErrorString(el));
+            cudaGetLastError();
+            return FPS_ERR_CUDA;
+        }
+    }
+    // the build's one host round-trip (K sizes the sampling kernel's shared memory; the non-finite flag)
+    unsigned hrb[RB_N];
+    RFPS_CUDA(cudaMemcpyAsync(hrb, rb, sizeof hrb, cudaMemcpyDeviceToHost, st));
+    RFPS_CUDA(cudaStreamSynchronize(st));
+    if (hrb[1 + 8 + 6]) { set_error("the cloud holds a NaN or infinite coordinate"); return FPS_ERR_NONFINITE; }
+    K_h[0] = (int32_t)hrb[0];
+    ix.max_voxel_points = (int)hrb[1];
+    ix.K_max = K_h[0];
+    ix.K_total = K_h[0];
+    ix.build_launches = log.launches;
+    const int rcs = choose_batched_shape(ix, o);
+    if (rcs != FPS_OK) return rcs;
+    if (ix.grid_ctas > 0) { set_error("fps_sample_noalloc: unexpected grid mode"); return FPS_ERR_INVALID; }   // (would allocate exchange blocks)
+    return launch_sample_batched(ix, M, start_idx, nullptr, (int64_t)(M - 1), out_idx, out_mindist, st);
+}
+
 }  // namespace rfps

@@ -108,6 +108,9 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
                           int32_t *out_idx, float *out_mindist, cudaStream_t stream);
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o);
 int measure_pick_chain(int cand_per_lane, int iters, float *cycles_per_pick);
+// fps_sample_noalloc: index in the static device array of index_build.cu, no device allocation anywhere
+int sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx, int32_t flags, int32_t *out_idx, float *out_mindist,
+                   cudaStream_t stream);
 
 }  // namespace rfps
 
