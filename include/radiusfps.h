@@ -59,7 +59,10 @@ typedef struct {
     int32_t cluster_size;  /* CTAs per cloud in the sampling kernel: 0 = choose; 1..16 = one thread-block cluster of
                               that size per cloud (per-pick kernel: 1,2,4,8,16); batched kernel only: -2..-148 =
                               that many CTAs per cloud spread over the whole grid (one picker, the others workers,
-                              exchanging through global memory; needs B * CTAs <= SMs)                      */
+                              exchanging through global memory; needs B * CTAs <= SMs).  With 0, an index whose
+                              clouds all hold <= 4 096 points is sampled by the one-CTA-per-cloud kernel that keeps
+                              the whole cloud in registers (fps_stats.whole_cloud_kernel); any explicit value, a
+                              local_warps other than 0 / 32, or FPS_FLAG_NO_BATCH selects the general kernel       */
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
     int32_t flags;         /* FPS_FLAG_* below                                                          */
     void   *stream;        /* cudaStream_t the build is issued on (0 = the legacy default stream)       */
@@ -135,6 +138,10 @@ typedef struct {
                                  workers: applying what is left of a batch once it is declared complete / the candidate
                                  extraction scans / waiting for the next message                              */
     int64_t worker_pieces;    /* pieces of <= 128 picks applied, summed over all workers                       */
+    int32_t whole_cloud_kernel; /* 1: every cloud holds <= 4 096 points and is sampled by the one-CTA-per-cloud
+                                 kernel (whole cloud in registers, radius prune on runs of 64 sorted points; the
+                                 voxel / point counters then count those runs); 0: the general kernel          */
+    int32_t reserved0;
 } fps_stats;
 
 /*

@@ -51,7 +51,7 @@ class fps_stats(ctypes.Structure):
                 ("cycles_local_update", ctypes.c_int64), ("cycles_local_pairs", ctypes.c_int64),
                 ("cycles_local_publish", ctypes.c_int64), ("cycles_worker_tail", ctypes.c_int64),
                 ("cycles_worker_extract", ctypes.c_int64), ("cycles_worker_idle", ctypes.c_int64),
-                ("worker_pieces", ctypes.c_int64)]
+                ("worker_pieces", ctypes.c_int64), ("whole_cloud_kernel", ctypes.c_int32), ("reserved0", ctypes.c_int32)]
 
     def as_dict(self) -> dict:
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

@@ -248,6 +248,7 @@ int fps_get_stats(fps_index_t *h, fps_stats *out)
     out->build_launches = ix.build_launches;
     out->grid_ctas = ix.grid_ctas;
     out->local_warps = ix.local_warps; out->cand_per_thread = ix.cand_per_thread;
+    out->whole_cloud_kernel = ix.whole ? 1 : 0;
     if (ix.flags & FPS_FLAG_STATS) {
         unsigned long long c[rfps::NUM_COUNTERS];
         RFPS_CUDA(cudaStreamSynchronize(ix.last_stream));

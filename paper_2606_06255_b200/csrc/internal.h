@@ -68,6 +68,7 @@ struct DeviceIndex {
     int32_t local_warps = 0, cand_per_thread = 0, Kc_cap = 0;   // batched kernel: local-phase shape, voxels per CTA
     int32_t grid_ctas = 0;              // batched kernel: > 0 = CTAs per cloud spread over the grid (cooperative launch,
                                         // exchange through global memory); 0 = one cluster of cluster_size CTAs per cloud
+    bool whole = false;                 // every cloud fits one CTA's registers: k_fps_whole (sample_whole.cu) samples it
     void *gx = nullptr;                 // grid mode: the clouds' exchange blocks (allocated by the first fps_sample)
     size_t gx_pitch = 0;
     int32_t flags = 0;

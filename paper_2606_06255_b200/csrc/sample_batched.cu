@@ -17,14 +17,10 @@ namespace rfps {
 
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
 {
-    // Local phase.  Clouds of <= 4 096 points are held whole in the picker's registers (4 candidates
-    // per thread up to 2 048 points, 8 up to 4 096: one round, nothing dies) -- there the hierarchical phase (one
-    // sequential pick warp, 15 warps following its picks) measures fastest; larger clouds work on the top ~1 024
-    // candidates per round with the parallel resolution
-    const bool whole = ix.N <= 4096;
-    // (grid mode: parallel resolution only; Euclidean mode: the parallel resolution applies picks in the squared domain
-    // and takes one square root per candidate and step, the hierarchical phase one per candidate and pick)
-    int LW = o.local_warps > 0 ? o.local_warps : (whole && ix.N > 1024 && o.cluster_size >= 0 && !(o.flags & FPS_FLAG_EUCLIDEAN) ? LW_HIER : LW_PAR);
+    // Local phase.  Clouds of <= 4 096 points are held whole in the registers of one CTA (2
+    // candidates per thread up to 1 024 points, 4 up to 2 048, 8 up to 4 096); larger clouds work on the top ~1 024
+    // candidates per round.  Both resolve the picks of a step in parallel (local_warps = 32) by default
+    int LW = o.local_warps > 0 ? o.local_warps : LW_PAR;
     int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW >= LW_HIER ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : 2))) : (LW == 8 ? 16 : 8));
     bool ok_shape = false;
 #define RFPS_OK(C_, L_) ok_shape |= (CPT == C_ && LW == L_);
@@ -40,6 +36,10 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         return FPS_ERR_INVALID;
     }
     int C = o.cluster_size;
+    // every cloud fits one CTA's registers: k_fps_whole (sample_whole.cu), one CTA per cloud, no workers.  An explicit
+    // cluster size, the flat / hierarchical local phases and FPS_FLAG_NO_BATCH keep the general kernel
+    ix.whole = LW == LW_PAR && CPT <= 8 && ix.N <= cand_capacity(CPT, LW) && C == 0 && !(o.flags & FPS_FLAG_NO_BATCH);
+    if (ix.whole) C = 1;
     const int sms = device_props().sm_count;
     if (C < -sms || C > 16) { set_error("cluster_size=%d must be 0 (choose), 1..16 (CTAs per cluster) or -2..-%d (CTAs per cloud, grid mode)", C, sms); return FPS_ERR_INVALID; }
     if (o.block_threads != 0 && o.block_threads != BT) { set_error("block_threads=%d: the batched kernel runs %d threads per CTA", o.block_threads, BT); return FPS_ERR_INVALID; }
@@ -80,7 +80,7 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
             if (p > 16 && (long long)p * ix.B <= batched_max_resident_ctas(max_smem)) { grid = p; C = p; }
         }
     }
-    if (!fits(C)) {
+    if (!ix.whole && !fits(C)) {
         set_error("K_max=%d voxels do not fit the shared memory of %d CTAs; use a smaller n_vox or a larger tile_points", K, C);
         return FPS_ERR_INVALID;
     }
@@ -129,6 +129,7 @@ int launch_sample_batched(DeviceIndex &ix, int32_t M, int32_t start_idx, const i
     if (ix.flags & FPS_FLAG_STATS) RFPS_CUDA(cudaMemsetAsync(ix.counters, 0, NUM_COUNTERS * sizeof(unsigned long long), st));
     ix.last_iterations = iterations;
     ix.last_stream = st;
+    if (ix.whole) return launch_sample_whole(bp, ix, st);
 #define RFPS_CASE(CPT, LW) if (ix.cand_per_thread == CPT && ix.local_warps == LW) return launch_batched_##CPT##_##LW(bp, ix, st);
     RFPS_BATCHED_SHAPES(RFPS_CASE)
 #undef RFPS_CASE

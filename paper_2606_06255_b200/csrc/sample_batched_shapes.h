@@ -128,6 +128,8 @@ __host__ __device__ inline SmemLayout smem_layout(int Kc_cap, int TC, int LW)
 #define RFPS_DECL_LAUNCH(CPT, LW) int launch_batched_##CPT##_##LW(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st);
 RFPS_BATCHED_SHAPES(RFPS_DECL_LAUNCH)
 #undef RFPS_DECL_LAUNCH
+// small clouds, one CTA per cloud (sample_whole.cu); cand_per_thread 2, 4 or 8
+int launch_sample_whole(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st);
 // how many clusters of `c` CTAs of the default kernel can be resident at once (0 on error)
 int batched_max_resident_clusters(int c, size_t smem);
 // grid mode: how many CTAs of the default kernel fit the device at once

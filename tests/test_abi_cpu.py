@@ -137,7 +137,8 @@ def test_no_packed_fma_in_the_built_kernels():
     for fn, (ffma, fmul, mufu) in counts.items():
         # the Euclidean-mode instantiations (fourth template flag = true) evaluate sqrt_rn at every update:
         # their FFMA are the Newton steps of those square roots; the squared-mode kernels have none there
-        euclid = re.search(r"k_fps_batchedILi\d+ELi\d+ELb[01]ELb1ELb[01]EE", fn) is not None
+        # (k_fps_whole: third template argument)
+        euclid = re.search(r"k_fps_batchedILi\d+ELi\d+ELb[01]ELb1ELb[01]EE|k_fps_wholeILi\d+ELb[01]ELb1EE", fn) is not None
         if "k_fps_" in fn and not euclid:
             assert ffma <= 8 * mufu + 16 and fmul > ffma, (fn, ffma, fmul, mufu)
             checked += 1

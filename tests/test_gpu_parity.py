@@ -599,6 +599,116 @@ def test_integer_grid_overflowing_ties(rf):
     assert st["extract_retries"] > 0 and st["single_picks"] > 0 and st["local_fallbacks"] > 0
 
 
+# ---- the small-cloud kernel (k_fps_whole: every cloud <= 4 096 points, one CTA per cloud, the whole cloud in
+# registers, radius prune on runs of 64 sorted points).  It is the default for such an index; an explicit
+# cluster_size, local_warps = 16 / 8 / 4 / 1 or FPS_FLAG_NO_BATCH select the general kernel (tests above). ----
+
+WHOLE_SIZES = [(1, 1, 0), (2, 2, 1), (63, 63, 5), (64, 20, 63), (65, 65, 64), (127, 40, 0), (129, 129, 128), (1023, 400, 7),
+               (1024, 1024, 1023), (1025, 300, 0), (2047, 2047, 3), (2048, 512, 2047), (2049, 600, 11), (4095, 1024, 4094),
+               (4096, 4096, 0)]
+
+
+@pytest.mark.parametrize("N,M,start", WHOLE_SIZES)
+def test_whole_cloud_kernel_sizes_around_blob_and_register_boundaries(rf, N, M, start):
+    # 64 points per blob, 1 024 points per register position, 512 x {2, 4, 8} capacity; M up to N (beyond the 1 024
+    # picks of the general kernel's batch buffer)
+    P = inputs.uniform_cube(N, 1000 + N)
+    ref = oracle.fps(P, M, start)
+    gi, gm, st = run_gpu(rf, P, M, start)
+    assert st["whole_cloud_kernel"] == 1 and st["cluster_size"] == 1
+    assert st["cand_per_thread"] == (2 if N <= 1024 else 4 if N <= 2048 else 8)
+    assert_same(gi, gm, *ref)
+
+
+@pytest.mark.parametrize("name", ["uniform4096", "lattice", "dups", "line"])
+@pytest.mark.parametrize("flags", [0, 1, 4, 5, 32, 36])
+def test_whole_cloud_kernel_flags(rf, name, flags):
+    # prune off (every pick applied to every blob), STATS build, Euclidean distances: same picks, bit for bit
+    P, M = SMALL[name]()
+    ref = oracle.fps_euclid(P, M, 0) if flags & rf.FPS_FLAG_EUCLIDEAN else oracle.fps(P, M, 0)
+    gi, gm, st = run_gpu(rf, P, M, flags=flags)
+    assert st["whole_cloud_kernel"] == 1
+    assert_same(gi, gm, *ref)
+    if flags & rf.FPS_FLAG_STATS:
+        assert st["iterations"] == M - 1 and st["rounds"] == 1 and st["group_tests"] == 0
+        assert st["voxel_tests"] > 0 and 0 < st["voxels_visited"] <= st["voxel_tests"]
+        if flags & rf.FPS_FLAG_NO_PRUNE:
+            assert st["voxels_visited"] * 2 > st["voxel_tests"]          # only blobs whose distances are all 0 are left out
+        elif name == "uniform4096":
+            assert st["voxels_visited"] * 4 < st["voxel_tests"]          # the prune does remove most (blob, pick) pairs
+
+
+def test_whole_cloud_kernel_tie_heavy_inputs(rf):
+    # exact ties everywhere: the first bin of the selection histogram overflows, the kernel falls back to runs of
+    # single block-wide argmax picks with the lowest-index tie-break; duplicates run out of positive distances
+    g = np.arange(64, dtype=np.float32)
+    grid = np.stack(np.meshgrid(g, g, np.zeros(1, dtype=np.float32)), -1).reshape(-1, 3).astype(np.float32)
+    grid = np.ascontiguousarray(grid[np.random.default_rng(5).permutation(grid.shape[0])])
+    same = np.full((777, 3), -3.5, dtype=np.float32)
+    few = inputs.with_duplicates(4000, 31, 50)
+    for P, M, start in ((grid, 2000, 17), (same, 50, 776), (few, 300, 3999), (inputs.cube_corners(), 8, 0)):
+        ref = oracle.fps(P, M, start)
+        gi, gm, st = run_gpu(rf, P, M, start, flags=rf.FPS_FLAG_STATS)
+        assert st["whole_cloud_kernel"] == 1
+        assert_same(gi, gm, *ref)
+    assert st["single_picks"] > 0
+
+
+def test_whole_cloud_kernel_batches_uniform_and_ragged(rf):
+    # more clouds than SMs; a ragged index with per-cloud M and start; repeat calls on one handle
+    P = np.stack([inputs.uniform_cube(1500, 300 + b) if b % 2 else inputs.room(1500, 300 + b) for b in range(170)])
+    ref = oracle.fps(P, 400, 3)
+    Pd = torch.from_numpy(P).cuda()
+    ix = rf.fps_index_build(Pd)
+    try:
+        assert rf.fps_get_stats(ix)["whole_cloud_kernel"] == 1
+        for _ in range(2):
+            idx, mind = rf.fps_sample(ix, 400, 3)
+            torch.cuda.synchronize()
+            assert_same(idx.cpu().numpy(), mind.cpu().numpy(), *ref)
+    finally:
+        rf.fps_index_destroy(ix)
+    clouds = [inputs.room(4096, 41), inputs.uniform_cube(1, 42), inputs.lidar(3001, 43, n_azimuth=60), inputs.shuffled_lattice(8, 44),
+              inputs.uniform_cube(33, 45), inputs.clustered(2500, 46), inputs.with_duplicates(900, 47, 200)]
+    Ms = [4096, 1, 1800, 512, 33, 600, 450]
+    starts = [0, 0, 3000, 5, 32, 17, 899]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])]).astype(np.int64)
+    Pr = torch.from_numpy(np.ascontiguousarray(np.concatenate(clouds, axis=0))).cuda()
+    ix = rf.fps_index_build_ragged(Pr, off.tolist())
+    try:
+        assert rf.fps_get_stats(ix)["whole_cloud_kernel"] == 1
+        for ms, ss in ((Ms, starts), ([min(m, 9) for m in Ms], None)):
+            idx, mind, ooff = rf.fps_sample_ragged(ix, ms, ss)
+            torch.cuda.synchronize()
+            idx, mind = idx.cpu().numpy(), mind.cpu().numpy()
+            for b, c in enumerate(clouds):
+                ref_i, ref_m = oracle.fps(c, ms[b], ss[b] if ss else 0)
+                assert_same(idx[ooff[b]:ooff[b + 1]], mind[ooff[b]:ooff[b + 1]], ref_i.reshape(-1), ref_m.reshape(-1))
+    finally:
+        rf.fps_index_destroy(ix)
+
+
+def test_whole_cloud_kernel_overflowing_distances_and_scales(rf):
+    # d2 overflows to +inf for the first picks (coordinates ~1e19..1e20): single picks until every distance is finite
+    base = inputs.uniform_cube(2000, 51)
+    big = (base * np.float32(2e19)).astype(np.float32)
+    for P in (big, (base * np.float32(1e-12)).astype(np.float32), (base + np.float32(4096.0)).astype(np.float32)):
+        ref = oracle.fps(P, 500, 0)
+        gi, gm, st = run_gpu(rf, P, 500)
+        assert st["whole_cloud_kernel"] == 1
+        assert_same(gi, gm, *ref)
+    assert np.isinf(oracle.fps(big, 3, 0)[1].reshape(-1)[1])       # the case does overflow
+
+
+def test_small_clouds_general_kernel_still_selectable(rf):
+    P, M = SMALL["uniform4096"]()
+    ref = oracle.fps(P, M, 0)
+    for opts in (dict(cluster_size=4), dict(local_warps=16), dict(flags=rf.FPS_FLAG_NO_BATCH), dict(cluster_size=1)):
+        gi, gm, st = run_gpu(rf, P, M, **opts)
+        assert st["whole_cloud_kernel"] == 0
+        assert_same(gi, gm, *ref)
+
+
 def test_host_entry_point(rf):
     w = inputs.scaled("C4", 4000, 900, B=2)
     P = inputs.make_batch(w)
