@@ -1412,9 +1412,14 @@ int sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx,
     ix.K_max = K_h[0];
     ix.K_total = K_h[0];
     ix.build_launches = log.launches;
-    const int rcs = choose_batched_shape(ix, o);
+    int rcs = choose_batched_shape(ix, o);
+    if (rcs == FPS_OK && ix.grid_ctas > 0) {               // grid mode would allocate exchange blocks: one cluster instead
+        fps_build_opts oc = o;
+        oc.cluster_size = std::max(1, std::min(8, N / 1024));
+        rcs = choose_batched_shape(ix, oc);
+    }
     if (rcs != FPS_OK) return rcs;
-    if (ix.grid_ctas > 0) { set_error("fps_sample_noalloc: unexpected grid mode"); return FPS_ERR_INVALID; }   // (would allocate exchange blocks)
+    if (ix.grid_ctas > 0) { set_error("fps_sample_noalloc: unexpected grid mode"); return FPS_ERR_INVALID; }
     return launch_sample_batched(ix, M, start_idx, nullptr, (int64_t)(M - 1), out_idx, out_mindist, st);
 }
 

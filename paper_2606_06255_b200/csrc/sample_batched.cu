@@ -71,13 +71,15 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
             if (batched_max_resident_clusters(c, max_smem) >= std::min(want, sms / c)) { C = c; break; }   // the launch takes all shared memory
         }
         while (C < 16 && !fits(C)) ++C;
-        // A batch of one or two large clouds leaves most of the GPU idle with one cluster per cloud: spread each cloud
-        // over the grid instead -- one picker CTA and up to sms / B - 1 workers, every worker >= 1 group of voxels
-        // and >= ~1 000 points (measured: C3 4.0 -> 3.9 ms, C5 9.3 -> 7.7 ms; no gain for four clouds or more)
-        if (LW == LW_PAR && C == 16 && ix.B * 64 <= sms) {
+        // Clusters leave part of the GPU idle (a cluster lives inside one GPC and holds <= 16 CTAs): where spreading each
+        // cloud over the grid gives it at least a third more CTAs -- one picker CTA and up to sms / B - 1 workers, every
+        // worker >= 1 group of voxels and >= ~1 000 points -- that is what runs (measured: C5 9.3 -> 7.7 ms with 148
+        // CTAs instead of 16, C3 4.0 -> 3.9 ms with 119, C4 3.69 -> 3.55 ms with 4 x 37, C2 1.07 -> 1.04 ms with 16 x 9
+        // instead of 16 x 6)
+        if (LW == LW_PAR && C > 1 && ix.B * 2 <= sms) {
             int p = std::min(sms / ix.B, std::min(G + 1, ix.N / 1024 + 1));
-            while (p > 16 && !fits(p)) --p;
-            if (p > 16 && (long long)p * ix.B <= batched_max_resident_ctas(max_smem)) { grid = p; C = p; }
+            while (p > C && !fits(p)) --p;
+            if (p >= C + std::max(2, C / 3) && (long long)p * ix.B <= batched_max_resident_ctas(max_smem)) { grid = p; C = p; }
         }
     }
     if (!ix.whole && !fits(C)) {

@@ -952,17 +952,19 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
             const int j0 = lane, j1 = lane + 32;
             const bool v0 = j0 < n, v1 = j1 < n;
             const float4 c0 = v0 ? ps->sC[j0] : make_float4(0.f, 0.f, 0.f, 0.f), c1 = v1 ? ps->sC[j1] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const unsigned o0 = v0 ? ps->sO[j0] : 0u, o1 = v1 ? ps->sO[j1] : 0u;
+            // rank key (distance bits, ~orig): unsigned order = "larger distance first, ties to the lowest index"; the keys
+            // of two different points differ, and an absent partner (key 0) ranks before nobody (members are > tau >= 0)
+            const unsigned long long k0 = v0 ? ((unsigned long long)__float_as_uint(c0.w) << 32) | ps->sO[j0] : 0ull;
+            const unsigned long long k1 = v1 ? ((unsigned long long)__float_as_uint(c1.w) << 32) | ps->sO[j1] : 0ull;
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
                 const int i = 4 * warp + ii;
                 if (i >= n) break;                           // warp-uniform
                 const float4 ci = ps->sC[i];
-                const unsigned oi = ps->sO[i];
+                const unsigned long long ki = ((unsigned long long)__float_as_uint(ci.w) << 32) | ps->sO[i];
                 const float d0 = distf<EUC>(d2_rn(ci.x, ci.y, ci.z, c0.x, c0.y, c0.z));
                 const float d1 = distf<EUC>(d2_rn(ci.x, ci.y, ci.z, c1.x, c1.y, c1.z));
-                const bool b0 = v0 && j0 != i && (c0.w > ci.w || (c0.w == ci.w && o0 > oi));
-                const bool b1 = v1 && j1 != i && (c1.w > ci.w || (c1.w == ci.w && o1 > oi));
+                const bool b0 = k0 > ki, b1 = k1 > ki;
                 const bool l0 = b0 && d0 < ci.w, l1 = b1 && d1 < ci.w;
                 const unsigned bw0 = __ballot_sync(FULL, b0), bw1 = __ballot_sync(FULL, b1);
                 const unsigned aw0 = __ballot_sync(FULL, l0), aw1 = __ballot_sync(FULL, l1);

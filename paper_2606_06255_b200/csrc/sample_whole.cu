@@ -42,8 +42,6 @@ struct __align__(16) WholeSmem {
     uint4 wb[16];
     unsigned wmax[16];
     unsigned stop[2];              // bit i: a member of aff_i may leave D_i >= the smallest member distance
-    int nmem;
-    unsigned minD;                 // smallest member distance (bits)
     int npk;                       // picks accepted by the step
     unsigned hi;                   // upper bound of every distance after the step (bits)
     float4 pick[KS];               // the step's picks {x, y, z, -}
@@ -130,7 +128,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     ws->hist[0][warp][lane] = 0;
     ws->hist[1][warp][lane] = 0;
     if (tid == 0) {
-        ws->nmem = 0; ws->minD = 0xffffffffu; ws->stop[0] = ws->stop[1] = 0u;
+        ws->stop[0] = ws->stop[1] = 0u;
         out_idx[0] = startb;
         out_mind[0] = inf;
     }
@@ -302,7 +300,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
         // positive constant are monotone
 #define RFPS_BIN(d) ((int)fminf(fmaxf(__fmul_rn(__fsub_rn(hi, (d)), scale), 0.0f), 31.0f))
         int bin[CPT1];
-        int bstar = 0, total = 0;
+        int bstar = 0, total = 0, nmem = 0, mbase = 0;
         if (finite) {
             // ---- (1) per-warp histogram of the points above blo; blobs whose Dist_v is not above it are skipped whole ----
             const unsigned blobits = __float_as_uint(blo);
@@ -321,9 +319,13 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             __syncthreads();
             ws->hist[hp ^ 1][warp][lane] = 0;                // the other buffer: every warp is done with it
             __syncwarp();
-            int tot = 0;
+            int tot = 0, before = 0;                         // bin `lane`: all warps / the warps before this one
 #pragma unroll
-            for (int w = 0; w < BT / 32; ++w) tot += ws->hist[hp][w][lane];
+            for (int w = 0; w < BT / 32; ++w) {
+                const int v = ws->hist[hp][w][lane];
+                tot += v;
+                before += w < warp ? v : 0;
+            }
             int incl = tot;
 #pragma unroll
             for (int o = 1; o < 32; o <<= 1) {
@@ -332,6 +334,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             }
             total = __shfl_sync(FULL, incl, 31);
             bstar = __popc(__ballot_sync(FULL, incl <= KS));
+            // members = the points of the bins < bstar: their number, and how many of them the warps before this one hold
+            nmem = bstar > 0 ? __shfl_sync(FULL, incl, bstar - 1) : 0;
+            mbase = __reduce_add_sync(FULL, lane < bstar ? before : 0);
             if (total == 0) {
                 // nothing above blo: blo is a bound of everything (it replaces hi), or -- blo == 0 -- nothing is left
                 if (blo == 0.0f) { hibits = 0u; break; }
@@ -376,10 +381,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
                 cntw += __popc(bal[c]);
             }
             if (cntw) {
-                int base = 0;
-                if (lane == 0) base = atomicAdd(&ws->nmem, cntw);
-                base = __shfl_sync(FULL, base, 0);
-                unsigned mind = 0xffffffffu;
+                int base = mbase;
 #pragma unroll
                 for (int c = 0; c < CPT1; ++c) {
                     if (bin[c] < bstar) {
@@ -390,36 +392,37 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
                         unpack2(Z[c >> 1], z0, z1);
                         ws->sC[sl] = make_float4((c & 1) ? x1 : x0, (c & 1) ? y1 : y0, (c & 1) ? z1 : z0, D[c]);
                         ws->sO[sl] = cO[(c >> 1) * 2 * BT + 2 * tid + (c & 1)];
-                        mind = min(mind, __float_as_uint(D[c]));
                     }
                     base += __popc(bal[c]);
                 }
-                mind = __reduce_min_sync(FULL, mind);
-                if (lane == 0) atomicMin(&ws->minD, mind);
             }
         }
         __syncthreads();
-        const int n = ws->nmem;
-        const unsigned thmbits = ws->minD;
+        const int n = nmem;
         if (STATS) { tt1 = clock64(); t_sel += tt1 - tt0; tt0 = tt1; }
         // ---- (3) all pairs: warp w takes the members i = 4w .. 4w+3 in turn, its lanes the partners j = lane and
         // lane + 32 (loaded once, consecutive addresses); a mask word is then ONE ballot ----
+        unsigned thmbits;
         {
-            const float thm = __uint_as_float(thmbits);
             const int j0 = lane, j1 = lane + 32;
             const bool v0 = j0 < n, v1 = j1 < n;
             const float4 c0 = v0 ? ws->sC[j0] : make_float4(0.f, 0.f, 0.f, 0.f), c1 = v1 ? ws->sC[j1] : make_float4(0.f, 0.f, 0.f, 0.f);
-            const unsigned o0 = v0 ? ws->sO[j0] : 0u, o1 = v1 ? ws->sO[j1] : 0u;
+            // rank key (distance bits, ~orig): unsigned order = "larger distance first, ties to the lowest index"; the keys
+            // of two different points differ, and an absent partner (key 0) ranks before nobody
+            const unsigned long long k0 = v0 ? ((unsigned long long)__float_as_uint(c0.w) << 32) | ws->sO[j0] : 0ull;
+            const unsigned long long k1 = v1 ? ((unsigned long long)__float_as_uint(c1.w) << 32) | ws->sO[j1] : 0ull;
+            // smallest member distance (members are > 0, so the bits order like the values)
+            thmbits = __reduce_min_sync(FULL, min(v0 ? __float_as_uint(c0.w) : 0xffffffffu, v1 ? __float_as_uint(c1.w) : 0xffffffffu));
+            const float thm = __uint_as_float(thmbits);
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
                 const int i = 4 * warp + ii;
                 if (i >= n) break;                           // warp-uniform
                 const float4 ci = ws->sC[i];
-                const unsigned oi = ws->sO[i];
+                const unsigned long long ki = ((unsigned long long)__float_as_uint(ci.w) << 32) | ws->sO[i];
                 const float d0 = distf<EUC>(d2_rn(ci.x, ci.y, ci.z, c0.x, c0.y, c0.z));
                 const float d1 = distf<EUC>(d2_rn(ci.x, ci.y, ci.z, c1.x, c1.y, c1.z));
-                const bool b0 = v0 && j0 != i && (c0.w > ci.w || (c0.w == ci.w && o0 > oi));
-                const bool b1 = v1 && j1 != i && (c1.w > ci.w || (c1.w == ci.w && o1 > oi));
+                const bool b0 = k0 > ki, b1 = k1 > ki;
                 const bool l0 = b0 && d0 < ci.w, l1 = b1 && d1 < ci.w;
                 const unsigned bw0 = __ballot_sync(FULL, b0), bw1 = __ballot_sync(FULL, b1);
                 const unsigned aw0 = __ballot_sync(FULL, l0), aw1 = __ballot_sync(FULL, l1);
@@ -442,7 +445,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             const float4 ca = va ? ws->sC[ia] : make_float4(0.f, 0.f, 0.f, 0.f), cb = vb ? ws->sC[ib] : make_float4(0.f, 0.f, 0.f, 0.f);
             const bool sta = (ws->stop[0] >> lane) & 1u, stb = (ws->stop[1] >> lane) & 1u;
             __syncwarp();
-            if (lane == 0) { ws->stop[0] = ws->stop[1] = 0u; ws->nmem = 0; ws->minD = 0xffffffffu; }   // for the next step
+            if (lane == 0) ws->stop[0] = ws->stop[1] = 0u;   // for the next step
             bool acca = false, accb = false, reja = !va, rejb = !vb;
             unsigned long long A = 0ull, R = ballot64(reja, rejb);
             for (;;) {
