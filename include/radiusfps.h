@@ -60,7 +60,7 @@ typedef struct {
                               that size per cloud (per-pick kernel: 1,2,4,8,16); batched kernel only: -2..-148 =
                               that many CTAs per cloud spread over the whole grid (one picker, the others workers,
                               exchanging through global memory; needs B * CTAs <= SMs).  With 0, an index whose
-                              clouds all hold <= 4 096 points is sampled by the one-CTA-per-cloud kernel that keeps
+                              clouds all hold <= 8 192 points is sampled by the one-CTA-per-cloud kernel that keeps
                               the whole cloud in registers (fps_stats.whole_cloud_kernel); any explicit value, a
                               local_warps other than 0 / 32, or FPS_FLAG_NO_BATCH selects the general kernel       */
     int32_t block_threads; /* threads per CTA: 0 = choose; 128..1024, multiple of 32                    */
@@ -71,7 +71,8 @@ typedef struct {
                               16 = hierarchical (all 16 warps hold candidates, one warp picks sequentially from the
                               top <= 96 of them); 4, 1, 8 = flat FPS on that many warps                          */
     int32_t cand_per_thread; /* candidates per thread (registers): 0 = choose; 2, 4, 8 with local_warps 32 / 16
-                              (capacity 512 * cand_per_thread); flat shapes: 8 with 4 or 1 warps, 16 with 8        */
+                              (capacity 512 * cand_per_thread; 16 with local_warps 32 for clouds of <= 8 192 points,
+                              small-cloud kernel only); flat shapes: 8 with 4 or 1 warps, 16 with 8                */
 } fps_build_opts;
 
 enum {
@@ -138,7 +139,7 @@ typedef struct {
                                  workers: applying what is left of a batch once it is declared complete / the candidate
                                  extraction scans / waiting for the next message                              */
     int64_t worker_pieces;    /* pieces of <= 128 picks applied, summed over all workers                       */
-    int32_t whole_cloud_kernel; /* 1: every cloud holds <= 4 096 points and is sampled by the one-CTA-per-cloud
+    int32_t whole_cloud_kernel; /* 1: every cloud holds <= 8 192 points and is sampled by the one-CTA-per-cloud
                                  kernel (whole cloud in registers, radius prune on runs of 64 sorted points; the
                                  voxel / point counters then count those runs); 0: the general kernel          */
     int32_t reserved0;

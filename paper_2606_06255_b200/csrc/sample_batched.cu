@@ -17,12 +17,18 @@ namespace rfps {
 
 int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
 {
-    // Local phase.  Clouds of <= 4 096 points are held whole in the registers of one CTA (2
-    // candidates per thread up to 1 024 points, 4 up to 2 048, 8 up to 4 096); larger clouds work on the top ~1 024
-    // candidates per round.  Both resolve the picks of a step in parallel (local_warps = 32) by default
+    // Local phase.  Clouds of <= 8 192 points are held whole in the registers of one CTA (2 points
+    // per thread up to 1 024 points, 4 up to 2 048, 8 up to 4 096, 16 up to 8 192: k_fps_whole, sample_whole.cu -- one
+    // CTA per cloud, no workers); larger clouds work on the top ~1 024 candidates per round.  Both resolve the picks of
+    // a step in parallel (local_warps = 32) by default.  An explicit cluster size, the flat / hierarchical local phases
+    // and FPS_FLAG_NO_BATCH keep the general kernel for small clouds too
     int LW = o.local_warps > 0 ? o.local_warps : LW_PAR;
-    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread : (LW >= LW_HIER ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : 2))) : (LW == 8 ? 16 : 8));
-    bool ok_shape = false;
+    int C = o.cluster_size;
+    const bool whole_ok = LW == LW_PAR && C == 0 && !(o.flags & FPS_FLAG_NO_BATCH);
+    int CPT = o.cand_per_thread > 0 ? o.cand_per_thread
+              : (LW >= LW_HIER ? (ix.N <= 1024 ? 2 : (ix.N <= 2048 ? 4 : (ix.N <= 4096 ? 8 : (ix.N <= 8192 && whole_ok ? 16 : 2)))) : (LW == 8 ? 16 : 8));
+    ix.whole = whole_ok && CPT <= 16 && ix.N <= cand_capacity(CPT, LW);
+    bool ok_shape = ix.whole && (CPT == 2 || CPT == 4 || CPT == 8 || CPT == 16);
 #define RFPS_OK(C_, L_) ok_shape |= (CPT == C_ && LW == L_);
     RFPS_BATCHED_SHAPES(RFPS_OK)
 #undef RFPS_OK
@@ -31,14 +37,10 @@ int choose_batched_shape(DeviceIndex &ix, const fps_build_opts &o)
         return FPS_ERR_INVALID;
     }
     if (!ok_shape) {
-        set_error("local_warps=%d / cand_per_thread=%d: use 32 (parallel resolution) or 16 (hierarchical) with 2, 4 or 8, or the flat "
-                  "shapes 4 x 8, 1 x 8, 8 x 16", LW, CPT);
+        set_error("local_warps=%d / cand_per_thread=%d: use 32 (parallel resolution) or 16 (hierarchical) with 2, 4 or 8 (32 with 16 "
+                  "for clouds of <= 8192 points), or the flat shapes 4 x 8, 1 x 8, 8 x 16", LW, CPT);
         return FPS_ERR_INVALID;
     }
-    int C = o.cluster_size;
-    // every cloud fits one CTA's registers: k_fps_whole (sample_whole.cu), one CTA per cloud, no workers.  An explicit
-    // cluster size, the flat / hierarchical local phases and FPS_FLAG_NO_BATCH keep the general kernel
-    ix.whole = LW == LW_PAR && CPT <= 8 && ix.N <= cand_capacity(CPT, LW) && C == 0 && !(o.flags & FPS_FLAG_NO_BATCH);
     if (ix.whole) C = 1;
     const int sms = device_props().sm_count;
     if (C < -sms || C > 16) { set_error("cluster_size=%d must be 0 (choose), 1..16 (CTAs per cluster) or -2..-%d (CTAs per cloud, grid mode)", C, sms); return FPS_ERR_INVALID; }

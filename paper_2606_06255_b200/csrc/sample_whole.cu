@@ -1,4 +1,4 @@
-// sample_whole.cu -- steps a7-a13 for SMALL clouds (every cloud of the index holds <= 4 096 points): the whole
+// sample_whole.cu -- steps a7-a13 for SMALL clouds (every cloud of the index holds <= 8 192 points): the whole
 // cloud lives in the registers of ONE CTA (k_fps_whole; one CTA per cloud, no cluster, no worker CTAs, no
 // global rounds).  It is the first sampling layer of a point-cloud network (B x 1 024 .. 4 096 points) and
 // BASELINE.json's config 1.
@@ -33,6 +33,8 @@ namespace rfps {
 // (24, 4, 5) is within 2 % of the best of six settings on every one of them
 constexpr int SINGLES_FIRST = 24, SINGLES_AFTER = 4, STEP_MIN_YIELD = 5;
 
+constexpr int WHOLE_HR16 = 2;       // 16 points per thread: coordinate pairs kept in registers (the other 6 live in shared memory)
+
 struct __align__(16) WholeSmem {
     float4 sC[KS];                 // members {x, y, z, D}
     unsigned long long aff[KS];    // members ranked before i whose pick would lower D_i
@@ -45,7 +47,7 @@ struct __align__(16) WholeSmem {
     int npk;                       // picks accepted by the step
     unsigned hi;                   // upper bound of every distance after the step (bits)
     float4 pick[KS];               // the step's picks {x, y, z, -}
-    float4 bmin[64], bmax[64];     // box of blob q = warp + 16 h
+    float4 bmin[128], bmax[128];   // box of blob q = warp + 16 h
     float4 sp[2][16];              // single picks: every warp's best point {x, y, z, ~orig}, double-buffered by pick parity
     unsigned spd[2][16];           //               and its distance (bits)
 };
@@ -74,11 +76,14 @@ __device__ __forceinline__ float box_lb(const float4 lo, const float4 hi, const 
 template <int CPT1, bool STATS, bool EUC>
 __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const int flags)
 {
-    static_assert(CPT1 % 2 == 0 && CPT1 <= 8 && BT == 512 && KS == 64, "shape");
-    constexpr int H1 = CPT1 / 2, TC = CPT1 * BT;
+    static_assert(CPT1 % 2 == 0 && CPT1 <= 16 && BT == 512 && KS == 64, "shape");
+    // H1 pairs of points per thread: the coordinates of the first HR pairs live in registers, those of the other HS
+    // (clouds of 4 097 .. 8 192 points) in shared memory; every distance lives in a register
+    constexpr int H1 = CPT1 / 2, TC = CPT1 * BT, HR = H1 <= 4 ? H1 : WHOLE_HR16, HS = H1 - HR;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     unsigned *cO = reinterpret_cast<unsigned *>(smem_raw);                    // [TC] ~orig of sorted position i
-    WholeSmem *ws = reinterpret_cast<WholeSmem *>(smem_raw + sizeof(unsigned) * TC);
+    f32x2 *sXYZ = reinterpret_cast<f32x2 *>(smem_raw + sizeof(unsigned) * TC);   // [3][HS][BT] packed coordinate pairs
+    WholeSmem *ws = reinterpret_cast<WholeSmem *>(smem_raw + sizeof(unsigned) * TC + sizeof(f32x2) * 3 * HS * BT);
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const unsigned lt = (1u << lane) - 1u;
     const bool no_prune = flags & FPS_FLAG_NO_PRUNE;
@@ -98,9 +103,14 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     // ---- a7 + the initial update (Eq. 13-14): Dist_p = d(p, s_0), straight into registers ----
     const int p0 = P.pinv[po + startb];
     const float s0x = px[p0], s0y = py[p0], s0z = pz[p0];
-    f32x2 X[H1], Y[H1], Z[H1];
+    f32x2 X[HR], Y[HR], Z[HR];
     float D[CPT1];
+    // coordinate pair h of this thread (h is a compile-time constant wherever this is called)
+    auto cx = [&](const int h) -> f32x2 { return h < HR ? X[h < HR ? h : 0] : sXYZ[(0 * HS + (h - HR)) * BT + tid]; };
+    auto cy = [&](const int h) -> f32x2 { return h < HR ? Y[h < HR ? h : 0] : sXYZ[(1 * HS + (h - HR)) * BT + tid]; };
+    auto cz = [&](const int h) -> f32x2 { return h < HR ? Z[h < HR ? h : 0] : sXYZ[(2 * HS + (h - HR)) * BT + tid]; };
     unsigned Dm[H1];                     // Dist_v of the warp's blobs (bits; warp-uniform)
+    unsigned long long c_eff = 0;        // STATS: effective updates (Eq. 2), the initial one included
     const float inf = __uint_as_float(F32_INF_BITS);
 #pragma unroll
     for (int h = 0; h < H1; ++h) {
@@ -108,11 +118,18 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
         const bool ok0 = i0 < Nb, ok1 = i1 < Nb;
         const float x0 = ok0 ? px[i0] : 0.0f, y0 = ok0 ? py[i0] : 0.0f, z0 = ok0 ? pz[i0] : 0.0f;
         const float x1 = ok1 ? px[i1] : 0.0f, y1 = ok1 ? py[i1] : 0.0f, z1 = ok1 ? pz[i1] : 0.0f;
-        X[h] = pack2(x0, x1);
-        Y[h] = pack2(y0, y1);
-        Z[h] = pack2(z0, z1);
+        if (h < HR) {
+            X[h < HR ? h : 0] = pack2(x0, x1);
+            Y[h < HR ? h : 0] = pack2(y0, y1);
+            Z[h < HR ? h : 0] = pack2(z0, z1);
+        } else {
+            sXYZ[(0 * HS + (h - HR)) * BT + tid] = pack2(x0, x1);
+            sXYZ[(1 * HS + (h - HR)) * BT + tid] = pack2(y0, y1);
+            sXYZ[(2 * HS + (h - HR)) * BT + tid] = pack2(z0, z1);
+        }
         D[2 * h] = ok0 ? distf<EUC>(d2_rn(x0, y0, z0, s0x, s0y, s0z)) : 0.0f;      // padding: D = 0 is never picked
         D[2 * h + 1] = ok1 ? distf<EUC>(d2_rn(x1, y1, z1, s0x, s0y, s0z)) : 0.0f;
+        if (STATS) c_eff += (ok0 ? 1 : 0) + (ok1 ? 1 : 0);
         cO[i0] = ok0 ? ~(unsigned)porig[i0] : 0u;
         cO[i1] = ok1 ? ~(unsigned)porig[i1] : 0u;
         // the blob's box over its real points (an empty blob gets lo = +inf, hi = -inf: every bound is +inf)
@@ -133,7 +150,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
         out_mind[0] = inf;
     }
     int jl = 1;
-    unsigned long long c_steps = 0, c_fallback = 0, c_vtest = 0, c_vvisit = 0, c_pvisit = 0, c_eff = 0;
+    unsigned long long c_steps = 0, c_fallback = 0, c_vtest = 0, c_vvisit = 0, c_pvisit = 0;
     long long t_sel = 0, t_pairs = 0, t_pick = 0, t_upd = 0, t_single = 0, tt0 = 0, tt1 = 0;
 
     auto block_max = [&]() -> unsigned {
@@ -167,8 +184,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             // Euclidean mode: min and the monotone sqrt_rn commute, so the picks are applied in the squared domain
             // and folded into the distances once
             float a0 = EUC ? inf : D[2 * h], a1 = EUC ? inf : D[2 * h + 1];
+            const f32x2 xh = cx(h), yh = cy(h), zh = cz(h);
             auto one = [&](const float4 s) {
-                const f32x2 dx = sub2(X[h], pack2(s.x, s.x)), dy = sub2(Y[h], pack2(s.y, s.y)), dz = sub2(Z[h], pack2(s.z, s.z));
+                const f32x2 dx = sub2(xh, pack2(s.x, s.x)), dy = sub2(yh, pack2(s.y, s.y)), dz = sub2(zh, pack2(s.z, s.z));
                 float x0, x1, y0, y1, z0, z1;
                 unpack2(mul2(dx, dx), x0, x1);
                 unpack2(mul2(dy, dy), y0, y1);
@@ -225,9 +243,9 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             for (int c = 0; c < CPT1; ++c)
                 if (c == ci) {
                     float a0, a1;
-                    unpack2(X[c >> 1], a0, a1); bx = (c & 1) ? a1 : a0;
-                    unpack2(Y[c >> 1], a0, a1); by = (c & 1) ? a1 : a0;
-                    unpack2(Z[c >> 1], a0, a1); bz = (c & 1) ? a1 : a0;
+                    unpack2(cx(c >> 1), a0, a1); bx = (c & 1) ? a1 : a0;
+                    unpack2(cy(c >> 1), a0, a1); by = (c & 1) ? a1 : a0;
+                    unpack2(cz(c >> 1), a0, a1); bz = (c & 1) ? a1 : a0;
                 }
             ws->sp[spar][warp] = make_float4(bx, by, bz, __uint_as_float(wo));
             ws->spd[spar][warp] = wm;
@@ -254,7 +272,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
                 if (distf<EUC>(lb) >= __uint_as_float(Dm[h])) continue;       // warp-uniform
             }
             if (STATS) { c_vvisit++; c_pvisit += 64ull; }
-            const f32x2 dx = sub2(X[h], pack2(s.x, s.x)), dy = sub2(Y[h], pack2(s.y, s.y)), dz = sub2(Z[h], pack2(s.z, s.z));
+            const f32x2 dx = sub2(cx(h), pack2(s.x, s.x)), dy = sub2(cy(h), pack2(s.y, s.y)), dz = sub2(cz(h), pack2(s.z, s.z));
             float x0, x1, y0, y1, z0, z1;
             unpack2(mul2(dx, dx), x0, x1);
             unpack2(mul2(dy, dy), y0, y1);
@@ -299,21 +317,16 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
         // bin(d): 0 for d = hi, growing as d falls; monotone because fp32 subtraction and multiplication by a
         // positive constant are monotone
 #define RFPS_BIN(d) ((int)fminf(fmaxf(__fmul_rn(__fsub_rn(hi, (d)), scale), 0.0f), 31.0f))
-        int bin[CPT1];
         int bstar = 0, total = 0, nmem = 0, mbase = 0;
+        const unsigned blobits = __float_as_uint(blo);
         if (finite) {
             // ---- (1) per-warp histogram of the points above blo; blobs whose Dist_v is not above it are skipped whole ----
-            const unsigned blobits = __float_as_uint(blo);
 #pragma unroll
             for (int h = 0; h < H1; ++h) {
-                bin[2 * h] = bin[2 * h + 1] = 32;
                 if (Dm[h] > blobits) {                       // warp-uniform
 #pragma unroll
                     for (int c = 2 * h; c < 2 * h + 2; ++c)
-                        if (D[c] > blo) {
-                            bin[c] = RFPS_BIN(D[c]);
-                            atomicAdd(&ws->hist[hp][warp][bin[c]], 1);
-                        }
+                        if (D[c] > blo) atomicAdd(&ws->hist[hp][warp][RFPS_BIN(D[c])], 1);
                 }
             }
             __syncthreads();
@@ -371,29 +384,30 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
             refine = 0;
             continue;
         }
-        // ---- (2) members (bin < bstar) -> shared memory ----
+        // ---- (2) members (bin < bstar) -> shared memory, in the order (warp, blob, point) the histogram rows give ----
         {
-            unsigned bal[CPT1];
-            int cntw = 0;
+            int base = mbase;
 #pragma unroll
-            for (int c = 0; c < CPT1; ++c) {
-                bal[c] = __ballot_sync(FULL, bin[c] < bstar);
-                cntw += __popc(bal[c]);
-            }
-            if (cntw) {
-                int base = mbase;
-#pragma unroll
-                for (int c = 0; c < CPT1; ++c) {
-                    if (bin[c] < bstar) {
-                        const int sl = base + __popc(bal[c] & lt);
-                        float x0, x1, y0, y1, z0, z1;
-                        unpack2(X[c >> 1], x0, x1);
-                        unpack2(Y[c >> 1], y0, y1);
-                        unpack2(Z[c >> 1], z0, z1);
-                        ws->sC[sl] = make_float4((c & 1) ? x1 : x0, (c & 1) ? y1 : y0, (c & 1) ? z1 : z0, D[c]);
-                        ws->sO[sl] = cO[(c >> 1) * 2 * BT + 2 * tid + (c & 1)];
+            for (int h = 0; h < H1; ++h) {
+                if (!(Dm[h] > blobits)) continue;                // warp-uniform: no point of this blob was counted
+                const bool m0 = D[2 * h] > blo && RFPS_BIN(D[2 * h]) < bstar, m1 = D[2 * h + 1] > blo && RFPS_BIN(D[2 * h + 1]) < bstar;
+                const unsigned b0 = __ballot_sync(FULL, m0), b1 = __ballot_sync(FULL, m1);
+                if (b0 | b1) {
+                    float x0, x1, y0, y1, z0, z1;
+                    unpack2(cx(h), x0, x1);
+                    unpack2(cy(h), y0, y1);
+                    unpack2(cz(h), z0, z1);
+                    if (m0) {
+                        const int sl = base + __popc(b0 & lt);
+                        ws->sC[sl] = make_float4(x0, y0, z0, D[2 * h]);
+                        ws->sO[sl] = cO[h * 2 * BT + 2 * tid];
                     }
-                    base += __popc(bal[c]);
+                    if (m1) {
+                        const int sl = base + __popc(b0) + __popc(b1 & lt);
+                        ws->sC[sl] = make_float4(x1, y1, z1, D[2 * h + 1]);
+                        ws->sO[sl] = cO[h * 2 * BT + 2 * tid + 1];
+                    }
+                    base += __popc(b0) + __popc(b1);
                 }
             }
         }
@@ -538,7 +552,11 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     }
 }
 
-size_t whole_smem_bytes(int cpt) { return sizeof(unsigned) * (size_t)cpt * BT + sizeof(WholeSmem); }
+size_t whole_smem_bytes(int cpt)
+{
+    const int h1 = cpt / 2, hs = h1 > 4 ? h1 - WHOLE_HR16 : 0;
+    return sizeof(unsigned) * (size_t)cpt * BT + sizeof(f32x2) * 3 * (size_t)hs * BT + sizeof(WholeSmem);
+}
 
 template <int CPT1, bool STATS, bool EUC>
 static int launch_whole_one(const BatchParams &bp, const DeviceIndex &ix, cudaStream_t st)
@@ -565,8 +583,9 @@ int launch_sample_whole(const BatchParams &bp, const DeviceIndex &ix, cudaStream
         case 2: return launch_whole_c<2>(bp, ix, st);
         case 4: return launch_whole_c<4>(bp, ix, st);
         case 8: return launch_whole_c<8>(bp, ix, st);
+        case 16: return launch_whole_c<16>(bp, ix, st);
     }
-    set_error("whole-cloud kernel: cand_per_thread=%d must be 2, 4 or 8", ix.cand_per_thread);
+    set_error("whole-cloud kernel: cand_per_thread=%d must be 2, 4, 8 or 16", ix.cand_per_thread);
     return FPS_ERR_INVALID;
 }
 

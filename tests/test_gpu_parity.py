@@ -234,10 +234,13 @@ def test_block_sizes(rf, threads):
 @pytest.mark.parametrize("flags", [1, 2, 3, 4, 7])
 def test_ablations_and_stats_are_bit_identical(rf, flags, kernel):
     # Table 4 structure: prune off / skip off / both off must not change a bit
+    # (cluster_size = 2: the general batched kernel; by default a cloud of this size runs the small-cloud kernel, whose
+    # flags and counters test_whole_cloud_kernel_flags covers)
     P, M = SMALL["room"]()
     ref = oracle.fps(P, M, 0)
-    gi, gm, st = run_gpu(rf, P, M, flags=flags | KERNELS[kernel])
+    gi, gm, st = run_gpu(rf, P, M, flags=flags | KERNELS[kernel], cluster_size=2)
     assert_same(gi, gm, *ref)
+    assert st["whole_cloud_kernel"] == 0
     if flags & rf.FPS_FLAG_STATS:
         assert st["iterations"] == M - 1
         if kernel == "per_pick":
@@ -268,12 +271,18 @@ def test_stats_match_cpu_pruned_variant_effective_updates(rf):
     P, M = SMALL["room"]()
     _, _, cpu = oracle.pruned_fps(P, M, 0, n_vox=16)
     for kernel, kflag in KERNELS.items():
-        _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS | kflag)
+        _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS | kflag, cluster_size=2)
+        assert st["whole_cloud_kernel"] == 0
         if kernel == "per_pick":
             assert st["effective"] == cpu["effective"]
         else:                       # the picks of the last batch are never applied (nothing needs them)
             assert 0.8 * cpu["effective"] <= st["effective"] <= cpu["effective"]
         assert st["points_visited"] < 0.2 * P.shape[0] * (M - 1)
+    # the small-cloud kernel (the default for this size) applies every pick to every point it can still lower
+    _, _, st = run_gpu(rf, P, M, flags=rf.FPS_FLAG_STATS)
+    assert st["whole_cloud_kernel"] == 1
+    assert 0.98 * cpu["effective"] <= st["effective"] <= cpu["effective"] + P.shape[0]      # (+ the last pick's updates)
+    assert st["points_visited"] < 0.35 * P.shape[0] * (M - 1)
 
 
 @pytest.mark.parametrize("kernel", sorted(KERNELS))
@@ -599,28 +608,28 @@ def test_integer_grid_overflowing_ties(rf):
     assert st["extract_retries"] > 0 and st["single_picks"] > 0 and st["local_fallbacks"] > 0
 
 
-# ---- the small-cloud kernel (k_fps_whole: every cloud <= 4 096 points, one CTA per cloud, the whole cloud in
+# ---- the small-cloud kernel (k_fps_whole: every cloud <= 8 192 points, one CTA per cloud, the whole cloud in
 # registers, radius prune on runs of 64 sorted points).  It is the default for such an index; an explicit
 # cluster_size, local_warps = 16 / 8 / 4 / 1 or FPS_FLAG_NO_BATCH select the general kernel (tests above). ----
 
 WHOLE_SIZES = [(1, 1, 0), (2, 2, 1), (63, 63, 5), (64, 20, 63), (65, 65, 64), (127, 40, 0), (129, 129, 128), (1023, 400, 7),
                (1024, 1024, 1023), (1025, 300, 0), (2047, 2047, 3), (2048, 512, 2047), (2049, 600, 11), (4095, 1024, 4094),
-               (4096, 4096, 0)]
+               (4096, 4096, 0), (4097, 1000, 4096), (6000, 1500, 17), (8191, 2000, 0), (8192, 8192, 8191)]
 
 
 @pytest.mark.parametrize("N,M,start", WHOLE_SIZES)
 def test_whole_cloud_kernel_sizes_around_blob_and_register_boundaries(rf, N, M, start):
-    # 64 points per blob, 1 024 points per register position, 512 x {2, 4, 8} capacity; M up to N (beyond the 1 024
-    # picks of the general kernel's batch buffer)
+    # 64 points per blob, 1 024 points per register position, 512 x {2, 4, 8, 16} capacity (with 16 most coordinates
+    # live in shared memory); M up to N (beyond the 1 024 picks of the general kernel's batch buffer)
     P = inputs.uniform_cube(N, 1000 + N)
     ref = oracle.fps(P, M, start)
     gi, gm, st = run_gpu(rf, P, M, start)
     assert st["whole_cloud_kernel"] == 1 and st["cluster_size"] == 1
-    assert st["cand_per_thread"] == (2 if N <= 1024 else 4 if N <= 2048 else 8)
+    assert st["cand_per_thread"] == (2 if N <= 1024 else 4 if N <= 2048 else 8 if N <= 4096 else 16)
     assert_same(gi, gm, *ref)
 
 
-@pytest.mark.parametrize("name", ["uniform4096", "lattice", "dups", "line"])
+@pytest.mark.parametrize("name", ["uniform4096", "lattice", "dups", "line", "room", "lidar"])
 @pytest.mark.parametrize("flags", [0, 1, 4, 5, 32, 36])
 def test_whole_cloud_kernel_flags(rf, name, flags):
     # prune off (every pick applied to every blob), STATS build, Euclidean distances: same picks, bit for bit
@@ -703,7 +712,8 @@ def test_whole_cloud_kernel_overflowing_distances_and_scales(rf):
 def test_small_clouds_general_kernel_still_selectable(rf):
     P, M = SMALL["uniform4096"]()
     ref = oracle.fps(P, M, 0)
-    for opts in (dict(cluster_size=4), dict(local_warps=16), dict(flags=rf.FPS_FLAG_NO_BATCH), dict(cluster_size=1)):
+    for opts in (dict(cluster_size=4), dict(local_warps=16), dict(flags=rf.FPS_FLAG_NO_BATCH), dict(cluster_size=1),
+                 dict(cand_per_thread=2)):
         gi, gm, st = run_gpu(rf, P, M, **opts)
         assert st["whole_cloud_kernel"] == 0
         assert_same(gi, gm, *ref)
