@@ -12,7 +12,7 @@ timed in the same run" for each config), each with the full --steps.
   value / ms_per_step   device-resident build + sample, CUDA events, L2 flushed between steps
   e2e                   the same metric through fps_sample_host with pinned HOST buffers (H2D + build +
                         sample + D2H inside the timed region)
-  roofline              dominant kernel (k_fps_batched): ALGORITHMIC bytes per launch / its mean launch
+  roofline              dominant kernel (k_fps_batched; k_fps_whole for C1): ALGORITHMIC bytes per launch / its mean launch
                         duration (CUDA events on the launching stream).  `achieved`/`frac` use SURVEY.md
                         8(d)'s formula exactly (28 B x K per iteration + 16 B per visited (point, pick) +
                         8 B per voxel visit + 4 B per effective update + 20 B per pick);
@@ -179,10 +179,15 @@ def schedule_bytes(st: dict) -> int:
                + 4 * st.get("extract_points", 0) + 20 * st.get("candidates", 0))
 
 
-def ncu_traffic(workload: str, per_pick: bool):
+def kernel_name(st: dict, per_pick: bool) -> str:
+    """The sampling kernel a handle runs: the per-pick persistent kernel (ablation), the small-cloud kernel (every
+    cloud <= 8 192 points: one CTA per cloud, the whole cloud in registers) or the general batched kernel."""
+    return "k_fps_sample" if per_pick else ("k_fps_whole" if st.get("whole_cloud_kernel") else "k_fps_batched")
+
+
+def ncu_traffic(workload: str, want: str):
     """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
     `ncu --set full` capture of this workload (profiles/r02_traffic.csv, else r01_traffic.csv), else None."""
-    want = "k_fps_sample" if per_pick else "k_fps_batched"
     for fn in ("r02_traffic.csv", "r01_traffic.csv"):
         try:
             for row in open(os.path.join(ROOT, "profiles", fn)).read().splitlines()[1:]:
@@ -197,13 +202,14 @@ def ncu_traffic(workload: str, per_pick: bool):
 def roofline_report(stc, kern_s, w, peak, peak_src, per_pick):
     sb, cb = survey_bytes(stc), schedule_bytes(stc)
     ach = sb / kern_s / 1e9
-    return {"bound": "hbm", "kernel": "k_fps_sample" if per_pick else "k_fps_batched", "achieved": ach, "peak": peak,
+    kern = kernel_name(stc, per_pick)
+    return {"bound": "hbm", "kernel": kern, "achieved": ach, "peak": peak,
             "unit": "GB/s", "frac": ach / peak, "frac_of_8000_nominal": ach / 8000.0, "peak_source": peak_src,
             "bytes_source": "SURVEY.md 8(d) formula: (28 K + 20) B per iteration + 16 B per visited (point, pick) + "
                             "8 B per voxel visit + 4 B per effective update",
             "algorithmic_bytes_per_launch": sb,
             "schedule_bytes_per_launch": cb, "schedule_achieved": cb / kern_s / 1e9, "schedule_frac": cb / kern_s / 1e9 / peak,
-            "traffic": ncu_traffic(w.name, per_pick),
+            "traffic": ncu_traffic(w.name, kern),
             "dense_equivalent_GBps": w.B * w.N * 16.0 * (w.M - 1) / kern_s / 1e9,
             "note": "not the binding limit: the working set is L2/SMEM resident (see traffic) and the picks are "
                     "sequentially dependent; see latency"}
@@ -419,11 +425,11 @@ def config_entry(rf, torch, name, flush, opts, peak, peak_src, steps, warmup, sm
     k = float(np.mean(r["kern_ms"])) * 1e-3
     step = float(np.mean(r["step_ms"]))
     roof = roofline_report(stc, k, w, peak, peak_src, per_pick)
-    for drop in ("peak_source", "bytes_source", "note", "kernel", "bound", "unit"):
+    for drop in ("peak_source", "bytes_source", "note", "bound", "unit"):
         roof.pop(drop, None)
     lat = latency_report(rf, k, w, sm_mhz)
     out = {"B": w.B, "N": w.N, "M": w.M, "n_vox": stc["n_vox"], "K_max": stc["K_max"], "cluster_size": stc["cluster_size"],
-           "steps": steps, "ms_per_step": step, "ms_per_cloud": step / w.B, "samples_per_s": w.B * w.M / (step * 1e-3),
+           "grid_ctas": stc["grid_ctas"], "steps": steps, "ms_per_step": step, "ms_per_cloud": step / w.B, "samples_per_s": w.B * w.M / (step * 1e-3),
            "sample_kernel_ms": k * 1e3, "index_build_ms": float(np.mean(r["build_ms"])),
            "sample_only_samples_per_s": w.B * w.M / k,
            "e2e": {"value": w.B * w.M * steps / e2e_s, "ms_per_step": e2e_s / steps * 1e3, "h2d_bytes_per_step": int(P.nbytes),
@@ -504,9 +510,11 @@ def main():
             "config": {"workload": f"{w.name}: {w.note}", "B": w.B, "N": w.N, "M": w.M, "start_idx": w.start_idx,
                        "step": "fps_index_build + fps_sample (a1-a13)", "l2": "flushed between iterations (256 MiB fill)",
                        "n_vox": st["n_vox"], "K_max": st["K_max"], "cluster_size": st["cluster_size"],
-                       "block_threads": st["block_threads"], "local_warps": st["local_warps"],
+                       "ctas_per_cloud_grid_mode": st["grid_ctas"], "block_threads": st["block_threads"], "local_warps": st["local_warps"],
                        "cand_per_thread": st["cand_per_thread"],
-                       "kernel": "per-pick persistent (ablation)" if args.per_pick else "exact batched picking",
+                       "kernel": "per-pick persistent (ablation)" if args.per_pick else
+                                 ("exact batched picking, small-cloud kernel (one CTA per cloud)" if st.get("whole_cloud_kernel")
+                                  else "exact batched picking"),
                        "parallelism": f"replicas x{world}"},
             "ms_per_cloud": total_ms / args.steps / w.B,
             "sample_kernel_ms": kern_s * 1e3, "index_build_ms": float(np.mean(r["build_ms"])),
