@@ -7,7 +7,9 @@ prints one markdown table per study: for M = N/64 .. N/2 at the automatic n_vox 
 latency (`fps_sample`, CUDA events, best of `reps`; and index build + sampling), memory (device bytes owned by the
 handle) and throughput (samples/s and input points/s of build + sample) -- and for n_vox = 8 .. 256 at the config's M
 the latency, memory and voxel count, for the batched kernel and the per-pick kernel.  Results never depend on either
-parameter (tests/test_gpu_parity.py); only time and memory do.  Needs a CUDA device; there is no CPU fallback.
+parameter (tests/test_gpu_parity.py); only time and memory do.  A third table times batches of small clouds (the
+sampling layers of a point-cloud network) on the small-cloud kernel and on the general one.  Needs a CUDA device; there
+is no CPU fallback.
 """
 from __future__ import annotations
 
@@ -48,11 +50,34 @@ def time_sample(Pd, M, start, reps, **opts):
     return best, st
 
 
+def small_cloud_table(reps):
+    """Batches shaped like the sampling layers of a point-cloud network (B clouds of 1 024 .. 16 384 points, M = N/4): the
+    small-cloud kernel (one CTA per cloud, the default up to 8 192 points) beside the general kernel (an explicit
+    cluster size selects it), and the index build."""
+    print("\n### Small-cloud batches: B x N -> N/4 (uniform cube), fps_sample and index build\n")
+    print("| B | N | M | default kernel | fps_sample ms | us per pick | general kernel ms (cluster of 4) | index build ms | M samples/s (build + sample) |")
+    print("|---|---|---|---|---|---|---|---|---|")
+    for B in (1, 32, 128):
+        for N in (1024, 2048, 4096, 8192, 16384):
+            if B * N > 1 << 21:
+                continue
+            M = N // 4
+            Pd = torch.from_numpy(np.stack([inputs.uniform_cube(N, 7000 + b) for b in range(B)])).cuda()
+            t, st = time_sample(Pd, M, 0, reps)
+            tg, _ = time_sample(Pd, M, 0, reps, cluster_size=4)
+            kern = "small-cloud" if st["whole_cloud_kernel"] else (f"general, grid {st['grid_ctas']}" if st["grid_ctas"] else f"general, cluster {st['cluster_size']}")
+            tot = t + st["build_ms"]
+            print(f"| {B} | {N} | {M} | {kern} | {t:.3f} | {t * 1e3 / max(1, M - 1):.3f} | {tg:.3f} | {st['build_ms']:.3f} | {B * M / tot / 1e3:.2f} |", flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--workloads", default="C1,C2,C3,C4,C5")
     ap.add_argument("--reps", type=int, default=3)
+    ap.add_argument("--no-small", action="store_true", help="skip the small-cloud batch table")
     args = ap.parse_args()
+    if not args.no_small:
+        small_cloud_table(args.reps)
     for name in args.workloads.split(","):
         w = inputs.WORKLOADS[name]
         Pd = torch.from_numpy(np.ascontiguousarray(inputs.make_batch(w))).cuda()
