@@ -103,7 +103,7 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     // ---- a7 + the initial update (Eq. 13-14): Dist_p = d(p, s_0), straight into registers ----
     const int p0 = P.pinv[po + startb];
     const float s0x = px[p0], s0y = py[p0], s0z = pz[p0];
-    f32x2 X[HR], Y[HR], Z[HR];
+    f32x2 X[HR] = {}, Y[HR] = {}, Z[HR] = {};
     float D[CPT1];
     // coordinate pair h of this thread (h is a compile-time constant wherever this is called)
     auto cx = [&](const int h) -> f32x2 { return h < HR ? X[h < HR ? h : 0] : sXYZ[(0 * HS + (h - HR)) * BT + tid]; };
