@@ -27,11 +27,12 @@
 
 namespace rfps {
 
-// picks taken one at a time (block-wide argmax: ~1 800 cycles each, a parallel step ~9 500) at the start of a cloud,
+// picks taken one at a time (block-wide argmax: ~1 500 cycles each, a parallel step ~9 500) at the start of a cloud,
 // after a parallel step that yielded fewer than STEP_MIN_YIELD picks, and when the first bin overflows (then in
 // runs that double while the steps keep failing).  Measured on C1, 32 x {1 024, 2 048, 4 096} and the tie-heavy lattice:
 // (24, 4, 5) is within 2 % of the best of six settings on every one of them
 constexpr int SINGLES_FIRST = 24, SINGLES_AFTER = 4, STEP_MIN_YIELD = 5;
+constexpr int SINGLES_UNTESTED = 16;   // the first picks of a cloud reach nearly every blob: no box tests for them
 
 constexpr int WHOLE_HR16 = 2;       // 16 points per thread: coordinate pairs kept in registers (the other 6 live in shared memory)
 
@@ -222,67 +223,79 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     // parallel step while a step yields few picks (the first picks of a cloud each reach most of it; many equal
     // distances).  Returns the maximum before the pick (bits; 0 = nothing left, no pick was made). ----
     int spar = 0;
-    auto single_pick = [&]() -> unsigned {
+    auto single_pick = [&](const bool test_boxes) -> unsigned {
+        // the warp's maximum is the largest blob maximum (warp-uniform, kept current by every update); only the blobs
+        // that attain it -- normally one -- are searched for the point, ties to the lowest original index
         unsigned wm = Dm[0];
 #pragma unroll
         for (int h = 1; h < H1; ++h) wm = max(wm, Dm[h]);
         const float wmf = __uint_as_float(wm);
         unsigned o = 0u;
-        int ci = -1;
+        bool have = false;
+        float bx = 0.0f, by = 0.0f, bz = 0.0f;
 #pragma unroll
-        for (int c = 0; c < CPT1; ++c)
-            if (D[c] == wmf) {
-                const unsigned oc = cO[(c >> 1) * 2 * BT + 2 * tid + (c & 1)];
-                if (ci < 0 || oc > o) { o = oc; ci = c; }
-            }
-        const unsigned wo = __reduce_max_sync(FULL, ci >= 0 ? o : 0u);
-        const int wl = __ffs(__ballot_sync(FULL, ci >= 0 && o == wo)) - 1;
-        if (lane == wl) {
-            float bx = 0.0f, by = 0.0f, bz = 0.0f;
-#pragma unroll
-            for (int c = 0; c < CPT1; ++c)
-                if (c == ci) {
-                    float a0, a1;
-                    unpack2(cx(c >> 1), a0, a1); bx = (c & 1) ? a1 : a0;
-                    unpack2(cy(c >> 1), a0, a1); by = (c & 1) ? a1 : a0;
-                    unpack2(cz(c >> 1), a0, a1); bz = (c & 1) ? a1 : a0;
+        for (int h = 0; h < H1; ++h) {
+            if (Dm[h] != wm) continue;                       // warp-uniform
+            const bool e0 = D[2 * h] == wmf, e1 = D[2 * h + 1] == wmf;
+            if (e0 || e1) {
+                const unsigned o0 = e0 ? cO[h * 2 * BT + 2 * tid] : 0u, o1 = e1 ? cO[h * 2 * BT + 2 * tid + 1] : 0u;
+                const bool second = e1 && (!e0 || o1 > o0);
+                const unsigned oc = second ? o1 : o0;
+                if (!have || oc > o) {
+                    float x0, x1, y0, y1, z0, z1;
+                    unpack2(cx(h), x0, x1);
+                    unpack2(cy(h), y0, y1);
+                    unpack2(cz(h), z0, z1);
+                    o = oc; have = true;
+                    bx = second ? x1 : x0; by = second ? y1 : y0; bz = second ? z1 : z0;
                 }
+            }
+        }
+        const unsigned wo = __reduce_max_sync(FULL, have ? o : 0u);
+        const int wl = __ffs(__ballot_sync(FULL, have && o == wo)) - 1;
+        if (lane == wl) {
             ws->sp[spar][warp] = make_float4(bx, by, bz, __uint_as_float(wo));
             ws->spd[spar][warp] = wm;
         }
         __syncthreads();
+        // every warp reduces the 16 offers (loaded together; the winner's coordinates travel by shuffle)
         const unsigned d = lane < BT / 32 ? ws->spd[spar][lane] : 0u;
+        const float4 off = lane < BT / 32 ? ws->sp[spar][lane] : make_float4(0.f, 0.f, 0.f, 0.f);
         const unsigned gm = __reduce_max_sync(FULL, d);
         if (gm == 0u) return 0u;
-        const unsigned oo = (lane < BT / 32 && d == gm) ? __float_as_uint(ws->sp[spar][lane].w) : 0u;
+        const unsigned oo = (lane < BT / 32 && d == gm) ? __float_as_uint(off.w) : 0u;
         const unsigned go = __reduce_max_sync(FULL, oo);
         const int wl2 = __ffs(__ballot_sync(FULL, lane < BT / 32 && d == gm && oo == go)) - 1;
-        const float4 s = ws->sp[spar][wl2];
+        const float4 s = make_float4(__shfl_sync(FULL, off.x, wl2), __shfl_sync(FULL, off.y, wl2), __shfl_sync(FULL, off.z, wl2), 0.0f);
         if (tid == 0) {
             out_idx[jl] = (int)(~go);
             out_mind[jl] = __uint_as_float(gm);
         }
         spar ^= 1;
+        // a9-a12 without a branch between the blobs, so that their box tests, updates and reductions overlap
+        bool reach[H1];
 #pragma unroll
         for (int h = 0; h < H1; ++h) {
-            if (Dm[h] == 0u) continue;
-            if (STATS) c_vtest++;
-            if (!no_prune) {
-                const float lb = box_lb(ws->bmin[warp + 16 * h], ws->bmax[warp + 16 * h], s);
-                if (distf<EUC>(lb) >= __uint_as_float(Dm[h])) continue;       // warp-uniform
-            }
-            if (STATS) { c_vvisit++; c_pvisit += 64ull; }
-            const f32x2 dx = sub2(cx(h), pack2(s.x, s.x)), dy = sub2(cy(h), pack2(s.y, s.y)), dz = sub2(cz(h), pack2(s.z, s.z));
+            reach[h] = Dm[h] != 0u;
+            if (test_boxes) reach[h] = reach[h] && !(distf<EUC>(box_lb(ws->bmin[warp + 16 * h], ws->bmax[warp + 16 * h], s)) >= __uint_as_float(Dm[h]));
+        }
+        const f32x2 SX = pack2(s.x, s.x), SY = pack2(s.y, s.y), SZ = pack2(s.z, s.z);
+#pragma unroll
+        for (int h = 0; h < H1; ++h) {
+            if (STATS) { if (Dm[h] != 0u) c_vtest++; if (reach[h]) { c_vvisit++; c_pvisit += 64ull; } }
+            if (h >= HR && !reach[h]) continue;              // (coordinates in shared memory: not loaded for nothing)
+            const f32x2 dx = sub2(cx(h), SX), dy = sub2(cy(h), SY), dz = sub2(cz(h), SZ);
             float x0, x1, y0, y1, z0, z1;
             unpack2(mul2(dx, dx), x0, x1);
             unpack2(mul2(dy, dy), y0, y1);
             unpack2(mul2(dz, dz), z0, z1);
             const float e0 = distf<EUC>(__fadd_rn(__fadd_rn(x0, y0), z0)), e1 = distf<EUC>(__fadd_rn(__fadd_rn(x1, y1), z1));
-            if (STATS) c_eff += (e0 < D[2 * h] ? 1 : 0) + (e1 < D[2 * h + 1] ? 1 : 0);
-            D[2 * h] = fminf(D[2 * h], e0);
-            D[2 * h + 1] = fminf(D[2 * h + 1], e1);
-            Dm[h] = __reduce_max_sync(FULL, __float_as_uint(fmaxf(D[2 * h], D[2 * h + 1])));
+            if (STATS && reach[h]) c_eff += (e0 < D[2 * h] ? 1 : 0) + (e1 < D[2 * h + 1] ? 1 : 0);
+            D[2 * h] = reach[h] ? fminf(D[2 * h], e0) : D[2 * h];
+            D[2 * h + 1] = reach[h] ? fminf(D[2 * h + 1], e1) : D[2 * h + 1];
         }
+#pragma unroll
+        for (int h = 0; h < H1; ++h) Dm[h] = __reduce_max_sync(FULL, __float_as_uint(fmaxf(D[2 * h], D[2 * h + 1])));
         return gm;
     };
 
@@ -296,7 +309,8 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     while (jl < M && hibits != 0u) {     // hi == +0: every distance is +0 (reading A7, after the loop)
         if (STATS) tt0 = clock64();
         if (singles > 0) {
-            hibits = single_pick();      // the maximum before the pick bounds everything after it
+            // (the first picks of a cloud reach nearly every blob: the box tests are left out there)
+            hibits = single_pick(!no_prune && jl > SINGLES_UNTESTED);      // the maximum before the pick bounds everything after it
             hi_exact = false;
             if (hibits == 0u) break;
             ++jl;
