@@ -166,21 +166,26 @@ __global__ void __launch_bounds__(BT, 1) k_fps_whole(const BatchParams P, const 
     auto apply_picks = [&](const int npk) {
         const float4 sa = lane < npk ? ws->pick[lane] : make_float4(0.f, 0.f, 0.f, 0.f);
         const float4 sb = lane + 32 < npk ? ws->pick[lane + 32] : make_float4(0.f, 0.f, 0.f, 0.f);
+        // the box tests of all blobs first, without a branch between them (their dependent chains overlap)
+        unsigned M0[H1], M1[H1];
 #pragma unroll
         for (int h = 0; h < H1; ++h) {
-            if (Dm[h] == 0u) continue;                       // warp-uniform: nothing left to lower (or an empty blob)
             const float dm = __uint_as_float(Dm[h]);
-            unsigned m0, m1;
             if (no_prune) {
-                m0 = npk >= 32 ? FULL : ((1u << npk) - 1u);
-                m1 = npk > 32 ? (npk >= 64 ? FULL : ((1u << (npk - 32)) - 1u)) : 0u;
+                M0[h] = Dm[h] == 0u ? 0u : (npk >= 32 ? FULL : ((1u << npk) - 1u));
+                M1[h] = Dm[h] == 0u || npk <= 32 ? 0u : (npk >= 64 ? FULL : ((1u << (npk - 32)) - 1u));
             } else {
                 const float4 lo = ws->bmin[warp + 16 * h], hi = ws->bmax[warp + 16 * h];
-                // Eq. 25 on the blob: the pick is skipped iff its lower bound to the box is >= Dist_v
-                m0 = __ballot_sync(FULL, lane < npk && !(distf<EUC>(box_lb(lo, hi, sa)) >= dm));
-                m1 = npk > 32 ? __ballot_sync(FULL, lane + 32 < npk && !(distf<EUC>(box_lb(lo, hi, sb)) >= dm)) : 0u;
+                // Eq. 25 on the blob: the pick is skipped iff its lower bound to the box is >= Dist_v (Dist_v = +0:
+                // nothing left to lower, or an empty blob -- every bound is >= 0)
+                M0[h] = __ballot_sync(FULL, lane < npk && !(distf<EUC>(box_lb(lo, hi, sa)) >= dm));
+                M1[h] = __ballot_sync(FULL, lane + 32 < npk && !(distf<EUC>(box_lb(lo, hi, sb)) >= dm));
             }
-            if (STATS) { c_vtest += (unsigned)npk; c_vvisit += __popc(m0) + __popc(m1); c_pvisit += 64ull * (__popc(m0) + __popc(m1)); }
+        }
+#pragma unroll
+        for (int h = 0; h < H1; ++h) {
+            unsigned m0 = M0[h], m1 = M1[h];
+            if (STATS && Dm[h] != 0u) { c_vtest += (unsigned)npk; c_vvisit += __popc(m0) + __popc(m1); c_pvisit += 64ull * (__popc(m0) + __popc(m1)); }
             if (!(m0 | m1)) continue;
             // Euclidean mode: min and the monotone sqrt_rn commute, so the picks are applied in the squared domain
             // and folded into the distances once
