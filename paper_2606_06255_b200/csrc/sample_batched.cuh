@@ -958,8 +958,10 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
             const unsigned long long k1 = v1 ? ((unsigned long long)__float_as_uint(c1.w) << 32) | ps->sO[j1] : 0ull;
 #pragma unroll
             for (int ii = 0; ii < 4; ++ii) {
-                const int i = 4 * warp + ii;
-                if (i >= n) break;                           // warp-uniform
+                // (no early exit: without a branch between the four members their dependent chains overlap; a member
+                // slot beyond n is computed on slot 0 and not stored)
+                const bool live = 4 * warp + ii < n;
+                const int i = live ? 4 * warp + ii : 0;
                 const float4 ci = ps->sC[i];
                 const unsigned long long ki = ((unsigned long long)__float_as_uint(ci.w) << 32) | ps->sO[i];
                 const float d0 = distf<EUC>(d2_rn(ci.x, ci.y, ci.z, c0.x, c0.y, c0.z));
@@ -969,7 +971,7 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
                 const unsigned bw0 = __ballot_sync(FULL, b0), bw1 = __ballot_sync(FULL, b1);
                 const unsigned aw0 = __ballot_sync(FULL, l0), aw1 = __ballot_sync(FULL, l1);
                 const bool sany = __any_sync(FULL, (l0 && !(d0 < thm)) || (l1 && !(d1 < thm)));
-                if (lane == 0) {
+                if (lane == 0 && live) {
                     ps->aff[i] = ((unsigned long long)aw1 << 32) | aw0;
                     ps->bef[i] = ((unsigned long long)bw1 << 32) | bw0;
                     if (sany) atomicOr(&ps->stop[i >> 5], 1u << (i & 31));
