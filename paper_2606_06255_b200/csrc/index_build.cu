@@ -552,7 +552,7 @@ __global__ void __launch_bounds__(256) k_ntiles(const int *__restrict__ voff, co
     ntiles[(size_t)base + k] = nt;
 }
 
-// vseg[b][tbase[k] + t] = {off + t*chunk, len}: equal-size tiles of the (Morton-ordered) voxel run
+// vseg[b][tbase[k] + t] = {off + t*chunk, len}: equal-size tiles of the voxel run (Morton sub-cell order inside the voxel)
 __global__ void __launch_bounds__(256) k_tiles(const int *__restrict__ voff, const int *__restrict__ Kv, const int *__restrict__ ntiles,
                                                 const int *__restrict__ tbase, const int *__restrict__ poff, int K_cap,
                                                 int2 *__restrict__ vseg)
@@ -645,7 +645,7 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
 }
 
 // ---------------------------------------------------------------------------------------------
-// a6': group spheres.  32 consecutive (Morton-ordered) voxels form a group; its sphere encloses the
+// a6': group spheres.  32 consecutive (Hilbert-ordered) voxels form a group; its sphere encloses the
 // member spheres:  c_g = midpoint of the box around the member spheres,
 //   R_g = max_l ( sqrt_rn(d2(c_l, c_g)) * (1 + 2^-20) + R_l ) * (1 + 2^-20)     (rounded up, as A9)
 // so every point p of a member voxel has ||p - c_g|| <= ||p - c_l|| + ||c_l - c_g|| <= R_g, and the
@@ -767,14 +767,22 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
     {
         float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
         bool bad = false;
-        for (int i = tid; i < N; i += FUSED_T) {
+        // (four points per trip, all twelve loads first: the memory round trips of a trip overlap)
+        for (int i0 = tid; i0 < N; i0 += 4 * FUSED_T) {
+            float c[4][3];
 #pragma unroll
-            for (int a = 0; a < 3; ++a) {
-                const float v = P[3 * (size_t)i + a];
-                bad |= !(fabsf(v) <= FLT_MAX);
-                mn[a] = fminf(mn[a], v);
-                mx[a] = fmaxf(mx[a], v);
-            }
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) c[u][a] = i0 + u * FUSED_T < N ? P[3 * (size_t)(i0 + u * FUSED_T) + a] : P[3 * (size_t)i0 + a];
+#pragma unroll
+            for (int u = 0; u < 4; ++u)
+#pragma unroll
+                for (int a = 0; a < 3; ++a) {
+                    const float v = c[u][a];
+                    bad |= !(fabsf(v) <= FLT_MAX);
+                    mn[a] = fminf(mn[a], v);
+                    mx[a] = fmaxf(mx[a], v);
+                }
         }
 #pragma unroll
         for (int a = 0; a < 3; ++a)
@@ -811,11 +819,20 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
         float L = (1.0f + 1e-3f) * E / (float)A.n_vox;
         if (!(L > 0.0f)) L = 1.0f;
         const float invsub = (float)(1 << A.sb);
-        for (int i = tid; i < N; i += FUSED_T) {
+        for (int i0 = tid; i0 < N; i0 += 4 * FUSED_T) {
+          float c[4][3];
+#pragma unroll
+          for (int u = 0; u < 4; ++u)
+#pragma unroll
+              for (int a = 0; a < 3; ++a) c[u][a] = i0 + u * FUSED_T < N ? P[3 * (size_t)(i0 + u * FUSED_T) + a] : 0.0f;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) {
+            const int i = i0 + u * FUSED_T;
+            if (i >= N) break;
             unsigned v[3], s[3];
 #pragma unroll
             for (int a = 0; a < 3; ++a) {
-                const float t = (P[3 * (size_t)i + a] - bb[a]) / L;
+                const float t = (c[u][a] - bb[a]) / L;
                 int c = (int)floorf(t);
                 c = max(0, min(A.n_vox - 1, c));
                 int sc = (int)floorf((t - (float)c) * invsub);
@@ -827,6 +844,7 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
             const unsigned sub = A.sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
             kin[i] = (vid << (3 * A.sb)) | sub;
             vin[i] = i;
+          }
         }
         __syncthreads();
     }
@@ -934,33 +952,79 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
         const int nt = tiles_of(cnt);
         const int chunk = (cnt + nt - 1) / nt;
         int2 *dst = vseg + tbase[k];
-        for (int t = 0; t < nt; ++t) dst[t] = make_int2(off + t * chunk, min(chunk, cnt - t * chunk));
+        // (a packed copy {first point, count << 16} stays in shared memory for the sphere phase: the keys are not needed
+        // any more, and N <= FUSED_MAX_N = 8 192 fits 16 bits)
+        for (int t = 0; t < nt; ++t) {
+            const int o = off + t * chunk, c = min(chunk, cnt - t * chunk);
+            dst[t] = make_int2(o, c);
+            kin[tbase[k] + t] = (unsigned)o | ((unsigned)c << 16);
+        }
     }
-    // ---- a4: gather AoS -> sorted SoA (+ permutation and its inverse) ----
+    __syncthreads();                                       // voff / tbase (F1 / F2) are free from here on
+    // ---- a4: gather AoS -> sorted SoA (+ permutation and its inverse).  Four points per trip with all loads first (the
+    // memory round trips overlap); the sorted coordinates also stay in shared memory (x in place of the sorted values,
+    // y and z in the two spare buffers) for the sphere phase ----
     float *px = A.px + base, *py = A.py + base, *pz = A.pz + base;
     int *porig = A.porig + base, *pinv = A.pinv + base;
-    for (int p = tid; p < N; p += FUSED_T) {
-        const int i = vin[p];
-        const float *s = P + 3 * (size_t)i;
-        px[p] = s[0]; py[p] = s[1]; pz[p] = s[2];
-        porig[p] = i;
-        pinv[i] = p;
+    const unsigned *const pseg = kin;
+    float *const sx = reinterpret_cast<float *>(vin), *const sy = reinterpret_cast<float *>(F1), *const sz = reinterpret_cast<float *>(F2);
+    for (int p0 = tid; p0 < N; p0 += 4 * FUSED_T) {
+        int idx[4];
+        float c[4][3];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) idx[u] = p0 + u * FUSED_T < N ? vin[p0 + u * FUSED_T] : 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) c[u][a] = P[3 * (size_t)idx[u] + a];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int q = p0 + u * FUSED_T;
+            if (q < N) {
+                px[q] = c[u][0]; py[q] = c[u][1]; pz[q] = c[u][2];
+                porig[q] = idx[u];
+                pinv[idx[u]] = q;
+                sx[q] = c[u][0]; sy[q] = c[u][1]; sz[q] = c[u][2];
+            }
+        }
     }
     __syncthreads();
     // ---- a6: tight bounding sphere per (tiled) voxel, 8 lanes per voxel (small clouds have small voxels: a whole
     // warp per voxel spends its time in shuffles); then the group spheres ----
     float4 *vgeom = A.vgeom + (size_t)b * A.K_cap;
     int local_max = 0;
-    {
+    if ((long long)N <= 8ll * K) {
+        // few points per voxel (uniform small clouds: 2-8): ONE thread per voxel, no shuffles -- eight lanes per voxel
+        // would spend ~120 instructions per warp and pass on two or three points.  min / max are order-independent, so
+        // the sphere is bit-identical either way
+        for (int k = tid; k < K; k += FUSED_T) {
+            const unsigned ps = pseg[k];
+            const int off = (int)(ps & 0xffffu), cnt = (int)(ps >> 16);
+            float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+            for (int p = off; p < off + cnt; ++p) {
+                mn[0] = fminf(mn[0], sx[p]); mx[0] = fmaxf(mx[0], sx[p]);
+                mn[1] = fminf(mn[1], sy[p]); mx[1] = fmaxf(mx[1], sy[p]);
+                mn[2] = fminf(mn[2], sz[p]); mx[2] = fmaxf(mx[2], sz[p]);
+            }
+            const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+            const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+            const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+            float r2 = 0.0f;
+            for (int p = off; p < off + cnt; ++p) r2 = fmaxf(r2, d2_rn(sx[p], sy[p], sz[p], cx, cy, cz));
+            vgeom[k] = make_float4(cx, cy, cz, __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f));
+            local_max = max(local_max, cnt);
+        }
+    } else {
         const int sub = lane & 7, grp = (w << 2) | (lane >> 3), NG = NWF * 4;
         for (int k0 = 0; k0 < K; k0 += NG) {
             const int k = k0 + grp;
-            const int2 sg = k < K ? vseg[k] : make_int2(0, 0);
+            const unsigned ps = k < K ? pseg[k] : 0u;
+            const int2 sg = make_int2((int)(ps & 0xffffu), (int)(ps >> 16));
             float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
             for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) {
-                mn[0] = fminf(mn[0], px[p]); mx[0] = fmaxf(mx[0], px[p]);
-                mn[1] = fminf(mn[1], py[p]); mx[1] = fmaxf(mx[1], py[p]);
-                mn[2] = fminf(mn[2], pz[p]); mx[2] = fmaxf(mx[2], pz[p]);
+                mn[0] = fminf(mn[0], sx[p]); mx[0] = fmaxf(mx[0], sx[p]);
+                mn[1] = fminf(mn[1], sy[p]); mx[1] = fmaxf(mx[1], sy[p]);
+                mn[2] = fminf(mn[2], sz[p]); mx[2] = fmaxf(mx[2], sz[p]);
             }
 #pragma unroll
             for (int a = 0; a < 3; ++a)
@@ -972,7 +1036,7 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
             const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
             const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
             float r2 = 0.0f;
-            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) r2 = fmaxf(r2, d2_rn(px[p], py[p], pz[p], cx, cy, cz));
+            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) r2 = fmaxf(r2, d2_rn(sx[p], sy[p], sz[p], cx, cy, cz));
             for (int o = 4; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
             if (sub == 0 && k < K) {
                 vgeom[k] = make_float4(cx, cy, cz, __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f));
@@ -1102,6 +1166,38 @@ struct Scratch {
     int *vA, *vB, *table, *bsum, *heads, *rank, *voff, *ntl, *tbase, *Kv;
 };
 
+// the single-launch build takes more than the default 48 KB of dynamic shared memory: opt in once per device
+static bool fused_attr_set()
+{
+    static std::mutex mu;
+    static bool done[64];
+    int dev = 0;
+    cudaGetDevice(&dev);
+    std::lock_guard<std::mutex> lock(mu);
+    if (dev >= 0 && dev < 64 && done[dev]) return true;
+    if (cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)) != cudaSuccess) return false;
+    if (dev >= 0 && dev < 64) done[dev] = true;
+    return true;
+}
+
+// Per-thread pinned host staging for the two small copies of a build (cloud offsets in, read-back block out): with a
+// pageable buffer both copies are staged by the driver and cost several microseconds of host time each, which is a
+// visible part of a small cloud's build.  Grown on demand, kept for the life of the thread (a build synchronises its
+// stream before it returns, so the buffer is free again by then); nullptr if pinned memory cannot be had.
+static unsigned *pinned_stage(size_t words)
+{
+    struct Stage { unsigned *p = nullptr; size_t cap = 0; };
+    static thread_local Stage t;
+    if (words > t.cap) {
+        if (t.p) cudaFreeHost(t.p);
+        t.p = nullptr; t.cap = 0;
+        const size_t want = std::max<size_t>(words * 2, 4096);
+        if (cudaHostAlloc((void **)&t.p, want * sizeof(unsigned), cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); t.p = nullptr; return nullptr; }
+        t.cap = want;
+    }
+    return t.p;
+}
+
 int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 {
     // ix.poff_host[0..B] = first point of every cloud in the concatenated arrays (set by the caller);
@@ -1169,12 +1265,14 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
             sc.Kv = c.take<int>(B);
         }
     };
+    const bool fused = N <= FUSED_MAX_N && !(o.flags & FPS_FLAG_CHAIN_BUILD);     // one launch, all intermediates in shared memory
     Carver sizeP, sizeS;
     carve(sizeP, true);
     carve(sizeS, false);
     void *arena = nullptr, *scratch = nullptr;
     ix.arena_pooled = build_pool() != nullptr;
-    if (pool_alloc(&arena, sizeP.off, st) != cudaSuccess || pool_alloc(&scratch, sizeS.off, st) != cudaSuccess) {
+    // (the single-launch build needs none of the chain's intermediate arrays)
+    if (pool_alloc(&arena, sizeP.off, st) != cudaSuccess || (!fused && pool_alloc(&scratch, sizeS.off, st) != cudaSuccess)) {
         set_error("device allocation of %zu + %zu bytes failed: %s", sizeP.off, sizeS.off, cudaGetErrorString(cudaGetLastError()));
         if (arena) { if (ix.arena_pooled) cudaFreeAsync(arena, st); else cudaFree(arena); }
         return FPS_ERR_NOMEM;
@@ -1185,22 +1283,26 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     cp.base = (char *)arena;
     cs.base = (char *)scratch;
     carve(cp, true);
-    carve(cs, false);
-    auto release_scratch = [&]() { if (ix.arena_pooled) cudaFreeAsync(scratch, st); else cudaFree(scratch); };
+    if (!fused) carve(cs, false);
+    auto release_scratch = [&]() { if (scratch) { if (ix.arena_pooled) cudaFreeAsync(scratch, st); else cudaFree(scratch); } };
 
     LaunchLog log;
     const int sms = device_props().sm_count;
     const dim3 gN((N + 255) / 256, B);
     // a failing enqueue below must not leak the scratch block: every exit goes through release_scratch()
+    const size_t rb_n = (size_t)B + 8 + (size_t)B * BBOX_STRIDE;
+    unsigned *const stage = pinned_stage((size_t)(B + 1) + rb_n);      // [B + 1] offsets in, [rb_n] read-back out
+    const void *poff_src = ph;
+    if (stage) { memcpy(stage, ph, sizeof(int32_t) * (B + 1)); poff_src = stage; }
     cudaError_t e0 = cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st);
-    if (e0 == cudaSuccess) e0 = cudaMemcpyAsync(ix.poff_dev, ph, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st);
+    if (e0 == cudaSuccess) e0 = cudaMemcpyAsync(ix.poff_dev, poff_src, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st);
     if (e0 != cudaSuccess) {
         set_error("index build: enqueueing the first copies failed: %s", cudaGetErrorString(e0));
         release_scratch();
         return FPS_ERR_CUDA;
     }
     const int *poff = ix.poff_dev;
-    if (N <= FUSED_MAX_N && !(o.flags & FPS_FLAG_CHAIN_BUILD)) {
+    if (fused) {
         // small clouds: the whole build in ONE launch, one CTA per cloud (k_build_fused)
         FusedArgs fa;
         fa.pts = points; fa.poff = poff; fa.bbox = sc.bbox;
@@ -1209,7 +1311,7 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
         fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
         fa.maxcnt = reinterpret_cast<int *>(meta);
-        if (cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)) != cudaSuccess) {
+        if (!fused_attr_set()) {
             set_error("cudaFuncSetAttribute(k_build_fused) failed: %s", cudaGetErrorString(cudaGetLastError()));
             release_scratch();
             return FPS_ERR_CUDA;
@@ -1258,17 +1360,17 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
 
     // the one host round-trip of the build: K per cloud, the non-finite flags, the largest segment
     ix.K_host = (int32_t *)malloc(sizeof(int32_t) * B);
-    const size_t rb_n = (size_t)B + 8 + (size_t)B * BBOX_STRIDE;
-    std::vector<unsigned> hrb(rb_n);
+    std::vector<unsigned> hrb_pageable(stage ? 0 : rb_n);
+    unsigned *const hrb = stage ? stage + (B + 1) : hrb_pageable.data();
     if (!ix.K_host) { set_error("host malloc failed"); release_scratch(); return FPS_ERR_NOMEM; }
-    cudaError_t e1 = cudaMemcpyAsync(hrb.data(), rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
+    cudaError_t e1 = cudaMemcpyAsync(hrb, rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
     release_scratch();
     cudaError_t e4 = cudaStreamSynchronize(st);
     if (e1 == cudaSuccess && e4 == cudaSuccess) {
-        memcpy(ix.K_host, hrb.data(), sizeof(int32_t) * B);
+        memcpy(ix.K_host, hrb, sizeof(int32_t) * B);
         ix.max_voxel_points = (int)hrb[B];
     }
-    const unsigned *hb = hrb.data() + B + 8;
+    const unsigned *hb = hrb + B + 8;
     if (e1 != cudaSuccess || e4 != cudaSuccess) {
         set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : e1));
         return FPS_ERR_CUDA;
@@ -1391,7 +1493,7 @@ int sample_noalloc(const float *points, int32_t N, int32_t M, int32_t start_idx,
     fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
     fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
     fa.maxcnt = reinterpret_cast<int *>(meta);
-    RFPS_CUDA(cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)));
+    if (!fused_attr_set()) { set_error("cudaFuncSetAttribute(k_build_fused) failed: %s", cudaGetErrorString(cudaGetLastError())); return FPS_ERR_CUDA; }
     LaunchLog log;
     launch_pdl_smem(log, fused_smem_bytes(N), k_build_fused, dim3(1), dim3(FUSED_T), st, fa);
     {

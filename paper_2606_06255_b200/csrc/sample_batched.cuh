@@ -1057,7 +1057,7 @@ __device__ __forceinline__ void local_fps_par(const float *cX, const float *cY, 
 }
 
 // ---------------------------------------------------------------------------------------------
-// the kernel: one cluster per cloud.  32 consecutive (Morton-ordered) voxels form a group with its
+// the kernel: one cluster per cloud.  32 consecutive (Hilbert-ordered) voxels form a group with its
 // own bounding sphere; CTA `rank` owns the groups g = rank + C*gl (round-robin, so that dense
 // regions of the cloud are spread over the CTAs); local voxel slot kl = 32*gl + l is voxel
 // k = 32*g + l.
