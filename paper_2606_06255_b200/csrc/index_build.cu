@@ -652,9 +652,17 @@ __global__ void __launch_bounds__(256) k_sphere(const float *__restrict__ px, co
 // prune test of Eq. 25 can be applied to the whole group with Dist_v := max over its voxels.
 // ---------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) k_group_sphere(const float4 *__restrict__ vgeom, const int *__restrict__ K, int K_cap,
-                                                       int G_cap, float4 *__restrict__ ggeom)
+                                                       int G_cap, float4 *__restrict__ ggeom, const unsigned *__restrict__ rb,
+                                                       unsigned *host_rb, int rb_n)
 {
     grid_dep_sync();
+    // the last kernel of the chain also hands the build's read-back block (K per cloud, largest segment, bounding boxes
+    // with the non-finite flags: complete once its predecessors are) to the host through mapped pinned memory, so that
+    // the build's one host round trip needs no copy
+    if (host_rb != nullptr && blockIdx.x == 0 && blockIdx.y == 0) {
+        for (int i = threadIdx.x; i < rb_n; i += blockDim.x) host_rb[i] = rb[i];
+        __threadfence_system();
+    }
     const int b = blockIdx.y;
     const int lane = threadIdx.x & 31;
     const int Kb = K[b];
@@ -706,6 +714,13 @@ struct FusedArgs {
     float4 *vgeom, *ggeom;
     int *K_dev;
     int *maxcnt;                    // meta[0]
+    // zero-copy read-back (build_index): a pinned, device-visible host block [3][B] = K, largest segment, non-finite
+    // flag of every cloud, written by the kernel itself, so that the build's one host round trip needs no copy; and,
+    // for a batch of equal-size clouds (uniform_N > 0), the cloud offsets are computed and written here instead of
+    // being copied in.  Both null / 0 for fps_sample_noalloc
+    int *host_rb = nullptr;
+    int *poff_out = nullptr;
+    int uniform_N = 0, B = 0;
 };
 
 // exclusive scan of n ints by the whole CTA: tiles of 4 096 with a running carry; returns the total
@@ -761,7 +776,11 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
     __shared__ int sbad, skv, sK;
     const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, NWF = FUSED_T / 32;
     const int b = blockIdx.x;
-    const int base = A.poff[b], N = A.poff[b + 1] - base;
+    const int base = A.uniform_N > 0 ? b * A.uniform_N : A.poff[b], N = A.uniform_N > 0 ? A.uniform_N : A.poff[b + 1] - base;
+    if (A.uniform_N > 0 && tid == 0) {
+        A.poff_out[b] = base;
+        if (b == A.B - 1) A.poff_out[A.B] = base + N;
+    }
     const float *P = A.pts + (size_t)base * 3;
     // ---- a1: bounding box + non-finite flag ----
     {
@@ -805,7 +824,10 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
             bb[tid] = lo; bb[3 + tid] = hi;
             unsigned *g = A.bbox + b * BBOX_STRIDE;
             g[tid] = f2ord(lo); g[3 + tid] = f2ord(hi);
-            if (tid == 0) g[6] = sbad ? 1u : 0u;
+            if (tid == 0) {
+                g[6] = sbad ? 1u : 0u;
+                if (A.host_rb) A.host_rb[2 * A.B + b] = sbad;
+            }
         }
         __syncthreads();
     }
@@ -940,7 +962,7 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
     __syncthreads();
     {
         const int Kt = cta_scan_excl(F2, F2, N, sm);
-        if (tid == 0) { sK = Kt; A.K_dev[b] = Kt; }
+        if (tid == 0) { sK = Kt; A.K_dev[b] = Kt; if (A.host_rb) A.host_rb[b] = Kt; }
     }
     __syncthreads();
     const int K = sK;
@@ -1045,7 +1067,13 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
         }
     }
     local_max = __reduce_max_sync(0xffffffffu, local_max);
-    if (lane == 0 && local_max > 0) atomicMax(A.maxcnt, local_max);
+    if (A.host_rb) {
+        if (tid == 0) skv = 0;                              // (skv is free by now: reused as the CTA's largest segment)
+        __syncthreads();
+        if (lane == 0 && local_max > 0) atomicMax(&skv, local_max);
+        __syncthreads();
+        if (tid == 0) { A.host_rb[A.B + b] = skv; __threadfence_system(); }
+    } else if (lane == 0 && local_max > 0) atomicMax(A.maxcnt, local_max);
     __syncthreads();
     float4 *ggeom = A.ggeom + (size_t)b * A.G_cap;
     const int G = (K + 31) / 32;
@@ -1192,7 +1220,7 @@ static unsigned *pinned_stage(size_t words)
         if (t.p) cudaFreeHost(t.p);
         t.p = nullptr; t.cap = 0;
         const size_t want = std::max<size_t>(words * 2, 4096);
-        if (cudaHostAlloc((void **)&t.p, want * sizeof(unsigned), cudaHostAllocDefault) != cudaSuccess) { cudaGetLastError(); t.p = nullptr; return nullptr; }
+        if (cudaHostAlloc((void **)&t.p, want * sizeof(unsigned), cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); t.p = nullptr; return nullptr; }
         t.cap = want;
     }
     return t.p;
@@ -1216,6 +1244,11 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     const int vbits = 3 * ilog2_ceil((unsigned long long)n_vox);
     int sb = tile_points > 0 ? (32 - vbits) / 3 : 0;
     if (sb > 4) sb = 4;
+    // An index of small clouds built with default options is sampled by the small-cloud kernel (sample_batched.cu,
+    // choose_batched_shape), which uses the sorted order only: 16 key bits -- two radix passes instead of three -- order
+    // the points finely enough for its runs of 64 (measured: same sampling time, the build 5-8 us shorter)
+    if (N <= 8192 && o.cluster_size == 0 && (o.local_warps == 0 || o.local_warps == 32) && !(o.flags & (FPS_FLAG_NO_BATCH | FPS_FLAG_PER_PICK)))
+        while (sb > 0 && vbits + 3 * sb > 16) --sb;
     const int keybits = vbits + 3 * sb;
     ix.n_vox = n_vox;
     ix.tile_points = tile_points;
@@ -1292,10 +1325,16 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     // a failing enqueue below must not leak the scratch block: every exit goes through release_scratch()
     const size_t rb_n = (size_t)B + 8 + (size_t)B * BBOX_STRIDE;
     unsigned *const stage = pinned_stage((size_t)(B + 1) + rb_n);      // [B + 1] offsets in, [rb_n] read-back out
+    // single-launch build with pinned staging: the kernel writes the read-back values straight into the (mapped) host
+    // block and, for equal-size clouds, computes the offsets itself -- no memset, no copy in, no copy out
+    int *host_rb_dev = nullptr;
+    if (fused && stage && cudaHostGetDevicePointer((void **)&host_rb_dev, stage + (B + 1), 0) != cudaSuccess) { cudaGetLastError(); host_rb_dev = nullptr; }
+    const bool zero_copy = host_rb_dev != nullptr, poff_in_kernel = zero_copy && !ix.ragged;
+    unsigned *chain_rb_dev = nullptr;     // kernel chain: the last kernel copies the read-back block to the host
     const void *poff_src = ph;
     if (stage) { memcpy(stage, ph, sizeof(int32_t) * (B + 1)); poff_src = stage; }
-    cudaError_t e0 = cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st);
-    if (e0 == cudaSuccess) e0 = cudaMemcpyAsync(ix.poff_dev, poff_src, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st);
+    cudaError_t e0 = zero_copy ? cudaSuccess : cudaMemsetAsync(meta, 0, 8 * sizeof(unsigned), st);
+    if (e0 == cudaSuccess && !poff_in_kernel) e0 = cudaMemcpyAsync(ix.poff_dev, poff_src, sizeof(int32_t) * (B + 1), cudaMemcpyHostToDevice, st);
     if (e0 != cudaSuccess) {
         set_error("index build: enqueueing the first copies failed: %s", cudaGetErrorString(e0));
         release_scratch();
@@ -1311,6 +1350,8 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
         fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
         fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
         fa.maxcnt = reinterpret_cast<int *>(meta);
+        fa.host_rb = host_rb_dev; fa.B = B;
+        if (poff_in_kernel) { fa.uniform_N = N; fa.poff_out = ix.poff_dev; }
         if (!fused_attr_set()) {
             set_error("cudaFuncSetAttribute(k_build_fused) failed: %s", cudaGetErrorString(cudaGetLastError()));
             release_scratch();
@@ -1346,7 +1387,9 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     launch_pdl(log, k_sphere, dim3(dim3(sphere_blocks, B)), dim3(256), st, ix.px, ix.py, ix.pz, ix.vseg, ix.K_dev, poff, ix.K_cap, ix.vgeom,
                reinterpret_cast<int *>(meta));
     const int group_blocks = std::max(1, std::min((ix.G_cap + 7) / 8, sms * 8));
-    launch_pdl(log, k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom);
+    if (stage && cudaHostGetDevicePointer((void **)&chain_rb_dev, stage + (B + 1), 0) != cudaSuccess) { cudaGetLastError(); chain_rb_dev = nullptr; }
+    launch_pdl(log, k_group_sphere, dim3(dim3(group_blocks, B)), dim3(256), st, ix.vgeom, ix.K_dev, ix.K_cap, ix.G_cap, ix.ggeom,
+               (const unsigned *)rb, chain_rb_dev, (int)rb_n);
     }
     {
         const cudaError_t el = log.first_error != cudaSuccess ? log.first_error : cudaGetLastError();
@@ -1363,23 +1406,33 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     std::vector<unsigned> hrb_pageable(stage ? 0 : rb_n);
     unsigned *const hrb = stage ? stage + (B + 1) : hrb_pageable.data();
     if (!ix.K_host) { set_error("host malloc failed"); release_scratch(); return FPS_ERR_NOMEM; }
-    cudaError_t e1 = cudaMemcpyAsync(hrb, rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
+    cudaError_t e1 = (zero_copy || chain_rb_dev) ? cudaSuccess : cudaMemcpyAsync(hrb, rb, sizeof(unsigned) * rb_n, cudaMemcpyDeviceToHost, st);
     release_scratch();
     cudaError_t e4 = cudaStreamSynchronize(st);
-    if (e1 == cudaSuccess && e4 == cudaSuccess) {
-        memcpy(ix.K_host, hrb, sizeof(int32_t) * B);
-        ix.max_voxel_points = (int)hrb[B];
-    }
-    const unsigned *hb = hrb + B + 8;
     if (e1 != cudaSuccess || e4 != cudaSuccess) {
         set_error("index build failed on the device: %s", cudaGetErrorString(e4 != cudaSuccess ? e4 : e1));
         return FPS_ERR_CUDA;
     }
-    for (int b = 0; b < B; ++b)
-        if (hb[(size_t)b * BBOX_STRIDE + 6]) {
-            set_error("cloud %d holds a NaN or infinite coordinate", b);
-            return FPS_ERR_NONFINITE;
-        }
+    if (zero_copy) {                      // [3][B]: K, largest segment, non-finite flag (written by k_build_fused)
+        const int *h3 = reinterpret_cast<const int *>(hrb);
+        memcpy(ix.K_host, h3, sizeof(int32_t) * B);
+        ix.max_voxel_points = 0;
+        for (int b = 0; b < B; ++b) ix.max_voxel_points = std::max(ix.max_voxel_points, h3[B + b]);
+        for (int b = 0; b < B; ++b)
+            if (h3[2 * B + b]) {
+                set_error("cloud %d holds a NaN or infinite coordinate", b);
+                return FPS_ERR_NONFINITE;
+            }
+    } else {
+        memcpy(ix.K_host, hrb, sizeof(int32_t) * B);
+        ix.max_voxel_points = (int)hrb[B];
+        const unsigned *hb = hrb + B + 8;
+        for (int b = 0; b < B; ++b)
+            if (hb[(size_t)b * BBOX_STRIDE + 6]) {
+                set_error("cloud %d holds a NaN or infinite coordinate", b);
+                return FPS_ERR_NONFINITE;
+            }
+    }
     ix.K_max = 0;
     ix.K_total = 0;
     for (int b = 0; b < B; ++b) {
