@@ -61,6 +61,29 @@ struct LaunchLog {
 template <typename... P, typename... A>
 static void launch_pdl_smem(LaunchLog &log, size_t smem, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args);
 
+// the same with a thread-block cluster dimension (the single-launch build of mid-size clouds)
+template <typename... P, typename... A>
+static void launch_pdl_cluster(LaunchLog &log, size_t smem, int cluster, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
+{
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid;
+    cfg.blockDim = block;
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute at[2];
+    at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    at[0].val.programmaticStreamSerializationAllowed = 1;
+    at[1].id = cudaLaunchAttributeClusterDimension;
+    at[1].val.clusterDim.x = (unsigned)cluster;
+    at[1].val.clusterDim.y = 1;
+    at[1].val.clusterDim.z = 1;
+    cfg.attrs = at;
+    cfg.numAttrs = 2;
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, kern, std::forward<A>(args)...);
+    if (e != cudaSuccess && log.first_error == cudaSuccess) log.first_error = e;
+    log.launches += 1;
+}
+
 template <typename... P, typename... A>
 static void launch_pdl(LaunchLog &log, void (*kern)(P...), dim3 grid, dim3 block, cudaStream_t st, A &&...args)
 {
@@ -1100,6 +1123,397 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------
+// a1-a6 in ONE launch for MID-SIZE clouds (FUSED_MAX_N < N <= CL_MAX_N, e.g. config 2's 24 000 points): one
+// thread-block CLUSTER of C CTAs per cloud.  CTA r owns the points (later: the sorted positions) [r Np, (r+1) Np);
+// keys and values live in its shared memory as in k_build_fused, and the radix passes exchange across the cluster:
+// every CTA publishes its 256 digit totals (read by the peers over DSMEM), derives the global output offset of each
+// of its (digit, chunk) cells -- digit-major, then CTA rank, then chunk, which keeps the sort stable --, and scatters
+// its keys straight into the owner's shared memory (st.shared::cluster).  The segment / tile phase scans every CTA's
+// share in shared memory and chains the shares through per-CTA totals (DSMEM); the spheres are dealt over all warps
+// of the cluster.  A dozen cluster barriers instead of 22 launches; same voxels, tiles and spheres as the chain
+// (tests compare them).
+// ---------------------------------------------------------------------------------------------
+constexpr int CL_MAX_N = 32768, CL_PER_CTA = 6144, CL_MAX_C = 8;
+static inline int cluster_build_ctas(int N) { return std::min(CL_MAX_C, std::max(2, (N + CL_PER_CTA - 1) / CL_PER_CTA)); }
+static inline size_t cluster_smem_bytes(int Np) { return (size_t)16 * Np + (size_t)1024 * (((Np + FUSED_CHUNK - 1) / FUSED_CHUNK) | 1); }
+
+struct ClusterArgs {
+    FusedArgs f;                    // (f.Nmax = positions per CTA of the largest cloud: sizes the shared-memory buffers)
+    int *F1g;                       // [all points] first point of every grid voxel (global scratch)
+};
+
+// exclusive prefix sums of two int sequences of 256 elements held by threads 0..255 (one element each); whole CTA
+__device__ __forceinline__ int2 scan256_pair(const int a, const int b, int *sm /* [34] */)
+{
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
+    int ia = a, ib = b;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int ta = __shfl_up_sync(0xffffffffu, ia, o), tb = __shfl_up_sync(0xffffffffu, ib, o);
+        if (lane >= o) { ia += ta; ib += tb; }
+    }
+    __syncthreads();
+    if (w < 8 && lane == 31) { sm[w] = ia; sm[8 + w] = ib; }
+    __syncthreads();
+    int ca = 0, cb = 0;
+#pragma unroll
+    for (int i = 0; i < 8; ++i) { ca += i < w ? sm[i] : 0; cb += i < w ? sm[8 + i] : 0; }
+    return make_int2(ca + ia - a, cb + ib - b);
+}
+
+__global__ void __launch_bounds__(FUSED_T, 1) k_build_cluster(const ClusterArgs CA)
+{
+    grid_dep_sync();
+    const FusedArgs &A = CA.f;
+    extern __shared__ __align__(16) unsigned char fsm[];
+    __shared__ int hist[FUSED_T / 32][256];
+    __shared__ float red[FUSED_T / 32][6];
+    __shared__ float cred[8];        // this CTA's {lo x y z, hi x y z, non-finite flag, largest segment}: read by the peers
+    __shared__ int tdig[256];        // this CTA's digit totals of the running radix pass: read by the peers
+    __shared__ int fix[256];
+    __shared__ int sm[34];
+    __shared__ float bb[8];
+    __shared__ int sbad, sK, smaxc;
+    __shared__ int xch[2];           // this CTA's head / tile totals: read by the peers
+    const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, NWF = FUSED_T / 32;
+    const int C = (int)cluster_nctarank(), r = (int)cluster_ctarank();
+    const int b = blockIdx.x / C;
+    const int base = A.uniform_N > 0 ? b * A.uniform_N : A.poff[b], N = A.uniform_N > 0 ? A.uniform_N : A.poff[b + 1] - base;
+    if (A.uniform_N > 0 && tid == 0 && r == 0) {
+        A.poff_out[b] = base;
+        if (b == A.B - 1) A.poff_out[A.B] = base + N;
+    }
+    const float *P = A.pts + (size_t)base * 3;
+    const int Np = (N + C - 1) / C;                          // points / sorted positions per CTA
+    const int p0 = min(N, r * Np), n = min(N, p0 + Np) - p0; // this CTA's share
+    // ---- a1: bounding box + non-finite flag: CTA partials, combined over the cluster ----
+    {
+        float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+        bool bad = false;
+        for (int j = tid; j < n; j += FUSED_T) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float v = P[3 * (size_t)(p0 + j) + a];
+                bad |= !(fabsf(v) <= FLT_MAX);
+                mn[a] = fminf(mn[a], v);
+                mx[a] = fmaxf(mx[a], v);
+            }
+        }
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            for (int o = 16; o > 0; o >>= 1) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+            }
+        bad = __any_sync(0xffffffffu, bad);
+        if (tid == 0) sbad = 0;
+        __syncthreads();
+        if (lane == 0) {
+#pragma unroll
+            for (int a = 0; a < 3; ++a) { red[w][a] = mn[a]; red[w][3 + a] = mx[a]; }
+            if (bad) sbad = 1;
+        }
+        __syncthreads();
+        if (tid < 3) {
+            float lo = red[0][tid], hi = red[0][3 + tid];
+            for (int i = 1; i < NWF; ++i) { lo = fminf(lo, red[i][tid]); hi = fmaxf(hi, red[i][3 + tid]); }
+            cred[tid] = lo; cred[3 + tid] = hi;
+            if (tid == 0) cred[6] = sbad ? 1.0f : 0.0f;
+        }
+        cluster_sync_all();
+        if (tid < 3) {
+            float lo = FLT_MAX, hi = -FLT_MAX;
+            for (int q = 0; q < C; ++q) {
+                lo = fminf(lo, __uint_as_float(ld_dsmem_u32(mapa(smem_u32(&cred[tid]), (unsigned)q))));
+                hi = fmaxf(hi, __uint_as_float(ld_dsmem_u32(mapa(smem_u32(&cred[3 + tid]), (unsigned)q))));
+            }
+            bb[tid] = lo; bb[3 + tid] = hi;
+            if (r == 0) {
+                unsigned *g = A.bbox + b * BBOX_STRIDE;
+                g[tid] = f2ord(lo); g[3 + tid] = f2ord(hi);
+            }
+            if (tid == 0 && r == 0) {
+                int anybad = 0;
+                for (int q = 0; q < C; ++q) anybad |= __uint_as_float(ld_dsmem_u32(mapa(smem_u32(&cred[6]), (unsigned)q))) != 0.0f ? 1 : 0;
+                A.bbox[b * BBOX_STRIDE + 6] = anybad ? 1u : 0u;
+                if (A.host_rb) A.host_rb[2 * A.B + b] = anybad;
+            }
+        }
+        __syncthreads();
+    }
+    unsigned *kin = reinterpret_cast<unsigned *>(fsm), *kout = kin + A.Nmax;
+    int *vin = reinterpret_cast<int *>(kout + A.Nmax), *vout = vin + A.Nmax;
+    int *const table = vout + A.Nmax;                              // digit-major [256][nchunk]
+    // ---- a2: sort keys of this CTA's points (the arithmetic of k_keys) ----
+    {
+        const float E = fmaxf(fmaxf(bb[3] - bb[0], bb[4] - bb[1]), bb[5] - bb[2]);
+        float L = (1.0f + 1e-3f) * E / (float)A.n_vox;
+        if (!(L > 0.0f)) L = 1.0f;
+        const float invsub = (float)(1 << A.sb);
+        for (int j = tid; j < n; j += FUSED_T) {
+            const int i = p0 + j;
+            unsigned v[3], s[3];
+#pragma unroll
+            for (int a = 0; a < 3; ++a) {
+                const float t = (P[3 * (size_t)i + a] - bb[a]) / L;
+                int c = (int)floorf(t);
+                c = max(0, min(A.n_vox - 1, c));
+                int sc = (int)floorf((t - (float)c) * invsub);
+                sc = max(0, min((1 << A.sb) - 1, sc));
+                v[a] = (unsigned)c;
+                s[a] = (unsigned)sc;
+            }
+            const unsigned vid = hilbert3(v[0], v[1], v[2], A.hb);
+            const unsigned sub = A.sb ? (spread3(s[0]) | (spread3(s[1]) << 1) | (spread3(s[2]) << 2)) : 0u;
+            kin[j] = (vid << (3 * A.sb)) | sub;
+            vin[j] = i;
+        }
+        __syncthreads();
+    }
+    // ---- a3: stable LSD radix sort across the cluster, 8 bits per pass ----
+    {
+        const int nchunk = (n + FUSED_CHUNK - 1) / FUSED_CHUNK;                 // this CTA's chunks (0 if it holds no point)
+        const int ts = ((A.Nmax + FUSED_CHUNK - 1) / FUSED_CHUNK) | 1;          // odd row stride of the digit table
+        const unsigned lt = (1u << lane) - 1u;
+        for (int shift = 0; shift < A.keybits; shift += 8) {
+            for (int i = tid; i < 256 * ts; i += FUSED_T) table[i] = 0;         // (chunks this CTA does not have count nothing)
+            __syncthreads();
+            for (int c0 = 0; c0 < nchunk; c0 += NWF) {
+                const int c = c0 + w;
+                for (int d = lane; d < 256; d += 32) hist[w][d] = 0;
+                __syncwarp();
+                if (c < nchunk) {
+                    const int end = min(n, (c + 1) * FUSED_CHUNK);
+                    unsigned kr[FUSED_CHUNK / 32];
+#pragma unroll
+                    for (int q = 0; q < FUSED_CHUNK / 32; ++q) { const int p = c * FUSED_CHUNK + 32 * q + lane; kr[q] = p < end ? kin[p] : 0u; }
+#pragma unroll
+                    for (int q = 0; q < FUSED_CHUNK / 32; ++q)
+                        if (c * FUSED_CHUNK + 32 * q + lane < end) atomicAdd(&hist[w][(kr[q] >> shift) & 255u], 1);
+                    __syncwarp();
+                    for (int d = lane; d < 256; d += 32) table[d * ts + c] = hist[w][d];
+                }
+                __syncwarp();
+            }
+            __syncthreads();
+            // this CTA's digit totals -> the peers; every CTA then knows where each of its digits starts in the output
+            int mine = 0;
+            if (tid < 256) {
+                for (int c = 0; c < nchunk; ++c) mine += table[tid * ts + c];
+                tdig[tid] = mine;
+            }
+            cluster_sync_all();
+            int all = 0, before = 0;
+            if (tid < 256)
+                for (int q = 0; q < C; ++q) {
+                    const int v = (int)ld_dsmem_u32(mapa(smem_u32(&tdig[tid]), (unsigned)q));
+                    all += v;
+                    before += q < r ? v : 0;
+                }
+            const int2 ex = scan256_pair(all, mine, sm);      // digits before d: in the whole cloud / in this CTA
+            // global offset of (digit d, chunk c) = (all digits < d) + (digit d in the CTAs before this one) + (digit d in
+            // this CTA's chunks before c); the local digit-major scan of the table below yields (this CTA's digits < d) +
+            // (digit d in its chunks before c): fix[d] is the difference
+            if (tid < 256) fix[tid] = ex.x + before - ex.y;
+            __syncthreads();
+            cta_scan_excl(table, table, 256 * ts, sm);
+            for (int c0 = 0; c0 < nchunk; c0 += NWF) {
+                const int c = c0 + w;
+                if (c < nchunk) {
+                    for (int d = lane; d < 256; d += 32) hist[w][d] = table[d * ts + c] + fix[d];
+                    __syncwarp();
+                    const int end = min(n, (c + 1) * FUSED_CHUNK);
+                    unsigned kr[FUSED_CHUNK / 32];
+                    int vr[FUSED_CHUNK / 32];
+#pragma unroll
+                    for (int q = 0; q < FUSED_CHUNK / 32; ++q) {
+                        const int p = c * FUSED_CHUNK + 32 * q + lane;
+                        kr[q] = p < end ? kin[p] : 0u;
+                        vr[q] = p < end ? vin[p] : 0;
+                    }
+#pragma unroll
+                    for (int q = 0; q < FUSED_CHUNK / 32; ++q) {
+                        if (c * FUSED_CHUNK + 32 * q >= end) break;      // warp-uniform
+                        const bool valid = c * FUSED_CHUNK + 32 * q + lane < end;
+                        const unsigned key = kr[q];
+                        const int val = vr[q];
+                        const unsigned d = valid ? ((key >> shift) & 255u) : 256u;
+                        const unsigned peers = same_digit_lanes(d, valid);
+                        const int rk = __popc(peers & lt);
+                        int dst = 0;
+                        if (valid) dst = hist[w][d] + rk;
+                        __syncwarp();
+                        if (valid && rk == 0) hist[w][d] += __popc(peers);
+                        __syncwarp();
+                        if (valid) {                                     // straight into the owner's shared memory
+                            const int q2 = dst / Np, li = dst - q2 * Np;
+                            st_dsmem_u32(mapa(smem_u32(kout + li), (unsigned)q2), key);
+                            st_dsmem_u32(mapa(smem_u32(vout + li), (unsigned)q2), (unsigned)val);
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+            cluster_sync_all();                                          // every CTA's scatter has landed
+            unsigned *tk = kin; kin = kout; kout = tk;
+            int *tv = vin; vin = vout; vout = tv;
+        }
+    }
+    // ---- a4: gather this CTA's sorted positions (AoS -> sorted SoA, permutation and its inverse) ----
+    float *px = A.px + base, *py = A.py + base, *pz = A.pz + base;
+    int *porig = A.porig + base, *pinv = A.pinv + base;
+    for (int j0 = tid; j0 < n; j0 += 4 * FUSED_T) {
+        int idx[4];
+        float c[4][3];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) idx[u] = j0 + u * FUSED_T < n ? vin[j0 + u * FUSED_T] : vin[j0];
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+            for (int a = 0; a < 3; ++a) c[u][a] = P[3 * (size_t)idx[u] + a];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+            const int j = j0 + u * FUSED_T;
+            if (j < n) {
+                const int q = p0 + j;
+                px[q] = c[u][0]; py[q] = c[u][1]; pz[q] = c[u][2];
+                porig[q] = idx[u];
+                pinv[idx[u]] = q;
+            }
+        }
+    }
+    __syncthreads();                                                     // (vin is free from here on)
+    // ---- a5: grid voxels (heads -> rank -> offsets) and tiles (counts -> base -> segments), spread over the cluster: every
+    // CTA scans its own share in shared memory; the shares are chained through per-CTA totals read over DSMEM ----
+    int2 *vseg = A.vseg + (size_t)b * A.K_cap;
+    {
+        int *const F1 = reinterpret_cast<int *>(kout), *const F2 = vout;         // (free since the sort)
+        int *const voffg = CA.F1g + base;                                        // first point of every grid voxel (global)
+        const int subbits = 3 * A.sb;
+        // heads of this CTA's positions; the key before its first position is the last key of the CTA before it
+        unsigned prevk = 0u;
+        if (r > 0 && n > 0) prevk = ld_dsmem_u32(mapa(smem_u32(kin + (Np - 1)), (unsigned)(r - 1)));
+        for (int j = tid; j < n; j += FUSED_T) {
+            const unsigned pk = j > 0 ? kin[j - 1] : prevk;
+            F1[j] = (p0 + j == 0 || (kin[j] >> subbits) != (pk >> subbits)) ? 1 : 0;
+        }
+        __syncthreads();
+        const int hc = cta_scan_excl(F1, F2, n, sm);                             // F2 = rank of a head among this CTA's heads
+        if (tid == 0) xch[0] = hc;
+        cluster_sync_all();
+        int vbase = 0, kv = 0;
+        for (int q = 0; q < C; ++q) {
+            const int v = (int)ld_dsmem_u32(mapa(smem_u32(&xch[0]), (unsigned)q));
+            vbase += q < r ? v : 0;
+            kv += v;
+        }
+        for (int j = tid; j < n; j += FUSED_T)
+            if (F1[j]) voffg[vbase + F2[j]] = p0 + j;
+        cluster_sync_all();                                                      // voffg is complete
+        // tiles: the grid voxels are dealt to the CTAs in contiguous shares
+        const int Kp = (kv + C - 1) / C, k0 = min(kv, r * Kp), nk = min(kv, k0 + Kp) - k0;
+        auto tiles_of = [&](const int cnt) { return A.tile_points > 0 ? (cnt + A.tile_points - 1) / A.tile_points : 1; };
+        for (int kl = tid; kl < nk; kl += FUSED_T) {
+            const int k = k0 + kl;
+            F1[kl] = tiles_of((k + 1 < kv ? voffg[k + 1] : N) - voffg[k]);
+        }
+        __syncthreads();
+        const int tc = cta_scan_excl(F1, F2, nk, sm);                            // F2 = first tile of a voxel among this CTA's tiles
+        if (tid == 0) xch[1] = tc;
+        cluster_sync_all();
+        int tb = 0, Kt = 0;
+        for (int q = 0; q < C; ++q) {
+            const int v = (int)ld_dsmem_u32(mapa(smem_u32(&xch[1]), (unsigned)q));
+            tb += q < r ? v : 0;
+            Kt += v;
+        }
+        if (r == 0 && tid == 0) { A.K_dev[b] = Kt; if (A.host_rb) A.host_rb[b] = Kt; }
+        for (int kl = tid; kl < nk; kl += FUSED_T) {
+            const int k = k0 + kl;
+            const int off = voffg[k];
+            const int cnt = (k + 1 < kv ? voffg[k + 1] : N) - off;
+            const int nt = F1[kl];
+            const int chunk = (cnt + nt - 1) / nt;
+            int2 *dst = vseg + tb + F2[kl];
+            for (int t = 0; t < nt; ++t) dst[t] = make_int2(off + t * chunk, min(chunk, cnt - t * chunk));
+        }
+        sK = Kt;                                                                  // (every thread writes the same value)
+    }
+    cluster_sync_all();                                                          // vseg is complete
+    const int K = sK;
+    // ---- a6: tight bounding sphere per (tiled) voxel: eight lanes per voxel, four voxels per warp in flight (the points
+    // come from global memory / L2: what counts is the number of round trips under way), voxels dealt over the cluster ----
+    float4 *vgeom = A.vgeom + (size_t)b * A.K_cap;
+    int local_max = 0;
+    {
+        const int sub = lane & 7, grp = (r * NWF + w) * 4 + (lane >> 3), NG = C * NWF * 4;
+        for (int k0 = 0; k0 < K; k0 += NG) {
+            const int k = k0 + grp;
+            const int2 sg = k < K ? vseg[k] : make_int2(0, 0);
+            float mn[3] = {FLT_MAX, FLT_MAX, FLT_MAX}, mx[3] = {-FLT_MAX, -FLT_MAX, -FLT_MAX};
+            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) {
+                mn[0] = fminf(mn[0], px[p]); mx[0] = fmaxf(mx[0], px[p]);
+                mn[1] = fminf(mn[1], py[p]); mx[1] = fmaxf(mx[1], py[p]);
+                mn[2] = fminf(mn[2], pz[p]); mx[2] = fmaxf(mx[2], pz[p]);
+            }
+#pragma unroll
+            for (int a = 0; a < 3; ++a)
+                for (int o = 4; o > 0; o >>= 1) {
+                    mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                    mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+                }
+            const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+            const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+            const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+            float r2 = 0.0f;
+            for (int p = sg.x + sub; p < sg.x + sg.y; p += 8) r2 = fmaxf(r2, d2_rn(px[p], py[p], pz[p], cx, cy, cz));
+            for (int o = 4; o > 0; o >>= 1) r2 = fmaxf(r2, __shfl_xor_sync(0xffffffffu, r2, o));
+            if (sub == 0 && k < K) {
+                vgeom[k] = make_float4(cx, cy, cz, __fmul_rn(__fsqrt_rn(r2), 1.0f + 0x1p-20f));
+                local_max = max(local_max, sg.y);
+            }
+        }
+    }
+    local_max = __reduce_max_sync(0xffffffffu, local_max);
+    if (tid == 0) smaxc = 0;
+    __syncthreads();
+    if (lane == 0 && local_max > 0) atomicMax(&smaxc, local_max);
+    __syncthreads();
+    if (tid == 0) cred[7] = __int_as_float(smaxc);
+    cluster_sync_all();
+    // ---- a6': group spheres (32 consecutive voxels), groups dealt over the cluster's warps ----
+    float4 *ggeom = A.ggeom + (size_t)b * A.G_cap;
+    const int G = (K + 31) / 32;
+    for (int g = r * NWF + w; g < G; g += C * NWF) {
+        const int k = g * 32 + lane;
+        const bool in = k < K;
+        const float4 v = in ? vgeom[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        float mn[3] = {in ? v.x - v.w : FLT_MAX, in ? v.y - v.w : FLT_MAX, in ? v.z - v.w : FLT_MAX};
+        float mx[3] = {in ? v.x + v.w : -FLT_MAX, in ? v.y + v.w : -FLT_MAX, in ? v.z + v.w : -FLT_MAX};
+#pragma unroll
+        for (int a = 0; a < 3; ++a)
+            for (int o = 16; o > 0; o >>= 1) {
+                mn[a] = fminf(mn[a], __shfl_xor_sync(0xffffffffu, mn[a], o));
+                mx[a] = fmaxf(mx[a], __shfl_xor_sync(0xffffffffu, mx[a], o));
+            }
+        const float cx = __fadd_rn(__fmul_rn(0.5f, mn[0]), __fmul_rn(0.5f, mx[0]));
+        const float cy = __fadd_rn(__fmul_rn(0.5f, mn[1]), __fmul_rn(0.5f, mx[1]));
+        const float cz = __fadd_rn(__fmul_rn(0.5f, mn[2]), __fmul_rn(0.5f, mx[2]));
+        float rr = 0.0f;
+        if (in) rr = __fmul_rn(__fadd_rn(__fmul_rn(__fsqrt_rn(d2_rn(v.x, v.y, v.z, cx, cy, cz)), 1.0f + 0x1p-20f), v.w), 1.0f + 0x1p-20f);
+        for (int o = 16; o > 0; o >>= 1) rr = fmaxf(rr, __shfl_xor_sync(0xffffffffu, rr, o));
+        if (lane == 0) ggeom[g] = make_float4(cx, cy, cz, rr);
+    }
+    if (r == 0 && tid == 0) {
+        int mc = 0;
+        for (int q = 0; q < C; ++q) mc = max(mc, (int)ld_dsmem_u32(mapa(smem_u32(&cred[7]), (unsigned)q)));
+        if (A.host_rb) { A.host_rb[A.B + b] = mc; __threadfence_system(); }
+        else if (mc > 0) atomicMax(A.maxcnt, mc);
+    }
+    cluster_sync_all();              // no CTA may exit while a peer can still read its shared memory
+}
+
+// ---------------------------------------------------------------------------------------------
 // host orchestration
 // ---------------------------------------------------------------------------------------------
 static int ilog2_ceil(unsigned long long v)
@@ -1204,6 +1618,7 @@ static bool fused_attr_set()
     std::lock_guard<std::mutex> lock(mu);
     if (dev >= 0 && dev < 64 && done[dev]) return true;
     if (cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)) != cudaSuccess) return false;
+    if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cluster_smem_bytes(CL_PER_CTA)) != cudaSuccess) return false;
     if (dev >= 0 && dev < 64) done[dev] = true;
     return true;
 }
@@ -1328,7 +1743,9 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     // single-launch build with pinned staging: the kernel writes the read-back values straight into the (mapped) host
     // block and, for equal-size clouds, computes the offsets itself -- no memset, no copy in, no copy out
     int *host_rb_dev = nullptr;
-    if (fused && stage && cudaHostGetDevicePointer((void **)&host_rb_dev, stage + (B + 1), 0) != cudaSuccess) { cudaGetLastError(); host_rb_dev = nullptr; }
+    // mid-size clouds: one launch too, one thread-block cluster per cloud (k_build_cluster)
+    const bool clustered = !fused && N <= CL_MAX_N && !(o.flags & FPS_FLAG_CHAIN_BUILD) && stage != nullptr;
+    if ((fused || clustered) && stage && cudaHostGetDevicePointer((void **)&host_rb_dev, stage + (B + 1), 0) != cudaSuccess) { cudaGetLastError(); host_rb_dev = nullptr; }
     const bool zero_copy = host_rb_dev != nullptr, poff_in_kernel = zero_copy && !ix.ragged;
     unsigned *chain_rb_dev = nullptr;     // kernel chain: the last kernel copies the read-back block to the host
     const void *poff_src = ph;
@@ -1358,6 +1775,25 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
             return FPS_ERR_CUDA;
         }
         launch_pdl_smem(log, fused_smem_bytes(N), k_build_fused, dim3(B), dim3(FUSED_T), st, fa);
+    } else if (clustered && zero_copy) {
+        const int C = cluster_build_ctas(N), Np = (N + C - 1) / C;
+        ClusterArgs ca;
+        FusedArgs &fa = ca.f;
+        fa.pts = points; fa.poff = poff; fa.bbox = sc.bbox;
+        fa.n_vox = n_vox; fa.hb = vbits / 3; fa.sb = sb; fa.keybits = keybits; fa.tile_points = tile_points;
+        fa.K_cap = ix.K_cap; fa.G_cap = ix.G_cap; fa.Nmax = Np;
+        fa.px = ix.px; fa.py = ix.py; fa.pz = ix.pz; fa.porig = ix.porig; fa.pinv = ix.pinv;
+        fa.vseg = ix.vseg; fa.vgeom = ix.vgeom; fa.ggeom = ix.ggeom; fa.K_dev = ix.K_dev;
+        fa.maxcnt = reinterpret_cast<int *>(meta);
+        fa.host_rb = host_rb_dev; fa.B = B;
+        if (poff_in_kernel) { fa.uniform_N = N; fa.poff_out = ix.poff_dev; }
+        ca.F1g = sc.heads;
+        if (!fused_attr_set()) {
+            set_error("cudaFuncSetAttribute(k_build_cluster) failed: %s", cudaGetErrorString(cudaGetLastError()));
+            release_scratch();
+            return FPS_ERR_CUDA;
+        }
+        launch_pdl_cluster(log, cluster_smem_bytes(Np), C, k_build_cluster, dim3(B * C), dim3(FUSED_T), st, ca);
     } else {
     launch_pdl(log, k_bbox_init, dim3((B * BBOX_STRIDE + 255) / 256), dim3(256), st, sc.bbox, B);
     launch_pdl(log, k_bbox, dim3(dim3(std::max(1, std::min((N + 4095) / 4096, sms)), B)), dim3(256), st, points, poff, sc.bbox);

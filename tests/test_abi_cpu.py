@@ -157,7 +157,7 @@ def test_every_build_kernel_waits_for_its_predecessor_grid():
         first = body[body.index("{") + 1:].lstrip().splitlines()[0].strip()
         assert first == "grid_dep_sync();", (k, first)
     assert "<<<" not in src.replace("// ", ""), "a build kernel is launched without launch_pdl"
-    assert set(re.findall(r"launch_pdl(?:_smem)?\(log, (?:[^,(]+\([^)]*\), )?(k_\w+),", src)) == set(kernels)
+    assert set(re.findall(r"launch_pdl(?:_smem|_cluster)?\(log, (?:[^,(]+\([^)]*\), )?(?:\w+, )?(k_\w+),", src)) == set(kernels)
     helper = src[src.index("void grid_dep_sync()"):]
     helper = helper[:helper.index("}")]
     assert helper.index("griddepcontrol.launch_dependents") < helper.index("griddepcontrol.wait")

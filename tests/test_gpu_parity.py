@@ -202,6 +202,48 @@ def test_single_launch_build_equals_the_kernel_chain(rf, name):
     assert_same(b[0], b[1], *ref)
 
 
+@pytest.mark.parametrize("gen,B,N", [("room", 3, 24000), ("cube", 2, 8193), ("lidar", 2, 32768), ("clustered", 1, 20011)])
+def test_cluster_build_equals_the_kernel_chain(rf, gen, B, N):
+    # clouds of 8 193 .. 32 768 points: one launch, one thread-block cluster per cloud, radix passes over distributed
+    # shared memory; same voxels, tiles and samples as the chain
+    mk = {"room": inputs.room, "cube": inputs.uniform_cube, "clustered": inputs.clustered,
+          "lidar": lambda n, s: inputs.lidar(n, s, n_azimuth=512)}[gen]
+    P = np.stack([mk(N, 900 + b) for b in range(B)])
+    M = 257
+    ref = oracle.fps(P, M, 5)
+    a = run_gpu(rf, P, M, 5, flags=rf.FPS_FLAG_STATS)
+    b = run_gpu(rf, P, M, 5, flags=rf.FPS_FLAG_STATS | rf.FPS_FLAG_CHAIN_BUILD)
+    assert a[2]["build_launches"] == 1 and b[2]["build_launches"] > 10
+    for key in ("K_total", "K_max", "max_voxel_points", "n_vox", "voxel_tests", "voxels_visited", "points_visited", "effective"):
+        assert a[2][key] == b[2][key], key
+    assert_same(a[0], a[1], *ref)
+    assert_same(b[0], b[1], *ref)
+
+
+def test_cluster_build_ragged_batch_and_bad_input(rf):
+    clouds = [inputs.room(20000, 31), inputs.uniform_cube(7, 32), inputs.lidar(9001, 33, n_azimuth=140), inputs.uniform_cube(1, 34),
+              inputs.clustered(30000, 35)]
+    Ms = [300, 7, 400, 1, 350]
+    off = np.concatenate([[0], np.cumsum([c.shape[0] for c in clouds])]).astype(np.int64)
+    P = torch.from_numpy(np.ascontiguousarray(np.concatenate(clouds, axis=0))).cuda()
+    ix = rf.fps_index_build_ragged(P, off.tolist())
+    try:
+        assert rf.fps_get_stats(ix)["build_launches"] == 1
+        idx, mind, ooff = rf.fps_sample_ragged(ix, Ms)
+        torch.cuda.synchronize()
+        idx, mind = idx.cpu().numpy(), mind.cpu().numpy()
+        for b, c in enumerate(clouds):
+            ref_i, ref_m = oracle.fps(c, Ms[b], 0)
+            assert_same(idx[ooff[b]:ooff[b + 1]], mind[ooff[b]:ooff[b + 1]], ref_i.reshape(-1), ref_m.reshape(-1))
+    finally:
+        rf.fps_index_destroy(ix)
+    bad = inputs.room(12000, 36).copy()
+    bad[11999, 1] = np.nan
+    with pytest.raises(rf.FpsError) as e:
+        rf.fps_index_build(torch.from_numpy(bad).cuda())
+    assert e.value.status == rf.FPS_ERR_NONFINITE
+
+
 def test_single_launch_build_ragged_batch(rf):
     clouds = [inputs.room(5000, 21), inputs.uniform_cube(1, 22), inputs.lidar(7001, 23, n_azimuth=110),
               inputs.shuffled_lattice(8, 24), inputs.uniform_cube(33, 25), inputs.clustered(2500, 26)]
