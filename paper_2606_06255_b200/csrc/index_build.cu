@@ -1123,7 +1123,7 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
 }
 
 // ---------------------------------------------------------------------------------------------
-// a1-a6 in ONE launch for MID-SIZE clouds (FUSED_MAX_N < N <= CL_MAX_N, e.g. config 2's 24 000 points): one
+// a1-a6 in ONE launch for MID-SIZE clouds (FUSED_MAX_N < N <= CL_MAX_N = 155 648, e.g. config 2's 24 000 points): one
 // thread-block CLUSTER of C CTAs per cloud.  CTA r owns the points (later: the sorted positions) [r Np, (r+1) Np);
 // keys and values live in its shared memory as in k_build_fused, and the radix passes exchange across the cluster:
 // every CTA publishes its 256 digit totals (read by the peers over DSMEM), derives the global output offset of each
@@ -1133,7 +1133,9 @@ __global__ void __launch_bounds__(FUSED_T, 1) k_build_fused(const FusedArgs A)
 // of the cluster.  A dozen cluster barriers instead of 22 launches; same voxels, tiles and spheres as the chain
 // (tests compare them).
 // ---------------------------------------------------------------------------------------------
-constexpr int CL_MAX_N = 32768, CL_PER_CTA = 6144, CL_MAX_C = 8;
+// ~6 000 points per CTA where that needs <= 16 CTAs (a cluster of more than 8 is "non-portable" but fits a B200 GPC);
+// up to CL_PER_CTA_MAX per CTA beyond (what the 227 KB of shared memory hold next to the 35 KB of static arrays)
+constexpr int CL_PER_CTA = 6144, CL_PER_CTA_MAX = 9728, CL_MAX_C = 16, CL_MAX_N = CL_MAX_C * CL_PER_CTA_MAX;
 static inline int cluster_build_ctas(int N) { return std::min(CL_MAX_C, std::max(2, (N + CL_PER_CTA - 1) / CL_PER_CTA)); }
 static inline size_t cluster_smem_bytes(int Np) { return (size_t)16 * Np + (size_t)1024 * (((Np + FUSED_CHUNK - 1) / FUSED_CHUNK) | 1); }
 
@@ -1618,7 +1620,8 @@ static bool fused_attr_set()
     std::lock_guard<std::mutex> lock(mu);
     if (dev >= 0 && dev < 64 && done[dev]) return true;
     if (cudaFuncSetAttribute(k_build_fused, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fused_smem_bytes(FUSED_MAX_N)) != cudaSuccess) return false;
-    if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cluster_smem_bytes(CL_PER_CTA)) != cudaSuccess) return false;
+    if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)cluster_smem_bytes(CL_PER_CTA_MAX)) != cudaSuccess) return false;
+    if (cudaFuncSetAttribute(k_build_cluster, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess) return false;
     if (dev >= 0 && dev < 64) done[dev] = true;
     return true;
 }
@@ -1744,7 +1747,11 @@ int build_index(DeviceIndex &ix, const float *points, const fps_build_opts &o)
     // block and, for equal-size clouds, computes the offsets itself -- no memset, no copy in, no copy out
     int *host_rb_dev = nullptr;
     // mid-size clouds: one launch too, one thread-block cluster per cloud (k_build_cluster)
-    const bool clustered = !fused && N <= CL_MAX_N && !(o.flags & FPS_FLAG_CHAIN_BUILD) && stage != nullptr;
+    // (measured: C2 0.172 -> 0.112 ms, C4 0.240 -> 0.152 ms; a single cloud of 150 000 points on 16 CTAs takes 0.203 ms
+    // against 0.164 ms for the chain, which spreads it over the whole GPU: beyond 8 192 points per CTA, or for one
+    // cloud of more than 65 536 points, the chain stays)
+    const bool clustered = !fused && N <= CL_MAX_N && (N + cluster_build_ctas(N) - 1) / cluster_build_ctas(N) <= 8192 && (N <= 65536 || B >= 2) &&
+                           !(o.flags & FPS_FLAG_CHAIN_BUILD) && stage != nullptr;
     if ((fused || clustered) && stage && cudaHostGetDevicePointer((void **)&host_rb_dev, stage + (B + 1), 0) != cudaSuccess) { cudaGetLastError(); host_rb_dev = nullptr; }
     const bool zero_copy = host_rb_dev != nullptr, poff_in_kernel = zero_copy && !ix.ragged;
     unsigned *chain_rb_dev = nullptr;     // kernel chain: the last kernel copies the read-back block to the host

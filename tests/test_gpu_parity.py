@@ -202,10 +202,11 @@ def test_single_launch_build_equals_the_kernel_chain(rf, name):
     assert_same(b[0], b[1], *ref)
 
 
-@pytest.mark.parametrize("gen,B,N", [("room", 3, 24000), ("cube", 2, 8193), ("lidar", 2, 32768), ("clustered", 1, 20011)])
+@pytest.mark.parametrize("gen,B,N", [("room", 3, 24000), ("cube", 2, 8193), ("lidar", 2, 32768), ("clustered", 1, 20011),
+                                     ("room", 1, 65536), ("lidar", 2, 120000)])
 def test_cluster_build_equals_the_kernel_chain(rf, gen, B, N):
-    # clouds of 8 193 .. 32 768 points: one launch, one thread-block cluster per cloud, radix passes over distributed
-    # shared memory; same voxels, tiles and samples as the chain
+    # clouds of 8 193 .. ~130 000 points (one cloud: .. 65 536): one launch, one thread-block cluster of 2-16 CTAs per
+    # cloud, radix passes over distributed shared memory; same voxels, tiles and samples as the chain
     mk = {"room": inputs.room, "cube": inputs.uniform_cube, "clustered": inputs.clustered,
           "lidar": lambda n, s: inputs.lidar(n, s, n_azimuth=512)}[gen]
     P = np.stack([mk(N, 900 + b) for b in range(B)])
