@@ -82,8 +82,9 @@ enum {
     FPS_FLAG_NO_BATCH = 8,  /* ablation: every batch of the batched kernel is the single global argmax  */
     FPS_FLAG_PER_PICK = 16, /* run the per-pick persistent kernel (one cluster-wide exchange per sample,
                                the paper's iteration structure) instead of exact batched picking        */
-    FPS_FLAG_CHAIN_BUILD = 64, /* build the index with the chain of ~22 kernels also for small clouds (N <= 32 768),
-                               which by default take the single-launch build (one CTA per cloud); same index    */
+    FPS_FLAG_CHAIN_BUILD = 64, /* build the index with the chain of ~22 kernels also for clouds that by default take a
+                               single-launch build (one CTA per cloud up to 8 192 points, one thread-block cluster
+                               per cloud up to 65 536 points -- batches: ~130 000); same voxels, tiles and samples */
     FPS_FLAG_EUCLIDEAN = 32 /* NOT an option that leaves results alone: sample with the Euclidean distance
                                sqrt_rn(d2), the paper's literal Eq. 1 / Eq. 29, instead of
                                d2.  out_mindist then holds distances.  In fp32 this is a different function:

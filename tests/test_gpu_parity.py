@@ -189,8 +189,8 @@ def test_result_independent_of_tiling(rf, name, tile):
 
 @pytest.mark.parametrize("name", sorted(SMALL))
 def test_single_launch_build_equals_the_kernel_chain(rf, name):
-    # clouds of <= 32 768 points are indexed by ONE kernel launch (one CTA per cloud); FPS_FLAG_CHAIN_BUILD forces the
-    # chain of ~22 kernels that larger clouds take: same voxels, same tiles, same samples
+    # clouds of <= 8 192 points are indexed by ONE kernel launch (one CTA per cloud); FPS_FLAG_CHAIN_BUILD forces the
+    # chain of ~22 kernels that large clouds take: same voxels, same tiles, same samples
     P, M = SMALL[name]()
     ref = oracle.fps(P, M, 0)
     a = run_gpu(rf, P, M, n_vox=8)
