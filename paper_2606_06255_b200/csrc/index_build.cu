@@ -1629,7 +1629,8 @@ static bool fused_attr_set()
 // Per-thread pinned host staging for the two small copies of a build (cloud offsets in, read-back block out): with a
 // pageable buffer both copies are staged by the driver and cost several microseconds of host time each, which is a
 // visible part of a small cloud's build.  Grown on demand, kept for the life of the thread (a build synchronises its
-// stream before it returns, so the buffer is free again by then); nullptr if pinned memory cannot be had.
+// stream before it returns, so the buffer is free again by then; portable + mapped, so that every device the thread
+// builds on can write its read-back block into it); nullptr if pinned memory cannot be had.
 static unsigned *pinned_stage(size_t words)
 {
     struct Stage { unsigned *p = nullptr; size_t cap = 0; };
@@ -1638,7 +1639,7 @@ static unsigned *pinned_stage(size_t words)
         if (t.p) cudaFreeHost(t.p);
         t.p = nullptr; t.cap = 0;
         const size_t want = std::max<size_t>(words * 2, 4096);
-        if (cudaHostAlloc((void **)&t.p, want * sizeof(unsigned), cudaHostAllocMapped) != cudaSuccess) { cudaGetLastError(); t.p = nullptr; return nullptr; }
+        if (cudaHostAlloc((void **)&t.p, want * sizeof(unsigned), cudaHostAllocMapped | cudaHostAllocPortable) != cudaSuccess) { cudaGetLastError(); t.p = nullptr; return nullptr; }
         t.cap = want;
     }
     return t.p;
